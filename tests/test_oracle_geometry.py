@@ -1,0 +1,120 @@
+"""Pins for O2 (oracle/geometry.py) and the sign conventions of O4: exact facts only.  CPU only."""
+import numpy as np
+import pytest
+
+from oracle import Oracle, geodesic
+from oracle import geometry as G
+
+
+def _ks_points(a, n=200, lo=0.15, hi=0.85, seed=0):
+    rng = np.random.default_rng(seed)
+    rh = 1 + np.sqrt(1 - a * a)
+    return np.stack([np.log(rng.uniform(0.9 * rh, 50, n)), rng.uniform(lo, hi, n), rng.uniform(0, 6.28, n)], -1)
+
+
+@pytest.mark.parametrize("a", [0.0, 0.9, 0.9375])
+def test_ks_tetrad_eq1_eq4_inverse(a):
+    X = _ks_points(a, lo=0.02, hi=0.98)
+    P = dict(a=a, hslope=0.3)
+    g = G.metric("ks_mks", P, X)
+    e, ei = G.tetrad("ks_mks", P, X)
+    eta = np.einsum("...ma,...nb,...mn->...ab", e, e, g)
+    assert np.abs(eta - G.ETA).max() < 5e-14                                           # Eq 1
+    assert np.abs(np.einsum("...am,...mb->...ab", ei, e) - np.eye(4)).max() < 5e-14     # L67
+    gi = np.linalg.inv(g)
+    e0 = -gi[..., 0, :] / np.sqrt(-gi[..., 0, 0])[..., None]
+    assert np.abs(e0 - e[..., :, 0]).max() < 5e-14                                      # Eq 4
+    assert np.all(e[..., 0, 1:] == 0)           # spatial legs have no time component => n^0 = 1/lapse for all s
+    # sqrt(-g) of Kerr-Schild is Sigma sin(theta), times the Jacobian of the logical map
+    r, th, drdx, dthdx = G._ks_map(P, X)
+    sg = (r * r + a * a * np.cos(th) ** 2) * np.sin(th) * drdx * dthdx
+    assert np.allclose(G.sqrt_neg_g("ks_mks", P, X), sg, rtol=1e-11)
+
+
+def test_ks_metric_is_vacuum_solution_inverse_component():
+    # g^{tt} of Kerr-Schild is -(1 + 2r/Sigma) exactly (lapse^-2), g^{t phi} = 0: independent textbook facts
+    a = 0.9
+    X = _ks_points(a)
+    P = dict(a=a, hslope=0.3)
+    r, th, _, _ = G._ks_map(P, X)
+    gi = np.linalg.inv(G.metric("ks_mks", P, X))
+    H = 2 * r / (r * r + a * a * np.cos(th) ** 2)
+    assert np.allclose(gi[..., 0, 0], -(1 + H), rtol=1e-11)
+    assert np.abs(gi[..., 0, 3]).max() < 1e-11
+
+
+def test_omega_antisymmetry_and_flat_values():
+    a = 0.9
+    X = _ks_points(a)
+    om = G.ricci_rotation("ks_mks", dict(a=a, hslope=0.3), X)
+    oml = np.einsum("ab,...bcd->...acd", G.ETA, om)
+    assert np.abs(oml + np.swapaxes(oml, -3, -1)).max() < 1e-10       # omega_{a c d} = -omega_{d c a}
+    assert np.abs(G.ricci_rotation("minkowski", {}, X)).max() == 0.0
+    # cylindrical tetrad in flat space: only omega^R_{phi phi} = -1/R and omega^phi_{phi R} = +1/R
+    X = np.array([[1.3, 0.7, 0.4]])
+    om = G.ricci_rotation("mink_cyl", {}, X)[0]
+    R = np.hypot(1.3, 0.7)
+    ref = np.zeros((4, 4, 4))
+    ref[1, 2, 2], ref[2, 2, 1] = -1 / R, 1 / R
+    assert np.abs(om - ref).max() < 1e-10
+
+
+def test_angular_acceleration_is_rate_of_change_of_tetrad_components():
+    """a^i(n) = -(omega^i_cd - n^i omega^0_cd) n^c n^d must equal d/dlambda of the tetrad components of a FIXED
+    Cartesian direction along its own straight ray (flat space, rotating tetrad): fixes the sign of Eq 7/8."""
+    x0 = np.array([1.3, 0.7, 0.4])
+    rng = np.random.default_rng(1)
+    for _ in range(5):
+        d = rng.normal(size=3)
+        d /= np.linalg.norm(d)                      # Cartesian direction of the ray
+
+        def comps(lam):
+            e, ei = G.tetrad("mink_cyl", {}, (x0 + lam * d)[None])
+            return ei[0, 1:, 1:] @ d                 # nhat^i = e^i_mu d^mu
+
+        h = 1e-4
+        exact = (-comps(2 * h) + 8 * comps(h) - 8 * comps(-h) + comps(-2 * h)) / (12 * h)
+        nh = comps(0.0)
+        om = G.ricci_rotation("mink_cyl", {}, x0[None])[0]
+        n4 = np.concatenate([[1.0], nh])
+        acc = -np.einsum("icd,c,d->i", om[1:], n4, n4) + nh * np.einsum("cd,c,d->", om[0], n4, n4)
+        assert np.abs(acc - exact).max() < 1e-9
+
+
+@pytest.mark.parametrize("level,tol", [(2, 3.0e-2), (4, 1.5e-2), (8, 0.8e-2)])
+def test_discrete_liouville(level, tol):
+    """For I = 1 in flat space with a rotating tetrad the spatial divergence d_a n^a_s and the angular
+    divergence D_Omega(s) of the oracle must cancel up to the (first-order) angular truncation error.
+    This fixes the relative sign of the spatial and angular terms, of u_e and of a.  SURVEY probe values:
+    1.7e-2 / 8.2e-3 / 4.0e-3 at 42 / 162 / 642 directions, with max|d_a n^a| = 0.68."""
+    x0 = np.array([1.3, 0.7, 0.4])
+    h = 1e-3
+    grid = dict(n=(1, 1, 1), x0=tuple(x0 - h / 2), dx=(h, h, h), bc_lo=("outflow",) * 3, bc_hi=("outflow",) * 3)
+    o = Oracle(grid, "mink_cyl", {}, level, dict(method=0, limiter=3))
+    I = np.ones((1, 1, 1, o.nd))
+    dt = 1e-3
+    # transport of a uniform field: I_out - 1 = -dt * div_x / (n^0 n_0) with n^0 n_0 = -1
+    divx = -(o.transport(I, I, dt) - I).reshape(-1) / dt * (-1.0)
+    divo = -(o.angular_flux(I, I, dt) - I).reshape(-1) / dt * (-1.0)
+    assert np.abs(divx).max() > 0.5                     # the terms are individually O(1) ...
+    assert np.abs(divx + divo).max() < tol              # ... and cancel
+    # and the angular update is conservative per cell: sum_s w_s delta(n^0 n_0 I)_s = 0
+    assert abs((o.ang["w"] * divo).sum()) < 1e-11      # (1e-16 / dt round-off)
+
+
+def test_photon_orbit_radii_eq53():
+    # Eq 53 (L569) as an exact formula; paper prints r1 ~ 2.34, r2 ~ 3.53 for a = 0.5 (L648)
+    a = 0.5
+    r1 = 2 * (1 + np.cos(2 / 3 * np.arccos(-a)))
+    r2 = 2 * (1 + np.cos(2 / 3 * np.arccos(+a)))
+    assert abs(r1 - 2.34) < 0.01 and abs(r2 - 3.53) < 0.01
+    # cross-check with the oracle's metric (equatorial plane, x2 = 0.5 <=> theta = pi/2):
+    # Omega of a circular photon orbit solves g_tt + 2 g_tphi Om + g_phiphi Om^2 = 0 and its r-derivative = 0
+    def disc(x1):
+        gg = G.metric("ks_mks", dict(a=a, hslope=0.3), np.array([[x1, 0.5, 0.0]]))[0]
+        return gg[0, 0], gg[0, 3], gg[3, 3]
+    gtt, gtp, gpp = disc(np.log(r1))
+    Om = (-gtp + np.sqrt(gtp ** 2 - gtt * gpp)) / gpp          # prograde null angular velocity
+    h = 1e-5
+    f = lambda x1: (lambda t: t[0] + 2 * t[1] * Om + t[2] * Om * Om)(disc(x1))
+    assert abs((f(np.log(r1) + h) - f(np.log(r1) - h)) / (2 * h)) < 1e-6
