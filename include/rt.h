@@ -1,0 +1,130 @@
+/* rt.h -- C ABI of the B200-native radiation hot path of arxiv 2508.15532 (cuHARM radiation module).
+ *
+ * Per spatial cell x per direction update of the gray tetrad-frame intensity I(x, n) on a geodesic angular grid:
+ *   (a) conservative spatial transport   PAPER.md Eq 18 (L193), PLI L225, Eq 20 (L245), Eq 21-23 (L252-278)
+ *   (b) angular fluxes                   Eq 19 (L239-241) with Eq 7-8 (L99-109)
+ *   (c) implicit radiation-fluid source  Eq 35 (L352), Eq 39-46 (L377-430), Eq 5 (L85)
+ *   (d) moments R^mu_nu and 4-force      Eq 13 (L141), Eq 36/48 (L361, L442)
+ *   predictor-corrector driver           L448-456
+ * Readings of silent/garbled passages: DESIGN.md (S1-S26).
+ *
+ * Conventions
+ *  - All array arguments named *_dev are DEVICE pointers (fp64), owned by the caller, unless marked host.
+ *  - Intensity layout I[k][j][i][s]: interior cells only, s (direction) fastest, cell pitch = rt_ndir_padded()
+ *    doubles (N_d rounded up to a multiple of 4; pad entries are ignored on input and written as 0).
+ *  - Cell fields (rho, T, ...) are [k][j][i]; multi-component cell fields are component-major: u4[4][N_c],
+ *    R[16][N_c] (R^mu_nu at index 4*mu+nu), G[4][N_c] (G_nu).
+ *  - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls enqueue work and return; they do
+ *    not synchronise.
+ *  - Every call returns RT_OK (0) or a negative RT_E* code; nothing is printed, nothing aborts.  Numerical
+ *    failure of a cell's temperature solve is NOT an error: the cell keeps T_-, skips the update and is counted.
+ *  - Same inputs => bit-identical outputs (no atomics in reductions).
+ */
+#ifndef RT_H_
+#define RT_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RT_OK 0
+#define RT_EINVAL (-1)  /* bad argument */
+#define RT_ECUDA (-2)   /* a CUDA runtime call failed (rt_last_cuda_error() has the code) */
+#define RT_ENOMEM (-3)
+#define RT_ESTATE (-4)  /* call order: fluid / boundary not set */
+
+enum { RT_BC_PERIODIC = 0, RT_BC_OUTFLOW = 1, RT_BC_ZERO = 2, RT_BC_FIXED = 3 };
+enum { RT_MINKOWSKI_CART = 0, RT_MINK_CYL_TETRAD = 1, RT_KS_MKS = 2 };
+enum { RT_LIM_MC = 0, RT_LIM_MINMOD = 1, RT_LIM_VANLEER = 2, RT_LIM_NONE = 3 };
+enum { RT_ANG_DONOR = 0, RT_ANG_MAPR = 1 };
+/* rt_get_geometry selectors (host output, for table-level parity of the init precompute) */
+enum { RT_GEOM_G_C = 0,     /* g_{mu nu} at centres        [E3][N2][N1][4][4]            */
+       RT_GEOM_E_C = 1,     /* e^mu_a at centres           [E3][N2][N1][4 mu][4 a]       */
+       RT_GEOM_EINV_C = 2,  /* e^a_mu at centres           [E3][N2][N1][4 a][4 mu]       */
+       RT_GEOM_SQRTG_C = 3, /* sqrt(-g) at centres         [E3][N2][N1]                  */
+       RT_GEOM_OMEGA_C = 4, /* omega^a_{cd} at centres     [E3][N2][N1][4][4][4]         */
+       RT_GEOM_N0_C = 5,    /* n_0 per (cell, s)           [E3][N2][N1][N_d]             */
+       RT_GEOM_ANGCOEF = 6  /* Delta-lambda_e n_0e V_e / w_s per (cell, edge slot, s)  [E3][N2][N1][6][N_d] */ };
+/* E3 = 1 when the geometry is x3-symmetric, else N3. */
+
+typedef struct rt_ctx rt_ctx; /* opaque; owns all precomputed tables and one scratch copy of I on the device */
+
+/* Logical uniform mesh (L201): interior cells n[0..2] along x^1, x^2, x^3; cell i spans x0 + [i, i+1] dx. */
+typedef struct {
+    int n[3];
+    double x0[3], dx[3];
+    int bc_lo[3], bc_hi[3];     /* RT_BC_*; ghost depth is 2 (PLI) */
+    int zero_lo[3], zero_hi[3]; /* bands of interior cells next to a boundary whose I is reset to 0 after every
+                                   update ("zero the specific intensity in the four cells closest to the poles", L709) */
+} rt_grid;
+
+/* Metric + tetrad (L57-79, App. A).  x3_symmetric: geometry independent of x^3 (tables stored per (x1,x2) column,
+ * the paper's own optimisation, L776); required for RT_KS_MKS, ignored (constant geometry) for RT_MINKOWSKI_CART. */
+typedef struct {
+    int kind;         /* RT_MINKOWSKI_CART | RT_MINK_CYL_TETRAD | RT_KS_MKS */
+    double a, hslope; /* RT_KS_MKS: spin, theta-map parameter h: r = exp(x1), theta = pi x2 + (1-h)/2 sin(2 pi x2), phi = x3 */
+    int x3_symmetric;
+} rt_metric;
+
+typedef struct {
+    int limiter;       /* RT_LIM_* (S7: monotonised central by default) */
+    int angular_recon; /* RT_ANG_DONOR (RT_ANG_MAPR: not implemented in this round -> RT_EINVAL) */
+    int source_method; /* 0 = no source step; 1, 2, 3 = Methods 1-3 of section 3.6.2 */
+    double n0_floor;   /* mask directions with n_0 > -n0_floor (L284; 0.1) */
+    double rho_floor;  /* no interaction below this density (L468; 5e-4) */
+    double kappa_a0;   /* absorption: alpha^a = kappa_a0 rho^2 T^-3.5 (L403) */
+    double kappa_s;    /* scattering: alpha^s = kappa_s rho */
+    double a_rad;      /* radiation constant in code units */
+    double Y_over_rho; /* k_B / ((Gamma-1) mu m_p), so that Y = Y_over_rho * rho (L399) */
+    double abar;       /* a-bar of tau = abar alpha dt (L262; 1) */
+} rt_options;
+
+/* Build the angular grid with N_d = 10 angle_level^2 + 2 directions (L207-213; angle_level = 2^generation is the
+ * paper's rule, other levels by the extension S1), tetrads and Ricci rotation coefficients (Eq 8, 4th-order finite
+ * differences, h = 1e-3), and every per-column table; upload them.  Host-side, not timed.  *out is owned by the
+ * library until rt_free. */
+int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_level, const rt_options *opt, rt_ctx **out);
+int rt_free(rt_ctx *ctx);
+int rt_ndir(const rt_ctx *ctx);
+int rt_ndir_padded(const rt_ctx *ctx);
+
+/* Angular tables to HOST buffers: nhat[N_d][3], w[N_d] (solid angles, sum = 4 pi), nnb[N_d] (5 or 6),
+ * nb[N_d][6] (neighbour per edge slot, -1 padded).  Any pointer may be NULL. */
+int rt_get_directions(const rt_ctx *ctx, double *nhat_host, double *w_host, int *nnb_host, int *nb_host);
+/* Geometry tables to a HOST buffer (shapes above). */
+int rt_get_geometry(const rt_ctx *ctx, int which, double *host_out);
+/* Time-step bounds to HOST: out[0] = half the light-crossing time of the smallest cell (L464), out[1] = the
+ * angular-flux bound dt * (outflow rate of an angular cell) <= 1/2 (S14; +inf when omega = 0). */
+int rt_cfl_dt(const rt_ctx *ctx, double out_host[2]);
+
+/* RT_BC_FIXED ghost values for side (0 lo, 1 hi) of dim: device array [2 layers][face cells][pitch], layer 0
+ * next to the interior, face cell index = (other dims, lower dim fastest).  The pointer is kept, not copied. */
+int rt_set_boundary(rt_ctx *ctx, int dim, int side, const double *ghost_dev);
+/* Fluid state: rho[N_c], T[N_c], u4[4][N_c] coordinate-frame u^mu (NULL = tetrad rest frame e_0).  Copied into
+ * library-owned buffers on `stream`; T is the temperature used for the transport opacities of rt_transport. */
+int rt_set_fluid(rt_ctx *ctx, const double *rho_dev, const double *T_dev, const double *u4_dev, void *stream);
+
+/* I_out = (n^0 n_0 I_base - dt D_x[I_in]) / (n^0 n_0), then mask + zero bands (O3 + O5).  I_out may alias I_base
+ * but not I_in.  I_base may equal I_in. */
+int rt_transport(rt_ctx *ctx, const double *I_in_dev, const double *I_base_dev, double *I_out_dev, double dt, void *stream);
+/* I_inout -= dt D_Omega[I_in] / (n^0 n_0), then mask + zero bands (O4 + O5).  No-op when omega = 0. */
+int rt_angular_flux(rt_ctx *ctx, const double *I_in_dev, double *I_inout_dev, double dt, void *stream);
+/* Implicit source step O6 in place on (I, T); *n_fail_dev (device int, may be NULL) += cells whose solve failed. */
+int rt_source_implicit(rt_ctx *ctx, double *I_inout_dev, double *T_inout_dev, double dt, int *n_fail_dev, void *stream);
+/* R[16][N_c] = R^mu_nu (O7). */
+int rt_moments(rt_ctx *ctx, const double *I_dev, double *R_dev, void *stream);
+/* One predictor-corrector step O8 in place on (I, T).  R_out[16][N_c] = moments after the step (may be NULL),
+ * G_out[4][N_c] = G_nu = -(R^0_nu after - before the corrector's source step)/dt (may be NULL).
+ * n_fail_dev as above.  The fluid (rho, u4) is the one last given to rt_set_fluid; T comes from T_inout. */
+int rt_step(rt_ctx *ctx, double *I_inout_dev, double *T_inout_dev, double *R_out_dev, double *G_out_dev, double dt,
+            int *n_fail_dev, void *stream);
+
+/* number of kernels the library launched since rt_init (for bench.py's gpu_launches) */
+long long rt_launch_count(const rt_ctx *ctx);
+int rt_last_cuda_error(void);
+const char *rt_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RT_H_ */

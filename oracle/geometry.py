@@ -16,11 +16,11 @@ Metric kinds
                theta = pi x2 + (1-h)/2 sin(2 pi x2), phi = x3 (S26).  Tetrad = A3-A4 with reading S25:
                alpha is the LAPSE (1+2r/Sigma)^(-1/2) (A5b prints its inverse; A4a and Eq 4 need the lapse),
                gamma^{ij} is the INVERSE of the 3-metric gamma_ij = g_ij (A5d as printed gives a non-unit e_r).
-Finite differences (S15): 4th-order central, h = 1e-4 in logical coordinates.
+Finite differences (S15): 4th-order central, h = 1e-3 in logical coordinates.
 """
 import numpy as np
 
-FD_H = 1e-4
+FD_H = 1e-3
 ETA = np.diag([-1.0, 1.0, 1.0, 1.0])
 
 

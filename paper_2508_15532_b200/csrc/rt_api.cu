@@ -1,0 +1,398 @@
+// C ABI of librt_b200 (include/rt.h): context, init-time precompute (a0), and the rt_* entry points.
+#include <cmath>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <vector>
+
+#include "rt_kernels.cuh"
+
+using namespace rt;
+
+struct rt_ctx {
+    rt_grid grid;
+    rt_metric metric;
+    rt_options opt;
+    int level, nd, pitch, ncol;
+    long long ncell;
+    bool curved;   // omega != 0 somewhere: the angular-flux kernel has work to do
+    bool matter;   // any opacity: Eq 23 faces may exist
+    bool fluid_set;
+    AngularGrid ang;
+    // host copies of the geometry tables (rt_get_geometry, rt_cfl_dt)
+    std::vector<double> h_g, h_e, h_einv, h_sqrtg, h_omega, h_n0, h_angcoef;
+    DeviceTables tab;
+    double *d_rho, *d_u4, *d_T, *d_Th, *d_Ih, *d_fcoef[3];
+    KParams kp;
+    long long launches;
+};
+
+static int g_last_cuda = 0;
+#define CK(call)                                                       \
+    do {                                                               \
+        cudaError_t e_ = (call);                                       \
+        if (e_ != cudaSuccess) { g_last_cuda = (int)e_; return RT_ECUDA; } \
+    } while (0)
+
+template <typename T>
+static cudaError_t upload(T **dst, const std::vector<T> &src) {
+    cudaError_t e = cudaMalloc((void **)dst, src.size() * sizeof(T));
+    if (e != cudaSuccess) return e;
+    return cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice);
+}
+
+static void fill_face_entry(double *f, const PointGeom &g, int a) {
+    for (int q = 0; q < FACE_STRIDE; ++q) f[q] = 0.0;
+    if (g.dead || !(g.sqrtg > 0)) return;
+    for (int b = 0; b < 4; ++b) {
+        f[b] = g.sqrtg * g.e[1 + a][b];
+        double c = 0;
+        for (int mu = 0; mu < 4; ++mu) c += g.g[0][mu] * g.e[mu][b];
+        f[4 + b] = c;
+        f[8 + b] = g.sqrtg * g.e[0][b];
+    }
+}
+
+extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_level, const rt_options *opt, rt_ctx **out) {
+    if (!grid || !metric || !opt || !out) return RT_EINVAL;
+    for (int a = 0; a < 3; ++a) {
+        if (grid->n[a] < 1 || !(grid->dx[a] > 0)) return RT_EINVAL;
+        if (grid->bc_lo[a] < 0 || grid->bc_lo[a] > 3 || grid->bc_hi[a] < 0 || grid->bc_hi[a] > 3) return RT_EINVAL;
+        if ((grid->bc_lo[a] == RT_BC_PERIODIC) != (grid->bc_hi[a] == RT_BC_PERIODIC)) return RT_EINVAL;
+        if (grid->zero_lo[a] < 0 || grid->zero_hi[a] < 0) return RT_EINVAL;
+    }
+    if (metric->kind < 0 || metric->kind > RT_KS_MKS) return RT_EINVAL;
+    if (metric->kind == RT_KS_MKS && (!metric->x3_symmetric || std::fabs(metric->a) >= 1.0)) return RT_EINVAL;
+    if (opt->angular_recon != RT_ANG_DONOR) return RT_EINVAL;
+    if (opt->limiter < 0 || opt->limiter > 3 || opt->source_method < 0 || opt->source_method > 3) return RT_EINVAL;
+    if (opt->source_method != 0 && !(opt->Y_over_rho > 0)) return RT_EINVAL;
+
+    rt_ctx *c = new (std::nothrow) rt_ctx();
+    if (!c) return RT_ENOMEM;
+    c->grid = *grid; c->metric = *metric; c->opt = *opt; c->level = angle_level;
+    c->launches = 0; c->fluid_set = false;
+    if (!build_angular_grid(angle_level, c->ang)) { delete c; return RT_EINVAL; }
+    const int nd = c->nd = c->ang.nd;
+    const int pitch = c->pitch = (nd + 3) / 4 * 4;
+    const int n1 = grid->n[0], n2 = grid->n[1], n3 = grid->n[2];
+    const int ncol = c->ncol = n1 * n2;
+    c->ncell = (long long)ncol * n3;
+    c->matter = (opt->kappa_a0 != 0.0 || opt->kappa_s != 0.0);
+    const double x3c = grid->x0[2] + 0.5 * grid->dx[2];
+
+    // ---- geometry at centres and faces ----
+    std::vector<double> cen((size_t)ncol * CEN_STRIDE, 0.0), ecen((size_t)ncol * 16);
+    c->h_g.resize((size_t)ncol * 16); c->h_e.resize((size_t)ncol * 16); c->h_einv.resize((size_t)ncol * 16);
+    c->h_sqrtg.resize(ncol); c->h_omega.resize((size_t)ncol * 64); c->h_n0.resize((size_t)ncol * nd);
+    c->h_angcoef.assign((size_t)ncol * 6 * nd, 0.0);
+    std::vector<double> face[3];
+    face[0].resize((size_t)(n1 + 1) * n2 * FACE_STRIDE);
+    face[1].resize((size_t)n1 * (n2 + 1) * FACE_STRIDE);
+    face[2].resize((size_t)ncol * FACE_STRIDE);
+    std::vector<double> angc((size_t)ncol * ANG_SLOTS * pitch, 0.0);
+    double omax = 0.0;
+    for (int j = 0; j < n2; ++j)
+        for (int i = 0; i < n1; ++i) {
+            const size_t col = (size_t)j * n1 + i;
+            const double x[3] = {grid->x0[0] + (i + 0.5) * grid->dx[0], grid->x0[1] + (j + 0.5) * grid->dx[1], x3c};
+            PointGeom g;
+            eval_point(*metric, x, g);
+            if (g.dead) { delete c; return RT_EINVAL; }   // a cell centre on the polar axis
+            double om[4][4][4];
+            eval_omega(*metric, x, om);
+            std::memcpy(&c->h_g[col * 16], g.g, 128); std::memcpy(&c->h_e[col * 16], g.e, 128);
+            std::memcpy(&c->h_einv[col * 16], g.einv, 128); std::memcpy(&c->h_omega[col * 64], om, 512);
+            c->h_sqrtg[col] = g.sqrtg;
+            double *ce = &cen[col * CEN_STRIDE];
+            for (int b = 0; b < 4; ++b) {
+                double s0 = 0;
+                for (int mu = 0; mu < 4; ++mu) s0 += g.g[0][mu] * g.e[mu][b];
+                ce[b] = s0;
+                ce[4 + b] = g.e[0][b];
+                for (int nu = 0; nu < 4; ++nu) {
+                    double l = 0;
+                    for (int lam = 0; lam < 4; ++lam) l += g.e[lam][b] * g.g[lam][nu];
+                    ce[28 + 4 * b + nu] = l;
+                }
+            }
+            ce[8] = 1.0 / g.sqrtg;
+            std::memcpy(ce + 12, g.einv, 128);
+            std::memcpy(&ecen[col * 16], g.e, 128);
+            fill_face_entry(&face[2][col * FACE_STRIDE], g, 2);
+            // per-direction n_0 and per-edge angular coefficients
+            const AngularGrid &A = c->ang;
+            for (int s = 0; s < nd; ++s)
+                c->h_n0[col * nd + s] = ce[0] + ce[1] * A.nhat[3 * s] + ce[2] * A.nhat[3 * s + 1] + ce[3] * A.nhat[3 * s + 2];
+            for (int s = 0; s < nd; ++s) {
+                double self = 0.0;
+                for (int e = 0; e < A.nnb[s]; ++e) {
+                    const double *m3 = &A.emid[3 * (6 * s + e)], *u3 = &A.eun[3 * (6 * s + e)];
+                    const double m[4] = {1.0, m3[0], m3[1], m3[2]};
+                    double V = 0.0;
+                    for (int ii = 1; ii < 4; ++ii) {
+                        double q = 0.0;
+                        for (int cc = 0; cc < 4; ++cc) for (int d = 0; d < 4; ++d) q += om[ii][cc][d] * m[cc] * m[d];
+                        V -= u3[ii - 1] * q;                                     // a(m_e) . u_e  (Eq 7-8, S4)
+                    }
+                    omax = std::fmax(omax, std::fabs(V));
+                    const double n0e = ce[0] + ce[1] * m3[0] + ce[2] * m3[1] + ce[3] * m3[2];
+                    const int t = A.nb[6 * s + e];
+                    const double n0s = c->h_n0[col * nd + s], n0t = c->h_n0[col * nd + t];
+                    const bool gate = ((n0s > 0) - (n0s < 0)) != ((n0t > 0) - (n0t < 0));   // L280
+                    const double coef = gate ? 0.0 : A.dlam[6 * s + e] * n0e * V / A.w[s];  // Eq 19 / Eq 18
+                    c->h_angcoef[(col * 6 + e) * nd + s] = coef;
+                    if (V > 0) self += coef;                                    // upwind: own value (S5)
+                    else angc[(col * ANG_SLOTS + e) * pitch + s] = coef;        // upwind: neighbour's value
+                }
+                angc[(col * ANG_SLOTS + 6) * pitch + s] = self;
+            }
+        }
+    for (int j = 0; j < n2; ++j)
+        for (int i = 0; i <= n1; ++i) {
+            const double x[3] = {grid->x0[0] + i * grid->dx[0], grid->x0[1] + (j + 0.5) * grid->dx[1], x3c};
+            PointGeom g;
+            eval_point(*metric, x, g);
+            fill_face_entry(&face[0][((size_t)j * (n1 + 1) + i) * FACE_STRIDE], g, 0);
+        }
+    for (int j = 0; j <= n2; ++j)
+        for (int i = 0; i < n1; ++i) {
+            const double x[3] = {grid->x0[0] + (i + 0.5) * grid->dx[0], grid->x0[1] + j * grid->dx[1], x3c};
+            PointGeom g;
+            eval_point(*metric, x, g);
+            fill_face_entry(&face[1][((size_t)j * n1 + i) * FACE_STRIDE], g, 1);
+        }
+    c->curved = omax > 0.0;
+
+    // ---- angular tables, padded ----
+    std::vector<double> nh(3 * (size_t)pitch, 0.0), w(pitch, 0.0);
+    std::vector<int> nb(6 * (size_t)pitch, 0);
+    for (int s = 0; s < pitch; ++s)
+        for (int e = 0; e < 6; ++e) nb[e * pitch + s] = (s < nd && c->ang.nb[6 * s + e] >= 0) ? c->ang.nb[6 * s + e] : (s < nd ? s : 0);
+    for (int s = 0; s < nd; ++s) {
+        for (int q = 0; q < 3; ++q) nh[q * pitch + s] = c->ang.nhat[3 * s + q];
+        w[s] = c->ang.w[s];
+    }
+
+    // ---- upload ----
+    DeviceTables &t = c->tab;
+    std::memset(&t, 0, sizeof t);
+    cudaError_t e = cudaSuccess;
+    for (int a = 0; a < 3 && e == cudaSuccess; ++a) e = upload(&t.face[a], face[a]);
+    if (e == cudaSuccess) e = upload(&t.cen, cen);
+    if (e == cudaSuccess) e = upload(&t.ecen, ecen);
+    if (e == cudaSuccess) e = upload(&t.angcoef, angc);
+    if (e == cudaSuccess) e = upload(&t.nhat, nh);
+    if (e == cudaSuccess) e = upload(&t.w, w);
+    if (e == cudaSuccess) e = upload(&t.nb, nb);
+    const size_t nI = (size_t)c->ncell * pitch;
+    c->d_rho = c->d_u4 = c->d_T = c->d_Th = c->d_Ih = nullptr;
+    c->d_fcoef[0] = c->d_fcoef[1] = c->d_fcoef[2] = nullptr;
+    if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_rho, c->ncell * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_u4, 4 * c->ncell * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_T, c->ncell * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_Th, c->ncell * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_Ih, nI * sizeof(double));
+    for (int a = 0; a < 3 && e == cudaSuccess; ++a) {
+        size_t nf = (size_t)(n1 + (a == 0)) * (n2 + (a == 1)) * (n3 + (a == 2));
+        e = cudaMalloc((void **)&c->d_fcoef[a], nf * 4 * sizeof(double));
+    }
+    if (e != cudaSuccess) { g_last_cuda = (int)e; rt_free(c); return e == cudaErrorMemoryAllocation ? RT_ENOMEM : RT_ECUDA; }
+
+    KParams &k = c->kp;
+    std::memset(&k, 0, sizeof k);
+    k.n1 = n1; k.n2 = n2; k.n3 = n3; k.nd = nd; k.pitch = pitch; k.ncol = ncol; k.ncell = c->ncell;
+    for (int a = 0; a < 3; ++a) {
+        k.inv_dx[a] = 1.0 / grid->dx[a];
+        k.bc_lo[a] = grid->bc_lo[a]; k.bc_hi[a] = grid->bc_hi[a];
+        k.zlo[a] = grid->zero_lo[a]; k.zhi[a] = grid->zero_hi[a];
+        k.face[a] = t.face[a];
+    }
+    k.limiter = opt->limiter; k.method = opt->source_method;
+    k.n0_floor = opt->n0_floor; k.rho_floor = opt->rho_floor; k.kappa_a0 = opt->kappa_a0; k.kappa_s = opt->kappa_s;
+    k.a_rad = opt->a_rad; k.Y_over_rho = opt->Y_over_rho; k.abar = opt->abar;
+    k.cen = t.cen; k.ecen = t.ecen; k.angcoef = t.angcoef; k.nhat = t.nhat; k.w = t.w; k.nb = t.nb;
+    k.rho = c->d_rho; k.u4 = c->d_u4;
+    *out = c;
+    return RT_OK;
+}
+
+extern "C" int rt_free(rt_ctx *c) {
+    if (!c) return RT_EINVAL;
+    for (int a = 0; a < 3; ++a) { cudaFree(c->tab.face[a]); cudaFree(c->d_fcoef[a]); }
+    cudaFree(c->tab.cen); cudaFree(c->tab.ecen); cudaFree(c->tab.angcoef); cudaFree(c->tab.nhat); cudaFree(c->tab.w);
+    cudaFree(c->tab.nb); cudaFree(c->d_rho); cudaFree(c->d_u4); cudaFree(c->d_T); cudaFree(c->d_Th); cudaFree(c->d_Ih);
+    delete c;
+    return RT_OK;
+}
+
+extern "C" int rt_ndir(const rt_ctx *c) { return c ? c->nd : RT_EINVAL; }
+extern "C" int rt_ndir_padded(const rt_ctx *c) { return c ? c->pitch : RT_EINVAL; }
+extern "C" long long rt_launch_count(const rt_ctx *c) { return c ? c->launches : -1; }
+extern "C" int rt_last_cuda_error(void) { return g_last_cuda; }
+
+extern "C" const char *rt_strerror(int code) {
+    switch (code) {
+        case RT_OK: return "ok";
+        case RT_EINVAL: return "invalid argument";
+        case RT_ECUDA: return "CUDA runtime error (see rt_last_cuda_error)";
+        case RT_ENOMEM: return "out of memory";
+        case RT_ESTATE: return "call order: fluid or boundary data not set";
+        default: return "unknown error";
+    }
+}
+
+extern "C" int rt_get_directions(const rt_ctx *c, double *nhat, double *w, int *nnb, int *nb) {
+    if (!c) return RT_EINVAL;
+    if (nhat) std::memcpy(nhat, c->ang.nhat.data(), sizeof(double) * 3 * c->nd);
+    if (w) std::memcpy(w, c->ang.w.data(), sizeof(double) * c->nd);
+    if (nnb) std::memcpy(nnb, c->ang.nnb.data(), sizeof(int) * c->nd);
+    if (nb) std::memcpy(nb, c->ang.nb.data(), sizeof(int) * 6 * c->nd);
+    return RT_OK;
+}
+
+extern "C" int rt_get_geometry(const rt_ctx *c, int which, double *out) {
+    if (!c || !out) return RT_EINVAL;
+    const std::vector<double> *v = nullptr;
+    switch (which) {
+        case RT_GEOM_G_C: v = &c->h_g; break;
+        case RT_GEOM_E_C: v = &c->h_e; break;
+        case RT_GEOM_EINV_C: v = &c->h_einv; break;
+        case RT_GEOM_SQRTG_C: v = &c->h_sqrtg; break;
+        case RT_GEOM_OMEGA_C: v = &c->h_omega; break;
+        case RT_GEOM_N0_C: v = &c->h_n0; break;
+        case RT_GEOM_ANGCOEF: v = &c->h_angcoef; break;
+        default: return RT_EINVAL;
+    }
+    std::memcpy(out, v->data(), v->size() * sizeof(double));
+    return RT_OK;
+}
+
+extern "C" int rt_cfl_dt(const rt_ctx *c, double out[2]) {
+    if (!c || !out) return RT_EINVAL;
+    const double INF = std::numeric_limits<double>::infinity();
+    double dts = INF, dta = INF;
+    const rt_grid &G = c->grid;
+    const AngularGrid &A = c->ang;
+    const int nd = c->nd;
+    for (int j = 0; j < G.n[1]; ++j)
+        for (int i = 0; i < G.n[0]; ++i) {
+            if (i < G.zero_lo[0] || i >= G.n[0] - G.zero_hi[0] || j < G.zero_lo[1] || j >= G.n[1] - G.zero_hi[1]) continue;
+            const size_t col = (size_t)j * G.n[0] + i;
+            const double *e = &c->h_e[col * 16];
+            for (int s = 0; s < nd; ++s) {
+                const double n0 = c->h_n0[col * nd + s];
+                if (n0 > -c->opt.n0_floor) continue;
+                const double *nh = &A.nhat[3 * s];
+                double n[4];
+                for (int mu = 0; mu < 4; ++mu) n[mu] = e[4 * mu] + e[4 * mu + 1] * nh[0] + e[4 * mu + 2] * nh[1] + e[4 * mu + 3] * nh[2];
+                for (int a = 0; a < 3; ++a)
+                    if (n[1 + a] != 0.0) dts = std::fmin(dts, 0.5 * G.dx[a] * n[0] / std::fabs(n[1 + a]));   // L464
+                double rate = 0.0;   // sum over edges with V > 0 of V |n_0e| dlam / w  (coef = dlam n_0e V / w)
+                for (int q = 0; q < A.nnb[s]; ++q) {
+                    const double *m3 = &A.emid[3 * (6 * s + q)], *u3 = &A.eun[3 * (6 * s + q)];
+                    const double m[4] = {1.0, m3[0], m3[1], m3[2]};
+                    const double *om = &c->h_omega[col * 64];
+                    double V = 0.0;
+                    for (int ii = 1; ii < 4; ++ii) {
+                        double qq = 0.0;
+                        for (int cc = 0; cc < 4; ++cc) for (int d = 0; d < 4; ++d) qq += om[(ii * 4 + cc) * 4 + d] * m[cc] * m[d];
+                        V -= u3[ii - 1] * qq;
+                    }
+                    if (V > 0) {
+                        const double *g0 = &c->h_g[col * 16];
+                        double n0e = 0.0;
+                        for (int mu = 0; mu < 4; ++mu)
+                            n0e += g0[mu] * (e[4 * mu] + e[4 * mu + 1] * m3[0] + e[4 * mu + 2] * m3[1] + e[4 * mu + 3] * m3[2]);
+                        rate += V * std::fabs(n0e) * A.dlam[6 * s + q] / A.w[s];
+                    }
+                }
+                if (rate > 0) dta = std::fmin(dta, 0.5 * std::fabs(n[0] * n0) / rate);                        // S14
+            }
+        }
+    out[0] = dts; out[1] = dta;
+    return RT_OK;
+}
+
+extern "C" int rt_set_boundary(rt_ctx *c, int dim, int side, const double *ghost_dev) {
+    if (!c || dim < 0 || dim > 2 || side < 0 || side > 1) return RT_EINVAL;
+    c->kp.ghost[dim][side] = ghost_dev;
+    return RT_OK;
+}
+
+extern "C" int rt_set_fluid(rt_ctx *c, const double *rho, const double *T, const double *u4, void *stream) {
+    if (!c || !rho || !T) return RT_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t nb = c->ncell * sizeof(double);
+    CK(cudaMemcpyAsync(c->d_rho, rho, nb, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpyAsync(c->d_T, T, nb, cudaMemcpyDeviceToDevice, st));
+    if (u4) {
+        CK(cudaMemcpyAsync(c->d_u4, u4, 4 * nb, cudaMemcpyDeviceToDevice, st));
+    } else {   // tetrad rest frame u^mu = e^mu_0
+        std::vector<double> h(4 * (size_t)c->ncell);
+        for (long long cell = 0; cell < c->ncell; ++cell)
+            for (int mu = 0; mu < 4; ++mu) h[mu * c->ncell + cell] = c->h_e[(cell % c->ncol) * 16 + 4 * mu];
+        CK(cudaStreamSynchronize(st));
+        CK(cudaMemcpy(c->d_u4, h.data(), 4 * nb, cudaMemcpyHostToDevice));
+    }
+    c->fluid_set = true;
+    return RT_OK;
+}
+
+static bool fixed_bc_missing(const rt_ctx *c) {
+    for (int a = 0; a < 3; ++a) {
+        if (c->grid.bc_lo[a] == RT_BC_FIXED && !c->kp.ghost[a][0]) return true;
+        if (c->grid.bc_hi[a] == RT_BC_FIXED && !c->kp.ghost[a][1]) return true;
+    }
+    return false;
+}
+
+extern "C" int rt_transport(rt_ctx *c, const double *I_in, const double *I_base, double *I_out, double dt, void *stream) {
+    if (!c || !I_in || !I_base || !I_out || I_in == I_out) return RT_EINVAL;
+    if (fixed_bc_missing(c) || (c->matter && !c->fluid_set)) return RT_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (c->matter) CK(launch_facecoef(c->kp, c->d_T, dt, c->d_fcoef, st, &c->launches));
+    CK(launch_transport(c->kp, I_in, I_base, I_out, c->d_fcoef, c->matter, dt, st, &c->launches));
+    return RT_OK;
+}
+
+extern "C" int rt_angular_flux(rt_ctx *c, const double *I_in, double *I_io, double dt, void *stream) {
+    if (!c || !I_in || !I_io || I_in == I_io) return RT_EINVAL;
+    if (!c->curved) return RT_OK;
+    CK(launch_angular(c->kp, I_in, I_io, dt, (cudaStream_t)stream, &c->launches));
+    return RT_OK;
+}
+
+extern "C" int rt_source_implicit(rt_ctx *c, double *I, double *T, double dt, int *n_fail, void *stream) {
+    if (!c || !I || !T) return RT_EINVAL;
+    if (!c->fluid_set) return RT_ESTATE;
+    if (c->opt.source_method == 0) return RT_OK;
+    CK(launch_source(c->kp, I, T, dt, n_fail, nullptr, nullptr, (cudaStream_t)stream, &c->launches));
+    return RT_OK;
+}
+
+extern "C" int rt_moments(rt_ctx *c, const double *I, double *R, void *stream) {
+    if (!c || !I || !R) return RT_EINVAL;
+    CK(launch_moments(c->kp, I, R, (cudaStream_t)stream, &c->launches));
+    return RT_OK;
+}
+
+// one stage of the predictor-corrector (L448-456): I* = O5(I_base; fluxes of I_flux, opacities at T_flux; delta),
+// then O6 on (I*, T) with T_- = T_base
+static int stage(rt_ctx *c, const double *I_flux, const double *T_flux, const double *I_base, double *I_out, double *T_io,
+                 double delta, int *n_fail, double *R, double *G, cudaStream_t st) {
+    if (c->matter) CK(launch_facecoef(c->kp, T_flux, delta, c->d_fcoef, st, &c->launches));
+    CK(launch_transport(c->kp, I_flux, I_base, I_out, c->d_fcoef, c->matter, delta, st, &c->launches));
+    if (c->curved) CK(launch_angular(c->kp, I_flux, I_out, delta, st, &c->launches));
+    if (c->opt.source_method != 0 || R || G) CK(launch_source(c->kp, I_out, T_io, delta, n_fail, R, G, st, &c->launches));
+    return RT_OK;
+}
+
+extern "C" int rt_step(rt_ctx *c, double *I, double *T, double *R_out, double *G_out, double dt, int *n_fail, void *stream) {
+    if (!c || !I || !T) return RT_EINVAL;
+    if (!c->fluid_set || fixed_bc_missing(c)) return RT_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaMemcpyAsync(c->d_Th, T, c->ncell * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    int rc = stage(c, I, T, I, c->d_Ih, c->d_Th, 0.5 * dt, n_fail, nullptr, nullptr, st);     // predictor
+    if (rc != RT_OK) return rc;
+    return stage(c, c->d_Ih, c->d_Th, I, I, T, dt, n_fail, R_out, G_out, st);               // corrector
+}

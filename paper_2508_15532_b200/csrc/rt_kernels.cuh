@@ -1,0 +1,46 @@
+// Device-side parameter block and launcher declarations shared by the .cu files of librt_b200.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "rt_internal.h"
+
+namespace rt {
+
+constexpr int FACE_STRIDE = 12;  // doubles per face entry   (see DeviceTables::face)
+constexpr int CEN_STRIDE = 44;   // doubles per centre entry (see below)
+// centre entry: [0..3] g_{0mu}e^mu_b (-> n_0)  [4..7] e^0_b (-> n^0)  [8] 1/sqrt(-g_c)  [9..11] unused
+//               [12..27] e^a_mu ([a][mu], -> u^a-hat)   [28..43] L[b][nu] = e^lam_b g_{lam nu} (-> n_nu)
+constexpr int ANG_SLOTS = 7;     // 6 neighbour coefficients + 1 self coefficient per (column, s)
+
+struct KParams {
+    int n1, n2, n3, nd, pitch;
+    int ncol;
+    long long ncell;
+    double inv_dx[3];
+    int bc_lo[3], bc_hi[3];
+    int zlo[3], zhi[3];
+    int limiter, method;
+    double n0_floor, rho_floor, kappa_a0, kappa_s, a_rad, Y_over_rho, abar;
+    const double *face[3];
+    const double *cen;
+    const double *ecen;
+    const double *angcoef;
+    const double *nhat;
+    const double *w;
+    const int *nb;
+    const double *ghost[3][2];
+    const double *rho, *u4;  // library-owned fluid copies
+};
+
+// launchers (rt_transport.cu, rt_source.cu); every launch increments *launches
+cudaError_t launch_facecoef(const KParams &p, const double *T, double dt, double *fcoef[3], cudaStream_t st, long long *launches);
+cudaError_t launch_transport(const KParams &p, const double *I_in, const double *I_base, double *I_out,
+                             double *const fcoef[3], bool matter, double dt, cudaStream_t st, long long *launches);
+cudaError_t launch_angular(const KParams &p, const double *I_in, double *I_io, double dt, cudaStream_t st, long long *launches);
+// source step; if R_after != nullptr also writes moments after the update; if G != nullptr writes
+// G_nu = -(R^0_nu after - before)/dt.
+cudaError_t launch_source(const KParams &p, double *I, double *T, double dt, int *n_fail, double *R_after, double *G,
+                          cudaStream_t st, long long *launches);
+cudaError_t launch_moments(const KParams &p, const double *I, double *R, cudaStream_t st, long long *launches);
+
+}  // namespace rt

@@ -1,0 +1,256 @@
+// Cell-local kernels of librt_b200 (sm_100a): implicit radiation-fluid source step (O6) fused with the moment
+// reduction (O7) and the 4-force (Eq 36/48).
+//
+// PAPER.md: fluid-frame boost Eq 5 (L85) with I/nu^4 and nu^2 dOmega invariance (S17); angular sums Eq 33, 41
+// (L344, L388-390); temperature equations Eq 42 / 43 / 46 (L396-426; S19: A' = alpha_- dt A); intensity update
+// Eq 35 (L352) with the coefficients the T-equation was built from (S19b); density floor L468; moments Eq 13
+// (L141); G_nu = -(R^0_nu after - before)/dt (Eq 36, 48).
+//
+// Design: one warp per cell; the cell's N_d intensities live in registers (MAXV per lane, s = lane + 32 v, so
+// every load/store is a 256-byte coalesced row); all angular sums are butterfly warp reductions (fixed order =>
+// bit-reproducible); the scalar temperature solve runs redundantly on all lanes (no divergence, no broadcast).
+// Moments are accumulated in the TETRAD frame, M^{ab} = sum_s w_s I_s n^a n^b (10 sums with constant n-hat), and
+// rotated once per cell: R^mu_nu = e^mu_a M^{ab} (e^lam_b g_{lam nu}).
+#include <cmath>
+
+#include "rt_kernels.cuh"
+
+namespace rt {
+namespace {
+
+constexpr double FOURPI = 12.566370614359172953850573533118;
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+struct TEq {
+    int method;
+    double a4, b1, c0;             // methods 1, 2: a4 g(T) + b1 T + c0
+    double k45, k4, k35, k1, k0;   // method 3: coefficients of Eq 46
+};
+__device__ __forceinline__ void teq_eval(const TEq &q, double T, double &f, double &df) {
+    if (q.method == 1) {
+        const double T3 = T * T * T;
+        f = q.a4 * T3 * T + q.b1 * T + q.c0;
+        df = 4.0 * q.a4 * T3 + q.b1;
+    } else if (q.method == 2) {
+        const double r = sqrt(T);
+        f = q.a4 * r + q.b1 * T + q.c0;
+        df = 0.5 * q.a4 / r + q.b1;
+    } else {
+        const double r = sqrt(T), T3 = T * T * T, T35 = T3 * r, T4 = T3 * T, T45 = T4 * r;
+        f = -(q.k45 * T45 + q.k4 * T4 + q.k35 * T35 + q.k1 * T + q.k0);
+        df = -(4.5 * q.k45 * T35 + 4.0 * q.k4 * T3 + 3.5 * q.k35 * T3 / r + q.k1);
+    }
+}
+// Newton-Raphson (L399) from T_-, kept inside the bracket (0, W/Y] on which the residual changes sign (S20).
+__device__ __forceinline__ bool solve_T(const TEq &q, double Tm, double Thi, double &Tp) {
+    double lo = 0.0, hi = Thi, f, df;
+    if (!(Thi > 0.0)) return false;
+    teq_eval(q, hi, f, df);
+    if (!(f >= 0.0)) return false;
+    if (q.method != 3 && !(q.c0 < 0.0)) return false;
+    double T = (Tm > lo && Tm < hi) ? Tm : 0.5 * (lo + hi);
+    for (int it = 0; it < 100; ++it) {
+        teq_eval(q, T, f, df);
+        if (f < 0) lo = T; else hi = T;
+        double Tn = T - f / df;
+        if (!(Tn > lo && Tn < hi)) Tn = 0.5 * (lo + hi);
+        const double d = Tn - T;
+        T = Tn;
+        if (fabs(d) <= 1e-14 * T) break;
+    }
+    Tp = T;
+    return true;
+}
+
+// 10 independent components of M^{ab}: 00 01 02 03 11 12 13 22 23 33
+__device__ __forceinline__ void mom_accumulate(double M[10], double wI, double nx, double ny, double nz) {
+    M[0] += wI;
+    M[1] += wI * nx; M[2] += wI * ny; M[3] += wI * nz;
+    M[4] += wI * nx * nx; M[5] += wI * nx * ny; M[6] += wI * nx * nz;
+    M[7] += wI * ny * ny; M[8] += wI * ny * nz; M[9] += wI * nz * nz;
+}
+__device__ __forceinline__ double mom_get(const double M[10], int a, int b) {
+    if (a > b) { int t = a; a = b; b = t; }
+    const int base[4] = {0, 4, 7, 9};
+    return M[base[a] + (b - a)];
+}
+// R^mu_nu for (mu, nu) from tetrad-frame M, e^mu_a (ecen) and L[b][nu] (cen + 28)
+__device__ __forceinline__ double rotate(const double M[10], const double *__restrict__ ecen, const double *__restrict__ L, int mu, int nu) {
+    double r = 0.0;
+    for (int a = 0; a < 4; ++a) {
+        double t = 0.0;
+        for (int b = 0; b < 4; ++b) t += mom_get(M, a, b) * L[4 * b + nu];
+        r += ecen[4 * mu + a] * t;
+    }
+    return r;
+}
+
+template <int MAXV, bool SRC, bool MOM>
+__global__ void __launch_bounds__(256)
+k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, double *G_out) {
+    extern __shared__ double tab[];   // nx[pitch] ny[pitch] nz[pitch] w[pitch]
+    for (int t = threadIdx.x; t < 3 * p.pitch; t += blockDim.x) tab[t] = p.nhat[t];
+    for (int t = threadIdx.x; t < p.pitch; t += blockDim.x) tab[3 * p.pitch + t] = p.w[t];
+    __syncthreads();
+    const double *snx = tab, *sny = tab + p.pitch, *snz = tab + 2 * p.pitch, *sw = tab + 3 * p.pitch;
+    const int lane = threadIdx.x & 31;
+    const long long warp0 = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5;
+    const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
+
+    for (long long cell = warp0; cell < p.ncell; cell += nwarps) {
+        const int col = int(cell % p.ncol);
+        const double *cen = p.cen + (long long)col * CEN_STRIDE;
+        double alpha = 0.0, aa = 0.0, as = 0.0, rho = 0.0, Tm = 0.0;
+        if (SRC) {
+            rho = p.rho[cell];
+            Tm = T[cell];
+            if (rho >= p.rho_floor) {
+                aa = (p.kappa_a0 != 0.0) ? p.kappa_a0 * rho * rho * pow(Tm, -3.5) : 0.0;
+                as = p.kappa_s * rho;
+            }
+            alpha = aa + as;
+        }
+        const bool interact = SRC && p.method != 0 && alpha != 0.0;
+        if (!interact && !MOM) continue;
+        double uh0 = 1.0, uh1 = 0.0, uh2 = 0.0, uh3 = 0.0;
+        if (interact) {
+            const double u0 = p.u4[cell], u1 = p.u4[p.ncell + cell], u2 = p.u4[2 * p.ncell + cell], u3 = p.u4[3 * p.ncell + cell];
+            uh0 = cen[12] * u0 + cen[13] * u1 + cen[14] * u2 + cen[15] * u3;
+            uh1 = cen[16] * u0 + cen[17] * u1 + cen[18] * u2 + cen[19] * u3;
+            uh2 = cen[20] * u0 + cen[21] * u1 + cen[22] * u2 + cen[23] * u3;
+            uh3 = cen[24] * u0 + cen[25] * u1 + cen[26] * u2 + cen[27] * u3;
+        }
+        double *Ic = I + cell * p.pitch;
+        double val[MAXV];
+        double E = 0.0, A1 = 0.0, A2 = 0.0;
+        double Mb[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+#pragma unroll
+        for (int v = 0; v < MAXV; ++v) {
+            const int s = lane + 32 * v;
+            val[v] = 0.0;
+            if (s < p.nd) {
+                const double x = Ic[s];
+                val[v] = x;
+                const double nx = snx[s], ny = sny[s], nz = snz[s], ws = sw[s];
+                if (MOM && G_out) mom_accumulate(Mb, ws * x, nx, ny, nz);
+                if (interact) {
+                    const double n0c = cen[0] + cen[1] * nx + cen[2] * ny + cen[3] * nz;
+                    if (!(n0c > -p.n0_floor)) {
+                        const double nup = cen[4] + cen[5] * nx + cen[6] * ny + cen[7] * nz;
+                        const double nbar = uh0 - (uh1 * nx + uh2 * ny + uh3 * nz);       // Eq 5, first row
+                        const double d = nup + nbar * alpha * dt;
+                        const double IbdOm = nbar * nbar * x * ws;                          // Ibar dOmegabar (S17)
+                        E += IbdOm;                                                         // Eq 33
+                        A1 += nup / d * IbdOm;                                              // Eq 41a
+                        A2 += ws / (nbar * d);                                              // Eq 41b
+                    }
+                }
+            }
+        }
+        bool updated = false;
+        if (interact) {
+            E = warp_sum(E); A1 = warp_sum(A1); A2 = warp_sum(A2) * (dt / FOURPI);
+            const double Y = p.Y_over_rho * rho, W = E + Y * Tm, Nbar = p.kappa_a0 * rho * rho;
+            TEq q;
+            q.method = p.method;
+            q.a4 = (p.method == 1) ? A2 * aa * p.a_rad : A2 * Nbar * p.a_rad;
+            q.b1 = Y * (1.0 - A2 * as);
+            q.c0 = A1 - Y * (1.0 - A2 * as) * Tm - (1.0 - A2 * as) * E;
+            if (p.method == 3) {
+                const double A1p = alpha * dt * A1, A2p = alpha * dt * A2;
+                q.k45 = Y * as * (A2p - dt);
+                q.k4 = -A2p * Nbar * p.a_rad;
+                q.k35 = -(A2p * as * W + A1p - W * as * dt);
+                q.k1 = -Y * Nbar * dt;
+                q.k0 = W * Nbar * dt;
+            }
+            double Tp;
+            if (solve_T(q, Tm, W / Y, Tp)) {
+                const double Ep = W - Y * Tp;                                               // Eq 39
+                const double emis = (p.method == 1) ? aa * p.a_rad * Tp * Tp * Tp * Tp : Nbar * p.a_rad * sqrt(Tp);
+                const double scale = (p.method == 3) ? alpha / (as + Nbar * pow(Tp, -3.5)) : 1.0;
+                const double S = emis + as * Ep;
+#pragma unroll
+                for (int v = 0; v < MAXV; ++v) {
+                    const int s = lane + 32 * v;
+                    if (s < p.nd) {
+                        const double nx = snx[s], ny = sny[s], nz = snz[s];
+                        const double n0c = cen[0] + cen[1] * nx + cen[2] * ny + cen[3] * nz;
+                        if (!(n0c > -p.n0_floor)) {
+                            const double nup = cen[4] + cen[5] * nx + cen[6] * ny + cen[7] * nz;
+                            const double nbar = uh0 - (uh1 * nx + uh2 * ny + uh3 * nz);
+                            const double d = nup + nbar * alpha * dt;
+                            const double n2 = nbar * nbar, n4 = n2 * n2;
+                            const double Ip = scale * (nup / d * (n4 * val[v]) + nbar * dt / (FOURPI * d) * S);   // Eq 35
+                            val[v] = Ip / n4;                                                                   // L432
+                            Ic[s] = val[v];
+                        }
+                    }
+                }
+                if (lane == 0) T[cell] = Tp;
+                updated = true;
+            } else if (lane == 0 && n_fail) {
+                atomicAdd(n_fail, 1);
+            }
+        }
+        if (MOM) {
+            double Ma[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+#pragma unroll
+            for (int v = 0; v < MAXV; ++v) {
+                const int s = lane + 32 * v;
+                if (s < p.nd) mom_accumulate(Ma, sw[s] * val[v], snx[s], sny[s], snz[s]);
+            }
+#pragma unroll
+            for (int c = 0; c < 10; ++c) Ma[c] = warp_sum(Ma[c]);
+            if (G_out) {
+#pragma unroll
+                for (int c = 0; c < 10; ++c) Mb[c] = warp_sum(Mb[c]);
+            }
+            const double *ecen = p.ecen + (long long)col * 16, *L = cen + 28;
+            if (lane < 16) {
+                const int mu = lane >> 2, nu = lane & 3;
+                const double Ra = rotate(Ma, ecen, L, mu, nu);
+                if (R_out) R_out[lane * p.ncell + cell] = Ra;
+                if (G_out && mu == 0) {
+                    const double Rb = updated ? rotate(Mb, ecen, L, 0, nu) : Ra;
+                    G_out[nu * p.ncell + cell] = -(Ra - Rb) / dt;
+                }
+            }
+        }
+    }
+}
+
+template <bool SRC, bool MOM>
+cudaError_t launch_cell(const KParams &p, double *I, double *T, double dt, int *n_fail, double *R, double *G, cudaStream_t st) {
+    const int threads = 256;
+    long long want = (p.ncell + 7) / 8;
+    const int blocks = (int)(want < 148LL * 8 * 4 ? want : 148LL * 8 * 4);
+    const size_t smem = 4 * p.pitch * sizeof(double);
+    if (p.nd <= 64) k_cell<2, SRC, MOM><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail, R, G);
+    else if (p.nd <= 192) k_cell<6, SRC, MOM><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail, R, G);
+    else if (p.nd <= 384) k_cell<12, SRC, MOM><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail, R, G);
+    else if (p.nd <= 672) k_cell<21, SRC, MOM><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail, R, G);
+    else return cudaErrorInvalidValue;
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t launch_source(const KParams &p, double *I, double *T, double dt, int *n_fail, double *R_after, double *G,
+                          cudaStream_t st, long long *launches) {
+    ++*launches;
+    if (R_after || G) return launch_cell<true, true>(p, I, T, dt, n_fail, R_after, G, st);
+    return launch_cell<true, false>(p, I, T, dt, n_fail, nullptr, nullptr, st);
+}
+
+cudaError_t launch_moments(const KParams &p, const double *I, double *R, cudaStream_t st, long long *launches) {
+    ++*launches;
+    return launch_cell<false, true>(p, const_cast<double *>(I), nullptr, 0.0, nullptr, R, nullptr, st);
+}
+
+}  // namespace rt

@@ -1,0 +1,200 @@
+"""Thin Python binding of librt_b200.so (include/rt.h): argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels.  torch is used for device memory and streams only.
+There is no CPU fallback: if the shared library is missing, importing this module raises.
+"""
+import ctypes
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "librt_b200.so")
+
+BC = {"periodic": 0, "outflow": 1, "zero": 2, "fixed": 3}
+METRIC = {"minkowski": 0, "mink_cyl": 1, "ks_mks": 2}
+GEOM = dict(g_c=0, e_c=1, einv_c=2, sqrtg_c=3, omega_c=4, n0_c=5, angcoef=6)
+SYMBOLS = ["rt_init", "rt_free", "rt_ndir", "rt_ndir_padded", "rt_get_directions", "rt_get_geometry", "rt_cfl_dt",
+           "rt_set_boundary", "rt_set_fluid", "rt_transport", "rt_angular_flux", "rt_source_implicit", "rt_moments",
+           "rt_step", "rt_launch_count", "rt_last_cuda_error", "rt_strerror"]
+
+
+class RtGrid(ctypes.Structure):
+    _fields_ = [("n", ctypes.c_int * 3), ("x0", ctypes.c_double * 3), ("dx", ctypes.c_double * 3),
+                ("bc_lo", ctypes.c_int * 3), ("bc_hi", ctypes.c_int * 3),
+                ("zero_lo", ctypes.c_int * 3), ("zero_hi", ctypes.c_int * 3)]
+
+
+class RtMetric(ctypes.Structure):
+    _fields_ = [("kind", ctypes.c_int), ("a", ctypes.c_double), ("hslope", ctypes.c_double), ("x3_symmetric", ctypes.c_int)]
+
+
+class RtOptions(ctypes.Structure):
+    _fields_ = [("limiter", ctypes.c_int), ("angular_recon", ctypes.c_int), ("source_method", ctypes.c_int),
+                ("n0_floor", ctypes.c_double), ("rho_floor", ctypes.c_double), ("kappa_a0", ctypes.c_double),
+                ("kappa_s", ctypes.c_double), ("a_rad", ctypes.c_double), ("Y_over_rho", ctypes.c_double),
+                ("abar", ctypes.c_double)]
+
+
+def load_library(path=LIB_PATH):
+    """dlopen the C-ABI library and declare its signatures.  Raises if it is missing (no fallback)."""
+    if not os.path.exists(path):
+        raise ImportError("librt_b200.so not built: run `python -m paper_2508_15532_b200.build` (needs nvcc); "
+                          "there is no CPU fallback")
+    lib = ctypes.CDLL(path)
+    vp, dbl, ci = ctypes.c_void_p, ctypes.c_double, ctypes.c_int
+    lib.rt_init.argtypes = [ctypes.POINTER(RtGrid), ctypes.POINTER(RtMetric), ci, ctypes.POINTER(RtOptions), ctypes.POINTER(vp)]
+    lib.rt_free.argtypes = [vp]
+    lib.rt_ndir.argtypes = [vp]
+    lib.rt_ndir_padded.argtypes = [vp]
+    lib.rt_get_directions.argtypes = [vp, vp, vp, vp, vp]
+    lib.rt_get_geometry.argtypes = [vp, ci, vp]
+    lib.rt_cfl_dt.argtypes = [vp, vp]
+    lib.rt_set_boundary.argtypes = [vp, ci, ci, vp]
+    lib.rt_set_fluid.argtypes = [vp, vp, vp, vp, vp]
+    lib.rt_transport.argtypes = [vp, vp, vp, vp, dbl, vp]
+    lib.rt_angular_flux.argtypes = [vp, vp, vp, dbl, vp]
+    lib.rt_source_implicit.argtypes = [vp, vp, vp, dbl, vp, vp]
+    lib.rt_moments.argtypes = [vp, vp, vp, vp]
+    lib.rt_step.argtypes = [vp, vp, vp, vp, vp, dbl, vp, vp]
+    lib.rt_launch_count.argtypes = [vp]
+    lib.rt_launch_count.restype = ctypes.c_longlong
+    lib.rt_strerror.argtypes = [ci]
+    lib.rt_strerror.restype = ctypes.c_char_p
+    return lib
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = load_library()
+    return _lib
+
+
+class RtError(RuntimeError):
+    pass
+
+
+def _check(rc):
+    if rc != 0:
+        raise RtError("%s (code %d, cuda %d)" % (lib().rt_strerror(rc).decode(), rc, lib().rt_last_cuda_error()))
+
+
+def _ptr(t):
+    if t is None:
+        return None
+    assert t.is_cuda and t.dtype in (torch.float64, torch.int32), "device fp64 tensor expected"
+    assert t.is_contiguous()
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _stream():
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+DEFAULT_OPTIONS = dict(limiter=0, angular_recon=0, source_method=2, n0_floor=0.1, rho_floor=5e-4, kappa_a0=0.0,
+                       kappa_s=0.0, a_rad=1.0, Y_over_rho=1.5, abar=1.0)
+
+
+class RtContext:
+    """rt_init .. rt_free.  Intensity tensors are [N3, N2, N1, pitch] fp64 on the device (pad entries zero)."""
+
+    def __init__(self, grid, metric_kind, metric_params, level, options=None, device="cuda:0"):
+        if not torch.cuda.is_available():
+            raise RtError("no CUDA device: librt_b200 has no CPU path")
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        g = RtGrid()
+        g.n[:] = grid["n"]; g.x0[:] = grid["x0"]; g.dx[:] = grid["dx"]
+        g.bc_lo[:] = [BC[b] for b in grid["bc_lo"]]; g.bc_hi[:] = [BC[b] for b in grid["bc_hi"]]
+        g.zero_lo[:] = grid.get("zero_lo", (0, 0, 0)); g.zero_hi[:] = grid.get("zero_hi", (0, 0, 0))
+        mp = dict(metric_params or {})
+        m = RtMetric(METRIC[metric_kind], mp.get("a", 0.0), mp.get("hslope", 0.3), 1)
+        od = dict(DEFAULT_OPTIONS)
+        for k, v in (options or {}).items():
+            od[{"method": "source_method", "ang_recon": "angular_recon"}.get(k, k)] = v
+        o = RtOptions(**od)
+        self._h = ctypes.c_void_p()
+        _check(lib().rt_init(ctypes.byref(g), ctypes.byref(m), int(level), ctypes.byref(o), ctypes.byref(self._h)))
+        self.n = tuple(int(x) for x in grid["n"])
+        self.shape = self.n[::-1]
+        self.nd = lib().rt_ndir(self._h)
+        self.pitch = lib().rt_ndir_padded(self._h)
+        self.ncell = self.n[0] * self.n[1] * self.n[2]
+        self._keep = {}
+        self._nfail = torch.zeros(1, dtype=torch.int32, device=self.device)
+
+    def close(self):
+        if self._h:
+            lib().rt_free(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- tables -------------------------------------------------------------------------------------------
+    def directions(self):
+        nhat, w = np.empty((self.nd, 3)), np.empty(self.nd)
+        nnb, nb = np.empty(self.nd, np.int32), np.empty((self.nd, 6), np.int32)
+        _check(lib().rt_get_directions(self._h, nhat.ctypes.data, w.ctypes.data, nnb.ctypes.data, nb.ctypes.data))
+        return dict(nhat=nhat, w=w, nnb=nnb, nb=nb)
+
+    def geometry(self, which):
+        ncol = self.n[0] * self.n[1]
+        shp = {"g_c": (4, 4), "e_c": (4, 4), "einv_c": (4, 4), "sqrtg_c": (), "omega_c": (4, 4, 4), "n0_c": (self.nd,),
+               "angcoef": (6, self.nd)}[which]
+        out = np.empty((1, self.n[1], self.n[0]) + shp)
+        assert out.size == ncol * int(np.prod(shp, dtype=np.int64))
+        _check(lib().rt_get_geometry(self._h, GEOM[which], out.ctypes.data))
+        return out
+
+    def cfl_dt(self):
+        out = np.zeros(2)
+        _check(lib().rt_cfl_dt(self._h, out.ctypes.data))
+        return float(out[0]), float(out[1])
+
+    # ---- helpers for the padded layout ----------------------------------------------------------------------
+    def to_device(self, I_host):
+        """numpy [N3,N2,N1,nd] -> device tensor [N3,N2,N1,pitch] (pad = 0)."""
+        I = torch.zeros(self.shape + (self.pitch,), dtype=torch.float64, device=self.device)
+        I[..., :self.nd] = torch.as_tensor(np.ascontiguousarray(I_host).reshape(self.shape + (self.nd,)), device=self.device)
+        return I
+
+    def to_host(self, I_dev):
+        return I_dev[..., :self.nd].cpu().numpy()
+
+    # ---- the rt_* calls -------------------------------------------------------------------------------------
+    def set_boundary(self, dim, side, ghost_dev):
+        self._keep[("ghost", dim, side)] = ghost_dev
+        _check(lib().rt_set_boundary(self._h, dim, side, _ptr(ghost_dev)))
+
+    def set_fluid(self, rho, T, u4=None):
+        _check(lib().rt_set_fluid(self._h, _ptr(rho), _ptr(T), _ptr(u4), _stream()))
+
+    def transport(self, I_in, I_base, I_out, dt):
+        _check(lib().rt_transport(self._h, _ptr(I_in), _ptr(I_base), _ptr(I_out), float(dt), _stream()))
+
+    def angular_flux(self, I_in, I_inout, dt):
+        _check(lib().rt_angular_flux(self._h, _ptr(I_in), _ptr(I_inout), float(dt), _stream()))
+
+    def source_implicit(self, I, T, dt):
+        _check(lib().rt_source_implicit(self._h, _ptr(I), _ptr(T), float(dt), _ptr(self._nfail), _stream()))
+
+    def moments(self, I, R):
+        _check(lib().rt_moments(self._h, _ptr(I), _ptr(R), _stream()))
+
+    def step(self, I, T, dt, R=None, G=None):
+        _check(lib().rt_step(self._h, _ptr(I), _ptr(T), _ptr(R), _ptr(G), float(dt), _ptr(self._nfail), _stream()))
+
+    def n_fail(self):
+        return int(self._nfail.item())
+
+    def launch_count(self):
+        return int(lib().rt_launch_count(self._h))
