@@ -119,6 +119,13 @@ int rt_moments(rt_ctx *ctx, const double *I_dev, double *R_dev, void *stream);
 int rt_step(rt_ctx *ctx, double *I_inout_dev, double *T_inout_dev, double *R_out_dev, double *G_out_dev, double dt,
             int *n_fail_dev, void *stream);
 
+/* Per-kernel device timing (bench.py's roofline): while enabled, every kernel launch is bracketed by CUDA events
+ * on its stream.  rt_profile_read synchronises on the last event, returns the accumulated milliseconds and launch
+ * counts per kernel class (HOST arrays of RT_K_COUNT entries) and resets the accumulators. */
+enum { RT_K_FACECOEF = 0, RT_K_TRANSPORT = 1, RT_K_ANGULAR = 2, RT_K_SOURCE = 3, RT_K_MOMENTS = 4, RT_K_COUNT = 5 };
+int rt_profile_enable(rt_ctx *ctx, int on);
+int rt_profile_read(rt_ctx *ctx, double *ms_host, long long *count_host);
+
 /* number of kernels the library launched since rt_init (for bench.py's gpu_launches) */
 long long rt_launch_count(const rt_ctx *ctx);
 int rt_last_cuda_error(void);

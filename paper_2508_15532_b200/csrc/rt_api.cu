@@ -25,6 +25,20 @@ struct rt_ctx {
     double *d_rho, *d_u4, *d_T, *d_Th, *d_Ih, *d_fcoef[3];
     KParams kp;
     long long launches;
+    bool profiling;
+    struct Span { int cls; cudaEvent_t a, b; };
+    std::vector<Span> spans;
+};
+
+// brackets one launcher call with events when profiling is on
+struct ProfScope {
+    rt_ctx *c; int cls; cudaStream_t st; cudaEvent_t a, b; bool on;
+    ProfScope(rt_ctx *c_, int cls_, cudaStream_t st_) : c(c_), cls(cls_), st(st_), on(c_->profiling) {
+        if (on) { cudaEventCreate(&a); cudaEventCreate(&b); cudaEventRecord(a, st); }
+    }
+    ~ProfScope() {
+        if (on) { cudaEventRecord(b, st); c->spans.push_back({cls, a, b}); }
+    }
 };
 
 static int g_last_cuda = 0;
@@ -70,7 +84,7 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     rt_ctx *c = new (std::nothrow) rt_ctx();
     if (!c) return RT_ENOMEM;
     c->grid = *grid; c->metric = *metric; c->opt = *opt; c->level = angle_level;
-    c->launches = 0; c->fluid_set = false;
+    c->launches = 0; c->fluid_set = false; c->profiling = false;
     if (!build_angular_grid(angle_level, c->ang)) { delete c; return RT_EINVAL; }
     const int nd = c->nd = c->ang.nd;
     const int pitch = c->pitch = (nd + 3) / 4 * 4;
@@ -230,6 +244,27 @@ extern "C" int rt_ndir_padded(const rt_ctx *c) { return c ? c->pitch : RT_EINVAL
 extern "C" long long rt_launch_count(const rt_ctx *c) { return c ? c->launches : -1; }
 extern "C" int rt_last_cuda_error(void) { return g_last_cuda; }
 
+extern "C" int rt_profile_enable(rt_ctx *c, int on) {
+    if (!c) return RT_EINVAL;
+    c->profiling = on != 0;
+    return RT_OK;
+}
+
+extern "C" int rt_profile_read(rt_ctx *c, double *ms, long long *count) {
+    if (!c || !ms || !count) return RT_EINVAL;
+    for (int q = 0; q < RT_K_COUNT; ++q) { ms[q] = 0.0; count[q] = 0; }
+    if (!c->spans.empty()) CK(cudaEventSynchronize(c->spans.back().b));
+    for (auto &sp : c->spans) {
+        float t = 0.f;
+        CK(cudaEventElapsedTime(&t, sp.a, sp.b));
+        ms[sp.cls] += t;
+        count[sp.cls] += 1;
+        cudaEventDestroy(sp.a); cudaEventDestroy(sp.b);
+    }
+    c->spans.clear();
+    return RT_OK;
+}
+
 extern "C" const char *rt_strerror(int code) {
     switch (code) {
         case RT_OK: return "ok";
@@ -350,15 +385,15 @@ extern "C" int rt_transport(rt_ctx *c, const double *I_in, const double *I_base,
     if (!c || !I_in || !I_base || !I_out || I_in == I_out) return RT_EINVAL;
     if (fixed_bc_missing(c) || (c->matter && !c->fluid_set)) return RT_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
-    if (c->matter) CK(launch_facecoef(c->kp, c->d_T, dt, c->d_fcoef, st, &c->launches));
-    CK(launch_transport(c->kp, I_in, I_base, I_out, c->d_fcoef, c->matter, dt, st, &c->launches));
+    if (c->matter) { ProfScope ps(c, RT_K_FACECOEF, st); CK(launch_facecoef(c->kp, c->d_T, dt, c->d_fcoef, st, &c->launches)); }
+    { ProfScope ps(c, RT_K_TRANSPORT, st); CK(launch_transport(c->kp, I_in, I_base, I_out, c->d_fcoef, c->matter, dt, st, &c->launches)); }
     return RT_OK;
 }
 
 extern "C" int rt_angular_flux(rt_ctx *c, const double *I_in, double *I_io, double dt, void *stream) {
     if (!c || !I_in || !I_io || I_in == I_io) return RT_EINVAL;
     if (!c->curved) return RT_OK;
-    CK(launch_angular(c->kp, I_in, I_io, dt, (cudaStream_t)stream, &c->launches));
+    { ProfScope ps(c, RT_K_ANGULAR, (cudaStream_t)stream); CK(launch_angular(c->kp, I_in, I_io, dt, (cudaStream_t)stream, &c->launches)); }
     return RT_OK;
 }
 
@@ -366,13 +401,13 @@ extern "C" int rt_source_implicit(rt_ctx *c, double *I, double *T, double dt, in
     if (!c || !I || !T) return RT_EINVAL;
     if (!c->fluid_set) return RT_ESTATE;
     if (c->opt.source_method == 0) return RT_OK;
-    CK(launch_source(c->kp, I, T, dt, n_fail, nullptr, nullptr, (cudaStream_t)stream, &c->launches));
+    { ProfScope ps(c, RT_K_SOURCE, (cudaStream_t)stream); CK(launch_source(c->kp, I, T, dt, n_fail, nullptr, nullptr, (cudaStream_t)stream, &c->launches)); }
     return RT_OK;
 }
 
 extern "C" int rt_moments(rt_ctx *c, const double *I, double *R, void *stream) {
     if (!c || !I || !R) return RT_EINVAL;
-    CK(launch_moments(c->kp, I, R, (cudaStream_t)stream, &c->launches));
+    { ProfScope ps(c, RT_K_MOMENTS, (cudaStream_t)stream); CK(launch_moments(c->kp, I, R, (cudaStream_t)stream, &c->launches)); }
     return RT_OK;
 }
 
@@ -380,10 +415,13 @@ extern "C" int rt_moments(rt_ctx *c, const double *I, double *R, void *stream) {
 // then O6 on (I*, T) with T_- = T_base
 static int stage(rt_ctx *c, const double *I_flux, const double *T_flux, const double *I_base, double *I_out, double *T_io,
                  double delta, int *n_fail, double *R, double *G, cudaStream_t st) {
-    if (c->matter) CK(launch_facecoef(c->kp, T_flux, delta, c->d_fcoef, st, &c->launches));
-    CK(launch_transport(c->kp, I_flux, I_base, I_out, c->d_fcoef, c->matter, delta, st, &c->launches));
-    if (c->curved) CK(launch_angular(c->kp, I_flux, I_out, delta, st, &c->launches));
-    if (c->opt.source_method != 0 || R || G) CK(launch_source(c->kp, I_out, T_io, delta, n_fail, R, G, st, &c->launches));
+    if (c->matter) { ProfScope ps(c, RT_K_FACECOEF, st); CK(launch_facecoef(c->kp, T_flux, delta, c->d_fcoef, st, &c->launches)); }
+    { ProfScope ps(c, RT_K_TRANSPORT, st); CK(launch_transport(c->kp, I_flux, I_base, I_out, c->d_fcoef, c->matter, delta, st, &c->launches)); }
+    if (c->curved) { ProfScope ps(c, RT_K_ANGULAR, st); CK(launch_angular(c->kp, I_flux, I_out, delta, st, &c->launches)); }
+    if (c->opt.source_method != 0 || R || G) {
+        ProfScope ps(c, RT_K_SOURCE, st);
+        CK(launch_source(c->kp, I_out, T_io, delta, n_fail, R, G, st, &c->launches));
+    }
     return RT_OK;
 }
 

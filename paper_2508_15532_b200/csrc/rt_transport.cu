@@ -39,8 +39,8 @@ __device__ __forceinline__ double slope_rt(int lim, double dm, double dp) {
 
 // index of a fluid cell along one dim: periodic wraps, everything else clamps (fluid ghosts)
 __device__ __forceinline__ int fluid_idx(int c, int N, int bc_lo, int bc_hi) {
-    if (c < 0) return bc_lo == RT_BC_PERIODIC ? c + N : 0;
-    if (c >= N) return bc_hi == RT_BC_PERIODIC ? c - N : N - 1;
+    if (c < 0) return bc_lo == RT_BC_PERIODIC ? ((c % N) + N) % N : 0;
+    if (c >= N) return bc_hi == RT_BC_PERIODIC ? c % N : N - 1;
     return c;
 }
 __device__ __forceinline__ double alpha_total(const KParams &p, double rho, double T) {
@@ -93,7 +93,7 @@ __device__ __forceinline__ const double *cell_ptr(const KParams &p, const double
     int c = q[a];
     if (c < 0 || c >= N) {
         const int bc = (c < 0) ? p.bc_lo[a] : p.bc_hi[a];
-        if (bc == RT_BC_PERIODIC) q[a] = (c < 0) ? c + N : c - N;
+        if (bc == RT_BC_PERIODIC) q[a] = ((c % N) + N) % N;   // N may be 1 or 2: a single wrap is not enough
         else if (bc == RT_BC_OUTFLOW) q[a] = (c < 0) ? 0 : N - 1;
         else if (bc == RT_BC_ZERO) return nullptr;
         else {

@@ -17,7 +17,7 @@ METRIC = {"minkowski": 0, "mink_cyl": 1, "ks_mks": 2}
 GEOM = dict(g_c=0, e_c=1, einv_c=2, sqrtg_c=3, omega_c=4, n0_c=5, angcoef=6)
 SYMBOLS = ["rt_init", "rt_free", "rt_ndir", "rt_ndir_padded", "rt_get_directions", "rt_get_geometry", "rt_cfl_dt",
            "rt_set_boundary", "rt_set_fluid", "rt_transport", "rt_angular_flux", "rt_source_implicit", "rt_moments",
-           "rt_step", "rt_launch_count", "rt_last_cuda_error", "rt_strerror"]
+           "rt_step", "rt_profile_enable", "rt_profile_read", "rt_launch_count", "rt_last_cuda_error", "rt_strerror"]
 
 
 class RtGrid(ctypes.Structure):
@@ -58,6 +58,8 @@ def load_library(path=LIB_PATH):
     lib.rt_source_implicit.argtypes = [vp, vp, vp, dbl, vp, vp]
     lib.rt_moments.argtypes = [vp, vp, vp, vp]
     lib.rt_step.argtypes = [vp, vp, vp, vp, vp, dbl, vp, vp]
+    lib.rt_profile_enable.argtypes = [vp, ci]
+    lib.rt_profile_read.argtypes = [vp, vp, vp]
     lib.rt_launch_count.argtypes = [vp]
     lib.rt_launch_count.restype = ctypes.c_longlong
     lib.rt_strerror.argtypes = [ci]
@@ -195,6 +197,16 @@ class RtContext:
 
     def n_fail(self):
         return int(self._nfail.item())
+
+    def profile_enable(self, on=True):
+        _check(lib().rt_profile_enable(self._h, int(on)))
+
+    def profile_read(self):
+        """dict kernel class -> (milliseconds, launches) since the last read."""
+        ms, cnt = np.zeros(5), np.zeros(5, np.int64)
+        _check(lib().rt_profile_read(self._h, ms.ctypes.data, cnt.ctypes.data))
+        names = ("facecoef", "transport", "angular", "source", "moments")
+        return {n: (float(ms[i]), int(cnt[i])) for i, n in enumerate(names)}
 
     def launch_count(self):
         return int(lib().rt_launch_count(self._h))
