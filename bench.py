@@ -1,0 +1,315 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the radiation hot path (one rt_step = predictor + corrector: transport, angular flux,
+implicit source, moments) on a synthetic workload shaped like BASELINE.json's configs.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl reference]
+
+Prints ONE JSON line.  metric = cell-direction updates/s (fp64): N_cells * N_dirs * steps / time of rt_step, with
+inputs resident in HBM.  `e2e` = the same through the C ABI with pinned HOST buffers (H2D of I, T and D2H of I, T,
+R, G inside the timed region).  `roofline` = dominant kernel, algorithmic bytes / CUDA-event time / measured HBM peak.
+`cpu_baseline` = the oracle timed on a bounded sample on this box's cores (a baseline, not the target).
+N > 1: replicas only this round: every rank runs the same workload on its own GPU,
+value = aggregate over ranks / max-over-ranks time.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "cell-direction updates/s (fp64)"
+UNIT = "cell-direction updates/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index 1..5 (4 = Kerr-Schild, the roofline config)")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--size", default=None, help="override grid, e.g. 64x48x32 (debug)")
+    return ap.parse_args()
+
+
+# ---- clocks ---------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi sampled DURING the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            pass
+        sm = sorted(float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit())
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) > 3 + i and r[3 + i].lower().startswith("active") for r in self.rows)]
+        pw = [float(r[2]) for r in self.rows if len(r) > 2 and r[2].replace(".", "").isdigit()]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": reasons}
+
+
+def measured_peak():
+    """(GB/s, which) -- MEASURED_PEAKS.json (driver-written), else the profiling guide's fallback."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ---- workload -------------------------------------------------------------------------------------------------------
+# Algorithmic bytes per cell-direction per LAUNCH of each kernel class:
+# what the method must move at this kernel boundary, fp64 = 8 B.  transport: read I_in, (read I_base when it is a
+# different array: corrector only), write I_out; angular: read I_in, read+write I_inout; source: read+write I.
+ALGO_BYTES = {"transport_pred": 16.0, "transport_corr": 24.0, "angular": 24.0, "source": 16.0}
+
+
+def make_config(args):
+    import rt_workloads as W
+    n = tuple(int(x) for x in args.size.split("x")) if args.size else None
+    return W.config(args.config, n=n)
+
+
+def workload_name(cfg):
+    n = cfg["grid"]["n"]
+    return "%s %dx%dx%d x %d dirs" % (cfg["name"], n[0], n[1], n[2], 10 * cfg["level"] ** 2 + 2)
+
+
+def setup_gpu(cfg, device):
+    """Context + device-resident seeded inputs.  Tables needed by the generator come from the LIBRARY (no oracle)."""
+    import numpy as np
+    import torch
+    import rt_workloads as W
+    from paper_2508_15532_b200 import rt
+
+    kind, params = cfg["metric"]
+    ctx = rt.RtContext(cfg["grid"], kind, params, cfg["level"], cfg["options"], device=device)
+    f = W.fields(cfg, ctx.directions()["nhat"], ctx.geometry("e_c"))
+    dev = ctx.device
+    rho = torch.as_tensor(f["rho"], device=dev).contiguous()
+    T = torch.as_tensor(f["T"], device=dev).contiguous()
+    u4 = None if f["u4"] is None else torch.as_tensor(f["u4"], device=dev).contiguous()
+    ctx.set_fluid(rho, T, u4)
+    for (dim, side), g in f["ghosts"].items():
+        gd = torch.zeros(g.shape[:2] + (ctx.pitch,), dtype=torch.float64, device=dev)
+        gd[..., :ctx.nd] = torch.as_tensor(g, device=dev)
+        ctx.set_boundary(dim, side, gd)
+    dt = cfg["dt"] if cfg["dt"] is not None else min(ctx.cfl_dt())
+    I = ctx.to_device(f["I0"])
+    return ctx, f, I, T.clone(), dt
+
+
+def run_gpu(args, rank, world):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    local = int(os.environ.get("LOCAL_RANK", 0))
+    device = "cuda:%d" % local
+    torch.cuda.set_device(local)
+    cfg = make_config(args)
+    ctx, f, I, T, dt = setup_gpu(cfg, device)
+    dev = ctx.device
+    R = torch.zeros((16,) + ctx.shape, dtype=torch.float64, device=dev)
+    G = torch.zeros((4,) + ctx.shape, dtype=torch.float64, device=dev)
+    units = ctx.ncell * ctx.nd                       # cell-direction updates per step
+    I0, T0 = I.clone(), T.clone()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+
+    for _ in range(max(args.warmup, 3)):
+        ctx.step(I, T, dt, R, G)
+    barrier()
+    I.copy_(I0); T.copy_(T0)
+    ctx.profile_enable(True)
+    ctx.profile_read()
+    l0 = ctx.launch_count()
+    clocks = ClockSampler(local)
+    clocks.start()
+    barrier()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(args.steps):
+        ctx.step(I, T, dt, R, G)
+    ev1.record()
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    clk = clocks.stop()
+    prof = ctx.profile_read()
+    ctx.profile_enable(False)
+    launches = ctx.launch_count() - l0
+    finite = bool(torch.isfinite(I).all().item())
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+
+    # ---- end to end through the C ABI with pinned HOST buffers (H2D + D2H inside the timed region) ----
+    e2e = None
+    if not args.no_e2e:
+        hI = torch.empty(I.shape, dtype=torch.float64, pin_memory=True); hI.copy_(I0)
+        hT = torch.empty(T.shape, dtype=torch.float64, pin_memory=True); hT.copy_(T0)
+        hR = torch.empty(R.shape, dtype=torch.float64, pin_memory=True)
+        hG = torch.empty(G.shape, dtype=torch.float64, pin_memory=True)
+        ksteps = min(args.steps, 5)
+        def one():
+            I.copy_(hI, non_blocking=True); T.copy_(hT, non_blocking=True)
+            ctx.step(I, T, dt, R, G)
+            hI.copy_(I, non_blocking=True); hT.copy_(T, non_blocking=True)
+            hR.copy_(R, non_blocking=True); hG.copy_(G, non_blocking=True)
+        one()
+        barrier()
+        t0 = time.perf_counter()
+        ev0.record()
+        for _ in range(ksteps):
+            one()
+        ev1.record()
+        barrier()
+        ems = ev0.elapsed_time(ev1)
+        if world > 1:
+            t = torch.tensor([ems], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ems = float(t.item())
+        h2d = (hI.numel() + hT.numel()) * 8
+        d2h = (hI.numel() + hT.numel() + hR.numel() + hG.numel()) * 8
+        e2e = {"value": units * ksteps * world / (ems * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "steps": ksteps, "ms_per_step": ems / ksteps}
+    return dict(cfg=cfg, ctx=ctx, ms=ms, units=units, prof=prof, launches=launches, clk=clk, e2e=e2e, finite=finite, dt=dt)
+
+
+# ---- oracle legs (the only places bench.py may execute oracle/) ----------------------------------------------------
+ORACLE_SAMPLE = {1: (64, 64, 1), 2: (24, 24, 24), 3: (24, 24, 24), 4: (64, 48, 16), 5: (32, 24, 8)}
+
+
+def run_oracle(cfg_index, steps, warmup=0):
+    """The oracle as it stands on this box's host cores, on a bounded sample of the workload: the same config
+    (metric, tetrad, opacities, seeded fields, CFL rule) on a coarser grid.  returns (updates/s, cores, sample)."""
+    import numpy as np
+    import rt_workloads as W
+    from oracle import Oracle
+
+    n = ORACLE_SAMPLE[cfg_index]
+    cfg = W.config(cfg_index, n=n)
+    kind, params = cfg["metric"]
+    orc = Oracle(cfg["grid"], kind, params, cfg["level"], cfg["options"])
+    f = W.fields(cfg, orc.ang["nhat"], orc.tab["e_c"])
+    orc.set_fluid(f["rho"], f["T"], f["u4"])
+    for (dim, side), g in f["ghosts"].items():
+        orc.set_boundary(dim, side, g)
+    dt = cfg["dt"] if cfg["dt"] is not None else min(orc.cfl())
+    I, T = f["I0"], f["T"]
+    for _ in range(warmup):
+        I, T, R, G, nf = orc.step(I, T, dt)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        I, T, R, G, nf = orc.step(I, T, dt)
+    el = time.perf_counter() - t0
+    units = n[0] * n[1] * n[2] * orc.nd
+    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    sample = "oracle rt_step x%d on %s at %dx%dx%d x %d dirs (same config, coarser grid), OpenMP over cells" % (
+        steps, cfg["name"], n[0], n[1], n[2], orc.nd)
+    return units * steps / el, cores, sample, el / steps * 1e3, cfg
+
+
+def main_reference(args):
+    rank = int(os.environ.get("RANK", 0))
+    if rank != 0:
+        return
+    val, cores, sample, ms, cfg = run_oracle(args.config, max(1, min(args.steps, 3)), warmup=min(args.warmup, 1))
+    import rt_workloads as W
+    full = W.config(args.config)
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(full), "timed_sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return main_reference(args)
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", 1))
+    rank = int(os.environ.get("RANK", 0))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda:%d" % int(os.environ.get("LOCAL_RANK", 0))))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device and no CPU fallback (use --impl reference for the oracle)")
+    r = run_gpu(args, rank, world)
+    if rank == 0:
+        ms, units, K = r["ms"], r["units"], args.steps
+        value = units * K * world / (ms * 1e-3)
+        peak, which = measured_peak()
+        prof = r["prof"]
+        dom = max(("transport", "angular", "source"), key=lambda k: prof[k][0])
+        dms, dcnt = prof[dom]
+        per_unit = {"transport": 0.5 * (ALGO_BYTES["transport_pred"] + ALGO_BYTES["transport_corr"]),
+                    "angular": ALGO_BYTES["angular"], "source": ALGO_BYTES["source"]}
+        achieved = per_unit[dom] * units / (dms / max(dcnt, 1) * 1e-3) / 1e9 if dcnt else 0.0
+        step_bytes = sum(per_unit[k] * units * prof[k][1] for k in per_unit) / K
+        roof = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": None, "peak_source": which,
+                "algorithmic_bytes_per_cell_dir_per_launch": per_unit[dom],
+                "kernel_ms_per_step": {k: prof[k][0] / K for k in prof},
+                "kernel_launches_per_step": {k: prof[k][1] / K for k in prof},
+                "step_algorithmic_GBps": step_bytes / (ms / K * 1e-3) / 1e9,
+                "step_frac_of_peak": step_bytes / (ms / K * 1e-3) / 1e9 / peak}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
+                "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                "data": "synthetic",
+                "config": {"workload": workload_name(r["cfg"]), "dt": r["dt"], "l2": "inputs larger than L2 (one I copy >= 1 GB vs 126 MB)"
+                           if units * 8 > 2.0e8 else "inputs FIT in L2 (latency-bound config; HBM fraction not meaningful)",
+                           "multi_gpu": "replicas only (no halo exchange this round)" if world > 1 else "single GPU",
+                           "finite": r["finite"]},
+                "clocks": r["clk"], "e2e": r["e2e"], "gpu_launches": r["launches"], "roofline": roof}
+        if not args.no_cpu_baseline and world == 1:
+            val, cores, sample, oms, _ = run_oracle(args.config, 2)
+            line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
