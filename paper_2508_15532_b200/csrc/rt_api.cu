@@ -23,6 +23,7 @@ struct rt_ctx {
     std::vector<double> h_g, h_e, h_einv, h_sqrtg, h_omega, h_n0, h_angcoef;
     DeviceTables tab;
     double *d_rho, *d_u4, *d_T, *d_Th, *d_Ih, *d_fcoef[3];
+    unsigned char *d_cflag;   // per cell: any non-vacuum face
     KParams kp;
     long long launches;
     bool profiling;
@@ -201,6 +202,8 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     const size_t nI = (size_t)c->ncell * pitch;
     c->d_rho = c->d_u4 = c->d_T = c->d_Th = c->d_Ih = nullptr;
     c->d_fcoef[0] = c->d_fcoef[1] = c->d_fcoef[2] = nullptr;
+    c->d_cflag = nullptr;
+    if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_cflag, c->ncell);
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_rho, c->ncell * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_u4, 4 * c->ncell * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_T, c->ncell * sizeof(double));
@@ -234,7 +237,7 @@ extern "C" int rt_free(rt_ctx *c) {
     if (!c) return RT_EINVAL;
     for (int a = 0; a < 3; ++a) { cudaFree(c->tab.face[a]); cudaFree(c->d_fcoef[a]); }
     cudaFree(c->tab.cen); cudaFree(c->tab.ecen); cudaFree(c->tab.angcoef); cudaFree(c->tab.nhat); cudaFree(c->tab.w);
-    cudaFree(c->tab.nb); cudaFree(c->d_rho); cudaFree(c->d_u4); cudaFree(c->d_T); cudaFree(c->d_Th); cudaFree(c->d_Ih);
+    cudaFree(c->tab.nb); cudaFree(c->d_cflag); cudaFree(c->d_rho); cudaFree(c->d_u4); cudaFree(c->d_T); cudaFree(c->d_Th); cudaFree(c->d_Ih);
     delete c;
     return RT_OK;
 }
@@ -385,8 +388,8 @@ extern "C" int rt_transport(rt_ctx *c, const double *I_in, const double *I_base,
     if (!c || !I_in || !I_base || !I_out || I_in == I_out) return RT_EINVAL;
     if (fixed_bc_missing(c) || (c->matter && !c->fluid_set)) return RT_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
-    if (c->matter) { ProfScope ps(c, RT_K_FACECOEF, st); CK(launch_facecoef(c->kp, c->d_T, dt, c->d_fcoef, st, &c->launches)); }
-    { ProfScope ps(c, RT_K_TRANSPORT, st); CK(launch_transport(c->kp, I_in, I_base, I_out, c->d_fcoef, c->matter, dt, st, &c->launches)); }
+    if (c->matter) { ProfScope ps(c, RT_K_FACECOEF, st); CK(launch_facecoef(c->kp, c->d_T, dt, c->d_fcoef, c->d_cflag, st, &c->launches)); }
+    { ProfScope ps(c, RT_K_TRANSPORT, st); CK(launch_transport(c->kp, I_in, I_base, I_out, c->d_fcoef, c->d_cflag, c->matter, dt, st, &c->launches)); }
     return RT_OK;
 }
 
@@ -415,8 +418,8 @@ extern "C" int rt_moments(rt_ctx *c, const double *I, double *R, void *stream) {
 // then O6 on (I*, T) with T_- = T_base
 static int stage(rt_ctx *c, const double *I_flux, const double *T_flux, const double *I_base, double *I_out, double *T_io,
                  double delta, int *n_fail, double *R, double *G, cudaStream_t st) {
-    if (c->matter) { ProfScope ps(c, RT_K_FACECOEF, st); CK(launch_facecoef(c->kp, T_flux, delta, c->d_fcoef, st, &c->launches)); }
-    { ProfScope ps(c, RT_K_TRANSPORT, st); CK(launch_transport(c->kp, I_flux, I_base, I_out, c->d_fcoef, c->matter, delta, st, &c->launches)); }
+    if (c->matter) { ProfScope ps(c, RT_K_FACECOEF, st); CK(launch_facecoef(c->kp, T_flux, delta, c->d_fcoef, c->d_cflag, st, &c->launches)); }
+    { ProfScope ps(c, RT_K_TRANSPORT, st); CK(launch_transport(c->kp, I_flux, I_base, I_out, c->d_fcoef, c->d_cflag, c->matter, delta, st, &c->launches)); }
     if (c->curved) { ProfScope ps(c, RT_K_ANGULAR, st); CK(launch_angular(c->kp, I_flux, I_out, delta, st, &c->launches)); }
     if (c->opt.source_method != 0 || R || G) {
         ProfScope ps(c, RT_K_SOURCE, st);

@@ -129,96 +129,190 @@ __device__ __forceinline__ bool sign_differs(double a, double b) {
     return ((a > 0) - (a < 0)) != ((b > 0) - (b < 0));
 }
 
-// flux through one face, times sqrt(-g_f).  IL/IR: PLI states; Il/Ir: cell-centre values left/right of the face.
-template <bool MATTER>
-__device__ __forceinline__ double face_flux(const FaceC &c, double IL, double IR, double Il, double Ir, const double4 &fc) {
-    if (!MATTER || fc.y < 0.0) return c.Q * c.P * (c.P > 0 ? IL : IR);                       // Eq 20
-    return c.Q * (c.P * fc.x * (IL + IR) - fabs(c.P) * fc.y * (Ir - Il) + c.Z * (fc.z * IL + fc.w * IR));   // Eq 23
+// Monotonised-central slope, same value as minmod3(2 dm, (dm+dp)/2, 2 dp) bit for bit, with 5 fp64-pipe operations:
+// equal signs => sign * min(2 min(|dm|,|dp|), |dm+dp|/2); opposite signs or a zero difference => 0.
+__device__ __forceinline__ double slope_mc(double dm, double dp) {
+    const double m2 = 2.0 * fmin(fabs(dm), fabs(dp));
+    const double r = fmin(m2, 0.5 * fabs(dm + dp));
+    const bool opp = (__double2hiint(dm) ^ __double2hiint(dp)) < 0;
+    return opp ? 0.0 : copysign(r, dm);
+}
+template <int LIM>
+__device__ __forceinline__ double slope_k(double dm, double dp) {
+    return (LIM == RT_LIM_MC) ? slope_mc(dm, dp) : slope<LIM>(dm, dp);
 }
 
-// both fluxes of one dim from the 5-point stencil (m2, m1, c0, p1, p2): lo = face (m1|c0), hi = face (c0|p1)
+// Per-face coefficients of one (column, s), with dt / (n^0 n_0 sqrt(-g_c) dx^a) folded in, so that
+// I_out = I_base - sum_faces (+-) flux.   A = [..] n_0f sqrt(-g_f) n^a_f,  Zq = [..] n_0f sqrt(-g_f) n^0_f.
+struct FaceK { double A, Zq; bool pos; };
+__device__ __forceinline__ FaceK fold(const FaceC &c, double scale) {
+    FaceK k;
+    k.A = c.Q * c.P * scale;
+    k.Zq = c.Q * c.Z * scale;
+    k.pos = c.P > 0;
+    return k;
+}
+// flux through one face.  IL/IR: PLI states; Il/Ir: cell-centre values left/right of the face.
+template <bool MATTER>
+__device__ __forceinline__ double face_flux(const FaceK &c, double IL, double IR, double Il, double Ir, const double4 &fc) {
+    if (!MATTER || fc.y < 0.0) return c.A * (c.pos ? IL : IR);                                     // Eq 20
+    const double B = c.pos ? c.A : -c.A;                                                           // [..] n_0 |n^a|
+    return c.A * fc.x * (IL + IR) - B * fc.y * (Ir - Il) + c.Zq * (fc.z * IL + fc.w * IR);          // Eq 23
+}
+// flux difference of one transverse dim from the 5-point stencil (m2, m1, c0, p1, p2)
 template <int LIM, bool MATTER>
-__device__ __forceinline__ double flux_diff(double m2, double m1, double c0, double p1, double p2, const FaceC &lo,
-                                            const FaceC &hi, const double4 &fclo, const double4 &fchi) {
+__device__ __forceinline__ double flux_diff(double m2, double m1, double c0, double p1, double p2, const FaceK &lo,
+                                            const FaceK &hi, const double4 &fclo, const double4 &fchi) {
     const double d0 = m1 - m2, d1 = c0 - m1, d2 = p1 - c0, d3 = p2 - p1;
-    const double sm = slope<LIM>(d0, d1), s0 = slope<LIM>(d1, d2), sp = slope<LIM>(d2, d3);
+    const double sm = slope_k<LIM>(d0, d1), s0 = slope_k<LIM>(d1, d2), sp = slope_k<LIM>(d2, d3);
     const double Flo = face_flux<MATTER>(lo, m1 + 0.5 * sm, c0 - 0.5 * s0, m1, c0, fclo);
     const double Fhi = face_flux<MATTER>(hi, c0 + 0.5 * s0, p1 - 0.5 * sp, c0, p1, fchi);
     return Fhi - Flo;
 }
 
+// cell flag: 1 if any of the six faces of the cell is a non-vacuum (Eq 23) face
+__global__ void k_cellflag(KParams p, const double4 *__restrict__ fc0, const double4 *__restrict__ fc1,
+                           const double4 *__restrict__ fc2, unsigned char *__restrict__ flag) {
+    const long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (c >= p.ncell) return;
+    const int i = int(c % p.n1), j = int((c / p.n1) % p.n2), k = int(c / p.ncol);
+    const long long x = ((long long)k * p.n2 + j) * (p.n1 + 1) + i, y = ((long long)k * (p.n2 + 1) + j) * p.n1 + i;
+    const bool m = fc0[x].y >= 0 || fc0[x + 1].y >= 0 || fc1[y].y >= 0 || fc1[y + p.n1].y >= 0 || fc2[c].y >= 0 ||
+                   fc2[c + p.ncol].y >= 0;
+    flag[c] = m ? 1 : 0;
+}
+
+// generic (boundary-aware) load, kept out of line: only threads next to a ZERO / FIXED boundary come here
+__device__ __noinline__ double slow_ld(const KParams &p, const double *I, int a, int i, int j, int k, int s) {
+    return ldI(cell_ptr(p, I, a, i, j, k), s);
+}
+// neighbour of coordinate c0 at offset d along a dim of extent N: interior index after periodic wrap / outflow
+// clamp, or -1 if it is a ZERO / FIXED ghost
+__device__ __forceinline__ int nb_index(int c, int N, int bc_lo, int bc_hi) {
+    if (c >= 0 && c < N) return c;
+    const int bc = (c < 0) ? bc_lo : bc_hi;
+    if (bc == RT_BC_PERIODIC) return ((c % N) + N) % N;
+    if (bc == RT_BC_OUTFLOW) return (c < 0) ? 0 : N - 1;
+    return -1;
+}
+
 // ---- spatial transport ------------------------------------------------------------------------------------------
+// One thread = one (column, s); marches x3.  Per step: 1 new x3 value + 8 transverse neighbours (coalesced), one
+// x3 slope and one x3 flux (the lower x3 flux and slope are carried), 3 slopes + 2 fluxes per transverse dim.
 template <int LIM, bool MATTER>
-__global__ void __launch_bounds__(256)
-k_transport(KParams p, const double *__restrict__ I_in, const double *I_base, double *I_out,
-            const double4 *__restrict__ fc0, const double4 *__restrict__ fc1, const double4 *__restrict__ fc2, double dt) {
+__global__ void __launch_bounds__(256, 2)
+k_transport(const __grid_constant__ KParams p, const double *__restrict__ I_in, const double *I_base, double *I_out,
+            const double4 *__restrict__ fc0, const double4 *__restrict__ fc1, const double4 *__restrict__ fc2,
+            const unsigned char *__restrict__ cflag, double dt) {
     const int e = blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= p.n1 * p.pitch) return;
     const int i = e / p.pitch, s = e - i * p.pitch, j = blockIdx.y;
-    const long long col = (long long)j * p.n1 + i;
-    const long long kstride = (long long)p.n1 * p.n2 * p.pitch;
-    double *out = I_out + col * p.pitch + s;
-    if (s >= p.nd) {   // pad lanes: keep the pad zero
+    const int col = j * p.n1 + i;
+    const long long kstride = (long long)p.ncol * p.pitch;
+    const long long pos0 = (long long)col * p.pitch + s;
+    double *out = I_out + pos0;
+    bool dead = s >= p.nd;   // pad lanes: keep the pad zero
+    double nx = 0, ny = 0, nz = 0, n0c = 0, scale = 0;
+    const double *cen = p.cen + (long long)col * CEN_STRIDE;
+    if (!dead) {
+        nx = __ldg(p.nhat + s); ny = __ldg(p.nhat + p.pitch + s); nz = __ldg(p.nhat + 2 * p.pitch + s);
+        n0c = centre_n0(cen, nx, ny, nz);
+        const double nup = cen[4] + cen[5] * nx + cen[6] * ny + cen[7] * nz;
+        scale = dt * cen[8] / (nup * n0c);
+        const bool band_ij = (i < p.zlo[0] || i >= p.n1 - p.zhi[0] || j < p.zlo[1] || j >= p.n2 - p.zhi[1]);
+        dead = band_ij || n0c > -p.n0_floor;   // masked direction (S14) or zero band (L709): stays zero, no work
+    }
+    if (dead) {
         for (int k = 0; k < p.n3; ++k) out[k * kstride] = 0.0;
         return;
     }
-    const double nx = __ldg(p.nhat + s), ny = __ldg(p.nhat + p.pitch + s), nz = __ldg(p.nhat + 2 * p.pitch + s);
-    const double *cen = p.cen + col * CEN_STRIDE;
-    const double n0c = centre_n0(cen, nx, ny, nz);
-    const double nup = cen[4] + cen[5] * nx + cen[6] * ny + cen[7] * nz;
-    const double n0n0 = nup * n0c, inv_n0n0 = 1.0 / n0n0, inv_sg = cen[8];
-    const bool band_ij = (i < p.zlo[0] || i >= p.n1 - p.zhi[0] || j < p.zlo[1] || j >= p.n2 - p.zhi[1]);
-    if (band_ij || n0c > -p.n0_floor) {   // masked direction (S14) or zero band (L709): stays zero, no work
-        for (int k = 0; k < p.n3; ++k) out[k * kstride] = 0.0;
-        return;
-    }
-    // face coefficients, formed once per column (geometry is x3-independent)
-    FaceC xl = face_coef(p.face[0] + ((long long)j * (p.n1 + 1) + i) * FACE_STRIDE, nx, ny, nz);
-    FaceC xh = face_coef(p.face[0] + ((long long)j * (p.n1 + 1) + i + 1) * FACE_STRIDE, nx, ny, nz);
-    FaceC yl = face_coef(p.face[1] + ((long long)j * p.n1 + i) * FACE_STRIDE, nx, ny, nz);
-    FaceC yh = face_coef(p.face[1] + ((long long)(j + 1) * p.n1 + i) * FACE_STRIDE, nx, ny, nz);
-    FaceC zf = face_coef(p.face[2] + col * FACE_STRIDE, nx, ny, nz);
-    // n_0 gate (L280): no flux between two mesh cells whose n_0 differ in sign
-    {
-        int in;
-        in = (i > 0) ? i - 1 : (p.bc_lo[0] == RT_BC_PERIODIC ? p.n1 - 1 : -1);
-        if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)j * p.n1 + in) * CEN_STRIDE, nx, ny, nz))) xl.Q = 0.0;
-        in = (i < p.n1 - 1) ? i + 1 : (p.bc_hi[0] == RT_BC_PERIODIC ? 0 : -1);
-        if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)j * p.n1 + in) * CEN_STRIDE, nx, ny, nz))) xh.Q = 0.0;
-        in = (j > 0) ? j - 1 : (p.bc_lo[1] == RT_BC_PERIODIC ? p.n2 - 1 : -1);
-        if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)in * p.n1 + i) * CEN_STRIDE, nx, ny, nz))) yl.Q = 0.0;
-        in = (j < p.n2 - 1) ? j + 1 : (p.bc_hi[1] == RT_BC_PERIODIC ? 0 : -1);
-        if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)in * p.n1 + i) * CEN_STRIDE, nx, ny, nz))) yh.Q = 0.0;
-    }
-    const double cx = p.inv_dx[0] * inv_sg, cy = p.inv_dx[1] * inv_sg, cz = p.inv_dx[2] * inv_sg;
+    // transverse neighbours: element offsets inside the x3-plane, resolved once (periodic / outflow map to interior
+    // cells); a ZERO / FIXED ghost makes the thread use the generic loader
+    const int im2 = nb_index(i - 2, p.n1, p.bc_lo[0], p.bc_hi[0]), im1 = nb_index(i - 1, p.n1, p.bc_lo[0], p.bc_hi[0]);
+    const int ip1 = nb_index(i + 1, p.n1, p.bc_lo[0], p.bc_hi[0]), ip2 = nb_index(i + 2, p.n1, p.bc_lo[0], p.bc_hi[0]);
+    const int jm2 = nb_index(j - 2, p.n2, p.bc_lo[1], p.bc_hi[1]), jm1 = nb_index(j - 1, p.n2, p.bc_lo[1], p.bc_hi[1]);
+    const int jp1 = nb_index(j + 1, p.n2, p.bc_lo[1], p.bc_hi[1]), jp2 = nb_index(j + 2, p.n2, p.bc_lo[1], p.bc_hi[1]);
+    const bool special = (im2 | im1 | ip1 | ip2 | jm2 | jm1 | jp1 | jp2) < 0;
+    const int rowp = p.n1 * p.pitch;
+    const int oxm2 = (im2 - i) * p.pitch, oxm1 = (im1 - i) * p.pitch, oxp1 = (ip1 - i) * p.pitch, oxp2 = (ip2 - i) * p.pitch;
+    const int oym2 = (jm2 - j) * rowp, oym1 = (jm1 - j) * rowp, oyp1 = (jp1 - j) * rowp, oyp2 = (jp2 - j) * rowp;
 
-    // x3 register window: I_in at k-2 .. k+2
-    double w0 = ldI(cell_ptr(p, I_in, 2, i, j, -2), s), w1 = ldI(cell_ptr(p, I_in, 2, i, j, -1), s);
-    double w2 = ldI(cell_ptr(p, I_in, 2, i, j, 0), s), w3 = ldI(cell_ptr(p, I_in, 2, i, j, 1), s);
+    // face coefficients, formed once per column (geometry is x3-independent); n_0 gate (L280) applied here
+    FaceK xl, xh, yl, yh, zf;
+    {
+        const double sx = scale * p.inv_dx[0], sy = scale * p.inv_dx[1], sz = scale * p.inv_dx[2];
+        FaceC c;
+        int in;
+        c = face_coef(p.face[0] + ((long long)j * (p.n1 + 1) + i) * FACE_STRIDE, nx, ny, nz);
+        in = (i > 0) ? i - 1 : (p.bc_lo[0] == RT_BC_PERIODIC ? p.n1 - 1 : -1);
+        if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)j * p.n1 + in) * CEN_STRIDE, nx, ny, nz))) c.Q = 0.0;
+        xl = fold(c, sx);
+        c = face_coef(p.face[0] + ((long long)j * (p.n1 + 1) + i + 1) * FACE_STRIDE, nx, ny, nz);
+        in = (i < p.n1 - 1) ? i + 1 : (p.bc_hi[0] == RT_BC_PERIODIC ? 0 : -1);
+        if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)j * p.n1 + in) * CEN_STRIDE, nx, ny, nz))) c.Q = 0.0;
+        xh = fold(c, sx);
+        c = face_coef(p.face[1] + ((long long)j * p.n1 + i) * FACE_STRIDE, nx, ny, nz);
+        in = (j > 0) ? j - 1 : (p.bc_lo[1] == RT_BC_PERIODIC ? p.n2 - 1 : -1);
+        if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)in * p.n1 + i) * CEN_STRIDE, nx, ny, nz))) c.Q = 0.0;
+        yl = fold(c, sy);
+        c = face_coef(p.face[1] + ((long long)(j + 1) * p.n1 + i) * FACE_STRIDE, nx, ny, nz);
+        in = (j < p.n2 - 1) ? j + 1 : (p.bc_hi[1] == RT_BC_PERIODIC ? 0 : -1);
+        if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)in * p.n1 + i) * CEN_STRIDE, nx, ny, nz))) c.Q = 0.0;
+        yh = fold(c, sy);
+        zf = fold(face_coef(p.face[2] + (long long)col * FACE_STRIDE, nx, ny, nz), sz);
+    }
+    const double *pin = I_in + pos0;
     const double4 vac = make_double4(0.5, -1.0, 0.0, 0.0);
+    auto ldk = [&](int kk) -> double {   // x3 neighbour with boundary conditions
+        return (kk >= 0 && kk < p.n3) ? __ldg(pin + kk * kstride) : slow_ld(p, I_in, 2, i, j, kk, s);
+    };
+    // prologue of the x3 march: carried state = (w2, w3) = I at (k, k+1), slope at k, lower x3 flux
+    double w2, w3, sk, Flo;
+    {
+        const double w0 = ldk(-2), w1 = ldk(-1);
+        w2 = ldk(0); w3 = ldk(1);
+        const double sm = slope_k<LIM>(w1 - w0, w2 - w1);
+        sk = slope_k<LIM>(w2 - w1, w3 - w2);
+        const double4 f = MATTER ? ld4(fc2 + col) : vac;
+        Flo = face_flux<MATTER>(zf, w1 + 0.5 * sm, w2 - 0.5 * sk, w1, w2, f);
+    }
+    const int zlo = p.zlo[2], zhi = p.n3 - p.zhi[2];
     for (int k = 0; k < p.n3; ++k) {
-        const double w4 = ldI(cell_ptr(p, I_in, 2, i, j, k + 2), s);
-        const double xm2 = ldI(cell_ptr(p, I_in, 0, i - 2, j, k), s), xm1 = ldI(cell_ptr(p, I_in, 0, i - 1, j, k), s);
-        const double xp1 = ldI(cell_ptr(p, I_in, 0, i + 1, j, k), s), xp2 = ldI(cell_ptr(p, I_in, 0, i + 2, j, k), s);
-        const double ym2 = ldI(cell_ptr(p, I_in, 1, i, j - 2, k), s), ym1 = ldI(cell_ptr(p, I_in, 1, i, j - 1, k), s);
-        const double yp1 = ldI(cell_ptr(p, I_in, 1, i, j + 1, k), s), yp2 = ldI(cell_ptr(p, I_in, 1, i, j + 2, k), s);
-        double4 fxl = vac, fxh = vac, fyl = vac, fyh = vac, fzl = vac, fzh = vac;
-        if (MATTER) {
-            fxl = ld4(fc0 + ((long long)k * p.n2 + j) * (p.n1 + 1) + i);
-            fxh = ld4(fc0 + ((long long)k * p.n2 + j) * (p.n1 + 1) + i + 1);
-            fyl = ld4(fc1 + ((long long)k * (p.n2 + 1) + j) * p.n1 + i);
-            fyh = ld4(fc1 + ((long long)k * (p.n2 + 1) + j + 1) * p.n1 + i);
-            fzl = ld4(fc2 + ((long long)k * p.n2 + j) * p.n1 + i);
-            fzh = ld4(fc2 + ((long long)(k + 1) * p.n2 + j) * p.n1 + i);
+        const double w4 = ldk(k + 2);
+        const double *pk = pin + k * kstride;
+        double xm2, xm1, xp1, xp2, ym2, ym1, yp1, yp2;
+        if (!special) {
+            xm2 = __ldg(pk + oxm2); xm1 = __ldg(pk + oxm1); xp1 = __ldg(pk + oxp1); xp2 = __ldg(pk + oxp2);
+            ym2 = __ldg(pk + oym2); ym1 = __ldg(pk + oym1); yp1 = __ldg(pk + oyp1); yp2 = __ldg(pk + oyp2);
+        } else {
+            xm2 = slow_ld(p, I_in, 0, i - 2, j, k, s); xm1 = slow_ld(p, I_in, 0, i - 1, j, k, s);
+            xp1 = slow_ld(p, I_in, 0, i + 1, j, k, s); xp2 = slow_ld(p, I_in, 0, i + 2, j, k, s);
+            ym2 = slow_ld(p, I_in, 1, i, j - 2, k, s); ym1 = slow_ld(p, I_in, 1, i, j - 1, k, s);
+            yp1 = slow_ld(p, I_in, 1, i, j + 1, k, s); yp2 = slow_ld(p, I_in, 1, i, j + 2, k, s);
         }
-        double D = cx * flux_diff<LIM, MATTER>(xm2, xm1, w2, xp1, xp2, xl, xh, fxl, fxh);
-        D += cy * flux_diff<LIM, MATTER>(ym2, ym1, w2, yp1, yp2, yl, yh, fyl, fyh);
-        D += cz * flux_diff<LIM, MATTER>(w0, w1, w2, w3, w4, zf, zf, fzl, fzh);
+        const long long cell = (long long)k * p.ncol + col;
+        const bool mat = MATTER && cflag[cell] != 0;
+        // x3: one new slope, one new flux
+        const double sk1 = slope_k<LIM>(w3 - w2, w4 - w3);
+        double D;
+        if (mat) {
+            const double Fhi = face_flux<MATTER>(zf, w2 + 0.5 * sk, w3 - 0.5 * sk1, w2, w3, ld4(fc2 + cell + p.ncol));
+            D = Fhi - Flo;
+            Flo = Fhi;
+            const long long fx = ((long long)k * p.n2 + j) * (p.n1 + 1) + i, fy = ((long long)k * (p.n2 + 1) + j) * p.n1 + i;
+            D += flux_diff<LIM, MATTER>(xm2, xm1, w2, xp1, xp2, xl, xh, ld4(fc0 + fx), ld4(fc0 + fx + 1));
+            D += flux_diff<LIM, MATTER>(ym2, ym1, w2, yp1, yp2, yl, yh, ld4(fc1 + fy), ld4(fc1 + fy + p.n1));
+        } else {
+            const double Fhi = face_flux<false>(zf, w2 + 0.5 * sk, w3 - 0.5 * sk1, w2, w3, vac);
+            D = Fhi - Flo;
+            Flo = Fhi;
+            D += flux_diff<LIM, false>(xm2, xm1, w2, xp1, xp2, xl, xh, vac, vac);
+            D += flux_diff<LIM, false>(ym2, ym1, w2, yp1, yp2, yl, yh, vac, vac);
+        }
         const long long off = k * kstride;
-        const double base = (I_base == I_in) ? w2 : I_base[col * p.pitch + s + off];
-        const bool band_k = (k < p.zlo[2] || k >= p.n3 - p.zhi[2]);
-        out[off] = band_k ? 0.0 : (n0n0 * base - dt * D) * inv_n0n0;          // Eq 18 (O5)
-        w0 = w1; w1 = w2; w2 = w3; w3 = w4;
+        const double base = (I_base == I_in) ? w2 : I_base[pos0 + off];
+        out[off] = (k < zlo || k >= zhi) ? 0.0 : base - D;          // Eq 18 (O5), dt/(n^0 n_0 sqrt(-g) dx) folded in
+        w2 = w3; w3 = w4; sk = sk1;
     }
 }
 
@@ -267,32 +361,38 @@ __global__ void k_angular(KParams p, const double *__restrict__ I_in, double *I_
 }  // namespace
 
 // ---- launchers ---------------------------------------------------------------------------------------------------
-cudaError_t launch_facecoef(const KParams &p, const double *T, double dt, double *fcoef[3], cudaStream_t st, long long *launches) {
+cudaError_t launch_facecoef(const KParams &p, const double *T, double dt, double *fcoef[3], unsigned char *cflag, cudaStream_t st,
+                            long long *launches) {
     for (int a = 0; a < 3; ++a) {
         long long nf = (long long)(p.n1 + (a == 0)) * (p.n2 + (a == 1)) * (p.n3 + (a == 2));
         k_facecoef<<<(unsigned)((nf + 255) / 256), 256, 0, st>>>(p, T, dt, a, reinterpret_cast<double4 *>(fcoef[a]));
         ++*launches;
     }
+    k_cellflag<<<(unsigned)((p.ncell + 255) / 256), 256, 0, st>>>(p, reinterpret_cast<const double4 *>(fcoef[0]),
+                                                                  reinterpret_cast<const double4 *>(fcoef[1]),
+                                                                  reinterpret_cast<const double4 *>(fcoef[2]), cflag);
+    ++*launches;
     return cudaGetLastError();
 }
 
 template <int LIM>
 static void launch_transport_lim(const KParams &p, const double *I_in, const double *I_base, double *I_out,
-                                 double *const fcoef[3], bool matter, double dt, cudaStream_t st) {
+                                 double *const fcoef[3], const unsigned char *cflag, bool matter, double dt, cudaStream_t st) {
     dim3 grid((p.n1 * p.pitch + 255) / 256, p.n2);
     const double4 *f0 = reinterpret_cast<const double4 *>(fcoef[0]), *f1 = reinterpret_cast<const double4 *>(fcoef[1]),
                   *f2 = reinterpret_cast<const double4 *>(fcoef[2]);
-    if (matter) k_transport<LIM, true><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, dt);
-    else k_transport<LIM, false><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, dt);
+    if (matter) k_transport<LIM, true><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, dt);
+    else k_transport<LIM, false><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, dt);
 }
 
 cudaError_t launch_transport(const KParams &p, const double *I_in, const double *I_base, double *I_out,
-                             double *const fcoef[3], bool matter, double dt, cudaStream_t st, long long *launches) {
+                             double *const fcoef[3], const unsigned char *cflag, bool matter, double dt, cudaStream_t st,
+                             long long *launches) {
     switch (p.limiter) {
-        case RT_LIM_MC: launch_transport_lim<RT_LIM_MC>(p, I_in, I_base, I_out, fcoef, matter, dt, st); break;
-        case RT_LIM_MINMOD: launch_transport_lim<RT_LIM_MINMOD>(p, I_in, I_base, I_out, fcoef, matter, dt, st); break;
-        case RT_LIM_NONE: launch_transport_lim<RT_LIM_NONE>(p, I_in, I_base, I_out, fcoef, matter, dt, st); break;
-        default: launch_transport_lim<RT_LIM_VANLEER>(p, I_in, I_base, I_out, fcoef, matter, dt, st); break;
+        case RT_LIM_MC: launch_transport_lim<RT_LIM_MC>(p, I_in, I_base, I_out, fcoef, cflag, matter, dt, st); break;
+        case RT_LIM_MINMOD: launch_transport_lim<RT_LIM_MINMOD>(p, I_in, I_base, I_out, fcoef, cflag, matter, dt, st); break;
+        case RT_LIM_NONE: launch_transport_lim<RT_LIM_NONE>(p, I_in, I_base, I_out, fcoef, cflag, matter, dt, st); break;
+        default: launch_transport_lim<RT_LIM_VANLEER>(p, I_in, I_base, I_out, fcoef, cflag, matter, dt, st); break;
     }
     ++*launches;
     return cudaGetLastError();
