@@ -24,6 +24,8 @@ struct rt_ctx {
     DeviceTables tab;
     double *d_rho, *d_u4, *d_T, *d_Th, *d_Ih, *d_fcoef[3];
     unsigned char *d_cflag;   // per cell: any non-vacuum face
+    unsigned char *d_cls;     // per (column, s): dead / general class (k_classify)
+    unsigned char *d_colflag; // per column: bit 0 has such a cell, bit 1 has an all-vacuum cell
     KParams kp;
     long long launches;
     bool profiling;
@@ -203,7 +205,10 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     c->d_rho = c->d_u4 = c->d_T = c->d_Th = c->d_Ih = nullptr;
     c->d_fcoef[0] = c->d_fcoef[1] = c->d_fcoef[2] = nullptr;
     c->d_cflag = nullptr;
+    c->d_colflag = nullptr; c->d_cls = nullptr;
+    if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_cls, (size_t)ncol * pitch);
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_cflag, c->ncell);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_colflag, (size_t)c->ncol * (2 + n3 / 8));   // column flags + x3-chunk flags (GEN_KC = 8)
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_rho, c->ncell * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_u4, 4 * c->ncell * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_T, c->ncell * sizeof(double));
@@ -229,6 +234,10 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     k.a_rad = opt->a_rad; k.Y_over_rho = opt->Y_over_rho; k.abar = opt->abar;
     k.cen = t.cen; k.ecen = t.ecen; k.angcoef = t.angcoef; k.nhat = t.nhat; k.w = t.w; k.nb = t.nb;
     k.rho = c->d_rho; k.u4 = c->d_u4;
+    k.cls = c->d_cls;
+    e = launch_classify(k, c->d_cls, 0);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) { g_last_cuda = (int)e; rt_free(c); return RT_ECUDA; }
     *out = c;
     return RT_OK;
 }
@@ -237,7 +246,7 @@ extern "C" int rt_free(rt_ctx *c) {
     if (!c) return RT_EINVAL;
     for (int a = 0; a < 3; ++a) { cudaFree(c->tab.face[a]); cudaFree(c->d_fcoef[a]); }
     cudaFree(c->tab.cen); cudaFree(c->tab.ecen); cudaFree(c->tab.angcoef); cudaFree(c->tab.nhat); cudaFree(c->tab.w);
-    cudaFree(c->tab.nb); cudaFree(c->d_cflag); cudaFree(c->d_rho); cudaFree(c->d_u4); cudaFree(c->d_T); cudaFree(c->d_Th); cudaFree(c->d_Ih);
+    cudaFree(c->tab.nb); cudaFree(c->d_cflag); cudaFree(c->d_colflag); cudaFree(c->d_cls); cudaFree(c->d_rho); cudaFree(c->d_u4); cudaFree(c->d_T); cudaFree(c->d_Th); cudaFree(c->d_Ih);
     delete c;
     return RT_OK;
 }
@@ -388,8 +397,8 @@ extern "C" int rt_transport(rt_ctx *c, const double *I_in, const double *I_base,
     if (!c || !I_in || !I_base || !I_out || I_in == I_out) return RT_EINVAL;
     if (fixed_bc_missing(c) || (c->matter && !c->fluid_set)) return RT_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
-    if (c->matter) { ProfScope ps(c, RT_K_FACECOEF, st); CK(launch_facecoef(c->kp, c->d_T, dt, c->d_fcoef, c->d_cflag, st, &c->launches)); }
-    { ProfScope ps(c, RT_K_TRANSPORT, st); CK(launch_transport(c->kp, I_in, I_base, I_out, c->d_fcoef, c->d_cflag, c->matter, dt, st, &c->launches)); }
+    if (c->matter) { ProfScope ps(c, RT_K_FACECOEF, st); CK(launch_facecoef(c->kp, c->d_T, dt, c->d_fcoef, c->d_cflag, c->d_colflag, st, &c->launches)); }
+    { ProfScope ps(c, RT_K_TRANSPORT, st); CK(launch_transport(c->kp, I_in, I_base, I_out, c->d_fcoef, c->d_cflag, c->d_colflag, c->matter, dt, st, &c->launches)); }
     return RT_OK;
 }
 
@@ -418,8 +427,8 @@ extern "C" int rt_moments(rt_ctx *c, const double *I, double *R, void *stream) {
 // then O6 on (I*, T) with T_- = T_base
 static int stage(rt_ctx *c, const double *I_flux, const double *T_flux, const double *I_base, double *I_out, double *T_io,
                  double delta, int *n_fail, double *R, double *G, cudaStream_t st) {
-    if (c->matter) { ProfScope ps(c, RT_K_FACECOEF, st); CK(launch_facecoef(c->kp, T_flux, delta, c->d_fcoef, c->d_cflag, st, &c->launches)); }
-    { ProfScope ps(c, RT_K_TRANSPORT, st); CK(launch_transport(c->kp, I_flux, I_base, I_out, c->d_fcoef, c->d_cflag, c->matter, delta, st, &c->launches)); }
+    if (c->matter) { ProfScope ps(c, RT_K_FACECOEF, st); CK(launch_facecoef(c->kp, T_flux, delta, c->d_fcoef, c->d_cflag, c->d_colflag, st, &c->launches)); }
+    { ProfScope ps(c, RT_K_TRANSPORT, st); CK(launch_transport(c->kp, I_flux, I_base, I_out, c->d_fcoef, c->d_cflag, c->d_colflag, c->matter, delta, st, &c->launches)); }
     if (c->curved) { ProfScope ps(c, RT_K_ANGULAR, st); CK(launch_angular(c->kp, I_flux, I_out, delta, st, &c->launches)); }
     if (c->opt.source_method != 0 || R || G) {
         ProfScope ps(c, RT_K_SOURCE, st);

@@ -28,16 +28,18 @@ struct KParams {
     const double *nhat;
     const double *w;
     const int *nb;
+    const unsigned char *cls;   // [ncol][pitch] class byte (k_classify)
     const double *ghost[3][2];
     const double *rho, *u4;  // library-owned fluid copies
 };
 
 // launchers (rt_transport.cu, rt_source.cu); every launch increments *launches
-cudaError_t launch_facecoef(const KParams &p, const double *T, double dt, double *fcoef[3], unsigned char *cflag, cudaStream_t st,
-                            long long *launches);
+cudaError_t launch_facecoef(const KParams &p, const double *T, double dt, double *fcoef[3], unsigned char *cflag, unsigned char *colflag,
+                            cudaStream_t st, long long *launches);
 cudaError_t launch_transport(const KParams &p, const double *I_in, const double *I_base, double *I_out,
-                             double *const fcoef[3], const unsigned char *cflag, bool matter, double dt, cudaStream_t st,
-                             long long *launches);
+                             double *const fcoef[3], const unsigned char *cflag, const unsigned char *colflag, bool matter,
+                             double dt, cudaStream_t st, long long *launches);
+cudaError_t launch_classify(const KParams &p, unsigned char *cls, cudaStream_t st);
 cudaError_t launch_angular(const KParams &p, const double *I_in, double *I_io, double dt, cudaStream_t st, long long *launches);
 // source step; if R_after != nullptr also writes moments after the update; if G != nullptr writes
 // G_nu = -(R^0_nu after - before)/dt.

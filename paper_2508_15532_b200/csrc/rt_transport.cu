@@ -132,8 +132,12 @@ __device__ __forceinline__ bool sign_differs(double a, double b) {
 // Monotonised-central slope, same value as minmod3(2 dm, (dm+dp)/2, 2 dp) bit for bit, with 5 fp64-pipe operations:
 // equal signs => sign * min(2 min(|dm|,|dp|), |dm+dp|/2); opposite signs or a zero difference => 0.
 __device__ __forceinline__ double slope_mc(double dm, double dp) {
-    const double m2 = 2.0 * fmin(fabs(dm), fabs(dp));
-    const double r = fmin(m2, 0.5 * fabs(dm + dp));
+    // plain compares + selects (DSETP + SEL); fmin() would add its NaN-propagation sequence to every call
+    const double a = fabs(dm), b = fabs(dp);
+    const double mn = (a < b) ? a : b;
+    const double m2 = mn + mn;
+    const double c = 0.5 * fabs(dm + dp);
+    const double r = (m2 < c) ? m2 : c;
     const bool opp = (__double2hiint(dm) ^ __double2hiint(dp)) < 0;
     return opp ? 0.0 : copysign(r, dm);
 }
@@ -196,123 +200,240 @@ __device__ __forceinline__ int nb_index(int c, int N, int bc_lo, int bc_hi) {
     return -1;
 }
 
+// column flags: bit 0 = the column has a cell with a non-vacuum face, bit 1 = it has an all-vacuum cell
+// colflag[ncol + kc * ncol + col]: the x3 chunk [kc*GEN_KC, (kc+1)*GEN_KC) of the column has such a cell
+constexpr int GEN_KC = 8;
+__global__ void k_colflag(KParams p, const unsigned char *__restrict__ cflag, unsigned char *__restrict__ colflag) {
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= p.ncol) return;
+    int m = 0, mc = 0;
+    for (int k = 0; k < p.n3; ++k) {
+        const int f = cflag[(long long)k * p.ncol + col];
+        m |= f ? 1 : 2;
+        mc |= f;
+        if ((k + 1) % GEN_KC == 0 || k + 1 == p.n3) {
+            colflag[p.ncol + (long long)(k / GEN_KC) * p.ncol + col] = (unsigned char)mc;
+            mc = 0;
+        }
+    }
+    colflag[col] = (unsigned char)m;
+}
+
 // ---- spatial transport ------------------------------------------------------------------------------------------
-// One thread = one (column, s); marches x3.  Per step: 1 new x3 value + 8 transverse neighbours (coalesced), one
-// x3 slope and one x3 flux (the lower x3 flux and slope are carried), 3 slopes + 2 fluxes per transverse dim.
-template <int LIM, bool MATTER>
-__global__ void __launch_bounds__(256, 2)
-k_transport(const __grid_constant__ KParams p, const double *__restrict__ I_in, const double *I_base, double *I_out,
-            const double4 *__restrict__ fc0, const double4 *__restrict__ fc1, const double4 *__restrict__ fc2,
-            const unsigned char *__restrict__ cflag, double dt) {
+// One thread = one (column, s); marches x3.  The work is split over two kernels that write disjoint (cell, s) sets:
+//   k_transport_vac  all-vacuum cells (Eq 20 on all six faces) of threads whose n^a has one sign across the cell:
+//                    lean upwind path, carried x3 flux, software-pipelined loads;
+//   k_transport_gen  everything else: cells with a non-vacuum (Eq 23) face, threads with a sign change of n^a
+//                    inside the cell, threads next to a ZERO / FIXED boundary.
+struct ColSetup {
+    int i, j, s, col;
+    bool dead, special, general;
+    FaceK xl, xh, yl, yh, zf;
+    int oxm2, oxm1, oxp1, oxp2, oym2, oym1, oyp1, oyp2;
+};
+__device__ __forceinline__ bool col_setup(const KParams &p, double dt, ColSetup &c) {
     const int e = blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= p.n1 * p.pitch) return;
-    const int i = e / p.pitch, s = e - i * p.pitch, j = blockIdx.y;
-    const int col = j * p.n1 + i;
-    const long long kstride = (long long)p.ncol * p.pitch;
-    const long long pos0 = (long long)col * p.pitch + s;
-    double *out = I_out + pos0;
-    bool dead = s >= p.nd;   // pad lanes: keep the pad zero
-    double nx = 0, ny = 0, nz = 0, n0c = 0, scale = 0;
-    const double *cen = p.cen + (long long)col * CEN_STRIDE;
-    if (!dead) {
-        nx = __ldg(p.nhat + s); ny = __ldg(p.nhat + p.pitch + s); nz = __ldg(p.nhat + 2 * p.pitch + s);
-        n0c = centre_n0(cen, nx, ny, nz);
-        const double nup = cen[4] + cen[5] * nx + cen[6] * ny + cen[7] * nz;
-        scale = dt * cen[8] / (nup * n0c);
-        const bool band_ij = (i < p.zlo[0] || i >= p.n1 - p.zhi[0] || j < p.zlo[1] || j >= p.n2 - p.zhi[1]);
-        dead = band_ij || n0c > -p.n0_floor;   // masked direction (S14) or zero band (L709): stays zero, no work
-    }
-    if (dead) {
-        for (int k = 0; k < p.n3; ++k) out[k * kstride] = 0.0;
-        return;
-    }
+    if (e >= p.n1 * p.pitch) return false;
+    const int i = c.i = e / p.pitch, s = c.s = e - c.i * p.pitch, j = c.j = blockIdx.y;
+    c.col = j * p.n1 + i;
+    c.dead = s >= p.nd;   // pad lanes: keep the pad zero
+    c.special = c.general = false;
+    if (c.dead) return true;
+    const double nx = __ldg(p.nhat + s), ny = __ldg(p.nhat + p.pitch + s), nz = __ldg(p.nhat + 2 * p.pitch + s);
+    const double *cen = p.cen + (long long)c.col * CEN_STRIDE;
+    const double n0c = centre_n0(cen, nx, ny, nz);
+    const double nup = cen[4] + cen[5] * nx + cen[6] * ny + cen[7] * nz;
+    const double scale = dt * cen[8] / (nup * n0c);
+    const bool band_ij = (i < p.zlo[0] || i >= p.n1 - p.zhi[0] || j < p.zlo[1] || j >= p.n2 - p.zhi[1]);
+    c.dead = band_ij || n0c > -p.n0_floor;   // masked direction (S14) or zero band (L709): stays zero, no work
+    if (c.dead) return true;
     // transverse neighbours: element offsets inside the x3-plane, resolved once (periodic / outflow map to interior
     // cells); a ZERO / FIXED ghost makes the thread use the generic loader
     const int im2 = nb_index(i - 2, p.n1, p.bc_lo[0], p.bc_hi[0]), im1 = nb_index(i - 1, p.n1, p.bc_lo[0], p.bc_hi[0]);
     const int ip1 = nb_index(i + 1, p.n1, p.bc_lo[0], p.bc_hi[0]), ip2 = nb_index(i + 2, p.n1, p.bc_lo[0], p.bc_hi[0]);
     const int jm2 = nb_index(j - 2, p.n2, p.bc_lo[1], p.bc_hi[1]), jm1 = nb_index(j - 1, p.n2, p.bc_lo[1], p.bc_hi[1]);
     const int jp1 = nb_index(j + 1, p.n2, p.bc_lo[1], p.bc_hi[1]), jp2 = nb_index(j + 2, p.n2, p.bc_lo[1], p.bc_hi[1]);
-    const bool special = (im2 | im1 | ip1 | ip2 | jm2 | jm1 | jp1 | jp2) < 0;
+    c.special = (im2 | im1 | ip1 | ip2 | jm2 | jm1 | jp1 | jp2) < 0;
     const int rowp = p.n1 * p.pitch;
-    const int oxm2 = (im2 - i) * p.pitch, oxm1 = (im1 - i) * p.pitch, oxp1 = (ip1 - i) * p.pitch, oxp2 = (ip2 - i) * p.pitch;
-    const int oym2 = (jm2 - j) * rowp, oym1 = (jm1 - j) * rowp, oyp1 = (jp1 - j) * rowp, oyp2 = (jp2 - j) * rowp;
-
+    c.oxm2 = (im2 - i) * p.pitch; c.oxm1 = (im1 - i) * p.pitch; c.oxp1 = (ip1 - i) * p.pitch; c.oxp2 = (ip2 - i) * p.pitch;
+    c.oym2 = (jm2 - j) * rowp; c.oym1 = (jm1 - j) * rowp; c.oyp1 = (jp1 - j) * rowp; c.oyp2 = (jp2 - j) * rowp;
     // face coefficients, formed once per column (geometry is x3-independent); n_0 gate (L280) applied here
-    FaceK xl, xh, yl, yh, zf;
+    const double sx = scale * p.inv_dx[0], sy = scale * p.inv_dx[1], sz = scale * p.inv_dx[2];
+    FaceC f;
+    int in;
+    f = face_coef(p.face[0] + ((long long)j * (p.n1 + 1) + i) * FACE_STRIDE, nx, ny, nz);
+    in = (i > 0) ? i - 1 : (p.bc_lo[0] == RT_BC_PERIODIC ? p.n1 - 1 : -1);
+    if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)j * p.n1 + in) * CEN_STRIDE, nx, ny, nz))) f.Q = 0.0;
+    c.xl = fold(f, sx);
+    f = face_coef(p.face[0] + ((long long)j * (p.n1 + 1) + i + 1) * FACE_STRIDE, nx, ny, nz);
+    in = (i < p.n1 - 1) ? i + 1 : (p.bc_hi[0] == RT_BC_PERIODIC ? 0 : -1);
+    if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)j * p.n1 + in) * CEN_STRIDE, nx, ny, nz))) f.Q = 0.0;
+    c.xh = fold(f, sx);
+    f = face_coef(p.face[1] + ((long long)j * p.n1 + i) * FACE_STRIDE, nx, ny, nz);
+    in = (j > 0) ? j - 1 : (p.bc_lo[1] == RT_BC_PERIODIC ? p.n2 - 1 : -1);
+    if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)in * p.n1 + i) * CEN_STRIDE, nx, ny, nz))) f.Q = 0.0;
+    c.yl = fold(f, sy);
+    f = face_coef(p.face[1] + ((long long)(j + 1) * p.n1 + i) * FACE_STRIDE, nx, ny, nz);
+    in = (j < p.n2 - 1) ? j + 1 : (p.bc_hi[1] == RT_BC_PERIODIC ? 0 : -1);
+    if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)in * p.n1 + i) * CEN_STRIDE, nx, ny, nz))) f.Q = 0.0;
+    c.yh = fold(f, sy);
+    c.zf = fold(face_coef(p.face[2] + (long long)c.col * FACE_STRIDE, nx, ny, nz), sz);
+    c.general = c.special || (c.xl.pos != c.xh.pos) || (c.yl.pos != c.yh.pos);
+    return true;
+}
+
+// Per-(column, s) class byte, computed once at rt_init: bit 0 = dead (pad lane, masked direction, zero band in x1/x2),
+// bit 1 = general (sign change of n^a inside the cell, or next to a ZERO / FIXED boundary).  Both transport kernels
+// read it, so they always agree on which of them owns a thread.
+__global__ void k_classify(const __grid_constant__ KParams p, unsigned char *__restrict__ cls) {
+    ColSetup c;
+    if (!col_setup(p, 1.0, c)) return;
+    cls[(long long)c.col * p.pitch + c.s] = (unsigned char)((c.dead ? 1 : 0) | (c.general ? 2 : 0));
+}
+
+// Upwind path for vacuum faces (Eq 20): the flux only needs the UPWIND PLI state, and the upwind side of a face is a
+// per-thread constant (the sign of n^a_f).  With (a, b, c, d) = four cells of a dim ordered along the propagation
+// direction (c = this cell) the flux difference is K_bc S_bc + K_cd S_cd, S_bc = b + slope(b-a, c-b)/2,
+// S_cd = c + slope(c-b, d-c)/2: 3 loads and 2 slopes per transverse dim; x3: 1 load, 1 slope, the lower flux carried.
+template <int LIM, bool MATTER>
+__global__ void __launch_bounds__(256, 3)
+k_transport_vac(const __grid_constant__ KParams p, const double *__restrict__ I_in, const double *I_base, double *I_out,
+                const unsigned char *__restrict__ cflag, const unsigned char *__restrict__ colflag, double dt) {
+    const int e0 = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e0 >= p.n1 * p.pitch) return;
+    const long long kstride = (long long)p.ncol * p.pitch;
+    const int n3 = p.n3, ncol = p.ncol;
     {
-        const double sx = scale * p.inv_dx[0], sy = scale * p.inv_dx[1], sz = scale * p.inv_dx[2];
-        FaceC c;
-        int in;
-        c = face_coef(p.face[0] + ((long long)j * (p.n1 + 1) + i) * FACE_STRIDE, nx, ny, nz);
-        in = (i > 0) ? i - 1 : (p.bc_lo[0] == RT_BC_PERIODIC ? p.n1 - 1 : -1);
-        if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)j * p.n1 + in) * CEN_STRIDE, nx, ny, nz))) c.Q = 0.0;
-        xl = fold(c, sx);
-        c = face_coef(p.face[0] + ((long long)j * (p.n1 + 1) + i + 1) * FACE_STRIDE, nx, ny, nz);
-        in = (i < p.n1 - 1) ? i + 1 : (p.bc_hi[0] == RT_BC_PERIODIC ? 0 : -1);
-        if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)j * p.n1 + in) * CEN_STRIDE, nx, ny, nz))) c.Q = 0.0;
-        xh = fold(c, sx);
-        c = face_coef(p.face[1] + ((long long)j * p.n1 + i) * FACE_STRIDE, nx, ny, nz);
-        in = (j > 0) ? j - 1 : (p.bc_lo[1] == RT_BC_PERIODIC ? p.n2 - 1 : -1);
-        if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)in * p.n1 + i) * CEN_STRIDE, nx, ny, nz))) c.Q = 0.0;
-        yl = fold(c, sy);
-        c = face_coef(p.face[1] + ((long long)(j + 1) * p.n1 + i) * FACE_STRIDE, nx, ny, nz);
-        in = (j < p.n2 - 1) ? j + 1 : (p.bc_hi[1] == RT_BC_PERIODIC ? 0 : -1);
-        if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)in * p.n1 + i) * CEN_STRIDE, nx, ny, nz))) c.Q = 0.0;
-        yh = fold(c, sy);
-        zf = fold(face_coef(p.face[2] + (long long)col * FACE_STRIDE, nx, ny, nz), sz);
+        const long long q = (long long)blockIdx.y * p.n1 * p.pitch + e0;
+        const int cl = p.cls[q];
+        if (cl & 1) {   // dead: this kernel keeps those entries zero
+            for (int k = 0; k < n3; ++k) I_out[q + k * kstride] = 0.0;
+            return;
+        }
+        if (cl & 2) return;
+        if (MATTER && !(colflag[blockIdx.y * p.n1 + e0 / p.pitch] & 2)) return;
     }
+    ColSetup c;
+    col_setup(p, dt, c);
+    const long long pos0 = (long long)c.col * p.pitch + c.s;
+    double *out = I_out + pos0;
+    const int i = c.i, j = c.j, s = c.s;
+    const bool xpos = c.xl.pos, ypos = c.yl.pos, zpos = c.zf.pos;
+    const int oxa = xpos ? c.oxm2 : c.oxp2, oxb = xpos ? c.oxm1 : c.oxp1, oxd = xpos ? c.oxp1 : c.oxm1;
+    const int oya = ypos ? c.oym2 : c.oyp2, oyb = ypos ? c.oym1 : c.oyp1, oyd = ypos ? c.oyp1 : c.oym1;
+    const double Kxbc = xpos ? -c.xl.A : c.xh.A, Kxcd = xpos ? c.xh.A : -c.xl.A;
+    const double Kybc = ypos ? -c.yl.A : c.yh.A, Kycd = ypos ? c.yh.A : -c.yl.A;
+    const double zA = c.zf.A, zhalf = zpos ? 0.5 : -0.5;
+    const double *pk = I_in + pos0;
+    auto ldk = [&](int kk) -> double {
+        return (kk >= 0 && kk < n3) ? __ldg(pk + kk * kstride) : slow_ld(p, I_in, 2, i, j, kk, s);
+    };
+    double w1 = ldk(-1), w2 = ldk(0), w3 = ldk(1), Flo;
+    {
+        const double w0 = ldk(-2);
+        const double sg = slope_k<LIM>(w2 - w1, zpos ? (w1 - w0) : (w3 - w2));
+        Flo = zA * fma(zhalf, sg, zpos ? w1 : w2);
+    }
+    const double *pb = I_base + pos0;
+    const bool same_base = (I_base == I_in);
+    const unsigned char *pflag = cflag + c.col;
+    const int zlo = p.zlo[2], zhi = n3 - p.zhi[2];
+    double qxa = __ldg(pk + oxa), qxb = __ldg(pk + oxb), qxd = __ldg(pk + oxd);
+    double qya = __ldg(pk + oya), qyb = __ldg(pk + oyb), qyd = __ldg(pk + oyd);
+    double qw4 = ldk(2);
+    unsigned char qflag = MATTER ? *pflag : 0;
+    for (int k = 0; k < n3; ++k) {
+        const double xa = qxa, xb = qxb, xd = qxd, ya = qya, yb = qyb, yd = qyd, w4 = qw4;
+        const bool mat = MATTER && qflag != 0;
+        if (k + 1 < n3) {   // request the operands of step k + 1 before computing step k
+            const double *pn = pk + kstride;
+            qxa = __ldg(pn + oxa); qxb = __ldg(pn + oxb); qxd = __ldg(pn + oxd);
+            qya = __ldg(pn + oya); qyb = __ldg(pn + oyb); qyd = __ldg(pn + oyd);
+            qw4 = (k + 3 < n3) ? __ldg(pn + 2 * kstride) : slow_ld(p, I_in, 2, i, j, k + 3, s);
+            if (MATTER) qflag = pflag[ncol];
+        }
+        // x3: upwind state at the upper face (always formed: it is the next cell's lower flux if that cell is vacuum)
+        const double sz = slope_k<LIM>(w3 - w2, zpos ? (w2 - w1) : (w4 - w3));
+        const double Fhi = zA * fma(zhalf, sz, zpos ? w2 : w3);
+        if (!mat) {
+            double D = Fhi - Flo;
+            {
+                const double d1 = xb - xa, d2 = w2 - xb, d3 = xd - w2;
+                D = fma(Kxbc, fma(0.5, slope_k<LIM>(d1, d2), xb), D);
+                D = fma(Kxcd, fma(0.5, slope_k<LIM>(d2, d3), w2), D);
+            }
+            {
+                const double d1 = yb - ya, d2 = w2 - yb, d3 = yd - w2;
+                D = fma(Kybc, fma(0.5, slope_k<LIM>(d1, d2), yb), D);
+                D = fma(Kycd, fma(0.5, slope_k<LIM>(d2, d3), w2), D);
+            }
+            const double base = same_base ? w2 : *pb;
+            *out = (k < zlo || k >= zhi) ? 0.0 : base - D;      // Eq 18 (O5), dt/(n^0 n_0 sqrt(-g) dx) folded in
+        }
+        Flo = Fhi;
+        w1 = w2; w2 = w3; w3 = w4;
+        pk += kstride; pb += kstride; out += kstride;
+        if (MATTER) pflag += ncol;
+    }
+}
+
+// General path: full 5-point stencils, both PLI states at all six faces, Eq 20 or Eq 23 per face.
+template <int LIM, bool MATTER>
+__global__ void __launch_bounds__(256, 2)
+k_transport_gen(const __grid_constant__ KParams p, const double *__restrict__ I_in, const double *I_base, double *I_out,
+                const double4 *__restrict__ fc0, const double4 *__restrict__ fc1, const double4 *__restrict__ fc2,
+                const unsigned char *__restrict__ cflag, const unsigned char *__restrict__ colflag, double dt) {
+    const int e0 = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e0 >= p.n1 * p.pitch) return;
+    const int kc = blockIdx.z;
+    {
+        const int cl = p.cls[(long long)blockIdx.y * p.n1 * p.pitch + e0];
+        if (cl & 1) return;
+        if (!(cl & 2) && !(MATTER && colflag[p.ncol + (long long)kc * p.ncol + blockIdx.y * p.n1 + e0 / p.pitch])) return;
+    }
+    ColSetup c;
+    col_setup(p, dt, c);
+    c.general = (p.cls[(long long)c.col * p.pitch + c.s] & 2) != 0;
+    const int i = c.i, j = c.j, s = c.s, n3 = p.n3;
+    const int k0 = kc * GEN_KC, k1 = min(n3, k0 + GEN_KC);
+    const long long kstride = (long long)p.ncol * p.pitch;
+    const long long pos0 = (long long)c.col * p.pitch + s;
     const double *pin = I_in + pos0;
     const double4 vac = make_double4(0.5, -1.0, 0.0, 0.0);
-    auto ldk = [&](int kk) -> double {   // x3 neighbour with boundary conditions
-        return (kk >= 0 && kk < p.n3) ? __ldg(pin + kk * kstride) : slow_ld(p, I_in, 2, i, j, kk, s);
+    auto ldk = [&](int kk) -> double {
+        return (kk >= 0 && kk < n3) ? __ldg(pin + kk * kstride) : slow_ld(p, I_in, 2, i, j, kk, s);
     };
-    // prologue of the x3 march: carried state = (w2, w3) = I at (k, k+1), slope at k, lower x3 flux
-    double w2, w3, sk, Flo;
-    {
-        const double w0 = ldk(-2), w1 = ldk(-1);
-        w2 = ldk(0); w3 = ldk(1);
-        const double sm = slope_k<LIM>(w1 - w0, w2 - w1);
-        sk = slope_k<LIM>(w2 - w1, w3 - w2);
-        const double4 f = MATTER ? ld4(fc2 + col) : vac;
-        Flo = face_flux<MATTER>(zf, w1 + 0.5 * sm, w2 - 0.5 * sk, w1, w2, f);
-    }
-    const int zlo = p.zlo[2], zhi = p.n3 - p.zhi[2];
-    for (int k = 0; k < p.n3; ++k) {
-        const double w4 = ldk(k + 2);
+    const int zlo = p.zlo[2], zhi = n3 - p.zhi[2];
+    for (int k = k0; k < k1; ++k) {
+        const long long cell = (long long)k * p.ncol + c.col;
+        const bool mat = MATTER && cflag[cell] != 0;
+        if (!mat && !c.general) continue;
         const double *pk = pin + k * kstride;
+        const double w0 = ldk(k - 2), w1 = ldk(k - 1), w2 = __ldg(pk), w3 = ldk(k + 1), w4 = ldk(k + 2);
         double xm2, xm1, xp1, xp2, ym2, ym1, yp1, yp2;
-        if (!special) {
-            xm2 = __ldg(pk + oxm2); xm1 = __ldg(pk + oxm1); xp1 = __ldg(pk + oxp1); xp2 = __ldg(pk + oxp2);
-            ym2 = __ldg(pk + oym2); ym1 = __ldg(pk + oym1); yp1 = __ldg(pk + oyp1); yp2 = __ldg(pk + oyp2);
+        if (!c.special) {
+            xm2 = __ldg(pk + c.oxm2); xm1 = __ldg(pk + c.oxm1); xp1 = __ldg(pk + c.oxp1); xp2 = __ldg(pk + c.oxp2);
+            ym2 = __ldg(pk + c.oym2); ym1 = __ldg(pk + c.oym1); yp1 = __ldg(pk + c.oyp1); yp2 = __ldg(pk + c.oyp2);
         } else {
             xm2 = slow_ld(p, I_in, 0, i - 2, j, k, s); xm1 = slow_ld(p, I_in, 0, i - 1, j, k, s);
             xp1 = slow_ld(p, I_in, 0, i + 1, j, k, s); xp2 = slow_ld(p, I_in, 0, i + 2, j, k, s);
             ym2 = slow_ld(p, I_in, 1, i, j - 2, k, s); ym1 = slow_ld(p, I_in, 1, i, j - 1, k, s);
             yp1 = slow_ld(p, I_in, 1, i, j + 1, k, s); yp2 = slow_ld(p, I_in, 1, i, j + 2, k, s);
         }
-        const long long cell = (long long)k * p.ncol + col;
-        const bool mat = MATTER && cflag[cell] != 0;
-        // x3: one new slope, one new flux
-        const double sk1 = slope_k<LIM>(w3 - w2, w4 - w3);
         double D;
         if (mat) {
-            const double Fhi = face_flux<MATTER>(zf, w2 + 0.5 * sk, w3 - 0.5 * sk1, w2, w3, ld4(fc2 + cell + p.ncol));
-            D = Fhi - Flo;
-            Flo = Fhi;
             const long long fx = ((long long)k * p.n2 + j) * (p.n1 + 1) + i, fy = ((long long)k * (p.n2 + 1) + j) * p.n1 + i;
-            D += flux_diff<LIM, MATTER>(xm2, xm1, w2, xp1, xp2, xl, xh, ld4(fc0 + fx), ld4(fc0 + fx + 1));
-            D += flux_diff<LIM, MATTER>(ym2, ym1, w2, yp1, yp2, yl, yh, ld4(fc1 + fy), ld4(fc1 + fy + p.n1));
+            D = flux_diff<LIM, MATTER>(w0, w1, w2, w3, w4, c.zf, c.zf, ld4(fc2 + cell), ld4(fc2 + cell + p.ncol));
+            D += flux_diff<LIM, MATTER>(xm2, xm1, w2, xp1, xp2, c.xl, c.xh, ld4(fc0 + fx), ld4(fc0 + fx + 1));
+            D += flux_diff<LIM, MATTER>(ym2, ym1, w2, yp1, yp2, c.yl, c.yh, ld4(fc1 + fy), ld4(fc1 + fy + p.n1));
         } else {
-            const double Fhi = face_flux<false>(zf, w2 + 0.5 * sk, w3 - 0.5 * sk1, w2, w3, vac);
-            D = Fhi - Flo;
-            Flo = Fhi;
-            D += flux_diff<LIM, false>(xm2, xm1, w2, xp1, xp2, xl, xh, vac, vac);
-            D += flux_diff<LIM, false>(ym2, ym1, w2, yp1, yp2, yl, yh, vac, vac);
+            D = flux_diff<LIM, false>(w0, w1, w2, w3, w4, c.zf, c.zf, vac, vac);
+            D += flux_diff<LIM, false>(xm2, xm1, w2, xp1, xp2, c.xl, c.xh, vac, vac);
+            D += flux_diff<LIM, false>(ym2, ym1, w2, yp1, yp2, c.yl, c.yh, vac, vac);
         }
         const long long off = k * kstride;
         const double base = (I_base == I_in) ? w2 : I_base[pos0 + off];
-        out[off] = (k < zlo || k >= zhi) ? 0.0 : base - D;          // Eq 18 (O5), dt/(n^0 n_0 sqrt(-g) dx) folded in
-        w2 = w3; w3 = w4; sk = sk1;
+        I_out[pos0 + off] = (k < zlo || k >= zhi) ? 0.0 : base - D;
     }
 }
 
@@ -340,29 +461,40 @@ __global__ void k_angular(KParams p, const double *__restrict__ I_in, double *I_
         for (int e = 0; e < 6; ++e) nb[e] = p.nb[e * p.pitch + s];
     }
     const long long kstride = (long long)p.n1 * p.n2 * p.pitch;
+    const bool inrow = s < p.pitch;
+    const double *pin = I_in + (long long)col * p.pitch + s;
+    double *pio = I_io + (long long)col * p.pitch + s;
+    // software pipeline over x3: the operands of step k+1 are requested before step k is computed; the staged cell is
+    // double-buffered in shared memory so that one barrier per step suffices
+    double v = inrow ? __ldg(pin) : 0.0, io = (live && !zero) ? *pio : 0.0;
     for (int k = 0; k < p.n3; ++k) {
-        const long long off = (long long)col * p.pitch + s + k * kstride;
-        double v = 0.0;
-        if (s < p.pitch) { v = I_in[off]; sI[s] = v; }
+        double *buf = sI + (k & 1) * p.pitch;
+        if (inrow) buf[s] = v;
+        double vn = 0.0, ion = 0.0;
+        if (k + 1 < p.n3) {
+            if (inrow) vn = __ldg(pin + kstride);
+            if (live && !zero) ion = pio[kstride];
+        }
         __syncthreads();
         if (live) {
             double D = c[6] * v;
 #pragma unroll
-            for (int e = 0; e < 6; ++e) D += c[e] * sI[nb[e]];
+            for (int e = 0; e < 6; ++e) D += c[e] * buf[nb[e]];
             const bool band_k = (k < p.zlo[2] || k >= p.n3 - p.zhi[2]);
-            I_io[off] = (zero || band_k) ? 0.0 : I_io[off] - scale * D;
-        } else if (s < p.pitch) {
-            I_io[off] = 0.0;
+            *pio = (zero || band_k) ? 0.0 : io - scale * D;
+        } else if (inrow) {
+            *pio = 0.0;
         }
-        __syncthreads();
+        v = vn; io = ion;
+        pin += kstride; pio += kstride;
     }
 }
 
 }  // namespace
 
 // ---- launchers ---------------------------------------------------------------------------------------------------
-cudaError_t launch_facecoef(const KParams &p, const double *T, double dt, double *fcoef[3], unsigned char *cflag, cudaStream_t st,
-                            long long *launches) {
+cudaError_t launch_facecoef(const KParams &p, const double *T, double dt, double *fcoef[3], unsigned char *cflag, unsigned char *colflag,
+                            cudaStream_t st, long long *launches) {
     for (int a = 0; a < 3; ++a) {
         long long nf = (long long)(p.n1 + (a == 0)) * (p.n2 + (a == 1)) * (p.n3 + (a == 2));
         k_facecoef<<<(unsigned)((nf + 255) / 256), 256, 0, st>>>(p, T, dt, a, reinterpret_cast<double4 *>(fcoef[a]));
@@ -371,36 +503,49 @@ cudaError_t launch_facecoef(const KParams &p, const double *T, double dt, double
     k_cellflag<<<(unsigned)((p.ncell + 255) / 256), 256, 0, st>>>(p, reinterpret_cast<const double4 *>(fcoef[0]),
                                                                   reinterpret_cast<const double4 *>(fcoef[1]),
                                                                   reinterpret_cast<const double4 *>(fcoef[2]), cflag);
-    ++*launches;
+    k_colflag<<<(p.ncol + 127) / 128, 128, 0, st>>>(p, cflag, colflag);
+    *launches += 2;
     return cudaGetLastError();
 }
 
 template <int LIM>
 static void launch_transport_lim(const KParams &p, const double *I_in, const double *I_base, double *I_out,
-                                 double *const fcoef[3], const unsigned char *cflag, bool matter, double dt, cudaStream_t st) {
-    dim3 grid((p.n1 * p.pitch + 255) / 256, p.n2);
+                                 double *const fcoef[3], const unsigned char *cflag, const unsigned char *colflag, bool matter,
+                                 double dt, cudaStream_t st) {
+    dim3 grid((p.n1 * p.pitch + 255) / 256, p.n2), ggen(grid.x, grid.y, (p.n3 + GEN_KC - 1) / GEN_KC);
     const double4 *f0 = reinterpret_cast<const double4 *>(fcoef[0]), *f1 = reinterpret_cast<const double4 *>(fcoef[1]),
                   *f2 = reinterpret_cast<const double4 *>(fcoef[2]);
-    if (matter) k_transport<LIM, true><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, dt);
-    else k_transport<LIM, false><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, dt);
+    if (matter) {
+        k_transport_vac<LIM, true><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
+        k_transport_gen<LIM, true><<<ggen, 256, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
+    } else {
+        k_transport_vac<LIM, false><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
+        k_transport_gen<LIM, false><<<ggen, 256, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
+    }
 }
 
 cudaError_t launch_transport(const KParams &p, const double *I_in, const double *I_base, double *I_out,
-                             double *const fcoef[3], const unsigned char *cflag, bool matter, double dt, cudaStream_t st,
-                             long long *launches) {
+                             double *const fcoef[3], const unsigned char *cflag, const unsigned char *colflag, bool matter,
+                             double dt, cudaStream_t st, long long *launches) {
     switch (p.limiter) {
-        case RT_LIM_MC: launch_transport_lim<RT_LIM_MC>(p, I_in, I_base, I_out, fcoef, cflag, matter, dt, st); break;
-        case RT_LIM_MINMOD: launch_transport_lim<RT_LIM_MINMOD>(p, I_in, I_base, I_out, fcoef, cflag, matter, dt, st); break;
-        case RT_LIM_NONE: launch_transport_lim<RT_LIM_NONE>(p, I_in, I_base, I_out, fcoef, cflag, matter, dt, st); break;
-        default: launch_transport_lim<RT_LIM_VANLEER>(p, I_in, I_base, I_out, fcoef, cflag, matter, dt, st); break;
+        case RT_LIM_MC: launch_transport_lim<RT_LIM_MC>(p, I_in, I_base, I_out, fcoef, cflag, colflag, matter, dt, st); break;
+        case RT_LIM_MINMOD: launch_transport_lim<RT_LIM_MINMOD>(p, I_in, I_base, I_out, fcoef, cflag, colflag, matter, dt, st); break;
+        case RT_LIM_NONE: launch_transport_lim<RT_LIM_NONE>(p, I_in, I_base, I_out, fcoef, cflag, colflag, matter, dt, st); break;
+        default: launch_transport_lim<RT_LIM_VANLEER>(p, I_in, I_base, I_out, fcoef, cflag, colflag, matter, dt, st); break;
     }
-    ++*launches;
+    *launches += 2;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_classify(const KParams &p, unsigned char *cls, cudaStream_t st) {
+    dim3 grid((p.n1 * p.pitch + 255) / 256, p.n2);
+    k_classify<<<grid, 256, 0, st>>>(p, cls);
     return cudaGetLastError();
 }
 
 cudaError_t launch_angular(const KParams &p, const double *I_in, double *I_io, double dt, cudaStream_t st, long long *launches) {
     const int threads = ((p.pitch + 31) / 32) * 32;
-    k_angular<<<p.ncol, threads, p.pitch * sizeof(double), st>>>(p, I_in, I_io, dt);
+    k_angular<<<p.ncol, threads, 2 * p.pitch * sizeof(double), st>>>(p, I_in, I_io, dt);
     ++*launches;
     return cudaGetLastError();
 }
