@@ -91,7 +91,7 @@ __device__ __forceinline__ double rotate(const double M[10], const double *__res
 }
 
 template <int MAXV, bool SRC, bool MOM>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 3)
 k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, double *G_out) {
     extern __shared__ double tab[];   // nx[pitch] ny[pitch] nz[pitch] w[pitch]
     for (int t = threadIdx.x; t < 3 * p.pitch; t += blockDim.x) tab[t] = p.nhat[t];
@@ -105,10 +105,19 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
     for (long long cell = warp0; cell < p.ncell; cell += nwarps) {
         const int col = int(cell % p.ncol);
         const double *cen = p.cen + (long long)col * CEN_STRIDE;
-        double alpha = 0.0, aa = 0.0, as = 0.0, rho = 0.0, Tm = 0.0;
+        double *Ic = I + cell * p.pitch;
+        // all independent loads first: the cell's intensities and its fluid state
+        double val[MAXV];
+#pragma unroll
+        for (int v = 0; v < MAXV; ++v) {
+            const int s = lane + 32 * v;
+            val[v] = (s < p.nd) ? Ic[s] : 0.0;
+        }
+        double alpha = 0.0, aa = 0.0, as = 0.0, rho = 0.0, Tm = 0.0, u0 = 1.0, u1 = 0.0, u2 = 0.0, u3 = 0.0;
         if (SRC) {
             rho = p.rho[cell];
             Tm = T[cell];
+            u0 = p.u4[cell]; u1 = p.u4[p.ncell + cell]; u2 = p.u4[2 * p.ncell + cell]; u3 = p.u4[3 * p.ncell + cell];
             if (rho >= p.rho_floor) {
                 aa = (p.kappa_a0 != 0.0) ? p.kappa_a0 * rho * rho * pow(Tm, -3.5) : 0.0;
                 as = p.kappa_s * rho;
@@ -117,43 +126,43 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
         }
         const bool interact = SRC && p.method != 0 && alpha != 0.0;
         if (!interact && !MOM) continue;
-        double uh0 = 1.0, uh1 = 0.0, uh2 = 0.0, uh3 = 0.0;
+        const double *ecen = p.ecen + (long long)col * 16, *L = cen + 28;
+        double Rb = 0.0;          // lanes 0..3: R^0_nu before the source step
+        bool updated = false;
         if (interact) {
-            const double u0 = p.u4[cell], u1 = p.u4[p.ncell + cell], u2 = p.u4[2 * p.ncell + cell], u3 = p.u4[3 * p.ncell + cell];
-            uh0 = cen[12] * u0 + cen[13] * u1 + cen[14] * u2 + cen[15] * u3;
-            uh1 = cen[16] * u0 + cen[17] * u1 + cen[18] * u2 + cen[19] * u3;
-            uh2 = cen[20] * u0 + cen[21] * u1 + cen[22] * u2 + cen[23] * u3;
-            uh3 = cen[24] * u0 + cen[25] * u1 + cen[26] * u2 + cen[27] * u3;
-        }
-        double *Ic = I + cell * p.pitch;
-        double val[MAXV];
-        double E = 0.0, A1 = 0.0, A2 = 0.0;
-        double Mb[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+            const double uh0 = cen[12] * u0 + cen[13] * u1 + cen[14] * u2 + cen[15] * u3;
+            const double uh1 = cen[16] * u0 + cen[17] * u1 + cen[18] * u2 + cen[19] * u3;
+            const double uh2 = cen[20] * u0 + cen[21] * u1 + cen[22] * u2 + cen[23] * u3;
+            const double uh3 = cen[24] * u0 + cen[25] * u1 + cen[26] * u2 + cen[27] * u3;
+            if (MOM && G_out) {   // moments before the update (only where the update can change them)
+                double Mb[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
 #pragma unroll
-        for (int v = 0; v < MAXV; ++v) {
-            const int s = lane + 32 * v;
-            val[v] = 0.0;
-            if (s < p.nd) {
-                const double x = Ic[s];
-                val[v] = x;
-                const double nx = snx[s], ny = sny[s], nz = snz[s], ws = sw[s];
-                if (MOM && G_out) mom_accumulate(Mb, ws * x, nx, ny, nz);
-                if (interact) {
+                for (int v = 0; v < MAXV; ++v) {
+                    const int s = lane + 32 * v;
+                    if (s < p.nd) mom_accumulate(Mb, sw[s] * val[v], snx[s], sny[s], snz[s]);
+                }
+#pragma unroll
+                for (int c = 0; c < 10; ++c) Mb[c] = warp_sum(Mb[c]);
+                if (lane < 4) Rb = rotate(Mb, ecen, L, 0, lane);
+            }
+            double E = 0.0, A1 = 0.0, A2 = 0.0;
+#pragma unroll
+            for (int v = 0; v < MAXV; ++v) {
+                const int s = lane + 32 * v;
+                if (s < p.nd) {
+                    const double nx = snx[s], ny = sny[s], nz = snz[s], ws = sw[s];
                     const double n0c = cen[0] + cen[1] * nx + cen[2] * ny + cen[3] * nz;
                     if (!(n0c > -p.n0_floor)) {
                         const double nup = cen[4] + cen[5] * nx + cen[6] * ny + cen[7] * nz;
                         const double nbar = uh0 - (uh1 * nx + uh2 * ny + uh3 * nz);       // Eq 5, first row
                         const double d = nup + nbar * alpha * dt;
-                        const double IbdOm = nbar * nbar * x * ws;                          // Ibar dOmegabar (S17)
+                        const double IbdOm = nbar * nbar * val[v] * ws;                     // Ibar dOmegabar (S17)
                         E += IbdOm;                                                         // Eq 33
                         A1 += nup / d * IbdOm;                                              // Eq 41a
                         A2 += ws / (nbar * d);                                              // Eq 41b
                     }
                 }
             }
-        }
-        bool updated = false;
-        if (interact) {
             E = warp_sum(E); A1 = warp_sum(A1); A2 = warp_sum(A2) * (dt / FOURPI);
             const double Y = p.Y_over_rho * rho, W = E + Y * Tm, Nbar = p.kappa_a0 * rho * rho;
             TEq q;
@@ -207,19 +216,11 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
             }
 #pragma unroll
             for (int c = 0; c < 10; ++c) Ma[c] = warp_sum(Ma[c]);
-            if (G_out) {
-#pragma unroll
-                for (int c = 0; c < 10; ++c) Mb[c] = warp_sum(Mb[c]);
-            }
-            const double *ecen = p.ecen + (long long)col * 16, *L = cen + 28;
             if (lane < 16) {
                 const int mu = lane >> 2, nu = lane & 3;
                 const double Ra = rotate(Ma, ecen, L, mu, nu);
                 if (R_out) R_out[lane * p.ncell + cell] = Ra;
-                if (G_out && mu == 0) {
-                    const double Rb = updated ? rotate(Mb, ecen, L, 0, nu) : Ra;
-                    G_out[nu * p.ncell + cell] = -(Ra - Rb) / dt;
-                }
+                if (G_out && mu == 0) G_out[nu * p.ncell + cell] = updated ? -(Ra - Rb) / dt : 0.0;
             }
         }
     }

@@ -377,7 +377,9 @@ k_transport_vac(const __grid_constant__ KParams p, const double *__restrict__ I_
     }
 }
 
-// General path: full 5-point stencils, both PLI states at all six faces, Eq 20 or Eq 23 per face.
+// General path: full 5-point stencils, both PLI states at all six faces, Eq 20 or Eq 23 per face.  Marches x3 with a
+// 5-deep register window; computes only the steps it owns (cells with a non-vacuum face, or every cell of a
+// "general" thread).
 template <int LIM, bool MATTER>
 __global__ void __launch_bounds__(256, 2)
 k_transport_gen(const __grid_constant__ KParams p, const double *__restrict__ I_in, const double *I_base, double *I_out,
@@ -385,55 +387,60 @@ k_transport_gen(const __grid_constant__ KParams p, const double *__restrict__ I_
                 const unsigned char *__restrict__ cflag, const unsigned char *__restrict__ colflag, double dt) {
     const int e0 = blockIdx.x * blockDim.x + threadIdx.x;
     if (e0 >= p.n1 * p.pitch) return;
-    const int kc = blockIdx.z;
+    bool general;
     {
         const int cl = p.cls[(long long)blockIdx.y * p.n1 * p.pitch + e0];
         if (cl & 1) return;
-        if (!(cl & 2) && !(MATTER && colflag[p.ncol + (long long)kc * p.ncol + blockIdx.y * p.n1 + e0 / p.pitch])) return;
+        general = (cl & 2) != 0;
+        if (!general && !(MATTER && (colflag[blockIdx.y * p.n1 + e0 / p.pitch] & 1))) return;
     }
     ColSetup c;
     col_setup(p, dt, c);
-    c.general = (p.cls[(long long)c.col * p.pitch + c.s] & 2) != 0;
-    const int i = c.i, j = c.j, s = c.s, n3 = p.n3;
-    const int k0 = kc * GEN_KC, k1 = min(n3, k0 + GEN_KC);
-    const long long kstride = (long long)p.ncol * p.pitch;
+    const int i = c.i, j = c.j, s = c.s, n3 = p.n3, ncol = p.ncol, n1 = p.n1;
+    const long long kstride = (long long)ncol * p.pitch;
     const long long pos0 = (long long)c.col * p.pitch + s;
-    const double *pin = I_in + pos0;
+    const double *pk = I_in + pos0;
     const double4 vac = make_double4(0.5, -1.0, 0.0, 0.0);
     auto ldk = [&](int kk) -> double {
-        return (kk >= 0 && kk < n3) ? __ldg(pin + kk * kstride) : slow_ld(p, I_in, 2, i, j, kk, s);
+        return (kk >= 0 && kk < n3) ? __ldg(pk + kk * kstride) : slow_ld(p, I_in, 2, i, j, kk, s);
     };
+    double w0 = ldk(-2), w1 = ldk(-1), w2 = ldk(0), w3 = ldk(1);
+    const double *pb = I_base + pos0;
+    double *out = I_out + pos0;
+    const bool same_base = (I_base == I_in);
+    const unsigned char *pflag = cflag + c.col;
+    const double4 *px = fc0 + ((long long)j * (n1 + 1) + i), *py = fc1 + ((long long)j * n1 + i), *pz = fc2 + c.col;
+    const int sx = p.n2 * (n1 + 1), sy = (p.n2 + 1) * n1;
     const int zlo = p.zlo[2], zhi = n3 - p.zhi[2];
-    for (int k = k0; k < k1; ++k) {
-        const long long cell = (long long)k * p.ncol + c.col;
-        const bool mat = MATTER && cflag[cell] != 0;
-        if (!mat && !c.general) continue;
-        const double *pk = pin + k * kstride;
-        const double w0 = ldk(k - 2), w1 = ldk(k - 1), w2 = __ldg(pk), w3 = ldk(k + 1), w4 = ldk(k + 2);
-        double xm2, xm1, xp1, xp2, ym2, ym1, yp1, yp2;
-        if (!c.special) {
-            xm2 = __ldg(pk + c.oxm2); xm1 = __ldg(pk + c.oxm1); xp1 = __ldg(pk + c.oxp1); xp2 = __ldg(pk + c.oxp2);
-            ym2 = __ldg(pk + c.oym2); ym1 = __ldg(pk + c.oym1); yp1 = __ldg(pk + c.oyp1); yp2 = __ldg(pk + c.oyp2);
-        } else {
-            xm2 = slow_ld(p, I_in, 0, i - 2, j, k, s); xm1 = slow_ld(p, I_in, 0, i - 1, j, k, s);
-            xp1 = slow_ld(p, I_in, 0, i + 1, j, k, s); xp2 = slow_ld(p, I_in, 0, i + 2, j, k, s);
-            ym2 = slow_ld(p, I_in, 1, i, j - 2, k, s); ym1 = slow_ld(p, I_in, 1, i, j - 1, k, s);
-            yp1 = slow_ld(p, I_in, 1, i, j + 1, k, s); yp2 = slow_ld(p, I_in, 1, i, j + 2, k, s);
+    for (int k = 0; k < n3; ++k) {
+        const double w4 = (k + 2 < n3) ? __ldg(pk + 2 * kstride) : slow_ld(p, I_in, 2, i, j, k + 2, s);
+        const bool mat = MATTER && *pflag != 0;
+        if (mat || general) {
+            double xm2, xm1, xp1, xp2, ym2, ym1, yp1, yp2;
+            if (!c.special) {
+                xm2 = __ldg(pk + c.oxm2); xm1 = __ldg(pk + c.oxm1); xp1 = __ldg(pk + c.oxp1); xp2 = __ldg(pk + c.oxp2);
+                ym2 = __ldg(pk + c.oym2); ym1 = __ldg(pk + c.oym1); yp1 = __ldg(pk + c.oyp1); yp2 = __ldg(pk + c.oyp2);
+            } else {
+                xm2 = slow_ld(p, I_in, 0, i - 2, j, k, s); xm1 = slow_ld(p, I_in, 0, i - 1, j, k, s);
+                xp1 = slow_ld(p, I_in, 0, i + 1, j, k, s); xp2 = slow_ld(p, I_in, 0, i + 2, j, k, s);
+                ym2 = slow_ld(p, I_in, 1, i, j - 2, k, s); ym1 = slow_ld(p, I_in, 1, i, j - 1, k, s);
+                yp1 = slow_ld(p, I_in, 1, i, j + 1, k, s); yp2 = slow_ld(p, I_in, 1, i, j + 2, k, s);
+            }
+            double D;
+            if (mat) {
+                D = flux_diff<LIM, MATTER>(w0, w1, w2, w3, w4, c.zf, c.zf, ld4(pz), ld4(pz + ncol));
+                D += flux_diff<LIM, MATTER>(xm2, xm1, w2, xp1, xp2, c.xl, c.xh, ld4(px), ld4(px + 1));
+                D += flux_diff<LIM, MATTER>(ym2, ym1, w2, yp1, yp2, c.yl, c.yh, ld4(py), ld4(py + n1));
+            } else {
+                D = flux_diff<LIM, false>(w0, w1, w2, w3, w4, c.zf, c.zf, vac, vac);
+                D += flux_diff<LIM, false>(xm2, xm1, w2, xp1, xp2, c.xl, c.xh, vac, vac);
+                D += flux_diff<LIM, false>(ym2, ym1, w2, yp1, yp2, c.yl, c.yh, vac, vac);
+            }
+            const double base = same_base ? w2 : *pb;
+            *out = (k < zlo || k >= zhi) ? 0.0 : base - D;
         }
-        double D;
-        if (mat) {
-            const long long fx = ((long long)k * p.n2 + j) * (p.n1 + 1) + i, fy = ((long long)k * (p.n2 + 1) + j) * p.n1 + i;
-            D = flux_diff<LIM, MATTER>(w0, w1, w2, w3, w4, c.zf, c.zf, ld4(fc2 + cell), ld4(fc2 + cell + p.ncol));
-            D += flux_diff<LIM, MATTER>(xm2, xm1, w2, xp1, xp2, c.xl, c.xh, ld4(fc0 + fx), ld4(fc0 + fx + 1));
-            D += flux_diff<LIM, MATTER>(ym2, ym1, w2, yp1, yp2, c.yl, c.yh, ld4(fc1 + fy), ld4(fc1 + fy + p.n1));
-        } else {
-            D = flux_diff<LIM, false>(w0, w1, w2, w3, w4, c.zf, c.zf, vac, vac);
-            D += flux_diff<LIM, false>(xm2, xm1, w2, xp1, xp2, c.xl, c.xh, vac, vac);
-            D += flux_diff<LIM, false>(ym2, ym1, w2, yp1, yp2, c.yl, c.yh, vac, vac);
-        }
-        const long long off = k * kstride;
-        const double base = (I_base == I_in) ? w2 : I_base[pos0 + off];
-        I_out[pos0 + off] = (k < zlo || k >= zhi) ? 0.0 : base - D;
+        w0 = w1; w1 = w2; w2 = w3; w3 = w4;
+        pk += kstride; pb += kstride; out += kstride; pflag += ncol; px += sx; py += sy; pz += ncol;
     }
 }
 
@@ -512,15 +519,15 @@ template <int LIM>
 static void launch_transport_lim(const KParams &p, const double *I_in, const double *I_base, double *I_out,
                                  double *const fcoef[3], const unsigned char *cflag, const unsigned char *colflag, bool matter,
                                  double dt, cudaStream_t st) {
-    dim3 grid((p.n1 * p.pitch + 255) / 256, p.n2), ggen(grid.x, grid.y, (p.n3 + GEN_KC - 1) / GEN_KC);
+    dim3 grid((p.n1 * p.pitch + 255) / 256, p.n2);
     const double4 *f0 = reinterpret_cast<const double4 *>(fcoef[0]), *f1 = reinterpret_cast<const double4 *>(fcoef[1]),
                   *f2 = reinterpret_cast<const double4 *>(fcoef[2]);
     if (matter) {
         k_transport_vac<LIM, true><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
-        k_transport_gen<LIM, true><<<ggen, 256, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
+        k_transport_gen<LIM, true><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
     } else {
         k_transport_vac<LIM, false><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
-        k_transport_gen<LIM, false><<<ggen, 256, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
+        k_transport_gen<LIM, false><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
     }
 }
 
