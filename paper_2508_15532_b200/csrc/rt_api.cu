@@ -24,6 +24,7 @@ struct rt_ctx {
     DeviceTables tab;
     double *d_rho, *d_u4, *d_T, *d_Th, *d_Ih, *d_fcoef[3];
     unsigned char *d_cflag;   // per cell: any non-vacuum face
+    int *d_genlist;
     unsigned char *d_cls;     // per (column, s): dead / general class (k_classify)
     unsigned char *d_colflag; // per column: bit 0 has such a cell, bit 1 has an all-vacuum cell
     KParams kp;
@@ -205,7 +206,7 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     c->d_rho = c->d_u4 = c->d_T = c->d_Th = c->d_Ih = nullptr;
     c->d_fcoef[0] = c->d_fcoef[1] = c->d_fcoef[2] = nullptr;
     c->d_cflag = nullptr;
-    c->d_colflag = nullptr; c->d_cls = nullptr;
+    c->d_colflag = nullptr; c->d_cls = nullptr; c->d_genlist = nullptr;
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_cls, (size_t)ncol * pitch);
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_cflag, c->ncell);
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_colflag, (size_t)c->ncol * (2 + n3 / 8));   // column flags + x3-chunk flags (GEN_KC = 8)
@@ -237,6 +238,15 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     k.cls = c->d_cls;
     e = launch_classify(k, c->d_cls, 0);
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) {   // compact list of the general (column, s) pairs, in memory order
+        std::vector<unsigned char> hc((size_t)ncol * pitch);
+        e = cudaMemcpy(hc.data(), c->d_cls, hc.size(), cudaMemcpyDeviceToHost);
+        std::vector<int> gl;
+        for (size_t q = 0; q < hc.size(); ++q)
+            if ((hc[q] & 2) && !(hc[q] & 1)) gl.push_back((int)q);
+        k.ngen = (int)gl.size();
+        if (e == cudaSuccess && k.ngen) { e = upload(&c->d_genlist, gl); k.genlist = c->d_genlist; }
+    }
     if (e != cudaSuccess) { g_last_cuda = (int)e; rt_free(c); return RT_ECUDA; }
     *out = c;
     return RT_OK;
@@ -246,7 +256,7 @@ extern "C" int rt_free(rt_ctx *c) {
     if (!c) return RT_EINVAL;
     for (int a = 0; a < 3; ++a) { cudaFree(c->tab.face[a]); cudaFree(c->d_fcoef[a]); }
     cudaFree(c->tab.cen); cudaFree(c->tab.ecen); cudaFree(c->tab.angcoef); cudaFree(c->tab.nhat); cudaFree(c->tab.w);
-    cudaFree(c->tab.nb); cudaFree(c->d_cflag); cudaFree(c->d_colflag); cudaFree(c->d_cls); cudaFree(c->d_rho); cudaFree(c->d_u4); cudaFree(c->d_T); cudaFree(c->d_Th); cudaFree(c->d_Ih);
+    cudaFree(c->tab.nb); cudaFree(c->d_cflag); cudaFree(c->d_colflag); cudaFree(c->d_cls); cudaFree(c->d_genlist); cudaFree(c->d_rho); cudaFree(c->d_u4); cudaFree(c->d_T); cudaFree(c->d_Th); cudaFree(c->d_Ih);
     delete c;
     return RT_OK;
 }

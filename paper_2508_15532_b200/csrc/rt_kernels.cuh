@@ -29,6 +29,8 @@ struct KParams {
     const double *w;
     const int *nb;
     const unsigned char *cls;   // [ncol][pitch] class byte (k_classify)
+    const int *genlist;         // compact list of the "general" (column * pitch + s) entries
+    int ngen;
     const double *ghost[3][2];
     const double *rho, *u4;  // library-owned fluid copies
 };

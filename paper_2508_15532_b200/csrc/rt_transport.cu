@@ -231,10 +231,8 @@ struct ColSetup {
     FaceK xl, xh, yl, yh, zf;
     int oxm2, oxm1, oxp1, oxp2, oym2, oym1, oyp1, oyp2;
 };
-__device__ __forceinline__ bool col_setup(const KParams &p, double dt, ColSetup &c) {
-    const int e = blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= p.n1 * p.pitch) return false;
-    const int i = c.i = e / p.pitch, s = c.s = e - c.i * p.pitch, j = c.j = blockIdx.y;
+__device__ __forceinline__ bool col_setup(const KParams &p, double dt, ColSetup &c, int i, int j, int s) {
+    c.i = i; c.j = j; c.s = s;
     c.col = j * p.n1 + i;
     c.dead = s >= p.nd;   // pad lanes: keep the pad zero
     c.special = c.general = false;
@@ -286,8 +284,10 @@ __device__ __forceinline__ bool col_setup(const KParams &p, double dt, ColSetup 
 // bit 1 = general (sign change of n^a inside the cell, or next to a ZERO / FIXED boundary).  Both transport kernels
 // read it, so they always agree on which of them owns a thread.
 __global__ void k_classify(const __grid_constant__ KParams p, unsigned char *__restrict__ cls) {
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= p.n1 * p.pitch) return;
     ColSetup c;
-    if (!col_setup(p, 1.0, c)) return;
+    col_setup(p, 1.0, c, e / p.pitch, blockIdx.y, e % p.pitch);
     cls[(long long)c.col * p.pitch + c.s] = (unsigned char)((c.dead ? 1 : 0) | (c.general ? 2 : 0));
 }
 
@@ -314,7 +314,7 @@ k_transport_vac(const __grid_constant__ KParams p, const double *__restrict__ I_
         if (MATTER && !(colflag[blockIdx.y * p.n1 + e0 / p.pitch] & 2)) return;
     }
     ColSetup c;
-    col_setup(p, dt, c);
+    col_setup(p, dt, c, e0 / p.pitch, blockIdx.y, e0 % p.pitch);
     const long long pos0 = (long long)c.col * p.pitch + c.s;
     double *out = I_out + pos0;
     const int i = c.i, j = c.j, s = c.s;
@@ -380,22 +380,30 @@ k_transport_vac(const __grid_constant__ KParams p, const double *__restrict__ I_
 // General path: full 5-point stencils, both PLI states at all six faces, Eq 20 or Eq 23 per face.  Marches x3 with a
 // 5-deep register window; computes only the steps it owns (cells with a non-vacuum face, or every cell of a
 // "general" thread).
-template <int LIM, bool MATTER>
+template <int LIM, bool MATTER, bool LIST>
 __global__ void __launch_bounds__(256, 2)
 k_transport_gen(const __grid_constant__ KParams p, const double *__restrict__ I_in, const double *I_base, double *I_out,
                 const double4 *__restrict__ fc0, const double4 *__restrict__ fc1, const double4 *__restrict__ fc2,
                 const unsigned char *__restrict__ cflag, const unsigned char *__restrict__ colflag, double dt) {
-    const int e0 = blockIdx.x * blockDim.x + threadIdx.x;
-    if (e0 >= p.n1 * p.pitch) return;
-    bool general;
-    {
-        const int cl = p.cls[(long long)blockIdx.y * p.n1 * p.pitch + e0];
-        if (cl & 1) return;
-        general = (cl & 2) != 0;
-        if (!general && !(MATTER && (colflag[blockIdx.y * p.n1 + e0 / p.pitch] & 1))) return;
+    // LIST = false: the non-general threads of columns that hold a cell with a non-vacuum face (grid over (i, s) x j).
+    // LIST = true:  the "general" (column, s) pairs, from the compact list built at rt_init (one thread per entry).
+    int ci, cj, cs;
+    const bool general = LIST;
+    if (LIST) {
+        const int t = blockIdx.x * blockDim.x + threadIdx.x;
+        if (t >= p.ngen) return;
+        const int q = p.genlist[t];
+        const int col = q / p.pitch;
+        cs = q - col * p.pitch; ci = col % p.n1; cj = col / p.n1;
+    } else {
+        const int e0 = blockIdx.x * blockDim.x + threadIdx.x;
+        if (e0 >= p.n1 * p.pitch) return;
+        if (p.cls[(long long)blockIdx.y * p.n1 * p.pitch + e0] != 0) return;      // dead or general
+        ci = e0 / p.pitch; cs = e0 - ci * p.pitch; cj = blockIdx.y;
+        if (!(MATTER && (colflag[cj * p.n1 + ci] & 1))) return;
     }
     ColSetup c;
-    col_setup(p, dt, c);
+    col_setup(p, dt, c, ci, cj, cs);
     const int i = c.i, j = c.j, s = c.s, n3 = p.n3, ncol = p.ncol, n1 = p.n1;
     const long long kstride = (long long)ncol * p.pitch;
     const long long pos0 = (long long)c.col * p.pitch + s;
@@ -524,10 +532,11 @@ static void launch_transport_lim(const KParams &p, const double *I_in, const dou
                   *f2 = reinterpret_cast<const double4 *>(fcoef[2]);
     if (matter) {
         k_transport_vac<LIM, true><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
-        k_transport_gen<LIM, true><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
+        k_transport_gen<LIM, true, false><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
+        if (p.ngen) k_transport_gen<LIM, true, true><<<(p.ngen + 127) / 128, 128, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
     } else {
         k_transport_vac<LIM, false><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
-        k_transport_gen<LIM, false><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
+        if (p.ngen) k_transport_gen<LIM, false, true><<<(p.ngen + 127) / 128, 128, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
     }
 }
 
@@ -540,7 +549,7 @@ cudaError_t launch_transport(const KParams &p, const double *I_in, const double 
         case RT_LIM_NONE: launch_transport_lim<RT_LIM_NONE>(p, I_in, I_base, I_out, fcoef, cflag, colflag, matter, dt, st); break;
         default: launch_transport_lim<RT_LIM_VANLEER>(p, I_in, I_base, I_out, fcoef, cflag, colflag, matter, dt, st); break;
     }
-    *launches += 2;
+    *launches += 1 + (matter ? 1 : 0) + (p.ngen ? 1 : 0);
     return cudaGetLastError();
 }
 
