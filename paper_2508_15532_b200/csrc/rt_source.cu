@@ -20,6 +20,11 @@ namespace {
 
 constexpr double FOURPI = 12.566370614359172953850573533118;
 
+// T^-3.5 = (1/T)^3 sqrt(1/T): a reciprocal and a square root instead of pow()
+__device__ __forceinline__ double t_m35(double T) {
+    const double r = 1.0 / T;
+    return r * r * r * sqrt(r);
+}
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -106,12 +111,15 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
         const int col = int(cell % p.ncol);
         const double *cen = p.cen + (long long)col * CEN_STRIDE;
         double *Ic = I + cell * p.pitch;
-        // all independent loads first: the cell's intensities and its fluid state
+        // all independent loads first: the cell's intensities (needed for every cell only when moments are wanted)
+        // and its fluid state
         double val[MAXV];
+        if (MOM) {
 #pragma unroll
-        for (int v = 0; v < MAXV; ++v) {
-            const int s = lane + 32 * v;
-            val[v] = (s < p.nd) ? Ic[s] : 0.0;
+            for (int v = 0; v < MAXV; ++v) {
+                const int s = lane + 32 * v;
+                val[v] = (s < p.nd) ? Ic[s] : 0.0;
+            }
         }
         double alpha = 0.0, aa = 0.0, as = 0.0, rho = 0.0, Tm = 0.0, u0 = 1.0, u1 = 0.0, u2 = 0.0, u3 = 0.0;
         if (SRC) {
@@ -119,13 +127,20 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
             Tm = T[cell];
             u0 = p.u4[cell]; u1 = p.u4[p.ncell + cell]; u2 = p.u4[2 * p.ncell + cell]; u3 = p.u4[3 * p.ncell + cell];
             if (rho >= p.rho_floor) {
-                aa = (p.kappa_a0 != 0.0) ? p.kappa_a0 * rho * rho * pow(Tm, -3.5) : 0.0;
+                aa = (p.kappa_a0 != 0.0) ? p.kappa_a0 * rho * rho * t_m35(Tm) : 0.0;
                 as = p.kappa_s * rho;
             }
             alpha = aa + as;
         }
         const bool interact = SRC && p.method != 0 && alpha != 0.0;
         if (!interact && !MOM) continue;
+        if (!MOM) {
+#pragma unroll
+            for (int v = 0; v < MAXV; ++v) {
+                const int s = lane + 32 * v;
+                val[v] = (s < p.nd) ? Ic[s] : 0.0;
+            }
+        }
         const double *ecen = p.ecen + (long long)col * 16, *L = cen + 28;
         double Rb = 0.0;          // lanes 0..3: R^0_nu before the source step
         bool updated = false;
@@ -155,11 +170,11 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
                     if (!(n0c > -p.n0_floor)) {
                         const double nup = cen[4] + cen[5] * nx + cen[6] * ny + cen[7] * nz;
                         const double nbar = uh0 - (uh1 * nx + uh2 * ny + uh3 * nz);       // Eq 5, first row
-                        const double d = nup + nbar * alpha * dt;
+                        const double rd = __drcp_rn(nup + nbar * alpha * dt), rn = __drcp_rn(nbar);
                         const double IbdOm = nbar * nbar * val[v] * ws;                     // Ibar dOmegabar (S17)
                         E += IbdOm;                                                         // Eq 33
-                        A1 += nup / d * IbdOm;                                              // Eq 41a
-                        A2 += ws / (nbar * d);                                              // Eq 41b
+                        A1 += nup * rd * IbdOm;                                             // Eq 41a
+                        A2 += ws * rn * rd;                                                 // Eq 41b
                     }
                 }
             }
@@ -182,8 +197,8 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
             if (solve_T(q, Tm, W / Y, Tp)) {
                 const double Ep = W - Y * Tp;                                               // Eq 39
                 const double emis = (p.method == 1) ? aa * p.a_rad * Tp * Tp * Tp * Tp : Nbar * p.a_rad * sqrt(Tp);
-                const double scale = (p.method == 3) ? alpha / (as + Nbar * pow(Tp, -3.5)) : 1.0;
-                const double S = emis + as * Ep;
+                const double scale = (p.method == 3) ? alpha / (as + Nbar * t_m35(Tp)) : 1.0;
+                const double Sdt = (emis + as * Ep) * (dt / FOURPI);
 #pragma unroll
                 for (int v = 0; v < MAXV; ++v) {
                     const int s = lane + 32 * v;
@@ -193,10 +208,9 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
                         if (!(n0c > -p.n0_floor)) {
                             const double nup = cen[4] + cen[5] * nx + cen[6] * ny + cen[7] * nz;
                             const double nbar = uh0 - (uh1 * nx + uh2 * ny + uh3 * nz);
-                            const double d = nup + nbar * alpha * dt;
-                            const double n2 = nbar * nbar, n4 = n2 * n2;
-                            const double Ip = scale * (nup / d * (n4 * val[v]) + nbar * dt / (FOURPI * d) * S);   // Eq 35
-                            val[v] = Ip / n4;                                                                   // L432
+                            const double rd = __drcp_rn(nup + nbar * alpha * dt), rn = __drcp_rn(nbar);
+                            // Eq 35 divided by nbar^4 (L432): I+ = [n^0/d] I- + [nbar dt/(4 pi d)] S / nbar^4
+                            val[v] = scale * rd * (nup * val[v] + Sdt * (rn * rn * rn));
                             Ic[s] = val[v];
                         }
                     }

@@ -479,29 +479,39 @@ __global__ void k_angular(KParams p, const double *__restrict__ I_in, double *I_
     const bool inrow = s < p.pitch;
     const double *pin = I_in + (long long)col * p.pitch + s;
     double *pio = I_io + (long long)col * p.pitch + s;
-    // software pipeline over x3: the operands of step k+1 are requested before step k is computed; the staged cell is
-    // double-buffered in shared memory so that one barrier per step suffices
-    double v = inrow ? __ldg(pin) : 0.0, io = (live && !zero) ? *pio : 0.0;
-    for (int k = 0; k < p.n3; ++k) {
-        double *buf = sI + (k & 1) * p.pitch;
-        if (inrow) buf[s] = v;
-        double vn = 0.0, ion = 0.0;
-        if (k + 1 < p.n3) {
-            if (inrow) vn = __ldg(pin + kstride);
-            if (live && !zero) ion = pio[kstride];
+    // software pipeline over x3, two planes per barrier: the operands of planes k+2, k+3 are requested before planes
+    // k, k+1 are computed; the staged cells are double-buffered in shared memory (4 x pitch doubles)
+    const bool upd = live && !zero;
+    const int n3 = p.n3;
+    double v0 = inrow ? __ldg(pin) : 0.0, v1 = (inrow && 1 < n3) ? __ldg(pin + kstride) : 0.0;
+    double io0 = upd ? *pio : 0.0, io1 = (upd && 1 < n3) ? pio[kstride] : 0.0;
+    for (int k = 0; k < n3; k += 2) {
+        double *buf0 = sI + ((k >> 1) & 1) * 2 * p.pitch, *buf1 = buf0 + p.pitch;
+        const bool two = k + 1 < n3;
+        if (inrow) { buf0[s] = v0; buf1[s] = v1; }
+        double vn0 = 0.0, vn1 = 0.0, ion0 = 0.0, ion1 = 0.0;
+        if (k + 2 < n3) {
+            if (inrow) vn0 = __ldg(pin + 2 * kstride);
+            if (upd) ion0 = pio[2 * kstride];
+            if (k + 3 < n3) {
+                if (inrow) vn1 = __ldg(pin + 3 * kstride);
+                if (upd) ion1 = pio[3 * kstride];
+            }
         }
         __syncthreads();
         if (live) {
-            double D = c[6] * v;
+            double D0 = c[6] * v0, D1 = c[6] * v1;
 #pragma unroll
-            for (int e = 0; e < 6; ++e) D += c[e] * buf[nb[e]];
-            const bool band_k = (k < p.zlo[2] || k >= p.n3 - p.zhi[2]);
-            *pio = (zero || band_k) ? 0.0 : io - scale * D;
+            for (int e = 0; e < 6; ++e) { D0 += c[e] * buf0[nb[e]]; D1 += c[e] * buf1[nb[e]]; }
+            const bool b0 = (k < p.zlo[2] || k >= n3 - p.zhi[2]), b1 = (k + 1 < p.zlo[2] || k + 1 >= n3 - p.zhi[2]);
+            pio[0] = (zero || b0) ? 0.0 : io0 - scale * D0;
+            if (two) pio[kstride] = (zero || b1) ? 0.0 : io1 - scale * D1;
         } else if (inrow) {
-            *pio = 0.0;
+            pio[0] = 0.0;
+            if (two) pio[kstride] = 0.0;
         }
-        v = vn; io = ion;
-        pin += kstride; pio += kstride;
+        v0 = vn0; v1 = vn1; io0 = ion0; io1 = ion1;
+        pin += 2 * kstride; pio += 2 * kstride;
     }
 }
 
@@ -561,7 +571,7 @@ cudaError_t launch_classify(const KParams &p, unsigned char *cls, cudaStream_t s
 
 cudaError_t launch_angular(const KParams &p, const double *I_in, double *I_io, double dt, cudaStream_t st, long long *launches) {
     const int threads = ((p.pitch + 31) / 32) * 32;
-    k_angular<<<p.ncol, threads, 2 * p.pitch * sizeof(double), st>>>(p, I_in, I_io, dt);
+    k_angular<<<p.ncol, threads, 4 * p.pitch * sizeof(double), st>>>(p, I_in, I_io, dt);
     ++*launches;
     return cudaGetLastError();
 }
