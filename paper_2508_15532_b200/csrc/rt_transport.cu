@@ -420,15 +420,28 @@ k_transport_gen(const __grid_constant__ KParams p, const double *__restrict__ I_
     const double4 *px = fc0 + ((long long)j * (n1 + 1) + i), *py = fc1 + ((long long)j * n1 + i), *pz = fc2 + c.col;
     const int sx = p.n2 * (n1 + 1), sy = (p.n2 + 1) * n1;
     const int zlo = p.zlo[2], zhi = n3 - p.zhi[2];
+    const bool special = c.special;
+    // software pipeline: transverse neighbours, x3 look-ahead and cell flag of step k+1 are requested during step k
+    // (special threads load through slow_ld inside the step instead)
+    const int oxm2 = special ? 0 : c.oxm2, oxm1 = special ? 0 : c.oxm1, oxp1 = special ? 0 : c.oxp1, oxp2 = special ? 0 : c.oxp2;
+    const int oym2 = special ? 0 : c.oym2, oym1 = special ? 0 : c.oym1, oyp1 = special ? 0 : c.oyp1, oyp2 = special ? 0 : c.oyp2;
+    double qxm2 = __ldg(pk + oxm2), qxm1 = __ldg(pk + oxm1), qxp1 = __ldg(pk + oxp1), qxp2 = __ldg(pk + oxp2);
+    double qym2 = __ldg(pk + oym2), qym1 = __ldg(pk + oym1), qyp1 = __ldg(pk + oyp1), qyp2 = __ldg(pk + oyp2);
+    double qw4 = ldk(2);
+    unsigned char qflag = MATTER ? *pflag : 0;
     for (int k = 0; k < n3; ++k) {
-        const double w4 = (k + 2 < n3) ? __ldg(pk + 2 * kstride) : slow_ld(p, I_in, 2, i, j, k + 2, s);
-        const bool mat = MATTER && *pflag != 0;
+        double xm2 = qxm2, xm1 = qxm1, xp1 = qxp1, xp2 = qxp2, ym2 = qym2, ym1 = qym1, yp1 = qyp1, yp2 = qyp2;
+        const double w4 = qw4;
+        const bool mat = MATTER && qflag != 0;
+        if (k + 1 < n3) {
+            const double *pn = pk + kstride;
+            qxm2 = __ldg(pn + oxm2); qxm1 = __ldg(pn + oxm1); qxp1 = __ldg(pn + oxp1); qxp2 = __ldg(pn + oxp2);
+            qym2 = __ldg(pn + oym2); qym1 = __ldg(pn + oym1); qyp1 = __ldg(pn + oyp1); qyp2 = __ldg(pn + oyp2);
+            qw4 = (k + 3 < n3) ? __ldg(pn + 2 * kstride) : slow_ld(p, I_in, 2, i, j, k + 3, s);
+            if (MATTER) qflag = pflag[ncol];
+        }
         if (mat || general) {
-            double xm2, xm1, xp1, xp2, ym2, ym1, yp1, yp2;
-            if (!c.special) {
-                xm2 = __ldg(pk + c.oxm2); xm1 = __ldg(pk + c.oxm1); xp1 = __ldg(pk + c.oxp1); xp2 = __ldg(pk + c.oxp2);
-                ym2 = __ldg(pk + c.oym2); ym1 = __ldg(pk + c.oym1); yp1 = __ldg(pk + c.oyp1); yp2 = __ldg(pk + c.oyp2);
-            } else {
+            if (special) {
                 xm2 = slow_ld(p, I_in, 0, i - 2, j, k, s); xm1 = slow_ld(p, I_in, 0, i - 1, j, k, s);
                 xp1 = slow_ld(p, I_in, 0, i + 1, j, k, s); xp2 = slow_ld(p, I_in, 0, i + 2, j, k, s);
                 ym2 = slow_ld(p, I_in, 1, i, j - 2, k, s); ym1 = slow_ld(p, I_in, 1, i, j - 1, k, s);
