@@ -405,20 +405,26 @@ k_transport_gen(const __grid_constant__ KParams p, const double *__restrict__ I_
     ColSetup c;
     col_setup(p, dt, c, ci, cj, cs);
     const int i = c.i, j = c.j, s = c.s, n3 = p.n3, ncol = p.ncol, n1 = p.n1;
+    // the list kernel splits x3 into gridDim.y chunks (few threads: more of them in flight); the column kernel marches all of it
+    const int kchunk = LIST ? (n3 + (int)gridDim.y - 1) / (int)gridDim.y : n3;
+    const int k0 = LIST ? (int)blockIdx.y * kchunk : 0, k1 = min(n3, k0 + kchunk);
+    if (k0 >= k1) return;
     const long long kstride = (long long)ncol * p.pitch;
     const long long pos0 = (long long)c.col * p.pitch + s;
-    const double *pk = I_in + pos0;
+    const double *pin = I_in + pos0;
+    const double *pk = pin + k0 * kstride;
     const double4 vac = make_double4(0.5, -1.0, 0.0, 0.0);
     auto ldk = [&](int kk) -> double {
-        return (kk >= 0 && kk < n3) ? __ldg(pk + kk * kstride) : slow_ld(p, I_in, 2, i, j, kk, s);
+        return (kk >= 0 && kk < n3) ? __ldg(pin + kk * kstride) : slow_ld(p, I_in, 2, i, j, kk, s);
     };
-    double w0 = ldk(-2), w1 = ldk(-1), w2 = ldk(0), w3 = ldk(1);
-    const double *pb = I_base + pos0;
-    double *out = I_out + pos0;
+    double w0 = ldk(k0 - 2), w1 = ldk(k0 - 1), w2 = ldk(k0), w3 = ldk(k0 + 1);
+    const double *pb = I_base + pos0 + k0 * kstride;
+    double *out = I_out + pos0 + k0 * kstride;
     const bool same_base = (I_base == I_in);
-    const unsigned char *pflag = cflag + c.col;
-    const double4 *px = fc0 + ((long long)j * (n1 + 1) + i), *py = fc1 + ((long long)j * n1 + i), *pz = fc2 + c.col;
     const int sx = p.n2 * (n1 + 1), sy = (p.n2 + 1) * n1;
+    const unsigned char *pflag = cflag + c.col + (long long)k0 * ncol;
+    const double4 *px = fc0 + ((long long)j * (n1 + 1) + i) + (long long)k0 * sx, *py = fc1 + ((long long)j * n1 + i) + (long long)k0 * sy,
+                  *pz = fc2 + c.col + (long long)k0 * ncol;
     const int zlo = p.zlo[2], zhi = n3 - p.zhi[2];
     const bool special = c.special;
     // software pipeline: transverse neighbours, x3 look-ahead and cell flag of step k+1 are requested during step k
@@ -427,13 +433,13 @@ k_transport_gen(const __grid_constant__ KParams p, const double *__restrict__ I_
     const int oym2 = special ? 0 : c.oym2, oym1 = special ? 0 : c.oym1, oyp1 = special ? 0 : c.oyp1, oyp2 = special ? 0 : c.oyp2;
     double qxm2 = __ldg(pk + oxm2), qxm1 = __ldg(pk + oxm1), qxp1 = __ldg(pk + oxp1), qxp2 = __ldg(pk + oxp2);
     double qym2 = __ldg(pk + oym2), qym1 = __ldg(pk + oym1), qyp1 = __ldg(pk + oyp1), qyp2 = __ldg(pk + oyp2);
-    double qw4 = ldk(2);
+    double qw4 = ldk(k0 + 2);
     unsigned char qflag = MATTER ? *pflag : 0;
-    for (int k = 0; k < n3; ++k) {
+    for (int k = k0; k < k1; ++k) {
         double xm2 = qxm2, xm1 = qxm1, xp1 = qxp1, xp2 = qxp2, ym2 = qym2, ym1 = qym1, yp1 = qyp1, yp2 = qyp2;
         const double w4 = qw4;
         const bool mat = MATTER && qflag != 0;
-        if (k + 1 < n3) {
+        if (k + 1 < k1) {
             const double *pn = pk + kstride;
             qxm2 = __ldg(pn + oxm2); qxm1 = __ldg(pn + oxm1); qxp1 = __ldg(pn + oxp1); qxp2 = __ldg(pn + oxp2);
             qym2 = __ldg(pn + oym2); qym1 = __ldg(pn + oym1); qyp1 = __ldg(pn + oyp1); qyp2 = __ldg(pn + oyp2);
@@ -556,10 +562,10 @@ static void launch_transport_lim(const KParams &p, const double *I_in, const dou
     if (matter) {
         k_transport_vac<LIM, true><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
         k_transport_gen<LIM, true, false><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
-        if (p.ngen) k_transport_gen<LIM, true, true><<<(p.ngen + 127) / 128, 128, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
+        if (p.ngen) k_transport_gen<LIM, true, true><<<dim3((p.ngen + 127) / 128, 8), 128, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
     } else {
         k_transport_vac<LIM, false><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
-        if (p.ngen) k_transport_gen<LIM, false, true><<<(p.ngen + 127) / 128, 128, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
+        if (p.ngen) k_transport_gen<LIM, false, true><<<dim3((p.ngen + 127) / 128, 8), 128, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
     }
 }
 
