@@ -24,7 +24,7 @@ struct rt_ctx {
     DeviceTables tab;
     double *d_rho, *d_u4, *d_T, *d_Th, *d_Ih, *d_fcoef[3];
     unsigned char *d_cflag;   // per cell: any non-vacuum face
-    int *d_genlist;
+    int *d_genlist, *d_srclist;
     unsigned char *d_cls;     // per (column, s): dead / general class (k_classify)
     unsigned char *d_colflag; // per column: bit 0 has such a cell, bit 1 has an all-vacuum cell
     KParams kp;
@@ -206,7 +206,7 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     c->d_rho = c->d_u4 = c->d_T = c->d_Th = c->d_Ih = nullptr;
     c->d_fcoef[0] = c->d_fcoef[1] = c->d_fcoef[2] = nullptr;
     c->d_cflag = nullptr;
-    c->d_colflag = nullptr; c->d_cls = nullptr; c->d_genlist = nullptr;
+    c->d_colflag = nullptr; c->d_cls = nullptr; c->d_genlist = nullptr; c->d_srclist = nullptr;
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_cls, (size_t)ncol * pitch);
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_cflag, c->ncell);
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_colflag, (size_t)c->ncol * (2 + n3 / 8));   // column flags + x3-chunk flags (GEN_KC = 8)
@@ -256,7 +256,7 @@ extern "C" int rt_free(rt_ctx *c) {
     if (!c) return RT_EINVAL;
     for (int a = 0; a < 3; ++a) { cudaFree(c->tab.face[a]); cudaFree(c->d_fcoef[a]); }
     cudaFree(c->tab.cen); cudaFree(c->tab.ecen); cudaFree(c->tab.angcoef); cudaFree(c->tab.nhat); cudaFree(c->tab.w);
-    cudaFree(c->tab.nb); cudaFree(c->d_cflag); cudaFree(c->d_colflag); cudaFree(c->d_cls); cudaFree(c->d_genlist); cudaFree(c->d_rho); cudaFree(c->d_u4); cudaFree(c->d_T); cudaFree(c->d_Th); cudaFree(c->d_Ih);
+    cudaFree(c->tab.nb); cudaFree(c->d_cflag); cudaFree(c->d_colflag); cudaFree(c->d_cls); cudaFree(c->d_genlist); cudaFree(c->d_srclist); cudaFree(c->d_rho); cudaFree(c->d_u4); cudaFree(c->d_T); cudaFree(c->d_Th); cudaFree(c->d_Ih);
     delete c;
     return RT_OK;
 }
@@ -390,6 +390,25 @@ extern "C" int rt_set_fluid(rt_ctx *c, const double *rho, const double *T, const
             for (int mu = 0; mu < 4; ++mu) h[mu * c->ncell + cell] = c->h_e[(cell % c->ncol) * 16 + 4 * mu];
         CK(cudaStreamSynchronize(st));
         CK(cudaMemcpy(c->d_u4, h.data(), 4 * nb, cudaMemcpyHostToDevice));
+    }
+    // interaction list: cells at or above the density floor (L468 (i)); below it alpha = 0 whatever T is
+    {
+        std::vector<double> hr((size_t)c->ncell);
+        CK(cudaStreamSynchronize(st));
+        CK(cudaMemcpy(hr.data(), c->d_rho, nb, cudaMemcpyDeviceToHost));
+        std::vector<int> sl;
+        if (c->matter && c->opt.source_method != 0)
+            for (long long q = 0; q < c->ncell; ++q)
+                if (hr[q] >= c->opt.rho_floor) sl.push_back((int)q);
+        cudaFree(c->d_srclist);
+        c->d_srclist = nullptr;
+        c->kp.nsrc = (int)sl.size();
+        c->kp.srclist = nullptr;
+        if (!sl.empty()) {
+            cudaError_t e = upload(&c->d_srclist, sl);
+            if (e != cudaSuccess) { g_last_cuda = (int)e; return RT_ECUDA; }
+            c->kp.srclist = c->d_srclist;
+        }
     }
     c->fluid_set = true;
     return RT_OK;

@@ -33,6 +33,8 @@ struct KParams {
     int ngen;
     const double *ghost[3][2];
     const double *rho, *u4;  // library-owned fluid copies
+    const int *srclist;      // cells with rho >= rho_floor (the only ones the source step can touch), built by rt_set_fluid
+    int nsrc;
 };
 
 // launchers (rt_transport.cu, rt_source.cu); every launch increments *launches

@@ -95,7 +95,7 @@ __device__ __forceinline__ double rotate(const double M[10], const double *__res
     return r;
 }
 
-template <int MAXV, bool SRC, bool MOM>
+template <int MAXV, bool SRC, bool MOM, bool LIST>
 __global__ void __launch_bounds__(256, 3)
 k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, double *G_out) {
     extern __shared__ double tab[];   // nx[pitch] ny[pitch] nz[pitch] w[pitch]
@@ -107,7 +107,10 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
     const long long warp0 = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5;
     const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
 
-    for (long long cell = warp0; cell < p.ncell; cell += nwarps) {
+    // LIST: the warp index runs over the compact list of cells above the density floor (built by rt_set_fluid)
+    const long long nwork = LIST ? (long long)p.nsrc : p.ncell;
+    for (long long widx = warp0; widx < nwork; widx += nwarps) {
+        const long long cell = LIST ? (long long)p.srclist[widx] : widx;
         const int col = int(cell % p.ncol);
         const double *cen = p.cen + (long long)col * CEN_STRIDE;
         double *Ic = I + cell * p.pitch;
@@ -240,32 +243,45 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
     }
 }
 
-template <bool SRC, bool MOM>
+template <bool SRC, bool MOM, bool LIST>
 cudaError_t launch_cell(const KParams &p, double *I, double *T, double dt, int *n_fail, double *R, double *G, cudaStream_t st) {
     const int threads = 256;
-    long long want = (p.ncell + 7) / 8;
+    const long long nwork = LIST ? (long long)p.nsrc : p.ncell;
+    long long want = (nwork + 7) / 8;
     const int blocks = (int)(want < 148LL * 8 * 4 ? want : 148LL * 8 * 4);
+    if (blocks == 0) return cudaSuccess;
     const size_t smem = 4 * p.pitch * sizeof(double);
-    if (p.nd <= 64) k_cell<2, SRC, MOM><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail, R, G);
-    else if (p.nd <= 192) k_cell<6, SRC, MOM><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail, R, G);
-    else if (p.nd <= 384) k_cell<12, SRC, MOM><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail, R, G);
-    else if (p.nd <= 672) k_cell<21, SRC, MOM><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail, R, G);
+    if (p.nd <= 64) k_cell<2, SRC, MOM, LIST><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail, R, G);
+    else if (p.nd <= 192) k_cell<6, SRC, MOM, LIST><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail, R, G);
+    else if (p.nd <= 384) k_cell<12, SRC, MOM, LIST><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail, R, G);
+    else if (p.nd <= 672) k_cell<21, SRC, MOM, LIST><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail, R, G);
     else return cudaErrorInvalidValue;
     return cudaGetLastError();
 }
 
 }  // namespace
 
+// Source step on the cells of the interaction list; G (if wanted) is zero elsewhere; R (if wanted) is reduced for all
+// cells by a second, source-free pass.
 cudaError_t launch_source(const KParams &p, double *I, double *T, double dt, int *n_fail, double *R_after, double *G,
                           cudaStream_t st, long long *launches) {
-    ++*launches;
-    if (R_after || G) return launch_cell<true, true>(p, I, T, dt, n_fail, R_after, G, st);
-    return launch_cell<true, false>(p, I, T, dt, n_fail, nullptr, nullptr, st);
+    cudaError_t e = cudaSuccess;
+    if (G) e = cudaMemsetAsync(G, 0, 4 * p.ncell * sizeof(double), st);
+    if (e == cudaSuccess && p.method != 0 && p.nsrc > 0) {
+        ++*launches;
+        e = G ? launch_cell<true, true, true>(p, I, T, dt, n_fail, nullptr, G, st)
+              : launch_cell<true, false, true>(p, I, T, dt, n_fail, nullptr, nullptr, st);
+    }
+    if (e == cudaSuccess && R_after) {
+        ++*launches;
+        e = launch_cell<false, true, false>(p, I, nullptr, 0.0, nullptr, R_after, nullptr, st);
+    }
+    return e;
 }
 
 cudaError_t launch_moments(const KParams &p, const double *I, double *R, cudaStream_t st, long long *launches) {
     ++*launches;
-    return launch_cell<false, true>(p, const_cast<double *>(I), nullptr, 0.0, nullptr, R, nullptr, st);
+    return launch_cell<false, true, false>(p, const_cast<double *>(I), nullptr, 0.0, nullptr, R, nullptr, st);
 }
 
 }  // namespace rt
