@@ -80,6 +80,22 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": reasons}
 
 
+def max_over_ranks(x, world, device=None):
+    """Multi-GPU timing rule: the slowest rank defines the time.  all_reduce(MAX) over the default process group."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(units_per_rank_step, steps, world, ms):
+    """Whole-job throughput: every rank processes the same units (replicas / weak scaling); time = max over ranks."""
+    return units_per_rank_step * steps * world / (ms * 1e-3)
+
+
 def measured_peak():
     """(GB/s, which) -- MEASURED_PEAKS.json (driver-written), else the profiling guide's fallback."""
     try:
@@ -174,10 +190,7 @@ def run_gpu(args, rank, world):
     ctx.profile_enable(False)
     launches = ctx.launch_count() - l0
     finite = bool(torch.isfinite(I).all().item())
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, world, dev)
 
     # ---- end to end through the C ABI with pinned HOST buffers (H2D + D2H inside the timed region) ----
     e2e = None
@@ -201,13 +214,10 @@ def run_gpu(args, rank, world):
         ev1.record()
         barrier()
         ems = ev0.elapsed_time(ev1)
-        if world > 1:
-            t = torch.tensor([ems], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ems = float(t.item())
+        ems = max_over_ranks(ems, world, dev)
         h2d = (hI.numel() + hT.numel()) * 8
         d2h = (hI.numel() + hT.numel() + hR.numel() + hG.numel()) * 8
-        e2e = {"value": units * ksteps * world / (ems * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+        e2e = {"value": aggregate_value(units, ksteps, world, ems), "unit": UNIT, "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "steps": ksteps, "ms_per_step": ems / ksteps}
     return dict(cfg=cfg, ctx=ctx, ms=ms, units=units, prof=prof, launches=launches, clk=clk, e2e=e2e, finite=finite, dt=dt)
 
@@ -278,7 +288,7 @@ def main():
     r = run_gpu(args, rank, world)
     if rank == 0:
         ms, units, K = r["ms"], r["units"], args.steps
-        value = units * K * world / (ms * 1e-3)
+        value = aggregate_value(units, K, world, ms)
         peak, which = measured_peak()
         prof = r["prof"]
         dom = max(("transport", "angular", "source"), key=lambda k: prof[k][0])
