@@ -341,12 +341,14 @@ k_transport_vac(const __grid_constant__ KParams p, const double *__restrict__ I_
     double qxa = __ldg(pk + oxa), qxb = __ldg(pk + oxb), qxd = __ldg(pk + oxd);
     double qya = __ldg(pk + oya), qyb = __ldg(pk + oyb), qyd = __ldg(pk + oyd);
     double qw4 = ldk(2);
+    double qbase = same_base ? 0.0 : *pb;
     unsigned char qflag = MATTER ? *pflag : 0;
     for (int k = 0; k < n3; ++k) {
-        const double xa = qxa, xb = qxb, xd = qxd, ya = qya, yb = qyb, yd = qyd, w4 = qw4;
+        const double xa = qxa, xb = qxb, xd = qxd, ya = qya, yb = qyb, yd = qyd, w4 = qw4, cbase = qbase;
         const bool mat = MATTER && qflag != 0;
         if (k + 1 < n3) {   // request the operands of step k + 1 before computing step k
             const double *pn = pk + kstride;
+            if (!same_base) qbase = pb[kstride];
             qxa = __ldg(pn + oxa); qxb = __ldg(pn + oxb); qxd = __ldg(pn + oxd);
             qya = __ldg(pn + oya); qyb = __ldg(pn + oyb); qyd = __ldg(pn + oyd);
             qw4 = (k + 3 < n3) ? __ldg(pn + 2 * kstride) : slow_ld(p, I_in, 2, i, j, k + 3, s);
@@ -367,7 +369,7 @@ k_transport_vac(const __grid_constant__ KParams p, const double *__restrict__ I_
                 D = fma(Kybc, fma(0.5, slope_k<LIM>(d1, d2), yb), D);
                 D = fma(Kycd, fma(0.5, slope_k<LIM>(d2, d3), w2), D);
             }
-            const double base = same_base ? w2 : *pb;
+            const double base = same_base ? w2 : cbase;
             *out = (k < zlo || k >= zhi) ? 0.0 : base - D;      // Eq 18 (O5), dt/(n^0 n_0 sqrt(-g) dx) folded in
         }
         Flo = Fhi;
@@ -434,12 +436,14 @@ k_transport_gen(const __grid_constant__ KParams p, const double *__restrict__ I_
     double qxm2 = __ldg(pk + oxm2), qxm1 = __ldg(pk + oxm1), qxp1 = __ldg(pk + oxp1), qxp2 = __ldg(pk + oxp2);
     double qym2 = __ldg(pk + oym2), qym1 = __ldg(pk + oym1), qyp1 = __ldg(pk + oyp1), qyp2 = __ldg(pk + oyp2);
     double qw4 = ldk(k0 + 2);
+    double qbase = same_base ? 0.0 : *pb;
     unsigned char qflag = MATTER ? *pflag : 0;
     for (int k = k0; k < k1; ++k) {
         double xm2 = qxm2, xm1 = qxm1, xp1 = qxp1, xp2 = qxp2, ym2 = qym2, ym1 = qym1, yp1 = qyp1, yp2 = qyp2;
-        const double w4 = qw4;
+        const double w4 = qw4, cbase = qbase;
         const bool mat = MATTER && qflag != 0;
         if (k + 1 < k1) {
+            if (!same_base) qbase = pb[kstride];
             const double *pn = pk + kstride;
             qxm2 = __ldg(pn + oxm2); qxm1 = __ldg(pn + oxm1); qxp1 = __ldg(pn + oxp1); qxp2 = __ldg(pn + oxp2);
             qym2 = __ldg(pn + oym2); qym1 = __ldg(pn + oym1); qyp1 = __ldg(pn + oyp1); qyp2 = __ldg(pn + oyp2);
@@ -463,7 +467,7 @@ k_transport_gen(const __grid_constant__ KParams p, const double *__restrict__ I_
                 D += flux_diff<LIM, false>(xm2, xm1, w2, xp1, xp2, c.xl, c.xh, vac, vac);
                 D += flux_diff<LIM, false>(ym2, ym1, w2, yp1, yp2, c.yl, c.yh, vac, vac);
             }
-            const double base = same_base ? w2 : *pb;
+            const double base = same_base ? w2 : cbase;
             *out = (k < zlo || k >= zhi) ? 0.0 : base - D;
         }
         w0 = w1; w1 = w2; w2 = w3; w3 = w4;
