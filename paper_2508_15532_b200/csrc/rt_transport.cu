@@ -225,6 +225,18 @@ __global__ void k_colflag(KParams p, const unsigned char *__restrict__ cflag, un
 //                    lean upwind path, carried x3 flux, software-pipelined loads;
 //   k_transport_gen  everything else: cells with a non-vacuum (Eq 23) face, threads with a sign change of n^a
 //                    inside the cell, threads next to a ZERO / FIXED boundary.
+// Block order of the marching kernels: a 1-D grid walked in bands of TILE_ROWS x2-rows with x2 fastest inside a band,
+// so that the CTAs resident at the same time cover a compact (x1, x2) patch and their transverse neighbours are
+// read from L2 instead of DRAM (row-major order re-reads ~4 halo rows per wave of ~5 rows).
+constexpr int TILE_ROWS = 24;
+__device__ __forceinline__ void tile_block(const KParams &p, int &bx, int &by) {
+    const int nbx = (p.n1 * p.pitch + (int)blockDim.x - 1) / (int)blockDim.x;
+    const int lin = blockIdx.x, band = lin / (nbx * TILE_ROWS), r = lin - band * nbx * TILE_ROWS;
+    const int th = min(TILE_ROWS, p.n2 - band * TILE_ROWS);
+    bx = r / th;
+    by = band * TILE_ROWS + (r - bx * th);
+}
+
 struct ColSetup {
     int i, j, s, col;
     bool dead, special, general;
@@ -299,22 +311,24 @@ template <int LIM, bool MATTER>
 __global__ void __launch_bounds__(256, 3)
 k_transport_vac(const __grid_constant__ KParams p, const double *__restrict__ I_in, const double *I_base, double *I_out,
                 const unsigned char *__restrict__ cflag, const unsigned char *__restrict__ colflag, double dt) {
-    const int e0 = blockIdx.x * blockDim.x + threadIdx.x;
+    int bx, by;
+    tile_block(p, bx, by);
+    const int e0 = bx * blockDim.x + threadIdx.x;
     if (e0 >= p.n1 * p.pitch) return;
     const long long kstride = (long long)p.ncol * p.pitch;
     const int n3 = p.n3, ncol = p.ncol;
     {
-        const long long q = (long long)blockIdx.y * p.n1 * p.pitch + e0;
+        const long long q = (long long)by * p.n1 * p.pitch + e0;
         const int cl = p.cls[q];
         if (cl & 1) {   // dead: this kernel keeps those entries zero
             for (int k = 0; k < n3; ++k) I_out[q + k * kstride] = 0.0;
             return;
         }
         if (cl & 2) return;
-        if (MATTER && !(colflag[blockIdx.y * p.n1 + e0 / p.pitch] & 2)) return;
+        if (MATTER && !(colflag[by * p.n1 + e0 / p.pitch] & 2)) return;
     }
     ColSetup c;
-    col_setup(p, dt, c, e0 / p.pitch, blockIdx.y, e0 % p.pitch);
+    col_setup(p, dt, c, e0 / p.pitch, by, e0 % p.pitch);
     const long long pos0 = (long long)c.col * p.pitch + c.s;
     double *out = I_out + pos0;
     const int i = c.i, j = c.j, s = c.s;
@@ -398,10 +412,12 @@ k_transport_gen(const __grid_constant__ KParams p, const double *__restrict__ I_
         const int col = q / p.pitch;
         cs = q - col * p.pitch; ci = col % p.n1; cj = col / p.n1;
     } else {
-        const int e0 = blockIdx.x * blockDim.x + threadIdx.x;
+        int bx, by;
+        tile_block(p, bx, by);
+        const int e0 = bx * blockDim.x + threadIdx.x;
         if (e0 >= p.n1 * p.pitch) return;
-        if (p.cls[(long long)blockIdx.y * p.n1 * p.pitch + e0] != 0) return;      // dead or general
-        ci = e0 / p.pitch; cs = e0 - ci * p.pitch; cj = blockIdx.y;
+        if (p.cls[(long long)by * p.n1 * p.pitch + e0] != 0) return;      // dead or general
+        ci = e0 / p.pitch; cs = e0 - ci * p.pitch; cj = by;
         if (!(MATTER && (colflag[cj * p.n1 + ci] & 1))) return;
     }
     ColSetup c;
@@ -560,7 +576,7 @@ template <int LIM>
 static void launch_transport_lim(const KParams &p, const double *I_in, const double *I_base, double *I_out,
                                  double *const fcoef[3], const unsigned char *cflag, const unsigned char *colflag, bool matter,
                                  double dt, cudaStream_t st) {
-    dim3 grid((p.n1 * p.pitch + 255) / 256, p.n2);
+    dim3 grid(((p.n1 * p.pitch + 255) / 256) * p.n2);   // walked in tiles, see tile_block()
     const double4 *f0 = reinterpret_cast<const double4 *>(fcoef[0]), *f1 = reinterpret_cast<const double4 *>(fcoef[1]),
                   *f2 = reinterpret_cast<const double4 *>(fcoef[2]);
     if (matter) {
