@@ -68,7 +68,7 @@ typedef struct {
 
 typedef struct {
     int limiter;       /* RT_LIM_* (S7: monotonised central by default) */
-    int angular_recon; /* RT_ANG_DONOR (RT_ANG_MAPR: not implemented in this round -> RT_EINVAL) */
+    int angular_recon; /* RT_ANG_DONOR (first order, L227) | RT_ANG_MAPR (minimum-angle plane reconstruction, reading S6) */
     int source_method; /* 0 = no source step; 1, 2, 3 = Methods 1-3 of section 3.6.2 */
     double n0_floor;   /* mask directions with n_0 > -n0_floor (L284; 0.1) */
     double rho_floor;  /* no interaction below this density (L468; 5e-4) */

@@ -71,6 +71,7 @@ def _load():
         _lib.orc_step.argtypes = [pp, _dp, _dp, _dp, _dp, ctypes.c_double, _dp, _dp, _dp]
         _lib.orc_step.restype = ctypes.c_int
         _lib.orc_cfl.argtypes = [pp, _dp]
+        _lib.orc_mapr_gradient.argtypes = [pp, _dp, ctypes.c_int, _dp]
     return _lib
 
 
@@ -186,6 +187,12 @@ class Oracle:
         nf = _load().orc_step(ctypes.byref(self.P), _ptr(I), _ptr(T), _ptr(R), _ptr(G), dt,
                               _ptr(Ih), _ptr(Th), _ptr(Rb))
         return I, T, R, G, nf
+
+    def mapr_gradient(self, Ic, s):
+        """O4' gradient (3-vector tangent at nhat_s) of direction s for one cell's intensities Ic[nd]."""
+        Ic, g = _c(Ic), np.zeros(3)
+        _load().orc_mapr_gradient(ctypes.byref(self.P), _ptr(Ic), int(s), _ptr(g))
+        return g
 
     def cfl(self):
         """(spatial bound L464, angular bound S14)."""

@@ -269,9 +269,14 @@ static void mapr_gradient(const orc_problem *P, const double *Ic /*[nd] one cell
         double c1 = (dI[e] * a22 - dI[e2] * a12) / det, c2 = (dI[e2] * a11 - dI[e] * a12) / det;
         double G[3], nrm = 0;
         for (int x = 0; x < 3; ++x) { G[x] = c1 * xi[e][x] + c2 * xi[e2][x]; nrm += G[x] * G[x]; }
-        if (nrm < best) { best = nrm; grad[0] = G[0]; grad[1] = G[1]; grad[2] = G[2]; }
+        /* ties -> lowest e, where a tie is agreement to round-off: equal (e.g. masked, zero) neighbours make
+         * consecutive candidates tie structurally, and the winner must not depend on the last bit (S6) */
+        if (nrm < best * (1.0 - 1e-12)) { best = nrm; grad[0] = G[0]; grad[1] = G[1]; grad[2] = G[2]; }
     }
 }
+/* test hook: the MAPR gradient of cell s for one cell's intensities */
+void orc_mapr_gradient(const orc_problem *P, const double *Ic, int s, double grad[3]) { mapr_gradient(P, Ic, s, grad); }
+
 static double mapr_edge_value(const orc_problem *P, const double *Ic, int s, int e, const double grad[3]) {
     const double *c0 = P->nhat + 3 * s, *m = P->emid + 3 * (6 * s + e);
     double dot = c0[0] * m[0] + c0[1] * m[1] + c0[2] * m[2];

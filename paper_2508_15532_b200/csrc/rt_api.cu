@@ -25,6 +25,9 @@ struct rt_ctx {
     double *d_rho, *d_u4, *d_T, *d_Th, *d_Ih, *d_fcoef[3];
     unsigned char *d_cflag;   // per cell: any non-vacuum face
     int *d_genlist, *d_srclist;
+    double *d_mapr_xi, *d_mapr_xim, *d_mapr_a, *d_angraw;
+    int *d_mapr_back, *d_mapr_nnb;
+    unsigned char *d_angup;
     unsigned char *d_cls;     // per (column, s): dead / general class (k_classify)
     unsigned char *d_colflag; // per column: bit 0 has such a cell, bit 1 has an all-vacuum cell
     KParams kp;
@@ -81,7 +84,7 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     }
     if (metric->kind < 0 || metric->kind > RT_KS_MKS) return RT_EINVAL;
     if (metric->kind == RT_KS_MKS && (!metric->x3_symmetric || std::fabs(metric->a) >= 1.0)) return RT_EINVAL;
-    if (opt->angular_recon != RT_ANG_DONOR) return RT_EINVAL;
+    if (opt->angular_recon != RT_ANG_DONOR && opt->angular_recon != RT_ANG_MAPR) return RT_EINVAL;
     if (opt->limiter < 0 || opt->limiter > 3 || opt->source_method < 0 || opt->source_method > 3) return RT_EINVAL;
     if (opt->source_method != 0 && !(opt->Y_over_rho > 0)) return RT_EINVAL;
 
@@ -108,6 +111,9 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     face[1].resize((size_t)n1 * (n2 + 1) * FACE_STRIDE);
     face[2].resize((size_t)ncol * FACE_STRIDE);
     std::vector<double> angc((size_t)ncol * ANG_SLOTS * pitch, 0.0);
+    const bool mapr = opt->angular_recon == RT_ANG_MAPR;
+    std::vector<double> angraw(mapr ? (size_t)ncol * 6 * pitch : 0, 0.0);
+    std::vector<unsigned char> angup(mapr ? (size_t)ncol * pitch : 0, 0);
     double omax = 0.0;
     for (int j = 0; j < n2; ++j)
         for (int i = 0; i < n1; ++i) {
@@ -159,6 +165,10 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
                     const bool gate = ((n0s > 0) - (n0s < 0)) != ((n0t > 0) - (n0t < 0));   // L280
                     const double coef = gate ? 0.0 : A.dlam[6 * s + e] * n0e * V / A.w[s];  // Eq 19 / Eq 18
                     c->h_angcoef[(col * 6 + e) * nd + s] = coef;
+                    if (mapr) {
+                        angraw[(col * 6 + e) * pitch + s] = coef;
+                        if (V > 0) angup[col * pitch + s] |= (unsigned char)(1u << e);
+                    }
                     if (V > 0) self += coef;                                    // upwind: own value (S5)
                     else angc[(col * ANG_SLOTS + e) * pitch + s] = coef;        // upwind: neighbour's value
                 }
@@ -207,6 +217,7 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     c->d_fcoef[0] = c->d_fcoef[1] = c->d_fcoef[2] = nullptr;
     c->d_cflag = nullptr;
     c->d_colflag = nullptr; c->d_cls = nullptr; c->d_genlist = nullptr; c->d_srclist = nullptr;
+    c->d_mapr_xi = c->d_mapr_xim = c->d_mapr_a = c->d_angraw = nullptr; c->d_mapr_back = c->d_mapr_nnb = nullptr; c->d_angup = nullptr;
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_cls, (size_t)ncol * pitch);
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_cflag, c->ncell);
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_colflag, (size_t)c->ncol * (2 + n3 / 8));   // column flags + x3-chunk flags (GEN_KC = 8)
@@ -236,6 +247,46 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     k.cen = t.cen; k.ecen = t.ecen; k.angcoef = t.angcoef; k.nhat = t.nhat; k.w = t.w; k.nb = t.nb;
     k.rho = c->d_rho; k.u4 = c->d_u4;
     k.cls = c->d_cls;
+    if (mapr) {   // grid-only MAPR tables (S6): log maps of the neighbours and of the edge centres, pair matrices
+        const AngularGrid &A = c->ang;
+        std::vector<double> xi(18 * (size_t)pitch, 0.0), xim(18 * (size_t)pitch, 0.0), am(24 * (size_t)pitch, 0.0);
+        std::vector<int> back(6 * (size_t)pitch, 0), nnb(pitch, 0);
+        auto logmap = [](const double *c0, const double *q, double out[3]) {
+            const double dot = c0[0] * q[0] + c0[1] * q[1] + c0[2] * q[2];
+            const double pv[3] = {q[0] - dot * c0[0], q[1] - dot * c0[1], q[2] - dot * c0[2]};
+            const double pn = std::sqrt(pv[0] * pv[0] + pv[1] * pv[1] + pv[2] * pv[2]);
+            const double ang = std::atan2(pn, dot);
+            for (int x = 0; x < 3; ++x) out[x] = ang * pv[x] / pn;
+        };
+        for (int s = 0; s < nd; ++s) {
+            nnb[s] = A.nnb[s];
+            double x6[6][3];
+            for (int e = 0; e < A.nnb[s]; ++e) {
+                logmap(&A.nhat[3 * s], &A.nhat[3 * A.nb[6 * s + e]], x6[e]);
+                double xm[3];
+                logmap(&A.nhat[3 * s], &A.emid[3 * (6 * s + e)], xm);
+                for (int x = 0; x < 3; ++x) { xi[(e * 3 + x) * pitch + s] = x6[e][x]; xim[(e * 3 + x) * pitch + s] = xm[x]; }
+                back[e * pitch + s] = A.back[6 * s + e];
+            }
+            for (int e = 0; e < A.nnb[s]; ++e) {
+                const int e2 = (e + 1) % A.nnb[s];
+                double a11 = 0, a12 = 0, a22 = 0;
+                for (int x = 0; x < 3; ++x) { a11 += x6[e][x] * x6[e][x]; a12 += x6[e][x] * x6[e2][x]; a22 += x6[e2][x] * x6[e2][x]; }
+                am[(e * 4 + 0) * pitch + s] = a11; am[(e * 4 + 1) * pitch + s] = a12; am[(e * 4 + 2) * pitch + s] = a22;
+                am[(e * 4 + 3) * pitch + s] = a11 * a22 - a12 * a12;
+            }
+        }
+        e = upload(&c->d_mapr_xi, xi);
+        if (e == cudaSuccess) e = upload(&c->d_mapr_xim, xim);
+        if (e == cudaSuccess) e = upload(&c->d_mapr_a, am);
+        if (e == cudaSuccess) e = upload(&c->d_mapr_back, back);
+        if (e == cudaSuccess) e = upload(&c->d_mapr_nnb, nnb);
+        if (e == cudaSuccess) e = upload(&c->d_angraw, angraw);
+        if (e == cudaSuccess) e = upload(&c->d_angup, angup);
+        if (e != cudaSuccess) { g_last_cuda = (int)e; rt_free(c); return RT_ECUDA; }
+        k.mapr_xi = c->d_mapr_xi; k.mapr_xim = c->d_mapr_xim; k.mapr_a = c->d_mapr_a; k.mapr_back = c->d_mapr_back;
+        k.mapr_nnb = c->d_mapr_nnb; k.angraw = c->d_angraw; k.angup = c->d_angup;
+    }
     e = launch_classify(k, c->d_cls, 0);
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     if (e == cudaSuccess) {   // compact list of the general (column, s) pairs, in memory order
@@ -256,7 +307,8 @@ extern "C" int rt_free(rt_ctx *c) {
     if (!c) return RT_EINVAL;
     for (int a = 0; a < 3; ++a) { cudaFree(c->tab.face[a]); cudaFree(c->d_fcoef[a]); }
     cudaFree(c->tab.cen); cudaFree(c->tab.ecen); cudaFree(c->tab.angcoef); cudaFree(c->tab.nhat); cudaFree(c->tab.w);
-    cudaFree(c->tab.nb); cudaFree(c->d_cflag); cudaFree(c->d_colflag); cudaFree(c->d_cls); cudaFree(c->d_genlist); cudaFree(c->d_srclist); cudaFree(c->d_rho); cudaFree(c->d_u4); cudaFree(c->d_T); cudaFree(c->d_Th); cudaFree(c->d_Ih);
+    cudaFree(c->tab.nb); cudaFree(c->d_cflag); cudaFree(c->d_colflag); cudaFree(c->d_cls); cudaFree(c->d_genlist); cudaFree(c->d_srclist); cudaFree(c->d_mapr_xi); cudaFree(c->d_mapr_xim); cudaFree(c->d_mapr_a);
+    cudaFree(c->d_angraw); cudaFree(c->d_mapr_back); cudaFree(c->d_mapr_nnb); cudaFree(c->d_angup); cudaFree(c->d_rho); cudaFree(c->d_u4); cudaFree(c->d_T); cudaFree(c->d_Th); cudaFree(c->d_Ih);
     delete c;
     return RT_OK;
 }
@@ -434,7 +486,7 @@ extern "C" int rt_transport(rt_ctx *c, const double *I_in, const double *I_base,
 extern "C" int rt_angular_flux(rt_ctx *c, const double *I_in, double *I_io, double dt, void *stream) {
     if (!c || !I_in || !I_io || I_in == I_io) return RT_EINVAL;
     if (!c->curved) return RT_OK;
-    { ProfScope ps(c, RT_K_ANGULAR, (cudaStream_t)stream); CK(launch_angular(c->kp, I_in, I_io, dt, (cudaStream_t)stream, &c->launches)); }
+    { ProfScope ps(c, RT_K_ANGULAR, (cudaStream_t)stream); CK((c->opt.angular_recon == RT_ANG_MAPR ? launch_angular_mapr : launch_angular)(c->kp, I_in, I_io, dt, (cudaStream_t)stream, &c->launches)); }
     return RT_OK;
 }
 
@@ -458,7 +510,7 @@ static int stage(rt_ctx *c, const double *I_flux, const double *T_flux, const do
                  double delta, int *n_fail, double *R, double *G, cudaStream_t st) {
     if (c->matter) { ProfScope ps(c, RT_K_FACECOEF, st); CK(launch_facecoef(c->kp, T_flux, delta, c->d_fcoef, c->d_cflag, c->d_colflag, st, &c->launches)); }
     { ProfScope ps(c, RT_K_TRANSPORT, st); CK(launch_transport(c->kp, I_flux, I_base, I_out, c->d_fcoef, c->d_cflag, c->d_colflag, c->matter, delta, st, &c->launches)); }
-    if (c->curved) { ProfScope ps(c, RT_K_ANGULAR, st); CK(launch_angular(c->kp, I_flux, I_out, delta, st, &c->launches)); }
+    if (c->curved) { ProfScope ps(c, RT_K_ANGULAR, st); CK((c->opt.angular_recon == RT_ANG_MAPR ? launch_angular_mapr : launch_angular)(c->kp, I_flux, I_out, delta, st, &c->launches)); }
     if (c->opt.source_method != 0 || R || G) {
         ProfScope ps(c, RT_K_SOURCE, st);
         CK(launch_source(c->kp, I_out, T_io, delta, n_fail, R, G, st, &c->launches));

@@ -29,6 +29,14 @@ struct KParams {
     const double *w;
     const int *nb;
     const unsigned char *cls;   // [ncol][pitch] class byte (k_classify)
+    // MAPR tables (only when angular_recon == RT_ANG_MAPR): grid-only tables are [slot][..][pitch]
+    const double *mapr_xi;    // [6][3][pitch]  log map of neighbour e in the tangent plane at n_s
+    const double *mapr_xim;   // [6][3][pitch]  log map of the centre of edge e
+    const double *mapr_a;     // [6][4][pitch]  a11, a12, a22, det of the pair (e, e+1)
+    const int *mapr_back;     // [6][pitch]     slot of s in neighbour e's list
+    const int *mapr_nnb;      // [pitch]        5 or 6
+    const double *angraw;     // [ncol][6][pitch] dlam n_0e V / w per edge (gated)
+    const unsigned char *angup;   // [ncol][pitch] bit e: V_e > 0
     const int *genlist;         // compact list of the "general" (column * pitch + s) entries
     int ngen;
     const double *ghost[3][2];
@@ -43,6 +51,7 @@ cudaError_t launch_facecoef(const KParams &p, const double *T, double dt, double
 cudaError_t launch_transport(const KParams &p, const double *I_in, const double *I_base, double *I_out,
                              double *const fcoef[3], const unsigned char *cflag, const unsigned char *colflag, bool matter,
                              double dt, cudaStream_t st, long long *launches);
+cudaError_t launch_angular_mapr(const KParams &p, const double *I_in, double *I_io, double dt, cudaStream_t st, long long *launches);
 cudaError_t launch_classify(const KParams &p, unsigned char *cls, cudaStream_t st);
 cudaError_t launch_angular(const KParams &p, const double *I_in, double *I_io, double dt, cudaStream_t st, long long *launches);
 // source step; if R_after != nullptr also writes moments after the update; if G != nullptr writes

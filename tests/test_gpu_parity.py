@@ -151,3 +151,30 @@ def test_determinism_bitwise():
         res.append((I.clone(), T.clone(), R.clone()))
     for a, b in zip(*res):
         assert torch.equal(a, b)
+
+
+@pytest.mark.parametrize("idx,n,steps", [(4, (16, 14, 4), 5), (5, (10, 8, 3), 2)])
+def test_mapr_angular_reconstruction(idx, n, steps):
+    """RT_ANG_MAPR against the oracle's O4' (reading S6; the oracle side is parity-unpinned beyond linear exactness).
+    The arg-min over candidate planes is discontinuous: both sides form the squared norms with the same rounded
+    operations, and the seeded noise keeps exact ties away."""
+    cfg = W.config(idx, n=n)
+    cfg["options"] = dict(cfg["options"], ang_recon=1)
+    orc, ctx, f, dt = make_pair(cfg)
+    _check(run_steps(orc, ctx, f, 0.5 * dt, steps))
+
+
+def test_mapr_rotating_tetrad_per_call():
+    import torch
+    cfg = W.config(3, n=(8, 7, 3))
+    cfg["grid"] = dict(cfg["grid"], x0=(0.6, 0.4, 0.0), bc_lo=("outflow", "outflow", "periodic"), bc_hi=("outflow", "outflow", "periodic"))
+    cfg["metric"] = ("mink_cyl", {})
+    cfg["options"] = dict(cfg["options"], ang_recon=1)
+    orc, ctx, f, dt = make_pair(cfg)
+    I0 = np.random.default_rng(3).uniform(0.5, 1.0, size=f["I0"].shape)
+    Ig = ctx.to_device(I0)
+    out = Ig.clone()
+    ctx.angular_flux(Ig, out, 0.1 * dt)
+    ref = orc.angular_flux(I0, I0, 0.1 * dt).reshape(I0.shape)
+    assert rel_err(ctx.to_host(out), ref) <= TOL
+    assert np.abs(ref - I0).max() > 1e-5

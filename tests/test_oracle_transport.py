@@ -158,3 +158,36 @@ def test_second_order_convergence_smooth_profile():
         ex = 1 + 0.5 * np.sin(2 * np.pi * (x - o.ang["nhat"][s, 0] * dt * nst))
         errs.append(np.abs(I[0, 0, :, s] - ex).mean())
     assert errs[0] / errs[1] > 3.0
+
+
+def test_mapr_linear_exactness_constant_reduction_and_conservation():
+    """O4' (MAPR, reading S6; PARITY UNPINNED beyond these facts): exact for fields linear in the tangent plane,
+    reduces to donor cell for a constant field, and stays conservative per cell."""
+    o = Oracle(dict(n=(1, 1, 1), x0=(0, 0, 0), dx=(1, 1, 1), bc_lo=PER, bc_hi=PER), "minkowski", {}, 4, dict(method=0, ang_recon=1))
+    nh, nb, nnb = o.ang["nhat"], o.ang["nb"], o.ang["nnb"]
+    rng = np.random.default_rng(11)
+    for s in (0, 7, 50, 161):
+        c0 = nh[s]
+        g = rng.normal(size=3)
+        g -= (g @ c0) * c0                                    # a gradient in the tangent plane at n_s
+        I = np.zeros(o.nd)
+        I[s] = 0.3
+        for t in nb[s, :nnb[s]]:
+            dot = c0 @ nh[t]
+            p = nh[t] - dot * c0
+            I[t] = 0.3 + g @ (np.arctan2(np.linalg.norm(p), dot) * p / np.linalg.norm(p))   # independent log map
+        assert np.abs(o.mapr_gradient(I, s) - g).max() < 1e-12
+    # constant field: gradient zero, MAPR == donor cell; and per-cell conservation in a curved metric
+    grid = dict(n=(3, 3, 1), x0=(np.log(4.0), 0.3, 0.0), dx=(0.2, 0.1, 0.1), bc_lo=("outflow", "outflow", "periodic"),
+                bc_hi=("outflow", "outflow", "periodic"), x3_symmetric=True)
+    om = Oracle(grid, "ks_mks", dict(a=0.9, hslope=0.3), 4, dict(method=0, ang_recon=1))
+    od = Oracle(grid, "ks_mks", dict(a=0.9, hslope=0.3), 4, dict(method=0, ang_recon=0))
+    Ic = np.tile(rng.uniform(0.5, 1.0, size=(1, 3, 3, 1)), (1, 1, 1, om.nd))
+    assert np.abs(om.angular_flux(Ic, Ic, 1e-3) - od.angular_flux(Ic, Ic, 1e-3)).max() < 1e-15
+    I = rng.uniform(0.5, 1.0, size=(1, 3, 3, om.nd))
+    out = om.angular_flux(I, I, 1e-3).reshape(I.shape)
+    e, g = om.tab["e_c"], om.tab["g_c"]
+    n = e[..., :, 0][..., None, :] + np.einsum("...mi,si->...sm", e[..., :, 1:], om.ang["nhat"])
+    n0 = np.einsum("...m,...sm->...s", g[..., 0, :], n)
+    assert np.abs(((out - I) * n[..., 0] * n0 * om.ang["w"]).sum(-1)).max() < 1e-16 * 50
+    assert np.abs(out - od.angular_flux(I, I, 1e-3).reshape(I.shape)).max() > 1e-7        # and it is not donor cell
