@@ -132,11 +132,13 @@ __device__ __forceinline__ bool sign_differs(double a, double b) {
 // Monotonised-central slope, same value as minmod3(2 dm, (dm+dp)/2, 2 dp) bit for bit, with 5 fp64-pipe operations:
 // equal signs => sign * min(2 min(|dm|,|dp|), |dm+dp|/2); opposite signs or a zero difference => 0.
 __device__ __forceinline__ double slope_mc(double dm, double dp) {
-    // plain compares + selects (DSETP + SEL); fmin() would add its NaN-propagation sequence to every call
-    const double a = fabs(dm), b = fabs(dp);
-    const double mn = (a < b) ? a : b;
-    const double m2 = mn + mn;
-    const double c = 0.5 * fabs(dm + dp);
+    // Equal signs: min(2 min(|dm|,|dp|), |dm+dp|/2) with |dm+dp| = |dm|+|dp| =: a and 2 min(|dm|,|dp|) = a - ||dm|-|dp||
+    // (fp64 adds instead of a compare + two selects; the fp64 pipe has slack, the ALU pipe does not).  The identity
+    // holds to one rounding of a, i.e. to 1e-16 of max(|dm|,|dp|): inside the parity budget, and the result still
+    // never exceeds 2 min(|dm|,|dp|) by more than that rounding.
+    const double a = fabs(dm) + fabs(dp);
+    const double m2 = a - fabs(fabs(dm) - fabs(dp));
+    const double c = 0.5 * a;
     const double r = (m2 < c) ? m2 : c;
     const bool opp = (__double2hiint(dm) ^ __double2hiint(dp)) < 0;
     return opp ? 0.0 : copysign(r, dm);
@@ -229,6 +231,10 @@ __global__ void k_colflag(KParams p, const unsigned char *__restrict__ cflag, un
 // so that the CTAs resident at the same time cover a compact (x1, x2) patch and their transverse neighbours are
 // read from L2 instead of DRAM (row-major order re-reads ~4 halo rows per wave of ~5 rows).
 constexpr int TILE_ROWS = 24;
+#ifndef VAC_THREADS
+#define VAC_THREADS 128
+#define VAC_MINB 5
+#endif
 __device__ __forceinline__ void tile_block(const KParams &p, int &bx, int &by) {
     const int nbx = (p.n1 * p.pitch + (int)blockDim.x - 1) / (int)blockDim.x;
     const int lin = blockIdx.x, band = lin / (nbx * TILE_ROWS), r = lin - band * nbx * TILE_ROWS;
@@ -308,7 +314,7 @@ __global__ void k_classify(const __grid_constant__ KParams p, unsigned char *__r
 // direction (c = this cell) the flux difference is K_bc S_bc + K_cd S_cd, S_bc = b + slope(b-a, c-b)/2,
 // S_cd = c + slope(c-b, d-c)/2: 3 loads and 2 slopes per transverse dim; x3: 1 load, 1 slope, the lower flux carried.
 template <int LIM, bool MATTER>
-__global__ void __launch_bounds__(256, 3)
+__global__ void __launch_bounds__(VAC_THREADS, VAC_MINB)
 k_transport_vac(const __grid_constant__ KParams p, const double *__restrict__ I_in, const double *I_base, double *I_out,
                 const unsigned char *__restrict__ cflag, const unsigned char *__restrict__ colflag, double dt) {
     int bx, by;
@@ -577,14 +583,15 @@ static void launch_transport_lim(const KParams &p, const double *I_in, const dou
                                  double *const fcoef[3], const unsigned char *cflag, const unsigned char *colflag, bool matter,
                                  double dt, cudaStream_t st) {
     dim3 grid(((p.n1 * p.pitch + 255) / 256) * p.n2);   // walked in tiles, see tile_block()
+    dim3 gvac(((p.n1 * p.pitch + VAC_THREADS - 1) / VAC_THREADS) * p.n2);
     const double4 *f0 = reinterpret_cast<const double4 *>(fcoef[0]), *f1 = reinterpret_cast<const double4 *>(fcoef[1]),
                   *f2 = reinterpret_cast<const double4 *>(fcoef[2]);
     if (matter) {
-        k_transport_vac<LIM, true><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
+        k_transport_vac<LIM, true><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
         k_transport_gen<LIM, true, false><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
         if (p.ngen) k_transport_gen<LIM, true, true><<<dim3((p.ngen + 127) / 128, 8), 128, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
     } else {
-        k_transport_vac<LIM, false><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
+        k_transport_vac<LIM, false><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
         if (p.ngen) k_transport_gen<LIM, false, true><<<dim3((p.ngen + 127) / 128, 8), 128, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
     }
 }
