@@ -111,6 +111,10 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
     const long long nwork = LIST ? (long long)p.nsrc : p.ncell;
     for (long long widx = warp0; widx < nwork; widx += nwarps) {
         const long long cell = LIST ? (long long)p.srclist[widx] : widx;
+        if (!LIST && widx + nwarps < nwork) {   // next cell of this warp: one 128-byte line per lane, into L2/L1
+            const char *nx = reinterpret_cast<const char *>(I + (widx + nwarps) * p.pitch) + lane * 128;
+            if (lane * 128 < p.pitch * 8) asm volatile("prefetch.global.L1 [%0];" ::"l"(nx));
+        }
         const int col = int(cell % p.ncol);
         const double *cen = p.cen + (long long)col * CEN_STRIDE;
         double *Ic = I + cell * p.pitch;

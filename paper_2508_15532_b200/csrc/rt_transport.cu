@@ -470,7 +470,15 @@ k_transport_gen(const __grid_constant__ KParams p, const double *__restrict__ I_
             qxm2 = __ldg(pn + oxm2); qxm1 = __ldg(pn + oxm1); qxp1 = __ldg(pn + oxp1); qxp2 = __ldg(pn + oxp2);
             qym2 = __ldg(pn + oym2); qym1 = __ldg(pn + oym1); qyp1 = __ldg(pn + oyp1); qyp2 = __ldg(pn + oyp2);
             qw4 = (k + 3 < n3) ? __ldg(pn + 2 * kstride) : slow_ld(p, I_in, 2, i, j, k + 3, s);
-            if (MATTER) qflag = pflag[ncol];
+            if (MATTER) {
+                qflag = pflag[ncol];
+                // the per-face coefficients of the next step: pulled into L1 now (no registers held), so that the
+                // ld4() of step k+1 do not expose an L2 round trip in front of the flux evaluation
+                asm volatile("prefetch.global.L1 [%0];" ::"l"(px + sx));
+                asm volatile("prefetch.global.L1 [%0];" ::"l"(py + sy));
+                asm volatile("prefetch.global.L1 [%0];" ::"l"(py + sy + n1));
+                asm volatile("prefetch.global.L1 [%0];" ::"l"(pz + 2 * ncol));
+            }
         }
         if (mat || general) {
             if (special) {
