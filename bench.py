@@ -110,6 +110,10 @@ def measured_peak():
 # what the method must move at this kernel boundary, fp64 = 8 B.  transport: read I_in, (read I_base when it is a
 # different array: corrector only), write I_out; angular: read I_in, read+write I_inout; source: read+write I.
 ALGO_BYTES = {"transport_pred": 16.0, "transport_corr": 24.0, "angular": 24.0, "source": 16.0}
+# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per launch of each kernel class on config 4 at full size,
+# from the `ncu --set full` capture summarised in profiles/r01_v15_kernels_full.md (transport = vacuum + general +
+# list kernels, mean of the predictor (2.72 GB) and corrector (3.71 GB) launches).  Other configs: not captured -> null.
+NCU_TRAFFIC = {4: {"transport": 3.22e9, "angular": 3.08e9, "source": 0.26e9}}
 
 
 def make_config(args):
@@ -298,7 +302,10 @@ def main():
         achieved = per_unit[dom] * units / (dms / max(dcnt, 1) * 1e-3) / 1e9 if dcnt else 0.0
         step_bytes = sum(per_unit[k] * units * prof[k][1] for k in per_unit) / K
         roof = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": None, "peak_source": which,
+                "frac": achieved / peak,
+                "traffic": NCU_TRAFFIC.get(args.config, {}).get(dom) if args.size is None else None,
+                "traffic_source": "profiles/r01_v15_kernels_full.md (bytes per launch)", "peak_source": which,
+                "algorithmic_bytes_per_launch": per_unit[dom] * units,
                 "algorithmic_bytes_per_cell_dir_per_launch": per_unit[dom],
                 "kernel_ms_per_step": {k: prof[k][0] / K for k in prof},
                 "kernel_launches_per_step": {k: prof[k][1] / K for k in prof},
