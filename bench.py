@@ -204,11 +204,8 @@ def run_gpu(args, rank, world):
         hR = torch.empty(R.shape, dtype=torch.float64, pin_memory=True)
         hG = torch.empty(G.shape, dtype=torch.float64, pin_memory=True)
         ksteps = min(args.steps, 5)
-        def one():
-            I.copy_(hI, non_blocking=True); T.copy_(hT, non_blocking=True)
-            ctx.step(I, T, dt, R, G)
-            hI.copy_(I, non_blocking=True); hT.copy_(T, non_blocking=True)
-            hR.copy_(R, non_blocking=True); hG.copy_(G, non_blocking=True)
+        def one():   # the user-facing C-ABI call with HOST buffers: H2D, rt_step, D2H inside rt_step_host; the state
+            ctx.step_host(hI, hT, dt, hR, hG)   # lives in pinned host memory and evolves from step to step
         one()
         barrier()
         t0 = time.perf_counter()

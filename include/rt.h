@@ -119,6 +119,12 @@ int rt_moments(rt_ctx *ctx, const double *I_dev, double *R_dev, void *stream);
 int rt_step(rt_ctx *ctx, double *I_inout_dev, double *T_inout_dev, double *R_out_dev, double *G_out_dev, double dt,
             int *n_fail_dev, void *stream);
 
+/* rt_step with HOST buffers (pinned memory recommended): copies I[N_c][pitch] and T[N_c] to library-owned device
+ * buffers, runs rt_step, copies I, T and (if not NULL) R[16][N_c], G[4][N_c] back, all on `stream`, and synchronises the
+ * stream before returning.  *n_fail_host (may be NULL) receives the number of cells whose temperature solve failed. */
+int rt_step_host(rt_ctx *ctx, double *I_inout_host, double *T_inout_host, double *R_out_host, double *G_out_host, double dt,
+                 int *n_fail_host, void *stream);
+
 /* Per-kernel device timing (bench.py's roofline): while enabled, every kernel launch is bracketed by CUDA events
  * on its stream.  rt_profile_read synchronises on the last event, returns the accumulated milliseconds and launch
  * counts per kernel class (HOST arrays of RT_K_COUNT entries) and resets the accumulators. */

@@ -25,6 +25,8 @@ struct rt_ctx {
     double *d_rho, *d_u4, *d_T, *d_Th, *d_Ih, *d_fcoef[3];
     unsigned char *d_cflag;   // per cell: any non-vacuum face
     int *d_genlist, *d_srclist;
+    double *d_hI, *d_hT, *d_hR, *d_hG;   // device staging of rt_step_host (allocated on first use)
+    int *d_hfail;
     double *d_mapr_xi, *d_mapr_xim, *d_mapr_a, *d_angraw;
     int *d_mapr_back, *d_mapr_nnb;
     unsigned char *d_angup;
@@ -217,6 +219,7 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     c->d_fcoef[0] = c->d_fcoef[1] = c->d_fcoef[2] = nullptr;
     c->d_cflag = nullptr;
     c->d_colflag = nullptr; c->d_cls = nullptr; c->d_genlist = nullptr; c->d_srclist = nullptr;
+    c->d_hI = c->d_hT = c->d_hR = c->d_hG = nullptr; c->d_hfail = nullptr;
     c->d_mapr_xi = c->d_mapr_xim = c->d_mapr_a = c->d_angraw = nullptr; c->d_mapr_back = c->d_mapr_nnb = nullptr; c->d_angup = nullptr;
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_cls, (size_t)ncol * pitch);
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_cflag, c->ncell);
@@ -307,7 +310,7 @@ extern "C" int rt_free(rt_ctx *c) {
     if (!c) return RT_EINVAL;
     for (int a = 0; a < 3; ++a) { cudaFree(c->tab.face[a]); cudaFree(c->d_fcoef[a]); }
     cudaFree(c->tab.cen); cudaFree(c->tab.ecen); cudaFree(c->tab.angcoef); cudaFree(c->tab.nhat); cudaFree(c->tab.w);
-    cudaFree(c->tab.nb); cudaFree(c->d_cflag); cudaFree(c->d_colflag); cudaFree(c->d_cls); cudaFree(c->d_genlist); cudaFree(c->d_srclist); cudaFree(c->d_mapr_xi); cudaFree(c->d_mapr_xim); cudaFree(c->d_mapr_a);
+    cudaFree(c->tab.nb); cudaFree(c->d_cflag); cudaFree(c->d_colflag); cudaFree(c->d_cls); cudaFree(c->d_genlist); cudaFree(c->d_srclist); cudaFree(c->d_hI); cudaFree(c->d_hT); cudaFree(c->d_hR); cudaFree(c->d_hG); cudaFree(c->d_hfail); cudaFree(c->d_mapr_xi); cudaFree(c->d_mapr_xim); cudaFree(c->d_mapr_a);
     cudaFree(c->d_angraw); cudaFree(c->d_mapr_back); cudaFree(c->d_mapr_nnb); cudaFree(c->d_angup); cudaFree(c->d_rho); cudaFree(c->d_u4); cudaFree(c->d_T); cudaFree(c->d_Th); cudaFree(c->d_Ih);
     delete c;
     return RT_OK;
@@ -526,4 +529,29 @@ extern "C" int rt_step(rt_ctx *c, double *I, double *T, double *R_out, double *G
     int rc = stage(c, I, T, I, c->d_Ih, c->d_Th, 0.5 * dt, n_fail, nullptr, nullptr, st);     // predictor
     if (rc != RT_OK) return rc;
     return stage(c, c->d_Ih, c->d_Th, I, I, T, dt, n_fail, R_out, G_out, st);               // corrector
+}
+
+extern "C" int rt_step_host(rt_ctx *c, double *I_h, double *T_h, double *R_h, double *G_h, double dt, int *n_fail_h, void *stream) {
+    if (!c || !I_h || !T_h) return RT_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t nI = (size_t)c->ncell * c->pitch * sizeof(double), nC = (size_t)c->ncell * sizeof(double);
+    if (!c->d_hI) {
+        CK(cudaMalloc((void **)&c->d_hI, nI));
+        CK(cudaMalloc((void **)&c->d_hT, nC));
+        CK(cudaMalloc((void **)&c->d_hR, 16 * nC));
+        CK(cudaMalloc((void **)&c->d_hG, 4 * nC));
+        CK(cudaMalloc((void **)&c->d_hfail, sizeof(int)));
+    }
+    CK(cudaMemcpyAsync(c->d_hI, I_h, nI, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(c->d_hT, T_h, nC, cudaMemcpyHostToDevice, st));
+    CK(cudaMemsetAsync(c->d_hfail, 0, sizeof(int), st));
+    const int rc = rt_step(c, c->d_hI, c->d_hT, R_h ? c->d_hR : nullptr, G_h ? c->d_hG : nullptr, dt, c->d_hfail, stream);
+    if (rc != RT_OK) return rc;
+    CK(cudaMemcpyAsync(I_h, c->d_hI, nI, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(T_h, c->d_hT, nC, cudaMemcpyDeviceToHost, st));
+    if (R_h) CK(cudaMemcpyAsync(R_h, c->d_hR, 16 * nC, cudaMemcpyDeviceToHost, st));
+    if (G_h) CK(cudaMemcpyAsync(G_h, c->d_hG, 4 * nC, cudaMemcpyDeviceToHost, st));
+    if (n_fail_h) CK(cudaMemcpyAsync(n_fail_h, c->d_hfail, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return RT_OK;
 }

@@ -17,7 +17,7 @@ METRIC = {"minkowski": 0, "mink_cyl": 1, "ks_mks": 2}
 GEOM = dict(g_c=0, e_c=1, einv_c=2, sqrtg_c=3, omega_c=4, n0_c=5, angcoef=6)
 SYMBOLS = ["rt_init", "rt_free", "rt_ndir", "rt_ndir_padded", "rt_get_directions", "rt_get_geometry", "rt_cfl_dt",
            "rt_set_boundary", "rt_set_fluid", "rt_transport", "rt_angular_flux", "rt_source_implicit", "rt_moments",
-           "rt_step", "rt_profile_enable", "rt_profile_read", "rt_launch_count", "rt_last_cuda_error", "rt_strerror"]
+           "rt_step", "rt_step_host", "rt_profile_enable", "rt_profile_read", "rt_launch_count", "rt_last_cuda_error", "rt_strerror"]
 
 
 class RtGrid(ctypes.Structure):
@@ -58,6 +58,7 @@ def load_library(path=LIB_PATH):
     lib.rt_source_implicit.argtypes = [vp, vp, vp, dbl, vp, vp]
     lib.rt_moments.argtypes = [vp, vp, vp, vp]
     lib.rt_step.argtypes = [vp, vp, vp, vp, vp, dbl, vp, vp]
+    lib.rt_step_host.argtypes = [vp, vp, vp, vp, vp, dbl, vp, vp]
     lib.rt_profile_enable.argtypes = [vp, ci]
     lib.rt_profile_read.argtypes = [vp, vp, vp]
     lib.rt_launch_count.argtypes = [vp]
@@ -194,6 +195,15 @@ class RtContext:
 
     def step(self, I, T, dt, R=None, G=None):
         _check(lib().rt_step(self._h, _ptr(I), _ptr(T), _ptr(R), _ptr(G), float(dt), _ptr(self._nfail), _stream()))
+
+    def step_host(self, I_host, T_host, dt, R_host=None, G_host=None):
+        """rt_step_host: HOST tensors (pinned fp64, padded layout); returns the failed-cell count of this call."""
+        nf = ctypes.c_int(0)
+        hp = lambda t: None if t is None else ctypes.c_void_p(t.data_ptr())
+        for t in (I_host, T_host, R_host, G_host):
+            assert t is None or (not t.is_cuda and t.dtype == torch.float64 and t.is_contiguous())
+        _check(lib().rt_step_host(self._h, hp(I_host), hp(T_host), hp(R_host), hp(G_host), float(dt), ctypes.byref(nf), _stream()))
+        return nf.value
 
     def n_fail(self):
         return int(self._nfail.item())

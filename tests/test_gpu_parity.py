@@ -178,3 +178,19 @@ def test_mapr_rotating_tetrad_per_call():
     ref = orc.angular_flux(I0, I0, 0.1 * dt).reshape(I0.shape)
     assert rel_err(ctx.to_host(out), ref) <= TOL
     assert np.abs(ref - I0).max() > 1e-5
+
+
+def test_step_host_equals_step_bitwise():
+    """rt_step_host (host buffers, copies inside the call) returns exactly what rt_step returns on device buffers."""
+    import torch
+    cfg = W.config(4, n=(12, 10, 4))
+    orc, ctx, f, dt = make_pair(cfg)
+    I = ctx.to_device(f["I0"]); T = torch.as_tensor(f["T"], device=ctx.device).contiguous().clone()
+    R = torch.zeros((16,) + ctx.shape, dtype=torch.float64, device=ctx.device); G = torch.zeros((4,) + ctx.shape, dtype=torch.float64, device=ctx.device)
+    hI, hT = I.cpu().pin_memory(), T.cpu().pin_memory()
+    hR, hG = torch.zeros(R.shape, dtype=torch.float64).pin_memory(), torch.zeros(G.shape, dtype=torch.float64).pin_memory()
+    for _ in range(2):
+        ctx.step(I, T, dt, R, G)
+        assert ctx.step_host(hI, hT, dt, hR, hG) == 0
+    for a, b in ((I, hI), (T, hT), (R, hR), (G, hG)):
+        assert torch.equal(a.cpu(), b)
