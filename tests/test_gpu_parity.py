@@ -194,3 +194,66 @@ def test_step_host_equals_step_bitwise():
         assert ctx.step_host(hI, hT, dt, hR, hG) == 0
     for a, b in ((I, hI), (T, hT), (R, hR), (G, hG)):
         assert torch.equal(a.cpu(), b)
+
+
+def test_geometry_tables_n0_and_angular_coefficients():
+    """rt_get_geometry RT_GEOM_N0_C and RT_GEOM_ANGCOEF against the same quantities formed from the oracle's tables."""
+    cfg = W.config(4, n=(10, 8, 3))
+    orc, ctx, f, dt = make_pair(cfg)
+    e, g, om = orc.tab["e_c"], orc.tab["g_c"], orc.tab["omega_c"]
+    A = orc.ang
+    n = e[..., :, 0][..., None, :] + np.einsum("...mi,si->...sm", e[..., :, 1:], A["nhat"])
+    n0 = np.einsum("...m,...sm->...s", g[..., 0, :], n)
+    assert rel_err(ctx.geometry("n0_c"), n0) < 1e-13
+    coef = np.zeros(n0.shape[:-1] + (6, orc.nd))
+    for s in range(orc.nd):
+        for ed in range(A["nnb"][s]):
+            m4 = np.concatenate([[1.0], A["emid"][s, ed]])
+            V = -np.einsum("i,...icd,c,d->...", A["eun"][s, ed], om[..., 1:, :, :], m4, m4)
+            n0e = np.einsum("...m,...ma,a->...", g[..., 0, :], e, m4)
+            t = A["nb"][s, ed]
+            gate = np.sign(n0[..., s]) != np.sign(n0[..., t])
+            coef[..., ed, s] = np.where(gate, 0.0, A["dlam"][s, ed] * n0e * V / A["w"][s])
+    assert rel_err(ctx.geometry("angcoef"), coef) < 1e-9
+
+
+def test_zero_and_fixed_boundaries_all_dims():
+    """ZERO ghosts and FIXED ghosts on x2 / x3 faces (config 1 only exercises a fixed x1-low face)."""
+    import torch
+    cfg = W.config(3, n=(7, 6, 5))
+    cfg["grid"] = dict(cfg["grid"], bc_lo=("zero", "fixed", "fixed"), bc_hi=("fixed", "zero", "outflow"))
+    cfg["options"] = dict(cfg["options"], kappa_s=2.0)
+    orc, ctx, f, dt = make_pair(cfg)
+    rng = np.random.default_rng(5)
+    f["I0"] = rng.uniform(0.1, 1.0, size=f["I0"].shape)
+    n1, n2, n3 = cfg["grid"]["n"]
+    for dim, side, nface in ((0, 1, n2 * n3), (1, 0, n1 * n3), (2, 0, n1 * n2)):
+        gh = rng.uniform(0.1, 1.0, size=(2, nface, orc.nd))
+        orc.set_boundary(dim, side, gh)
+        gd = torch.zeros((2, nface, ctx.pitch), dtype=torch.float64, device=ctx.device)
+        gd[..., :ctx.nd] = torch.as_tensor(gh, device=ctx.device)
+        ctx.set_boundary(dim, side, gd)
+    _check(run_steps(orc, ctx, f, dt, 4))
+
+
+def test_error_codes():
+    import ctypes
+    import torch
+    from paper_2508_15532_b200 import rt
+    lib = rt.lib()
+    cfg = W.config(1, n=(8, 8, 1))
+    kind, params = cfg["metric"]
+    ctx = rt.RtContext(cfg["grid"], kind, params, cfg["level"], cfg["options"])
+    I = torch.zeros(ctx.shape + (ctx.pitch,), dtype=torch.float64, device=ctx.device)
+    T = torch.ones(ctx.shape, dtype=torch.float64, device=ctx.device)
+    with pytest.raises(rt.RtError, match="call order"):          # fluid not set
+        ctx.step(I, T, 0.01)
+    ctx.set_fluid(torch.zeros_like(T), T)
+    with pytest.raises(rt.RtError, match="call order"):          # FIXED boundary without ghost values
+        ctx.step(I, T, 0.01)
+    with pytest.raises(rt.RtError, match="invalid argument"):    # in-place transport is not allowed
+        ctx.transport(I, I, I, 0.01)
+    bad = dict(cfg["grid"], bc_lo=("periodic", "outflow", "periodic"))   # periodic on one side only
+    with pytest.raises(rt.RtError, match="invalid argument"):
+        rt.RtContext(bad, kind, params, cfg["level"], cfg["options"])
+    assert lib.rt_strerror(-4) == b"call order: fluid or boundary data not set"
