@@ -95,8 +95,12 @@ __device__ __forceinline__ double rotate(const double M[10], const double *__res
     return r;
 }
 
+#ifndef CELL_THREADS
+#define CELL_THREADS 256
+#define CELL_MINB 3
+#endif
 template <int MAXV, bool SRC, bool MOM, bool LIST>
-__global__ void __launch_bounds__(256, 3)
+__global__ void __launch_bounds__(CELL_THREADS, CELL_MINB)
 k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, double *G_out) {
     extern __shared__ double tab[];   // nx[pitch] ny[pitch] nz[pitch] w[pitch]
     for (int t = threadIdx.x; t < 3 * p.pitch; t += blockDim.x) tab[t] = p.nhat[t];
@@ -249,9 +253,9 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
 
 template <bool SRC, bool MOM, bool LIST>
 cudaError_t launch_cell(const KParams &p, double *I, double *T, double dt, int *n_fail, double *R, double *G, cudaStream_t st) {
-    const int threads = 256;
+    const int threads = CELL_THREADS;
     const long long nwork = LIST ? (long long)p.nsrc : p.ncell;
-    long long want = (nwork + 7) / 8;
+    long long want = (nwork + threads / 32 - 1) / (threads / 32);
     const int blocks = (int)(want < 148LL * 8 * 4 ? want : 148LL * 8 * 4);
     if (blocks == 0) return cudaSuccess;
     const size_t smem = 4 * p.pitch * sizeof(double);
