@@ -223,7 +223,7 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     c->d_mapr_xi = c->d_mapr_xim = c->d_mapr_a = c->d_angraw = nullptr; c->d_mapr_back = c->d_mapr_nnb = nullptr; c->d_angup = nullptr;
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_cls, (size_t)ncol * pitch);
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_cflag, c->ncell);
-    if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_colflag, (size_t)c->ncol * (2 + n3 / 8));   // column flags + x3-chunk flags (GEN_KC = 8)
+    if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_colflag, colflag_bytes(c->ncol, n3));   // column flags, x3-chunk flags, cell-flag masks
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_rho, c->ncell * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_u4, 4 * c->ncell * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_T, c->ncell * sizeof(double));

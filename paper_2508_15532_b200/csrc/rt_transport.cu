@@ -205,18 +205,28 @@ __device__ __forceinline__ int nb_index(int c, int N, int bc_lo, int bc_hi) {
 
 // column flags: bit 0 = the column has a cell with a non-vacuum face, bit 1 = it has an all-vacuum cell
 // colflag[ncol + kc * ncol + col]: the x3 chunk [kc*GEN_KC, (kc+1)*GEN_KC) of the column has such a cell
+// column masks (32-bit words behind the flags, colmask_offset()): bit (k & 31) of word [(k >> 5) * ncol + col] = cell
+// flag of (col, k).  The marching kernels test a bit per step and load one word per 32 steps: a per-step flag load sat
+// in front of every step's branch and exposed its L2 latency (it was 70 % of the vacuum kernel's long-scoreboard stalls).
 constexpr int GEN_KC = 8;
 __global__ void k_colflag(KParams p, const unsigned char *__restrict__ cflag, unsigned char *__restrict__ colflag) {
     const int col = blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= p.ncol) return;
+    unsigned *cmask = reinterpret_cast<unsigned *>(colflag + colmask_offset(p.ncol, p.n3));
     int m = 0, mc = 0;
+    unsigned mw = 0;
     for (int k = 0; k < p.n3; ++k) {
         const int f = cflag[(long long)k * p.ncol + col];
         m |= f ? 1 : 2;
         mc |= f;
+        if (f) mw |= 1u << (k & 31);
         if ((k + 1) % GEN_KC == 0 || k + 1 == p.n3) {
             colflag[p.ncol + (long long)(k / GEN_KC) * p.ncol + col] = (unsigned char)mc;
             mc = 0;
+        }
+        if ((k & 31) == 31 || k + 1 == p.n3) {
+            cmask[(long long)(k >> 5) * p.ncol + col] = mw;
+            mw = 0;
         }
     }
     colflag[col] = (unsigned char)m;
@@ -231,6 +241,11 @@ __global__ void k_colflag(KParams p, const unsigned char *__restrict__ cflag, un
 // Block order of the marching kernels: a 1-D grid walked in bands of TILE_ROWS x2-rows with x2 fastest inside a band,
 // so that the CTAs resident at the same time cover a compact (x1, x2) patch and their transverse neighbours are
 // read from L2 instead of DRAM (row-major order re-reads ~4 halo rows per wave of ~5 rows).
+// how many x3-planes beyond the register pipeline the vacuum kernel prefetches its operands (0 = off)
+#ifndef VAC_PF
+#define VAC_PF 2
+#endif
+__device__ __forceinline__ void pf_l1(const void *q) { asm volatile("prefetch.global.L1 [%0];" ::"l"(q)); }
 constexpr int TILE_ROWS = 24;
 #ifndef VAC_THREADS
 #define VAC_THREADS 128
@@ -314,7 +329,7 @@ __global__ void k_classify(const __grid_constant__ KParams p, unsigned char *__r
 // per-thread constant (the sign of n^a_f).  With (a, b, c, d) = four cells of a dim ordered along the propagation
 // direction (c = this cell) the flux difference is K_bc S_bc + K_cd S_cd, S_bc = b + slope(b-a, c-b)/2,
 // S_cd = c + slope(c-b, d-c)/2: 3 loads and 2 slopes per transverse dim; x3: 1 load, 1 slope, the lower flux carried.
-template <int LIM, bool MATTER>
+template <int LIM, bool MATTER, bool SAME_BASE>
 __global__ void __launch_bounds__(VAC_THREADS, VAC_MINB)
 k_transport_vac(const __grid_constant__ KParams p, const double *__restrict__ I_in, const double *I_base, double *I_out,
                 const unsigned char *__restrict__ cflag, const unsigned char *__restrict__ colflag, double dt) {
@@ -356,24 +371,31 @@ k_transport_vac(const __grid_constant__ KParams p, const double *__restrict__ I_
         Flo = zA * fma(zhalf, sg, zpos ? w1 : w2);
     }
     const double *pb = I_base + pos0;
-    const bool same_base = (I_base == I_in);
-    const unsigned char *pflag = cflag + c.col;
+    const unsigned *pmask = reinterpret_cast<const unsigned *>(colflag + colmask_offset(ncol, n3)) + c.col;
     const int zlo = p.zlo[2], zhi = n3 - p.zhi[2];
+    unsigned mcur = MATTER ? __ldg(pmask) : 0u, mnext = (MATTER && n3 > 32) ? __ldg(pmask + ncol) : 0u;
     double qxa = __ldg(pk + oxa), qxb = __ldg(pk + oxb), qxd = __ldg(pk + oxd);
     double qya = __ldg(pk + oya), qyb = __ldg(pk + oyb), qyd = __ldg(pk + oyd);
     double qw4 = ldk(2);
-    double qbase = same_base ? 0.0 : *pb;
-    unsigned char qflag = MATTER ? *pflag : 0;
+    double qbase = SAME_BASE ? 0.0 : *pb;
     for (int k = 0; k < n3; ++k) {
         const double xa = qxa, xb = qxb, xd = qxd, ya = qya, yb = qyb, yd = qyd, w4 = qw4, cbase = qbase;
-        const bool mat = MATTER && qflag != 0;
+        const bool mat = MATTER && ((mcur >> (k & 31)) & 1u);
         if (k + 1 < n3) {   // request the operands of step k + 1 before computing step k
             const double *pn = pk + kstride;
-            if (!same_base) qbase = pb[kstride];
+            if (!SAME_BASE) qbase = pb[kstride];
             qxa = __ldg(pn + oxa); qxb = __ldg(pn + oxb); qxd = __ldg(pn + oxd);
             qya = __ldg(pn + oya); qyb = __ldg(pn + oyb); qyd = __ldg(pn + oyd);
             qw4 = (k + 3 < n3) ? __ldg(pn + 2 * kstride) : slow_ld(p, I_in, 2, i, j, k + 3, s);
-            if (MATTER) qflag = pflag[ncol];
+#if VAC_PF
+            if (k + VAC_PF + 1 < n3) {   // operands of step k + 1 + VAC_PF: pulled towards the SM now (no registers held)
+                const double *pf = pn + VAC_PF * kstride;
+                pf_l1(pf + oxa); pf_l1(pf + oxb); pf_l1(pf + oxd);
+                pf_l1(pf + oya); pf_l1(pf + oyb); pf_l1(pf + oyd);
+                if (k + VAC_PF + 3 < n3) pf_l1(pf + 2 * kstride);
+                if (!SAME_BASE) pf_l1(pb + (VAC_PF + 1) * kstride);
+            }
+#endif
         }
         // x3: upwind state at the upper face (always formed: it is the next cell's lower flux if that cell is vacuum)
         const double sz = slope_k<LIM>(w3 - w2, zpos ? (w2 - w1) : (w4 - w3));
@@ -390,13 +412,22 @@ k_transport_vac(const __grid_constant__ KParams p, const double *__restrict__ I_
                 D = fma(Kybc, fma(0.5, slope_k<LIM>(d1, d2), yb), D);
                 D = fma(Kycd, fma(0.5, slope_k<LIM>(d2, d3), w2), D);
             }
-            const double base = same_base ? w2 : cbase;
-            *out = (k < zlo || k >= zhi) ? 0.0 : base - D;      // Eq 18 (O5), dt/(n^0 n_0 sqrt(-g) dx) folded in
+            const double base = SAME_BASE ? w2 : cbase;
+            *out = base - D;      // Eq 18 (O5), dt/(n^0 n_0 sqrt(-g) dx) folded in; the x3 zero band is reset below
         }
         Flo = Fhi;
         w1 = w2; w2 = w3; w3 = w4;
         pk += kstride; pb += kstride; out += kstride;
-        if (MATTER) pflag += ncol;
+        if (MATTER && (k & 31) == 31) {   // next mask word (requested 32 steps ago)
+            mcur = mnext;
+            pmask += ncol;
+            mnext = (k + 33 < n3) ? __ldg(pmask + ncol) : 0u;
+        }
+    }
+    if (zlo > 0 || zhi < n3) {   // zero band in x3 (L709): reset after the march instead of a select in every step
+        double *o = I_out + pos0;
+        for (int k = 0; k < n3; ++k)
+            if (k < zlo || k >= zhi) o[k * kstride] = 0.0;
     }
 }
 
@@ -447,7 +478,7 @@ k_transport_gen(const __grid_constant__ KParams p, const double *__restrict__ I_
     double *out = I_out + pos0 + k0 * kstride;
     const bool same_base = (I_base == I_in);
     const int sx = p.n2 * (n1 + 1), sy = (p.n2 + 1) * n1;
-    const unsigned char *pflag = cflag + c.col + (long long)k0 * ncol;
+    const unsigned *pmask = reinterpret_cast<const unsigned *>(colflag + colmask_offset(ncol, n3)) + c.col + (long long)(k0 >> 5) * ncol;
     const double4 *px = fc0 + ((long long)j * (n1 + 1) + i) + (long long)k0 * sx, *py = fc1 + ((long long)j * n1 + i) + (long long)k0 * sy,
                   *pz = fc2 + c.col + (long long)k0 * ncol;
     const int zlo = p.zlo[2], zhi = n3 - p.zhi[2];
@@ -460,11 +491,11 @@ k_transport_gen(const __grid_constant__ KParams p, const double *__restrict__ I_
     double qym2 = __ldg(pk + oym2), qym1 = __ldg(pk + oym1), qyp1 = __ldg(pk + oyp1), qyp2 = __ldg(pk + oyp2);
     double qw4 = ldk(k0 + 2);
     double qbase = same_base ? 0.0 : *pb;
-    unsigned char qflag = MATTER ? *pflag : 0;
+    unsigned mcur = MATTER ? __ldg(pmask) : 0u, mnext = (MATTER && (k0 | 31) + 1 < k1) ? __ldg(pmask + ncol) : 0u;
     for (int k = k0; k < k1; ++k) {
         double xm2 = qxm2, xm1 = qxm1, xp1 = qxp1, xp2 = qxp2, ym2 = qym2, ym1 = qym1, yp1 = qyp1, yp2 = qyp2;
         const double w4 = qw4, cbase = qbase;
-        const bool mat = MATTER && qflag != 0;
+        const bool mat = MATTER && ((mcur >> (k & 31)) & 1u);
         if (k + 1 < k1) {
             if (!same_base) qbase = pb[kstride];
             const double *pn = pk + kstride;
@@ -472,7 +503,6 @@ k_transport_gen(const __grid_constant__ KParams p, const double *__restrict__ I_
             qym2 = __ldg(pn + oym2); qym1 = __ldg(pn + oym1); qyp1 = __ldg(pn + oyp1); qyp2 = __ldg(pn + oyp2);
             qw4 = (k + 3 < n3) ? __ldg(pn + 2 * kstride) : slow_ld(p, I_in, 2, i, j, k + 3, s);
             if (MATTER) {
-                qflag = pflag[ncol];
                 // the per-face coefficients of the next step: pulled into L1 now (no registers held), so that the
                 // ld4() of step k+1 do not expose an L2 round trip in front of the flux evaluation
                 asm volatile("prefetch.global.L1 [%0];" ::"l"(px + sx));
@@ -502,7 +532,12 @@ k_transport_gen(const __grid_constant__ KParams p, const double *__restrict__ I_
             *out = (k < zlo || k >= zhi) ? 0.0 : base - D;
         }
         w0 = w1; w1 = w2; w2 = w3; w3 = w4;
-        pk += kstride; pb += kstride; out += kstride; pflag += ncol; px += sx; py += sy; pz += ncol;
+        pk += kstride; pb += kstride; out += kstride; px += sx; py += sy; pz += ncol;
+        if (MATTER && (k & 31) == 31) {   // next mask word (requested 32 steps ago)
+            mcur = mnext;
+            pmask += ncol;
+            mnext = (k + 33 < k1) ? __ldg(pmask + ncol) : 0u;
+        }
     }
 }
 
@@ -596,11 +631,13 @@ static void launch_transport_lim(const KParams &p, const double *I_in, const dou
     const double4 *f0 = reinterpret_cast<const double4 *>(fcoef[0]), *f1 = reinterpret_cast<const double4 *>(fcoef[1]),
                   *f2 = reinterpret_cast<const double4 *>(fcoef[2]);
     if (matter) {
-        k_transport_vac<LIM, true><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
+        if (I_base == I_in) k_transport_vac<LIM, true, true><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
+        else k_transport_vac<LIM, true, false><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
         k_transport_gen<LIM, true, false><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
         if (p.ngen) k_transport_gen<LIM, true, true><<<dim3((p.ngen + 127) / 128, 8), 128, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
     } else {
-        k_transport_vac<LIM, false><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
+        if (I_base == I_in) k_transport_vac<LIM, false, true><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
+        else k_transport_vac<LIM, false, false><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
         if (p.ngen) k_transport_gen<LIM, false, true><<<dim3((p.ngen + 127) / 128, 8), 128, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
     }
 }
