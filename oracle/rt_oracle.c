@@ -369,8 +369,10 @@ static void teq_eval(const teq *q, double T, double *f, double *df) {
         *f = -F; *df = -dF;
     }
 }
-/* Newton-Raphson (L399) from the guess T_-, safeguarded by the bracket (0, W/Y] (S20).  returns 0 on
- * success, 1 if there is no positive root (T left unchanged). */
+/* Newton-Raphson (L399) from the guess T_-, safeguarded by the bracket (0, W/Y] (S20): an iterate outside the
+ * CLOSED current bracket [lo, hi] (or not positive) is replaced by the midpoint.  Closed, because for pure scattering
+ * the root is T_- itself, i.e. the first iterate lands on a bracket end; an open test would reject it and bisect ~45
+ * times towards the same number.  returns 0 on success, 1 if there is no positive root (T left unchanged). */
 static int solve_T(const teq *q, double Tminus, double Thi, double *Tplus) {
     double lo = 0.0, hi = Thi, f, df;
     if (!(Thi > 0.0)) return 1;
@@ -382,7 +384,7 @@ static int solve_T(const teq *q, double Tminus, double Thi, double *Tplus) {
         teq_eval(q, T, &f, &df);
         if (f < 0) lo = T; else hi = T;
         double Tn = T - f / df;
-        if (!(Tn > lo && Tn < hi)) Tn = 0.5 * (lo + hi);
+        if (!(Tn > 0.0 && Tn >= lo && Tn <= hi)) Tn = 0.5 * (lo + hi);   /* closed bracket: a root AT an end (T+ = T-) is kept */
         double d = Tn - T;
         T = Tn;
         if (fabs(d) <= 1e-14 * T) break;

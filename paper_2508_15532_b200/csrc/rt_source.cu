@@ -63,7 +63,7 @@ __device__ __forceinline__ bool solve_T(const TEq &q, double Tm, double Thi, dou
         teq_eval(q, T, f, df);
         if (f < 0) lo = T; else hi = T;
         double Tn = T - f / df;
-        if (!(Tn > lo && Tn < hi)) Tn = 0.5 * (lo + hi);
+        if (!(Tn > 0.0 && Tn >= lo && Tn <= hi)) Tn = 0.5 * (lo + hi);   // closed bracket (S20): a root at an end is kept
         const double d = Tn - T;
         T = Tn;
         if (fabs(d) <= 1e-14 * T) break;
