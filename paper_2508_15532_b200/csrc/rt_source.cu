@@ -100,7 +100,7 @@ __device__ __forceinline__ double rotate(const double M[10], const double *__res
 #define CELL_MINB 3
 #endif
 template <int MAXV, bool SRC, bool MOM, bool LIST>
-__global__ void __launch_bounds__(CELL_THREADS, CELL_MINB)
+__global__ void __launch_bounds__(CELL_THREADS, (MAXV > 6 ? CELL_MINB - 1 : CELL_MINB))   // 362 directions: 12 values + 24 kept coefficients per lane
 k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, double *G_out) {
     extern __shared__ double tab[];   // nx[pitch] ny[pitch] nz[pitch] w[pitch]
     for (int t = threadIdx.x; t < 3 * p.pitch; t += blockDim.x) tab[t] = p.nhat[t];
@@ -172,9 +172,12 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
                 if (lane < 4) Rb = rotate(Mb, ecen, L, 0, lane);
             }
             double E = 0.0, A1 = 0.0, A2 = 0.0;
+            // kept for the update loop below: ca = n^0/d (0 marks a masked or pad entry), cb = 1/(d nbar^3)
+            double ca[MAXV], cb[MAXV];
 #pragma unroll
             for (int v = 0; v < MAXV; ++v) {
                 const int s = lane + 32 * v;
+                ca[v] = 0.0; cb[v] = 0.0;
                 if (s < p.nd) {
                     const double nx = snx[s], ny = sny[s], nz = snz[s], ws = sw[s];
                     const double n0c = cen[0] + cen[1] * nx + cen[2] * ny + cen[3] * nz;
@@ -186,6 +189,8 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
                         E += IbdOm;                                                         // Eq 33
                         A1 += nup * rd * IbdOm;                                             // Eq 41a
                         A2 += ws * rn * rd;                                                 // Eq 41b
+                        ca[v] = nup * rd;
+                        cb[v] = rd * (rn * rn * rn);
                     }
                 }
             }
@@ -212,18 +217,10 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
                 const double Sdt = (emis + as * Ep) * (dt / FOURPI);
 #pragma unroll
                 for (int v = 0; v < MAXV; ++v) {
-                    const int s = lane + 32 * v;
-                    if (s < p.nd) {
-                        const double nx = snx[s], ny = sny[s], nz = snz[s];
-                        const double n0c = cen[0] + cen[1] * nx + cen[2] * ny + cen[3] * nz;
-                        if (!(n0c > -p.n0_floor)) {
-                            const double nup = cen[4] + cen[5] * nx + cen[6] * ny + cen[7] * nz;
-                            const double nbar = uh0 - (uh1 * nx + uh2 * ny + uh3 * nz);
-                            const double rd = __drcp_rn(nup + nbar * alpha * dt), rn = __drcp_rn(nbar);
-                            // Eq 35 divided by nbar^4 (L432): I+ = [n^0/d] I- + [nbar dt/(4 pi d)] S / nbar^4
-                            val[v] = scale * rd * (nup * val[v] + Sdt * (rn * rn * rn));
-                            Ic[s] = val[v];
-                        }
+                    if (ca[v] != 0.0) {   // (n^0/d > 0 for every unmasked direction)
+                        // Eq 35 divided by nbar^4 (L432): I+ = [n^0/d] I- + [nbar dt/(4 pi d)] S / nbar^4
+                        val[v] = scale * (ca[v] * val[v] + Sdt * cb[v]);
+                        Ic[lane + 32 * v] = val[v];
                     }
                 }
                 if (lane == 0) T[cell] = Tp;
