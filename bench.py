@@ -31,7 +31,7 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index 1..5 (4 = Kerr-Schild, the roofline config)")
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index 1..5 (4 = Kerr-Schild, the roofline config); 6 = snake-coordinates beam (PAPER 4.6)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -224,7 +224,7 @@ def run_gpu(args, rank, world):
 
 
 # ---- oracle legs (the only places bench.py may execute oracle/) ----------------------------------------------------
-ORACLE_SAMPLE = {1: (64, 64, 1), 2: (24, 24, 24), 3: (24, 24, 24), 4: (64, 48, 16), 5: (32, 24, 8)}
+ORACLE_SAMPLE = {1: (64, 64, 1), 2: (24, 24, 24), 3: (24, 24, 24), 4: (64, 48, 16), 5: (32, 24, 8), 6: (64, 64, 1)}
 
 
 def run_oracle(cfg_index, steps, warmup=0):

@@ -34,7 +34,7 @@ extern "C" {
 #define RT_ESTATE (-4)  /* call order: fluid / boundary not set */
 
 enum { RT_BC_PERIODIC = 0, RT_BC_OUTFLOW = 1, RT_BC_ZERO = 2, RT_BC_FIXED = 3 };
-enum { RT_MINKOWSKI_CART = 0, RT_MINK_CYL_TETRAD = 1, RT_KS_MKS = 2 };
+enum { RT_MINKOWSKI_CART = 0, RT_MINK_CYL_TETRAD = 1, RT_KS_MKS = 2, RT_SNAKE = 3 };
 enum { RT_LIM_MC = 0, RT_LIM_MINMOD = 1, RT_LIM_VANLEER = 2, RT_LIM_NONE = 3 };
 enum { RT_ANG_DONOR = 0, RT_ANG_MAPR = 1 };
 /* rt_get_geometry selectors (host output, for table-level parity of the init precompute) */
@@ -61,9 +61,11 @@ typedef struct {
 /* Metric + tetrad (L57-79, App. A).  x3_symmetric: geometry independent of x^3 (tables stored per (x1,x2) column,
  * the paper's own optimisation, L776); required for RT_KS_MKS, ignored (constant geometry) for RT_MINKOWSKI_CART. */
 typedef struct {
-    int kind;         /* RT_MINKOWSKI_CART | RT_MINK_CYL_TETRAD | RT_KS_MKS */
+    int kind;         /* RT_MINKOWSKI_CART | RT_MINK_CYL_TETRAD | RT_KS_MKS | RT_SNAKE */
     double a, hslope; /* RT_KS_MKS: spin, theta-map parameter h: r = exp(x1), theta = pi x2 + (1-h)/2 sin(2 pi x2), phi = x3 */
     int x3_symmetric;
+    double snake_A, snake_k; /* RT_SNAKE (App A.1): flat space in (t, w, y, z), w = x - A sin(k pi y); metric Eq A1,
+                                Cartesian-aligned tetrad (Eq A2 read as the co-frame, DESIGN S27): omega = 0, n^w = n^x - delta n^y */
 } rt_metric;
 
 typedef struct {

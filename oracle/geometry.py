@@ -16,6 +16,11 @@ Metric kinds
                theta = pi x2 + (1-h)/2 sin(2 pi x2), phi = x3 (S26).  Tetrad = A3-A4 with reading S25:
                alpha is the LAPSE (1+2r/Sigma)^(-1/2) (A5b prints its inverse; A4a and Eq 4 need the lapse),
                gamma^{ij} is the INVERSE of the 3-metric gamma_ij = g_ij (A5d as printed gives a non-unit e_r).
+  'snake'      flat space in snake coordinates (t, w, y, z), w = x - A sin(k pi y) (App A.1): metric A1
+               with delta = A k pi cos(k pi y); tetrad A2 under reading S27: the printed matrix is the CO-frame
+               e^{a-hat}_mu = [[1,0,0,0],[0,1,delta,0],[0,0,1,0],[0,0,0,1]] (rows dt, dx = dw + delta dy, dy, dz) with
+               its second row's two entries transposed in print -- as printed neither the matrix nor its transpose is
+               orthonormal in A1 (Eq 1 fails), the co-frame reading is.  It is the Cartesian frame, so omega = 0.
 Finite differences (S15): 4th-order central, h = 1e-3 in logical coordinates.
 """
 import numpy as np
@@ -49,11 +54,24 @@ def _ks_metric_phys(a, r, th):
     return g, Sig, H
 
 
+def _snake_delta(params, X):
+    """delta = A k pi cos(k pi y) (below Eq A1); y is the second logical coordinate."""
+    A, k = params["A"], params["k"]
+    return A * k * np.pi * np.cos(k * np.pi * X[..., 1])
+
+
 def metric(kind, params, X):
     """Covariant metric g_{mu nu} at logical points X[..., 3]."""
     X = np.asarray(X, dtype=np.float64)
     if kind in ("minkowski", "mink_cyl"):
         return np.broadcast_to(ETA, X.shape[:-1] + (4, 4)).copy()
+    if kind == "snake":
+        d = _snake_delta(params, X)
+        g = np.broadcast_to(ETA, X.shape[:-1] + (4, 4)).copy()   # Eq A1
+        g[..., 1, 2] = d
+        g[..., 2, 1] = d
+        g[..., 2, 2] = 1.0 + d * d
+        return g
     if kind == "ks_mks":
         r, th, drdx, dthdx = _ks_map(params, X)
         g, _, _ = _ks_metric_phys(params["a"], r, th)
@@ -83,6 +101,11 @@ def tetrad(kind, params, X):
         e[..., 3, 3] = 1.0
         einv = np.swapaxes(e, -1, -2).copy()  # orthogonal matrix in flat space
         return e, einv
+    if kind == "snake":
+        d = _snake_delta(params, X)
+        einv = np.broadcast_to(np.eye(4), shp + (4, 4)).copy()   # Eq A2 read as the co-frame (S27)
+        einv[..., 1, 2] = d
+        return np.linalg.inv(einv), einv
     if kind == "ks_mks":
         r, th, drdx, dthdx = _ks_map(params, X)
         g, Sig, H = _ks_metric_phys(params["a"], r, th)

@@ -44,11 +44,19 @@ bool invert44(const double a[4][4], double inv[4][4], double *det_out) {
     return true;
 }
 
+// d x / d y at fixed w in snake coordinates (L806)
+double snake_delta(const rt_metric &mt, double y) { return mt.snake_A * mt.snake_k * PI * std::cos(mt.snake_k * PI * y); }
+
 // covariant metric in logical coordinates
 void metric_at(const rt_metric &mt, const double x[3], double g[4][4]) {
     zero44(g);
     if (mt.kind != RT_KS_MKS) {
         g[0][0] = -1; g[1][1] = g[2][2] = g[3][3] = 1;
+        if (mt.kind == RT_SNAKE) {   // x = w + A sin(k pi y):  dx = dw + delta dy  =>  ds^2 = -dt^2 + (dw + delta dy)^2 + dy^2 + dz^2
+            const double dl = snake_delta(mt, x[1]);
+            g[1][2] = g[2][1] = dl;
+            g[2][2] += dl * dl;
+        }
         return;
     }
     const double a = mt.a, h = mt.hslope;
@@ -92,6 +100,13 @@ void eval_point(const rt_metric &mt, const double x[3], PointGeom &o) {
         o.e[1][1] = x[0] / R; o.e[2][1] = x[1] / R;
         o.e[1][2] = -x[1] / R; o.e[2][2] = x[0] / R;
         for (int a = 0; a < 4; ++a) for (int mu = 0; mu < 4; ++mu) o.einv[a][mu] = o.e[mu][a];
+        return;
+    }
+    if (mt.kind == RT_SNAKE) {   // the Cartesian frame written in (w, y, z): d_x = d_w, d_y|_x = d_y - delta d_w
+        const double dl = snake_delta(mt, x[1]);
+        for (int i = 0; i < 4; ++i) o.e[i][i] = o.einv[i][i] = 1.0;
+        o.e[1][2] = -dl;      // e^w_{y-hat}
+        o.einv[1][2] = dl;    // e^{x-hat}_y:  dx = dw + delta dy
         return;
     }
     if (!ok || !(o.sqrtg > 1e-300) || !(o.g[3][3] > 0)) {  // polar axis: gamma_phiphi = 0

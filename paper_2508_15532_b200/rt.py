@@ -13,7 +13,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "librt_b200.so")
 
 BC = {"periodic": 0, "outflow": 1, "zero": 2, "fixed": 3}
-METRIC = {"minkowski": 0, "mink_cyl": 1, "ks_mks": 2}
+METRIC = {"minkowski": 0, "mink_cyl": 1, "ks_mks": 2, "snake": 3}
 GEOM = dict(g_c=0, e_c=1, einv_c=2, sqrtg_c=3, omega_c=4, n0_c=5, angcoef=6)
 SYMBOLS = ["rt_init", "rt_free", "rt_ndir", "rt_ndir_padded", "rt_get_directions", "rt_get_geometry", "rt_cfl_dt",
            "rt_set_boundary", "rt_set_fluid", "rt_transport", "rt_angular_flux", "rt_source_implicit", "rt_moments",
@@ -27,7 +27,8 @@ class RtGrid(ctypes.Structure):
 
 
 class RtMetric(ctypes.Structure):
-    _fields_ = [("kind", ctypes.c_int), ("a", ctypes.c_double), ("hslope", ctypes.c_double), ("x3_symmetric", ctypes.c_int)]
+    _fields_ = [("kind", ctypes.c_int), ("a", ctypes.c_double), ("hslope", ctypes.c_double), ("x3_symmetric", ctypes.c_int),
+                ("snake_A", ctypes.c_double), ("snake_k", ctypes.c_double)]
 
 
 class RtOptions(ctypes.Structure):
@@ -116,7 +117,7 @@ class RtContext:
         g.bc_lo[:] = [BC[b] for b in grid["bc_lo"]]; g.bc_hi[:] = [BC[b] for b in grid["bc_hi"]]
         g.zero_lo[:] = grid.get("zero_lo", (0, 0, 0)); g.zero_hi[:] = grid.get("zero_hi", (0, 0, 0))
         mp = dict(metric_params or {})
-        m = RtMetric(METRIC[metric_kind], mp.get("a", 0.0), mp.get("hslope", 0.3), 1)
+        m = RtMetric(METRIC[metric_kind], mp.get("a", 0.0), mp.get("hslope", 0.3), 1, mp.get("A", 0.0), mp.get("k", 0.0))
         od = dict(DEFAULT_OPTIONS)
         for k, v in (options or {}).items():
             od[{"method": "source_method", "ang_recon": "angular_recon"}.get(k, k)] = v

@@ -1,4 +1,5 @@
-"""Seeded synthetic workloads shaped like BASELINE.json's five configs.
+"""Seeded synthetic workloads shaped like BASELINE.json's five configs,
+plus config 6 = the snake-coordinates beam of PAPER.md 4.6 (L557-559).
 
 This module serves BOTH the oracle and the CUDA path and therefore holds NONE of the method's arithmetic:
 it only fills arrays (random fields, profiles) from `numpy.random.default_rng(seed)`, seed = 1000 + config
@@ -14,11 +15,11 @@ import math
 
 import numpy as np
 
-FULL_SIZES = {1: (64, 64, 1), 2: (64, 64, 64), 3: (128, 128, 128), 4: (128, 96, 64), 5: (192, 128, 96)}
-LEVELS = {1: 2, 2: 4, 3: 4, 4: 4, 5: 6}
-NSTEPS = {1: 100, 2: 200, 3: 500, 4: 50, 5: 20}
+FULL_SIZES = {1: (64, 64, 1), 2: (64, 64, 64), 3: (128, 128, 128), 4: (128, 96, 64), 5: (192, 128, 96), 6: (128, 128, 1)}
+LEVELS = {1: 2, 2: 4, 3: 4, 4: 4, 5: 6, 6: 4}
+NSTEPS = {1: 100, 2: 200, 3: 500, 4: 50, 5: 20, 6: 400}
 NAMES = {1: "flat_beam_2d", 2: "flat_thermal_relaxation", 3: "scattering_diffusion",
-         4: "kerr_schild_torus", 5: "coupled_accretion_step"}
+         4: "kerr_schild_torus", 5: "coupled_accretion_step", 6: "snake_beam"}
 
 
 def config(idx, n=None, level=None):
@@ -60,6 +61,16 @@ def config(idx, n=None, level=None):
         c["metric"] = ("ks_mks", dict(a=a, hslope=0.3))
         c["options"] = dict(method=2, kappa_a0=10.0, kappa_s=20.0, a_rad=1.0, Y_over_rho=1.5)
         c["dt"] = None      # from the CFL bounds of whichever side runs it (L464 + angular bound, S14)
+    elif idx == 6:
+        # PAPER.md 4.6 (L559): A = 0.1, k = 2.0, 128 x 128, G2 angular grid; [0,1]^2 in (w, y); a beam enters through
+        # the w-low boundary and must be straight once mapped back to x = w + A sin(k pi y)
+        N = n[0]
+        c["grid"] = dict(n=n, x0=(0.0, 0.0, 0.0), dx=(1.0 / N, 1.0 / n[1], 1.0 / N),
+                         bc_lo=("fixed", "outflow", "periodic"), bc_hi=("outflow", "outflow", "periodic"),
+                         x3_symmetric=True)
+        c["metric"] = ("snake", dict(A=0.1, k=2.0))
+        c["options"] = dict(method=0, kappa_a0=0.0, kappa_s=0.0)
+        c["dt"] = 0.2 / N      # |n^w| <= 1 + A k pi = 1.63
     else:
         raise ValueError(idx)
     return c
@@ -96,7 +107,7 @@ def fields(cfg, nhat, e_c=None):
     X3, X2, X1 = np.meshgrid(ax[2], ax[1], ax[0], indexing="ij")
     shp = (n3, n2, n1)
     out = dict(u4=None, ghosts={})
-    if idx == 1:
+    if idx in (1, 6):
         s_star = beam_direction(nhat)
         out["I0"] = np.zeros(shp + (nd,))
         out["rho"] = np.zeros(shp)

@@ -135,3 +135,50 @@ def test_config1_full_run_matches_oracle():
         assert rel_err(*out[k]) <= TOL, k
     beam = out["I"][0][0, :, :, f["beam_dir"]]
     assert beam.max() > 0.9 and beam.min() > -1e-6      # (the two-stage scheme is not strictly positivity preserving)
+
+
+def test_config6_snake_beam_full_size_is_straight():
+    """PAPER.md 4.6 at the paper's resolution (128 x 128, G2 = 162 directions, A = 0.1, k = 2): the beam computed by the
+    CUDA path, mapped back to Cartesian coordinates, follows its straight central ray within 2 cells (Fig 7), while
+    the straight line in (w, y) is more than 4 cells away."""
+    import math
+    import torch
+    from parity_util import make_pair
+    cfg = W.config(6)
+    N = cfg["grid"]["n"][0]
+    kind, params = cfg["metric"]
+    from paper_2508_15532_b200 import rt
+    ctx = rt.RtContext(cfg["grid"], kind, params, cfg["level"], cfg["options"])
+    f = W.fields(cfg, ctx.directions()["nhat"], ctx.geometry("e_c"))
+    dev = ctx.device
+    ctx.set_fluid(torch.as_tensor(f["rho"], device=dev).contiguous(), torch.as_tensor(f["T"], device=dev).contiguous(), None)
+    for (dim, side), g in f["ghosts"].items():
+        gd = torch.zeros(g.shape[:2] + (ctx.pitch,), dtype=torch.float64, device=dev)
+        gd[..., :ctx.nd] = torch.as_tensor(g, device=dev)
+        ctx.set_boundary(dim, side, gd)
+    I = ctx.to_device(f["I0"])
+    T = torch.as_tensor(f["T"], device=dev).contiguous().clone()
+    dt = cfg["dt"]
+    for _ in range(int(0.9 / dt)):
+        ctx.step(I, T, dt, None, None)
+    torch.cuda.synchronize()
+    s = f["beam_dir"]
+    n = ctx.directions()["nhat"][s]
+    Ib = ctx.to_host(I)[0, :, :, s]
+    assert np.isfinite(Ib).all()
+    A, k = params["A"], params["k"]
+    y = (np.arange(N) + 0.5) / N
+    y0 = 0.5 * (N // 8 + N // 4) / N
+    ts = np.linspace(0.0, 1.5, 60001)
+    xr, yr = A * math.sin(k * math.pi * y0) + n[0] * ts, y0 + n[1] * ts
+    wr = xr - A * np.sin(k * np.pi * yr)
+    worst, bent = 0.0, 0.0
+    for i in range(8, int(0.45 * N), 4):
+        col = Ib[:, i]
+        assert col.sum() > 1.0
+        yb = (col * y).sum() / col.sum()
+        wi = (i + 0.5) / N
+        worst = max(worst, abs(yb - yr[np.argmax(wr >= wi)]) * N)
+        bent = max(bent, abs(yb - (y0 + n[1] / n[0] * wi)) * N)
+    assert worst < 2.0, worst
+    assert bent > 4.0, bent

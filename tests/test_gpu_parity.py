@@ -114,6 +114,22 @@ def test_mink_cyl_rotating_tetrad():
     assert np.abs(orc.tab["omega_c"]).max() > 0.1
 
 
+def test_snake_coordinates_beam_and_tables():
+    """Config 6 (PAPER.md 4.6, App A.1): flat space in snake coordinates -- off-diagonal metric, x2-dependent tetrad
+    with e^w_y-hat = -delta, omega = 0 up to the finite-difference error.  Tables, then 60 steps of the beam, then a
+    seeded full-sphere field so that every direction sees the sheared faces."""
+    cfg = W.config(6, n=(40, 36, 3))
+    orc, ctx, f, dt = make_pair(cfg)
+    for name in ("g_c", "e_c", "einv_c", "sqrtg_c"):
+        assert rel_err(ctx.geometry(name), orc.tab[name]) < 1e-13, name
+    assert np.abs(ctx.geometry("omega_c") - orc.tab["omega_c"]).max() < 1e-10      # both ~1e-9 of FD error around 0
+    out = run_steps(orc, ctx, f, dt, 60)
+    _check(out)
+    assert out["I"][1].max() > 0.5
+    f["I0"] = np.random.default_rng(11).uniform(0.5, 1.0, size=f["I0"].shape) / (4 * np.pi)
+    _check(run_steps(orc, ctx, f, dt, 8))
+
+
 def test_individual_calls_compose():
     """rt_transport, rt_angular_flux, rt_source_implicit, rt_moments one by one against the oracle's."""
     import torch

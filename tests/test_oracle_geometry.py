@@ -118,3 +118,35 @@ def test_photon_orbit_radii_eq53():
     h = 1e-5
     f = lambda x1: (lambda t: t[0] + 2 * t[1] * Om + t[2] * Om * Om)(disc(x1))
     assert abs((f(np.log(r1) + h) - f(np.log(r1) - h)) / (2 * h)) < 1e-6
+
+
+def test_snake_metric_tetrad_and_zero_connection():
+    """App A.1 (L802-806): snake coordinates w = x - A sin(k pi y).  The metric must be the pull-back of the flat metric
+    through the coordinate map (Jacobian by finite differences of the MAP, independent of the oracle's A1 formula);
+    the tetrad (A2 under reading S27) must satisfy Eq 1, be the Cartesian frame, and therefore have omega = 0."""
+    P = dict(A=0.1, k=2.0)
+    rng = np.random.default_rng(5)
+    X = rng.uniform(0.0, 1.0, (40, 3))
+
+    def cart(Xw):   # (w, y, z) -> (x, y, z)
+        return np.stack([Xw[..., 0] + P["A"] * np.sin(P["k"] * np.pi * Xw[..., 1]), Xw[..., 1], Xw[..., 2]], -1)
+
+    h = 1e-5
+    J = np.zeros((40, 3, 3))   # J[p, a, i] = d x^a / d X^i
+    for i in range(3):
+        d = np.zeros(3); d[i] = h
+        J[:, :, i] = (cart(X + d) - cart(X - d)) / (2 * h)
+    g = G.metric("snake", P, X)
+    assert np.abs(g[:, 1:, 1:] - np.einsum("pai,paj->pij", J, J)).max() < 1e-9
+    assert np.abs(g[:, 0, 0] + 1).max() == 0 and np.abs(g[:, 0, 1:]).max() == 0
+    assert np.abs(G.sqrt_neg_g("snake", P, X) - 1.0).max() < 1e-14           # det J = 1
+    e, einv = G.tetrad("snake", P, X)
+    assert np.abs(np.einsum("pma,pmn,pnb->pab", e, g, e) - G.ETA).max() < 1e-14      # Eq 1
+    assert np.abs(np.einsum("pam,pmb->pab", einv, e) - np.eye(4)).max() < 1e-14
+    # Cartesian frame: pushing e_a forward with J gives the unit vectors
+    assert np.abs(np.einsum("pai,pib->pab", J, e[:, 1:, 1:]) - np.eye(3)).max() < 1e-9
+    # a parallel frame in flat space: all Ricci rotation coefficients vanish (to the FD truncation error)
+    assert np.abs(G.ricci_rotation("snake", P, X)).max() < 1e-8
+    # n^w = n^x - delta n^y: a ray along y-hat moves backwards in w where delta > 0
+    delta = P["A"] * P["k"] * np.pi * np.cos(P["k"] * np.pi * X[:, 1])
+    assert np.abs(e[:, 1, 2] + delta).max() < 1e-14

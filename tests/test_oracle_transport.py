@@ -191,3 +191,44 @@ def test_mapr_linear_exactness_constant_reduction_and_conservation():
     n0 = np.einsum("...m,...sm->...s", g[..., 0, :], n)
     assert np.abs(((out - I) * n[..., 0] * n0 * om.ang["w"]).sum(-1)).max() < 1e-16 * 50
     assert np.abs(out - od.angular_flux(I, I, 1e-3).reshape(I.shape)).max() > 1e-7        # and it is not donor cell
+
+
+def test_snake_coordinates_beam_is_straight_in_cartesian():
+    """PAPER.md 4.6 (L559, Fig 7; A = 0.1, k = 2): a beam in snake coordinates bends in (w, y) but is a straight line
+    once mapped back to x = w + A sin(k pi y).  The intensity centroid of every mesh column must sit on the central
+    ray within 1.5 cells, while the straight line in (w, y) is several cells away (so a wrong sign or a missing
+    delta in n^w fails)."""
+    import math
+    import rt_workloads as W
+    N = 48
+    cfg = W.config(6, n=(N, N, 1), level=2)
+    kind, params = cfg["metric"]
+    orc = Oracle(cfg["grid"], kind, params, cfg["level"], cfg["options"])
+    f = W.fields(cfg, orc.ang["nhat"], orc.tab["e_c"])
+    orc.set_fluid(f["rho"], f["T"], f["u4"])
+    for (d, s), g in f["ghosts"].items():
+        orc.set_boundary(d, s, g)
+    dt = cfg["dt"]
+    I, T = f["I0"].copy(), f["T"].copy()
+    for _ in range(int(0.9 / dt)):
+        out = orc.step(I, T, dt)
+        I, T = out[0], out[1]
+    s = f["beam_dir"]
+    n = orc.ang["nhat"][s]
+    Ib = I.reshape(N, N, -1)[:, :, s]          # [j, i]
+    A, k = params["A"], params["k"]
+    y = (np.arange(N) + 0.5) / N
+    y0 = 0.5 * (N // 8 + N // 4) / N             # centre of the illuminated rows
+    ts = np.linspace(0.0, 1.5, 30001)            # the central ray, straight in Cartesian coordinates
+    xr, yr = A * math.sin(k * math.pi * y0) + n[0] * ts, y0 + n[1] * ts
+    wr = xr - A * np.sin(k * np.pi * yr)
+    worst, bent = 0.0, 0.0
+    for i in range(4, 22, 2):
+        col = Ib[:, i]
+        assert col.sum() > 1.0
+        yb = (col * y).sum() / col.sum()
+        wi = (i + 0.5) / N
+        worst = max(worst, abs(yb - yr[np.argmax(wr >= wi)]) * N)
+        bent = max(bent, abs(yb - (y0 + n[1] / n[0] * wi)) * N)
+    assert worst < 1.5, worst
+    assert bent > 4.0, bent
