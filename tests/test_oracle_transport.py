@@ -232,3 +232,33 @@ def test_snake_coordinates_beam_is_straight_in_cartesian():
         bent = max(bent, abs(yb - (y0 + n[1] / n[0] * wi)) * N)
     assert worst < 1.5, worst
     assert bent > 4.0, bent
+
+
+@pytest.mark.parametrize("v", [0.05, -0.05])
+def test_dynamic_diffusion_pulse_is_advected_with_the_flow(v):
+    """PAPER.md 4.9 (L656-664): in a scattering-dominated medium moving uniformly with v^x = 0.05 "the radiation should
+    be advected with the flow": after t = 2 the pulse has moved by v t (here to 0.5 %; either sign).  This is the pin of
+    Eq 23's advective term (readings S10/S11: n^0 v^a I, upwinded on v): without it the pulse does not move, with the
+    downwind choice it is unstable, with a wrong sign it moves the other way."""
+    import math
+    N = 64
+    grid = dict(n=(N, 1, 1), x0=(0.0, 0.0, 0.0), dx=(1.0 / N,) * 3, bc_lo=("periodic",) * 3, bc_hi=("periodic",) * 3)
+    o = Oracle(grid, "minkowski", {}, 2, dict(method=1, kappa_a0=0.0, kappa_s=10.0 * N, a_rad=1.0, Y_over_rho=1.5))
+    nd, w = o.nd, o.ang["w"]
+    x = (np.arange(N) + 0.5) / N
+    gam = 1.0 / math.sqrt(1.0 - v * v)
+    u4 = np.zeros((4, 1, 1, N)); u4[0] = gam; u4[1] = gam * v
+    o.set_fluid(np.ones((1, 1, N)), np.ones((1, 1, N)), u4)
+    I = np.repeat(np.exp(-(x - 0.5) ** 2 / (2 * 0.08 ** 2))[:, None] / (4 * np.pi), nd, axis=1).reshape(1, 1, N, nd).copy()
+    T = np.ones((1, 1, N))
+
+    def centroid(I):   # periodic centroid of the lab-frame energy density
+        E = (I.reshape(N, nd) * w).sum(1)
+        return (np.angle((E * np.exp(2j * np.pi * x)).sum()) / (2 * np.pi)) % 1.0
+
+    c0, dt, t = centroid(I), 0.5 / N, 0.0
+    for _ in range(256):
+        out = o.step(I, T, dt)
+        I, T = out[0], out[1]
+        t += dt
+    assert abs((centroid(I) - c0) - v * t) < 0.005 * abs(v * t)
