@@ -130,6 +130,26 @@ def test_snake_coordinates_beam_and_tables():
     _check(run_steps(orc, ctx, f, dt, 8))
 
 
+def test_flat_moving_fluid_advective_term():
+    """Eq 23 with a moving fluid in flat space (PAPER.md 4.9): uniform v^x = 0.05 plus a seeded transverse velocity
+    field, tau_cell = 10, on a grid with a 1-cell-thick dimension (periodic wrap of a single cell)."""
+    import math
+    import torch
+    cfg = W.config(3, n=(24, 5, 1))
+    orc, ctx, f, dt = make_pair(cfg)
+    rng = np.random.default_rng(21)
+    shp = f["rho"].shape
+    vx = 0.05 + 0.02 * rng.uniform(-1, 1, shp); vy = 0.1 * rng.uniform(-1, 1, shp); vz = 0.1 * rng.uniform(-1, 1, shp)
+    gam = 1.0 / np.sqrt(1.0 - vx * vx - vy * vy - vz * vz)
+    u4 = np.stack([gam, gam * vx, gam * vy, gam * vz])
+    orc.set_fluid(f["rho"], f["T"], u4)
+    dev = ctx.device
+    ctx.set_fluid(torch.as_tensor(f["rho"], device=dev).contiguous(), torch.as_tensor(f["T"], device=dev).contiguous(),
+                  torch.as_tensor(u4, device=dev).contiguous())
+    f["I0"] = rng.uniform(0.5, 1.0, size=f["I0"].shape) / (4 * np.pi)
+    _check(run_steps(orc, ctx, f, dt, 10))
+
+
 def test_individual_calls_compose():
     """rt_transport, rt_angular_flux, rt_source_implicit, rt_moments one by one against the oracle's."""
     import torch
