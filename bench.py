@@ -8,8 +8,9 @@ Prints ONE JSON line.  metric = cell-direction updates/s (fp64): N_cells * N_dir
 inputs resident in HBM.  `e2e` = the same through the C ABI with pinned HOST buffers (H2D of I, T and D2H of I, T,
 R, G inside the timed region).  `roofline` = dominant kernel, algorithmic bytes / CUDA-event time / measured HBM peak.
 `cpu_baseline` = the oracle timed on a bounded sample on this box's cores (a baseline, not the target).
-N > 1: replicas only this round: every rank runs the same workload on its own GPU,
-value = aggregate over ranks / max-over-ranks time.
+N > 1: the mesh grows with N along x3 and is cut into slabs, one per rank, with a 4-plane halo
+exchanged point to point once per step (inside the timed region); value = owned cell-directions of all ranks * steps /
+max-over-ranks time ("weak").  --multi replicas: N independent copies instead.
 """
 import argparse
 import json
@@ -33,6 +34,8 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index 1..5 (4 = Kerr-Schild, the roofline config); 6 = snake-coordinates beam (PAPER 4.6)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--multi", default="slab", choices=["slab", "replicas"],
+                    help="N > 1: slab decomposition along x3 with halo exchange (default) or independent replicas")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--size", default=None, help="override grid, e.g. 64x48x32 (debug)")
@@ -151,20 +154,60 @@ def setup_gpu(cfg, device):
     return ctx, f, I, T.clone(), dt
 
 
+def setup_slab(args, cfg, rank, world, device):
+    """N > 1: the mesh grows with N along x3 (weak scaling: every rank owns the config's n3 planes) and is cut into
+    slabs; each rank generates the seeded fields of its own extended slab and one halo exchange makes the margins
+    consistent.  returns (SlabDomain, global cfg, dt)."""
+    import torch
+    import torch.distributed as dist
+    import rt_workloads as W
+    from paper_2508_15532_b200.dist import SlabDomain
+
+    n = cfg["grid"]["n"]
+    gcfg = W.config(args.config, n=(n[0], n[1], n[2] * world))
+    slab = SlabDomain(gcfg, rank, world, device=device)
+    gen = dict(gcfg, grid=dict(slab.grid), seed=gcfg["seed"] + rank)
+    f = W.fields(gen, slab.ctx.directions()["nhat"], slab.ctx.geometry("e_c"))
+    slab.set_fields(f, local=True)
+    slab.exchange_halo()
+    dt = gcfg["dt"] if gcfg["dt"] is not None else min(slab.ctx.cfl_dt())
+    t = torch.tensor([dt], dtype=torch.float64, device=slab.device)
+    dist.all_reduce(t, op=dist.ReduceOp.MIN)       # one global time step (not on the data path)
+    return slab, gcfg, float(t.item())
+
+
 def run_gpu(args, rank, world):
     import numpy as np
     import torch
     import torch.distributed as dist
 
-    local = int(os.environ.get("LOCAL_RANK", 0))
+    local = int(os.environ.get("LOCAL_RANK", 0)) % max(torch.cuda.device_count(), 1)
     device = "cuda:%d" % local
     torch.cuda.set_device(local)
     cfg = make_config(args)
-    ctx, f, I, T, dt = setup_gpu(cfg, device)
-    dev = ctx.device
-    R = torch.zeros((16,) + ctx.shape, dtype=torch.float64, device=dev)
-    G = torch.zeros((4,) + ctx.shape, dtype=torch.float64, device=dev)
-    units = ctx.ncell * ctx.nd                       # cell-direction updates per step
+    slab, multi = None, "single GPU"
+    if world > 1 and args.multi == "slab":
+        try:
+            slab, cfg, dt = setup_slab(args, cfg, rank, world, device)
+            multi = ("slab decomposition along x3 (weak: %d planes per rank), deep halo: 4 planes of I and T per neighbour "
+                     "per step over %s send/recv, %d planes computed per rank" % (slab.layout.k1 - slab.layout.k0, dist.get_backend(), slab.layout.n3_local))
+        except Exception as e:   # e.g. slabs thinner than the halo: fall back to independent replicas, and say so
+            slab, multi = None, "replicas only (slab decomposition unavailable: %s)" % str(e)[:120]
+    elif world > 1:
+        multi = "replicas only (--multi replicas)"
+    if slab is not None:
+        ctx, I, T, R, G = slab.ctx, slab.I, slab.T, slab.R, slab.G
+        dev = ctx.device
+        units = slab.owned_units                     # cells this rank OWNS x directions (halo planes are not counted)
+        step = lambda: slab.step(dt)
+    else:
+        ctx, f, I, T, dt = setup_gpu(cfg, device)
+        dev = ctx.device
+        R = torch.zeros((16,) + ctx.shape, dtype=torch.float64, device=dev)
+        G = torch.zeros((4,) + ctx.shape, dtype=torch.float64, device=dev)
+        units = ctx.ncell * ctx.nd                   # cell-direction updates per step
+        step = lambda: ctx.step(I, T, dt, R, G)
+    kernel_units = ctx.ncell * ctx.nd                # what one launch processes (incl. halo planes)
     I0, T0 = I.clone(), T.clone()
 
     def barrier():
@@ -173,7 +216,7 @@ def run_gpu(args, rank, world):
             dist.barrier()
 
     for _ in range(max(args.warmup, 3)):
-        ctx.step(I, T, dt, R, G)
+        step()
     barrier()
     I.copy_(I0); T.copy_(T0)
     ctx.profile_enable(True)
@@ -185,7 +228,7 @@ def run_gpu(args, rank, world):
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev0.record()
     for _ in range(args.steps):
-        ctx.step(I, T, dt, R, G)
+        step()
     ev1.record()
     barrier()
     ms = ev0.elapsed_time(ev1)
@@ -205,7 +248,13 @@ def run_gpu(args, rank, world):
         hG = torch.empty(G.shape, dtype=torch.float64, pin_memory=True)
         ksteps = min(args.steps, 5)
         def one():   # the user-facing C-ABI call with HOST buffers: H2D, rt_step, D2H inside rt_step_host; the state
-            ctx.step_host(hI, hT, dt, hR, hG)   # lives in pinned host memory and evolves from step to step
+            if slab is None:
+                ctx.step_host(hI, hT, dt, hR, hG)   # lives in pinned host memory and evolves from step to step
+            else:                                   # sharded: the halo exchange sits between the step and the D2H
+                I.copy_(hI, non_blocking=True); T.copy_(hT, non_blocking=True)
+                slab.step(dt)
+                hI.copy_(I, non_blocking=True); hT.copy_(T, non_blocking=True)
+                hR.copy_(R, non_blocking=True); hG.copy_(G, non_blocking=True)
         one()
         barrier()
         t0 = time.perf_counter()
@@ -220,7 +269,8 @@ def run_gpu(args, rank, world):
         d2h = (hI.numel() + hT.numel() + hR.numel() + hG.numel()) * 8
         e2e = {"value": aggregate_value(units, ksteps, world, ems), "unit": UNIT, "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "steps": ksteps, "ms_per_step": ems / ksteps}
-    return dict(cfg=cfg, ctx=ctx, ms=ms, units=units, prof=prof, launches=launches, clk=clk, e2e=e2e, finite=finite, dt=dt)
+    return dict(cfg=cfg, ctx=ctx, ms=ms, units=units, kernel_units=kernel_units, prof=prof, launches=launches, clk=clk, e2e=e2e,
+                finite=finite, dt=dt, multi=multi)
 
 
 # ---- oracle legs (the only places bench.py may execute oracle/) ----------------------------------------------------
@@ -283,13 +333,20 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", 1))
     rank = int(os.environ.get("RANK", 0))
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda:%d" % int(os.environ.get("LOCAL_RANK", 0))))
+        # RT_BENCH_BACKEND=gloo: functional check of the N > 1 path on a box with fewer GPUs than ranks (halo staged
+        # through the host; never a measurement)
+        backend = os.environ.get("RT_BENCH_BACKEND", "nccl")
+        if backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda:%d" % int(os.environ.get("LOCAL_RANK", 0))))
+        else:
+            dist.init_process_group(backend)
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device and no CPU fallback (use --impl reference for the oracle)")
     r = run_gpu(args, rank, world)
     if rank == 0:
-        ms, units, K = r["ms"], r["units"], args.steps
-        value = aggregate_value(units, K, world, ms)
+        ms, K = r["ms"], args.steps
+        value = aggregate_value(r["units"], K, world, ms)
+        units = r["kernel_units"]                 # per-launch units of the roofline figures
         peak, which = measured_peak()
         prof = r["prof"]
         dom = max(("transport", "angular", "source"), key=lambda k: prof[k][0])
@@ -313,7 +370,7 @@ def main():
                 "data": "synthetic",
                 "config": {"workload": workload_name(r["cfg"]), "dt": r["dt"], "l2": "inputs larger than L2 (one I copy >= 1 GB vs 126 MB)"
                            if units * 8 > 2.0e8 else "inputs FIT in L2 (latency-bound config; HBM fraction not meaningful)",
-                           "multi_gpu": "replicas only (no halo exchange this round)" if world > 1 else "single GPU",
+                           "multi_gpu": r["multi"],
                            "finite": r["finite"]},
                 "clocks": r["clk"], "e2e": r["e2e"], "gpu_launches": r["launches"], "roofline": roof}
         if not args.no_cpu_baseline and world == 1:

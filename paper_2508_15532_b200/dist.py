@@ -61,21 +61,37 @@ def exchange(layout, tensors, group=None):
     Point-to-point only (no collective): per tensor at most two sends and two receives, posted in an order that also
     matches when the left and the right neighbour are the same rank (world = 2, periodic): sends (to left, to right),
     receives (from right, from left)."""
+    import torch
     import torch.distributed as dist
     if layout.world == 1:
         return
-    ops = []
+    # NCCL moves device memory directly (NVLink / NVSwitch peer copies); gloo has no point-to-point path for CUDA
+    # tensors, so there the halo planes are staged through host memory (functional fallback, used by the tests)
+    stage = dist.get_backend(group) == "gloo" and any(t.is_cuda for t in tensors)
+    ops, landed = [], []
+
+    def send(t, sl, peer):
+        ops.append(dist.P2POp(dist.isend, t[sl].cpu() if stage else t[sl], peer, group))
+
+    def recv(t, sl, peer):
+        buf = torch.empty(t[sl].shape, dtype=t.dtype) if stage else t[sl]
+        if stage:
+            landed.append((t, sl, buf))
+        ops.append(dist.P2POp(dist.irecv, buf, peer, group))
+
     for t in tensors:
         if layout.lo_cut:
-            ops.append(dist.P2POp(dist.isend, t[layout.send_lo()], layout.left, group))
+            send(t, layout.send_lo(), layout.left)
         if layout.hi_cut:
-            ops.append(dist.P2POp(dist.isend, t[layout.send_hi()], layout.right, group))
+            send(t, layout.send_hi(), layout.right)
         if layout.hi_cut:
-            ops.append(dist.P2POp(dist.irecv, t[layout.recv_hi()], layout.right, group))
+            recv(t, layout.recv_hi(), layout.right)
         if layout.lo_cut:
-            ops.append(dist.P2POp(dist.irecv, t[layout.recv_lo()], layout.left, group))
+            recv(t, layout.recv_lo(), layout.left)
     for req in dist.batch_isend_irecv(ops):
         req.wait()
+    for t, sl, buf in landed:
+        t[sl].copy_(buf)
 
 
 def local_grid(grid, layout):
