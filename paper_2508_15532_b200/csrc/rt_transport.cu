@@ -241,6 +241,10 @@ __global__ void k_colflag(KParams p, const unsigned char *__restrict__ cflag, un
 // Block order of the marching kernels: a 1-D grid walked in bands of TILE_ROWS x2-rows with x2 fastest inside a band,
 // so that the CTAs resident at the same time cover a compact (x1, x2) patch and their transverse neighbours are
 // read from L2 instead of DRAM (row-major order re-reads ~4 halo rows per wave of ~5 rows).
+// how many x3-planes beyond its two-plane register pipeline the angular kernel prefetches (0 = off)
+#ifndef ANG_PF
+#define ANG_PF 2
+#endif
 // how many x3-planes beyond the register pipeline the vacuum kernel prefetches its operands (0 = off)
 #ifndef VAC_PF
 #define VAC_PF 2
@@ -586,6 +590,12 @@ __global__ void k_angular(KParams p, const double *__restrict__ I_in, double *I_
                 if (inrow) vn1 = __ldg(pin + 3 * kstride);
                 if (upd) ion1 = pio[3 * kstride];
             }
+#if ANG_PF
+            if (k + 2 + ANG_PF + 1 < n3) {   // planes further ahead: towards the SM now, no registers held
+                if (inrow) { pf_l1(pin + (2 + ANG_PF) * kstride); pf_l1(pin + (3 + ANG_PF) * kstride); }
+                if (upd) { pf_l1(pio + (2 + ANG_PF) * kstride); pf_l1(pio + (3 + ANG_PF) * kstride); }
+            }
+#endif
         }
         __syncthreads();
         if (live) {
