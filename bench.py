@@ -114,9 +114,9 @@ def measured_peak():
 # different array: corrector only), write I_out; angular: read I_in, read+write I_inout; source: read+write I.
 ALGO_BYTES = {"transport_pred": 16.0, "transport_corr": 24.0, "angular": 24.0, "source": 16.0}
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per launch of each kernel class on config 4 at full size,
-# from the `ncu --set full` capture summarised in profiles/r01_v16_kernels_full.md (transport = vacuum + general +
-# list kernels, mean of the predictor (2.66 GB) and corrector (3.64 GB) launches).  Other configs: not captured -> null.
-NCU_TRAFFIC = {4: {"transport": 3.15e9, "angular": 3.08e9, "source": 0.26e9}}
+# from the `ncu --set full` capture summarised in profiles/r01_v17_kernels_full.md (transport = vacuum + general +
+# list kernels, mean of the predictor (2.65 GB) and corrector (3.63 GB) launches).  Other configs: not captured -> null.
+NCU_TRAFFIC = {4: {"transport": 3.14e9, "angular": 3.09e9, "source": 0.26e9}}
 
 
 def make_config(args):
@@ -336,10 +336,12 @@ def main():
         # RT_BENCH_BACKEND=gloo: functional check of the N > 1 path on a box with fewer GPUs than ranks (halo staged
         # through the host; never a measurement)
         backend = os.environ.get("RT_BENCH_BACKEND", "nccl")
+        import datetime
+        tmo = datetime.timedelta(minutes=5)      # a stuck exchange aborts instead of hanging the job
         if backend == "nccl":
-            dist.init_process_group("nccl", device_id=torch.device("cuda:%d" % int(os.environ.get("LOCAL_RANK", 0))))
+            dist.init_process_group("nccl", device_id=torch.device("cuda:%d" % int(os.environ.get("LOCAL_RANK", 0))), timeout=tmo)
         else:
-            dist.init_process_group(backend)
+            dist.init_process_group(backend, timeout=tmo)
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device and no CPU fallback (use --impl reference for the oracle)")
     r = run_gpu(args, rank, world)
@@ -358,7 +360,7 @@ def main():
         roof = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak,
                 "traffic": NCU_TRAFFIC.get(args.config, {}).get(dom) if args.size is None else None,
-                "traffic_source": "profiles/r01_v16_kernels_full.md (bytes per launch)", "peak_source": which,
+                "traffic_source": "profiles/r01_v17_kernels_full.md (bytes per launch)", "peak_source": which,
                 "algorithmic_bytes_per_launch": per_unit[dom] * units,
                 "algorithmic_bytes_per_cell_dir_per_launch": per_unit[dom],
                 "kernel_ms_per_step": {k: prof[k][0] / K for k in prof},
