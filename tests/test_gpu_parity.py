@@ -150,6 +150,19 @@ def test_flat_moving_fluid_advective_term():
     _check(run_steps(orc, ctx, f, dt, 10))
 
 
+@pytest.mark.parametrize("idx,n,level,steps", [(4, (8, 8, 3), 8, 2),      # G3 = 642 directions (L213), 21 values per lane
+                                               (2, (6, 5, 4), 1, 4),      # the bare icosahedron: 12 directions, all pentagons
+                                               (2, (1, 1, 1), 2, 3),      # a single cell, periodic onto itself
+                                               (3, (2, 1, 3), 2, 3),      # extents smaller than the stencil
+                                               (4, (5, 8, 1), 4, 3)])     # one x3 plane in Kerr-Schild
+def test_degenerate_sizes_and_other_angular_levels(idx, n, level, steps):
+    cfg = W.config(idx, n=n, level=level)
+    orc, ctx, f, dt = make_pair(cfg)
+    if idx == 3:
+        f["I0"] = f["I0"] + np.random.default_rng(2).uniform(0.5, 1.0, size=f["I0"].shape) / (4 * np.pi)
+    _check(run_steps(orc, ctx, f, dt, steps))
+
+
 def test_individual_calls_compose():
     """rt_transport, rt_angular_flux, rt_source_implicit, rt_moments one by one against the oracle's."""
     import torch
