@@ -33,7 +33,11 @@ extern "C" {
 #define RT_ENOMEM (-3)
 #define RT_ESTATE (-4)  /* call order: fluid / boundary not set */
 
-enum { RT_BC_PERIODIC = 0, RT_BC_OUTFLOW = 1, RT_BC_ZERO = 2, RT_BC_FIXED = 3 };
+enum { RT_BC_PERIODIC = 0, RT_BC_OUTFLOW = 1, RT_BC_ZERO = 2, RT_BC_FIXED = 3,
+       RT_BC_REFLECT = 4 /* "symmetric" boundary (L709, DESIGN S23): ghost = mirror-image cell read in the direction with the
+                            normal tetrad component flipped, normal fluid velocity reversed.  Only on x^2 boundaries: the
+                            geodesic grid (pole along 3-hat, a vertex at azimuth 0) is mirror symmetric across 2-hat
+                            only; rt_init returns RT_EINVAL for the other dims */ };
 enum { RT_MINKOWSKI_CART = 0, RT_MINK_CYL_TETRAD = 1, RT_KS_MKS = 2, RT_SNAKE = 3 };
 enum { RT_LIM_MC = 0, RT_LIM_MINMOD = 1, RT_LIM_VANLEER = 2, RT_LIM_NONE = 3 };
 enum { RT_ANG_DONOR = 0, RT_ANG_MAPR = 1 };

@@ -24,7 +24,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "rt_oracle.c")
 _LIB = os.path.join(_HERE, "_build", "librt_oracle.so")
 
-BC = {"periodic": 0, "outflow": 1, "zero": 2, "fixed": 3}
+BC = {"periodic": 0, "outflow": 1, "zero": 2, "fixed": 3, "reflect": 4}
 _dp = ctypes.POINTER(ctypes.c_double)
 _ip = ctypes.POINTER(ctypes.c_int)
 
@@ -42,7 +42,7 @@ class _Problem(ctypes.Structure):
         ("n0_floor", ctypes.c_double), ("rho_floor", ctypes.c_double), ("kappa_a0", ctypes.c_double),
         ("kappa_s", ctypes.c_double), ("a_rad", ctypes.c_double), ("Y_over_rho", ctypes.c_double),
         ("abar", ctypes.c_double),
-        ("rho", _dp), ("u4", _dp), ("ghost", (_dp * 2) * 3),
+        ("rho", _dp), ("u4", _dp), ("ghost", (_dp * 2) * 3), ("mirror", _ip * 3),
     ]
 
 
@@ -81,6 +81,18 @@ def _c(a, dtype=np.float64):
 
 def _ptr(a):
     return a.ctypes.data_as(_ip if a.dtype == np.int32 else _dp)
+
+
+def mirror_map(nhat, a):
+    """Permutation m with nhat[m[s]] = nhat[s] with component a negated, or None if the grid lacks that symmetry."""
+    nhat = np.asarray(nhat)
+    flipped = nhat.copy()
+    flipped[:, a] *= -1.0
+    d = np.abs(flipped[:, None, :] - nhat[None, :, :]).max(-1)       # [s, t]
+    m = d.argmin(1)
+    if d[np.arange(len(nhat)), m].max() > 1e-9 or len(set(m.tolist())) != len(nhat):
+        return None
+    return m.astype(np.int32)
 
 
 DEFAULT_OPTIONS = dict(limiter=0, ang_recon=0, method=2, n0_floor=0.1, rho_floor=5e-4, kappa_a0=0.0,
@@ -128,6 +140,15 @@ class Oracle:
                 getattr(P, name)[a_] = _ptr(a)
         for k, v in self.opt.items():
             setattr(P, k, v)
+        # reflecting ("symmetric", L709, S23) boundaries: the direction with the normal tetrad component flipped.  Only
+        # a dim whose flip maps the geodesic grid onto itself can reflect (with the pole along 3-hat and a vertex at
+        # azimuth 0 that is dim 2-hat = x2: the x-z plane is a mirror plane of the icosahedron, the others are not)
+        self.mirror = [mirror_map(self.ang["nhat"], a_) for a_ in range(3)]
+        for a_ in range(3):
+            if "reflect" in (self.grid["bc_lo"][a_], self.grid["bc_hi"][a_]):
+                if self.mirror[a_] is None:
+                    raise ValueError("the angular grid has no mirror symmetry across dim %d" % a_)
+                m = _c(self.mirror[a_], np.int32); self._keep.append(m); P.mirror[a_] = _ptr(m)
         self.P = P
         self.set_fluid(np.zeros(self.n[::-1]), np.ones(self.n[::-1]), None)
 

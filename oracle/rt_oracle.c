@@ -26,6 +26,7 @@
 #define BC_OUTFLOW 1
 #define BC_ZERO 2
 #define BC_FIXED 3
+#define BC_REFLECT 4  /* "symmetric" boundary (L709, S23): mirror cell, direction with the normal tetrad component flipped */
 
 typedef struct {
     int n[3];
@@ -45,6 +46,7 @@ typedef struct {
     double n0_floor, rho_floor, kappa_a0, kappa_s, a_rad, Y_over_rho, abar;
     const double *rho, *u4;     /* rho[Nc]; u4[4][Nc] coordinate-frame u^mu */
     const double *ghost[3][2];  /* BC_FIXED: [2 layers][face cells][nd], layer 0 next to the interior */
+    const int *mirror[3];       /* BC_REFLECT: mirror[a][s] = the direction with n-hat^a flipped (a permutation) */
 } orc_problem;
 
 static const double FOURPI = 12.566370614359172953850573533118;
@@ -93,7 +95,8 @@ static double slope(int limiter, double dm, double dp) {
 }
 
 /* resolve a possibly out-of-range index along dim a.  returns 1 and the interior index in *c if the
- * value lives in the interior array; 0 if it is zero; 2 + layer if it is a fixed ghost. */
+ * value lives in the interior array; 0 if it is zero; 2 if it is a fixed ghost (*c = layer); 3 if it is the
+ * mirror image of interior cell *c (reflecting boundary: read it in the mirrored direction). */
 static int resolve(const orc_problem *P, int a, int c, int *cout) {
     int N = P->n[a];
     if (c >= 0 && c < N) { *cout = c; return 1; }
@@ -101,6 +104,7 @@ static int resolve(const orc_problem *P, int a, int c, int *cout) {
     if (bc == BC_PERIODIC) { *cout = ((c % N) + N) % N; return 1; }
     if (bc == BC_OUTFLOW) { *cout = (c < 0) ? 0 : N - 1; return 1; }
     if (bc == BC_ZERO) return 0;
+    if (bc == BC_REFLECT) { *cout = (c < 0) ? (-1 - c) : (2 * N - 1 - c); return 3; }   /* mirror image cell */
     *cout = (c < 0) ? (-1 - c) : (c - N); /* ghost layer 0 or 1 */
     return 2;
 }
@@ -108,10 +112,10 @@ static int resolve(const orc_problem *P, int a, int c, int *cout) {
 static double getI(const orc_problem *P, const double *I, int a, int idx[3], int s) {
     int c, r = resolve(P, a, idx[a], &c);
     if (r == 0) return 0.0;
-    if (r == 1) {
+    if (r == 1 || r == 3) {
         int q[3] = {idx[0], idx[1], idx[2]};
         q[a] = c;
-        return I[cidx(P, q[0], q[1], q[2]) * P->nd + s];
+        return I[cidx(P, q[0], q[1], q[2]) * P->nd + (r == 3 ? P->mirror[a][s] : s)];
     }
     /* fixed ghost: face-cell index runs over the two other dims, lower dim fastest */
     int b1 = (a == 0) ? 1 : 0, b2 = (a == 2) ? 1 : 2;
@@ -120,15 +124,23 @@ static double getI(const orc_problem *P, const double *I, int a, int idx[3], int
     int side = idx[a] < 0 ? 0 : 1;
     return P->ghost[a][side][((long)c * nface + fc) * P->nd + s];
 }
-/* fluid quantities in ghost zones: periodic wraps, everything else copies the nearest interior cell */
+/* fluid quantities in ghost zones: periodic wraps, reflecting mirrors, everything else copies the nearest interior cell */
 static long fluid_cell(const orc_problem *P, int a, int idx[3]) {
     int q[3] = {idx[0], idx[1], idx[2]};
     int N = P->n[a], c = q[a];
     if (c < 0 || c >= N) {
         int bc = (c < 0) ? P->bc_lo[a] : P->bc_hi[a];
-        q[a] = (bc == BC_PERIODIC) ? ((c % N) + N) % N : (c < 0 ? 0 : N - 1);
+        if (bc == BC_REFLECT) q[a] = (c < 0) ? (-1 - c) : (2 * N - 1 - c);
+        else q[a] = (bc == BC_PERIODIC) ? ((c % N) + N) % N : (c < 0 ? 0 : N - 1);
     }
     return cidx(P, q[0], q[1], q[2]);
+}
+/* +1, or -1 for a mirror-image cell behind a reflecting boundary of dim a (its normal velocity is reversed) */
+static double mirror_sign(const orc_problem *P, int a, const int idx[3]) {
+    int c = idx[a];
+    if (c < 0) return P->bc_lo[a] == BC_REFLECT ? -1.0 : 1.0;
+    if (c >= P->n[a]) return P->bc_hi[a] == BC_REFLECT ? -1.0 : 1.0;
+    return 1.0;
 }
 /* fluid-frame total opacity alpha = rho (kappa_a + kappa_s), kappa_a = kappa_a0 rho T^-3.5 (S13, S21);
  * zero below the density floor (L468 (i)) */
@@ -195,9 +207,10 @@ static double face_flux(const orc_problem *P, const double *I, const double *T, 
     double etau = exp(-tau);
     /* PLI-reconstructed fluid 3-velocity at the face (L276) */
     int qq[3];
-    memcpy(qq, L, sizeof qq); qq[a] -= 1; long fm = fluid_cell(P, a, qq);
-    memcpy(qq, R, sizeof qq); qq[a] += 1; long fp = fluid_cell(P, a, qq);
-    double vm = vel(P, fm, a), v0 = vel(P, fl, a), v1 = vel(P, fr, a), v2 = vel(P, fp, a);
+    memcpy(qq, L, sizeof qq); qq[a] -= 1; long fm = fluid_cell(P, a, qq); double sm = mirror_sign(P, a, qq);
+    memcpy(qq, R, sizeof qq); qq[a] += 1; long fp = fluid_cell(P, a, qq); double sp = mirror_sign(P, a, qq);
+    double vm = sm * vel(P, fm, a), v0 = mirror_sign(P, a, L) * vel(P, fl, a), v1 = mirror_sign(P, a, R) * vel(P, fr, a),
+           v2 = sp * vel(P, fp, a);
     double vL = v0 + 0.5 * slope(P->limiter, v0 - vm, v1 - v0);
     double vR = v1 - 0.5 * slope(P->limiter, v1 - v0, v2 - v1);
     double adv;

@@ -80,7 +80,8 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     if (!grid || !metric || !opt || !out) return RT_EINVAL;
     for (int a = 0; a < 3; ++a) {
         if (grid->n[a] < 1 || !(grid->dx[a] > 0)) return RT_EINVAL;
-        if (grid->bc_lo[a] < 0 || grid->bc_lo[a] > 3 || grid->bc_hi[a] < 0 || grid->bc_hi[a] > 3) return RT_EINVAL;
+        if (grid->bc_lo[a] < 0 || grid->bc_lo[a] > RT_BC_REFLECT || grid->bc_hi[a] < 0 || grid->bc_hi[a] > RT_BC_REFLECT) return RT_EINVAL;
+        if (a != 1 && (grid->bc_lo[a] == RT_BC_REFLECT || grid->bc_hi[a] == RT_BC_REFLECT)) return RT_EINVAL;   // no mirror symmetry of the angular grid there
         if ((grid->bc_lo[a] == RT_BC_PERIODIC) != (grid->bc_hi[a] == RT_BC_PERIODIC)) return RT_EINVAL;
         if (grid->zero_lo[a] < 0 || grid->zero_hi[a] < 0) return RT_EINVAL;
     }
@@ -203,10 +204,33 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
         w[s] = c->ang.w[s];
     }
 
+    // reflecting x2 boundary: the permutation s -> direction with n-hat^2 flipped (the x-z plane is a mirror plane of the
+    // grid: pole along 3-hat, a vertex at azimuth 0).  Looked up by nearest direction and verified.
+    std::vector<int> mir;
+    if (grid->bc_lo[1] == RT_BC_REFLECT || grid->bc_hi[1] == RT_BC_REFLECT) {
+        mir.assign(pitch, 0);
+        bool ok = true;
+        for (int s = 0; s < nd; ++s) {
+            int best = -1;
+            double bd = 1e300;
+            for (int t2 = 0; t2 < nd; ++t2) {
+                const double dxn = c->ang.nhat[3 * t2] - c->ang.nhat[3 * s], dyn = c->ang.nhat[3 * t2 + 1] + c->ang.nhat[3 * s + 1],
+                             dzn = c->ang.nhat[3 * t2 + 2] - c->ang.nhat[3 * s + 2];
+                const double d = dxn * dxn + dyn * dyn + dzn * dzn;
+                if (d < bd) { bd = d; best = t2; }
+            }
+            if (!(bd < 1e-18)) ok = false;
+            mir[s] = best;
+        }
+        for (int s = 0; s < nd && ok; ++s) ok = mir[mir[s]] == s;
+        if (!ok) { delete c; return RT_EINVAL; }
+    }
+
     // ---- upload ----
     DeviceTables &t = c->tab;
     std::memset(&t, 0, sizeof t);
     cudaError_t e = cudaSuccess;
+    if (!mir.empty()) e = upload(&t.mirror, mir);
     for (int a = 0; a < 3 && e == cudaSuccess; ++a) e = upload(&t.face[a], face[a]);
     if (e == cudaSuccess) e = upload(&t.cen, cen);
     if (e == cudaSuccess) e = upload(&t.ecen, ecen);
@@ -247,7 +271,7 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     k.limiter = opt->limiter; k.method = opt->source_method;
     k.n0_floor = opt->n0_floor; k.rho_floor = opt->rho_floor; k.kappa_a0 = opt->kappa_a0; k.kappa_s = opt->kappa_s;
     k.a_rad = opt->a_rad; k.Y_over_rho = opt->Y_over_rho; k.abar = opt->abar;
-    k.cen = t.cen; k.ecen = t.ecen; k.angcoef = t.angcoef; k.nhat = t.nhat; k.w = t.w; k.nb = t.nb;
+    k.cen = t.cen; k.ecen = t.ecen; k.angcoef = t.angcoef; k.nhat = t.nhat; k.w = t.w; k.nb = t.nb; k.mirror = t.mirror;
     k.rho = c->d_rho; k.u4 = c->d_u4;
     k.cls = c->d_cls;
     if (mapr) {   // grid-only MAPR tables (S6): log maps of the neighbours and of the edge centres, pair matrices
@@ -310,7 +334,7 @@ extern "C" int rt_free(rt_ctx *c) {
     if (!c) return RT_EINVAL;
     for (int a = 0; a < 3; ++a) { cudaFree(c->tab.face[a]); cudaFree(c->d_fcoef[a]); }
     cudaFree(c->tab.cen); cudaFree(c->tab.ecen); cudaFree(c->tab.angcoef); cudaFree(c->tab.nhat); cudaFree(c->tab.w);
-    cudaFree(c->tab.nb); cudaFree(c->d_cflag); cudaFree(c->d_colflag); cudaFree(c->d_cls); cudaFree(c->d_genlist); cudaFree(c->d_srclist); cudaFree(c->d_hI); cudaFree(c->d_hT); cudaFree(c->d_hR); cudaFree(c->d_hG); cudaFree(c->d_hfail); cudaFree(c->d_mapr_xi); cudaFree(c->d_mapr_xim); cudaFree(c->d_mapr_a);
+    cudaFree(c->tab.nb); cudaFree(c->tab.mirror); cudaFree(c->d_cflag); cudaFree(c->d_colflag); cudaFree(c->d_cls); cudaFree(c->d_genlist); cudaFree(c->d_srclist); cudaFree(c->d_hI); cudaFree(c->d_hT); cudaFree(c->d_hR); cudaFree(c->d_hG); cudaFree(c->d_hfail); cudaFree(c->d_mapr_xi); cudaFree(c->d_mapr_xim); cudaFree(c->d_mapr_a);
     cudaFree(c->d_angraw); cudaFree(c->d_mapr_back); cudaFree(c->d_mapr_nnb); cudaFree(c->d_angup); cudaFree(c->d_rho); cudaFree(c->d_u4); cudaFree(c->d_T); cudaFree(c->d_Th); cudaFree(c->d_Ih);
     delete c;
     return RT_OK;

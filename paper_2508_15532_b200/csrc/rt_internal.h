@@ -49,6 +49,7 @@ struct DeviceTables {
     double *ecen;     // [ncol][16] e^mu_a, for the moment transform
     double *angcoef;  // [ncol][6][pitch]  dlam_e n_0e V_e / w_s, gated (0 across an n_0 sign change / missing slot)
     double *nhat;     // [3][pitch] direction cosines, component-major (pad = 0)
+    int *mirror;      // [pitch] direction with n-hat^2 flipped (RT_BC_REFLECT on x2), nullptr if unused
     double *w;        // [pitch] solid angles (pad = 0)
     int *nb;          // [6][pitch] neighbour per slot (pad / missing slot = own index)
 };

@@ -40,6 +40,7 @@ struct KParams {
     const int *genlist;         // compact list of the "general" (column * pitch + s) entries
     int ngen;
     const double *ghost[3][2];
+    const int *mirror;        // [pitch] RT_BC_REFLECT (x2 only): index of the direction with n-hat^2 flipped
     const double *rho, *u4;  // library-owned fluid copies
     const int *srclist;      // cells with rho >= rho_floor (the only ones the source step can touch), built by rt_set_fluid
     int nsrc;

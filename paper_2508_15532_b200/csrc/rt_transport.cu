@@ -37,11 +37,15 @@ __device__ __forceinline__ double slope_rt(int lim, double dm, double dp) {
     }
 }
 
-// index of a fluid cell along one dim: periodic wraps, everything else clamps (fluid ghosts)
+// index of a fluid cell along one dim: periodic wraps, reflecting mirrors, everything else clamps (fluid ghosts)
 __device__ __forceinline__ int fluid_idx(int c, int N, int bc_lo, int bc_hi) {
-    if (c < 0) return bc_lo == RT_BC_PERIODIC ? ((c % N) + N) % N : 0;
-    if (c >= N) return bc_hi == RT_BC_PERIODIC ? c % N : N - 1;
+    if (c < 0) return bc_lo == RT_BC_PERIODIC ? ((c % N) + N) % N : (bc_lo == RT_BC_REFLECT ? -1 - c : 0);
+    if (c >= N) return bc_hi == RT_BC_PERIODIC ? c % N : (bc_hi == RT_BC_REFLECT ? 2 * N - 1 - c : N - 1);
     return c;
+}
+// -1 for a mirror-image cell behind a reflecting boundary (its normal velocity is reversed), else +1
+__device__ __forceinline__ double mirror_sign(int c, int N, int bc_lo, int bc_hi) {
+    return ((c < 0 && bc_lo == RT_BC_REFLECT) || (c >= N && bc_hi == RT_BC_REFLECT)) ? -1.0 : 1.0;
 }
 __device__ __forceinline__ double alpha_total(const KParams &p, double rho, double T) {
     if (rho < p.rho_floor) return 0.0;   // L468 (i)
@@ -72,7 +76,8 @@ __global__ void k_facecoef(KParams p, const double *__restrict__ T, double dt, i
         const double et = exp(-tau);
         const double ft = sqrt(-expm1(-tau * tau) / (tau * tau));
         double v[4];
-        for (int o = 0; o < 4; ++o) v[o] = p.u4[(1 + a) * p.ncell + cell[o]] / p.u4[cell[o]];
+        for (int o = 0; o < 4; ++o)
+            v[o] = mirror_sign(q[a] + o - 2, N[a], p.bc_lo[a], p.bc_hi[a]) * (p.u4[(1 + a) * p.ncell + cell[o]] / p.u4[cell[o]]);
         const double vL = v[1] + 0.5 * slope_rt(p.limiter, v[1] - v[0], v[2] - v[1]);
         const double vR = v[2] - 0.5 * slope_rt(p.limiter, v[2] - v[1], v[3] - v[2]);
         double wL, wR;
@@ -96,6 +101,7 @@ __device__ __forceinline__ const double *cell_ptr(const KParams &p, const double
         if (bc == RT_BC_PERIODIC) q[a] = ((c % N) + N) % N;   // N may be 1 or 2: a single wrap is not enough
         else if (bc == RT_BC_OUTFLOW) q[a] = (c < 0) ? 0 : N - 1;
         else if (bc == RT_BC_ZERO) return nullptr;
+        else if (bc == RT_BC_REFLECT) q[a] = (c < 0) ? (-1 - c) : (2 * N - 1 - c);   // mirror image (slow_ld flips the direction)
         else {
             const int layer = (c < 0) ? (-1 - c) : (c - N), side = (c < 0) ? 0 : 1;
             long long fc, nface;
@@ -191,6 +197,8 @@ __global__ void k_cellflag(KParams p, const double4 *__restrict__ fc0, const dou
 
 // generic (boundary-aware) load, kept out of line: only threads next to a ZERO / FIXED boundary come here
 __device__ __noinline__ double slow_ld(const KParams &p, const double *I, int a, int i, int j, int k, int s) {
+    // reflecting boundary (x2 only): the mirror image holds the direction with n-hat^2 flipped
+    if (a == 1 && ((j < 0 && p.bc_lo[1] == RT_BC_REFLECT) || (j >= p.n2 && p.bc_hi[1] == RT_BC_REFLECT))) s = p.mirror[s];
     return ldI(cell_ptr(p, I, a, i, j, k), s);
 }
 // neighbour of coordinate c0 at offset d along a dim of extent N: interior index after periodic wrap / outflow

@@ -163,6 +163,53 @@ def test_degenerate_sizes_and_other_angular_levels(idx, n, level, steps):
     _check(run_steps(orc, ctx, f, dt, steps))
 
 
+@pytest.mark.parametrize("case", ["flat_matter", "kerr_schild_poles"])
+def test_reflecting_x2_boundary(case):
+    """RT_BC_REFLECT ('symmetric' theta boundary, L709 / S23): mirror-image cell, direction with n-hat^2 flipped, normal
+    fluid velocity reversed.  Flat space with a moving opaque fluid, and Kerr-Schild with reflecting poles and no zero
+    band (the pole faces have zero area; the ghosts enter through the PLI slopes of the first two rows)."""
+    import torch
+    if case == "flat_matter":
+        cfg = W.config(3, n=(7, 9, 4))
+        cfg["grid"] = dict(cfg["grid"], bc_lo=("periodic", "reflect", "outflow"), bc_hi=("periodic", "reflect", "outflow"))
+    else:
+        cfg = W.config(4, n=(10, 12, 4))
+        cfg["grid"] = dict(cfg["grid"], bc_lo=("outflow", "reflect", "periodic"), bc_hi=("outflow", "reflect", "periodic"),
+                           zero_lo=(0, 0, 0), zero_hi=(0, 0, 0))
+    orc, ctx, f, dt = make_pair(cfg)
+    rng = np.random.default_rng(31)
+    if case == "flat_matter":
+        shp = f["rho"].shape
+        v = 0.2 * rng.uniform(-1, 1, (3,) + shp)
+        gam = 1.0 / np.sqrt(1.0 - (v ** 2).sum(0))
+        u4 = np.concatenate([gam[None], gam[None] * v])
+        orc.set_fluid(f["rho"], f["T"], u4)
+        dev = ctx.device
+        ctx.set_fluid(torch.as_tensor(f["rho"], device=dev).contiguous(), torch.as_tensor(f["T"], device=dev).contiguous(),
+                      torch.as_tensor(u4, device=dev).contiguous())
+    f["I0"] = rng.uniform(0.5, 1.0, size=f["I0"].shape) / (4 * np.pi)
+    out = run_steps(orc, ctx, f, dt, 5)
+    _check(out)
+    # the wall matters: an open boundary gives something else in the first row
+    cfg2 = dict(cfg, grid=dict(cfg["grid"], bc_lo=(cfg["grid"]["bc_lo"][0], "outflow", cfg["grid"]["bc_lo"][2]),
+                               bc_hi=(cfg["grid"]["bc_hi"][0], "outflow", cfg["grid"]["bc_hi"][2])))
+    orc2, ctx2, f2, _ = make_pair(cfg2)
+    f2["I0"] = f["I0"]
+    out2 = run_steps(orc2, ctx2, f2, dt, 5)
+    assert np.abs(out2["I"][0] - out["I"][0])[:, 0].max() > 1e-6
+
+
+def test_reflect_rejected_where_the_angular_grid_has_no_mirror_plane():
+    from paper_2508_15532_b200 import rt
+    cfg = W.config(3, n=(4, 4, 4))
+    kind, params = cfg["metric"]
+    for a in (0, 2):
+        bl, bh = ["outflow"] * 3, ["outflow"] * 3
+        bl[a] = "reflect"
+        with pytest.raises(rt.RtError):
+            rt.RtContext(dict(cfg["grid"], bc_lo=tuple(bl), bc_hi=tuple(bh)), kind, params, cfg["level"], cfg["options"])
+
+
 def test_individual_calls_compose():
     """rt_transport, rt_angular_flux, rt_source_implicit, rt_moments one by one against the oracle's."""
     import torch

@@ -262,3 +262,57 @@ def test_dynamic_diffusion_pulse_is_advected_with_the_flow(v):
         I, T = out[0], out[1]
         t += dt
     assert abs((centroid(I) - c0) - v * t) < 0.005 * abs(v * t)
+
+
+@pytest.mark.parametrize("matter", [False, True])
+def test_reflecting_boundary_is_the_mirror_image_problem(matter):
+    """'Symmetric boundaries for the polar angle' (L709; reading S23: mirror cell, direction with the normal tetrad
+    component flipped, normal fluid velocity reversed).  A reflecting wall at x2 = 0 must give exactly what the doubled
+    domain with mirror-symmetric data gives in its upper half -- intensities, temperature and moments."""
+    import math
+    from oracle import mirror_map
+    n1, n2, n3 = 5, 6, 3
+    opt = dict(method=2, kappa_a0=8.0, kappa_s=4.0, a_rad=1.0, Y_over_rho=1.5) if matter else dict(method=0)
+    dx = (0.1, 0.1, 0.1)
+    half = dict(n=(n1, n2, n3), x0=(0.0, 0.0, 0.0), dx=dx, bc_lo=("periodic", "reflect", "periodic"),
+                bc_hi=("periodic", "outflow", "periodic"))
+    full = dict(n=(n1, 2 * n2, n3), x0=(0.0, -n2 * dx[1], 0.0), dx=dx, bc_lo=("periodic", "outflow", "periodic"),
+                bc_hi=("periodic", "outflow", "periodic"))
+    oh, of = Oracle(half, "minkowski", {}, 2, opt), Oracle(full, "minkowski", {}, 2, opt)
+    nd = oh.nd
+    m = mirror_map(oh.ang["nhat"], 1)
+    assert m is not None and (m[m] == np.arange(nd)).all() and (m != np.arange(nd)).any()
+    assert mirror_map(oh.ang["nhat"], 0) is None and mirror_map(oh.ang["nhat"], 2) is None   # no such symmetry (S2)
+    with pytest.raises(ValueError):
+        Oracle(dict(half, bc_lo=("reflect", "outflow", "periodic"), bc_hi=("outflow", "outflow", "periodic")), "minkowski", {}, 2, opt)
+    rng = np.random.default_rng(12)
+    I = rng.uniform(0.2, 1.0, (n3, n2, n1, nd))
+    rho, T = rng.uniform(0.5, 1.5, (n3, n2, n1)), rng.uniform(0.8, 1.2, (n3, n2, n1))
+    v = 0.3 * rng.uniform(-1, 1, (3, n3, n2, n1))
+    gam = 1.0 / np.sqrt(1.0 - (v ** 2).sum(0))
+    u4 = np.concatenate([gam[None], gam[None] * v])
+    flip = lambda a: a[:, ::-1]                                         # mirror in x2 (arrays are [k, j, i, ...])
+    If = np.concatenate([flip(I)[..., m], I], axis=1)
+    rhof, Tf = np.concatenate([flip(rho), rho], 1), np.concatenate([flip(T), T], 1)
+    u4m = u4[:, :, ::-1].copy(); u4m[2] *= -1.0                          # u^y reversed in the image
+    u4f = np.concatenate([u4m, u4], axis=2)
+    if matter:
+        oh.set_fluid(rho, T, u4); of.set_fluid(rhof, Tf, u4f)
+    dt = 0.03
+    Th, Tfull = T.copy(), Tf.copy()
+    for _ in range(4):
+        I, Th, Rh, Gh, _ = oh.step(I, Th, dt)
+        If, Tfull, Rf, Gf, _ = of.step(If, Tfull, dt)
+    I, If = I.reshape(n3, n2, n1, nd), If.reshape(n3, 2 * n2, n1, nd)
+    tol = 1e-13      # (the grid's mirror pairs agree to 3e-16 only, so not bit for bit)
+    assert np.abs(If[:, n2:] - I).max() < tol
+    assert np.abs(If[:, :n2] - I[:, ::-1][..., m]).max() < tol          # and the image stays the image
+    assert np.abs(Tfull.reshape(n3, 2 * n2, n1)[:, n2:] - Th.reshape(n3, n2, n1)).max() < tol
+    assert np.abs(Rf.reshape(16, n3, 2 * n2, n1)[:, :, n2:] - Rh.reshape(16, n3, n2, n1)).max() < tol
+    # and it is not what an open boundary gives
+    oo = Oracle(dict(half, bc_lo=("periodic", "outflow", "periodic")), "minkowski", {}, 2, opt)
+    if matter:
+        oo.set_fluid(rho, T, u4)
+    Io = oo.step(I.copy(), Th.copy(), dt)[0].reshape(I.shape)
+    Ir = oh.step(I.copy(), Th.copy(), dt)[0].reshape(I.shape)
+    assert np.abs(Io - Ir)[:, 0].max() > 1e-4
