@@ -117,6 +117,11 @@ ALGO_BYTES = {"transport_pred": 16.0, "transport_corr": 24.0, "angular": 24.0, "
 # from the `ncu --set full` capture summarised in profiles/r01_v17_kernels_full.md (transport = vacuum + general +
 # list kernels, mean of the predictor (2.65 GB) and corrector (3.63 GB) launches).  Other configs: not captured -> null.
 NCU_TRAFFIC = {4: {"transport": 3.14e9, "angular": 3.09e9, "source": 0.26e9}}
+# Warp instructions (smsp__inst_executed.sum) per launch of each kernel class, same capture (transport: mean of
+# 879.9 M predictor and 901.4 M corrector; source: mean of the three k_cell launches).  The transport and source kernels
+# are bound by instruction issue, not by HBM: `roofline.issue` reports that second roof.
+NCU_WARP_INSTR = {4: {"transport": 890.7e6, "angular": 439.2e6, "source": 254.1e6}}
+ISSUE_PEAK = 148 * 4 * 1.965e9          # warp instructions / s: 148 SMs x 4 schedulers x 1 issue per clock at 1965 MHz
 
 
 def make_config(args):
@@ -365,6 +370,11 @@ def main():
                 "algorithmic_bytes_per_cell_dir_per_launch": per_unit[dom],
                 "kernel_ms_per_step": {k: prof[k][0] / K for k in prof},
                 "kernel_launches_per_step": {k: prof[k][1] / K for k in prof},
+                "issue": ({"warp_instr_per_launch": NCU_WARP_INSTR[args.config][dom],
+                           "achieved": NCU_WARP_INSTR[args.config][dom] / (dms / max(dcnt, 1) * 1e-3), "peak": ISSUE_PEAK,
+                           "unit": "warp-instr/s", "frac": NCU_WARP_INSTR[args.config][dom] / (dms / max(dcnt, 1) * 1e-3) / ISSUE_PEAK,
+                           "source": "instruction count from profiles/r01_v17_kernels_full.md, time live"}
+                          if args.config in NCU_WARP_INSTR and args.size is None and dcnt and world == 1 else None),
                 "step_algorithmic_GBps": step_bytes / (ms / K * 1e-3) / 1e9,
                 "step_frac_of_peak": step_bytes / (ms / K * 1e-3) / 1e9 / peak}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
