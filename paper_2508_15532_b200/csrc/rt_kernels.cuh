@@ -44,6 +44,8 @@ struct KParams {
     const double *rho, *u4;  // library-owned fluid copies
     const int *srclist;      // cells with rho >= rho_floor (the only ones the source step can touch), built by rt_set_fluid
     int nsrc;
+    const int *vaclist;      // the other cells (only when both lists are non-empty)
+    int nvac;
 };
 
 // Layout of the column-flag buffer: [ncol] column flags, [ceil(n3/8)][ncol] x3-chunk flags, then (4-byte aligned)

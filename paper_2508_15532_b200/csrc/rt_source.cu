@@ -115,8 +115,9 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
     const long long nwork = LIST ? (long long)p.nsrc : p.ncell;
     for (long long widx = warp0; widx < nwork; widx += nwarps) {
         const long long cell = LIST ? (long long)p.srclist[widx] : widx;
-        if (!LIST && widx + nwarps < nwork) {   // next cell of this warp: one 128-byte line per lane, into L2/L1
-            const char *nx = reinterpret_cast<const char *>(I + (widx + nwarps) * p.pitch) + lane * 128;
+        if (!SRC && widx + nwarps < nwork) {   // moments-only passes stream: next cell of this warp, one 128-byte line per lane, into L2/L1
+            const long long nc = LIST ? (long long)p.srclist[widx + nwarps] : widx + nwarps;
+            const char *nx = reinterpret_cast<const char *>(I + nc * p.pitch) + lane * 128;
             if (lane * 128 < p.pitch * 8) asm volatile("prefetch.global.L1 [%0];" ::"l"(nx));
         }
         const int col = int(cell % p.ncol);
@@ -266,20 +267,29 @@ cudaError_t launch_cell(const KParams &p, double *I, double *T, double dt, int *
 
 }  // namespace
 
-// Source step on the cells of the interaction list; G (if wanted) is zero elsewhere; R (if wanted) is reduced for all
-// cells by a second, source-free pass.
+// Source step on the cells of the interaction list, with their moments (R after, G from before / after) when wanted;
+// G is zero elsewhere; R of the cells not on the list comes from a second, source-free pass over the complement list.
 cudaError_t launch_source(const KParams &p, double *I, double *T, double dt, int *n_fail, double *R_after, double *G,
                           cudaStream_t st, long long *launches) {
     cudaError_t e = cudaSuccess;
     if (G) e = cudaMemsetAsync(G, 0, 4 * p.ncell * sizeof(double), st);
-    if (e == cudaSuccess && p.method != 0 && p.nsrc > 0) {
+    const bool listed = p.method != 0 && p.nsrc > 0;
+    if (e == cudaSuccess && listed) {
         ++*launches;
-        e = G ? launch_cell<true, true, true>(p, I, T, dt, n_fail, nullptr, G, st)
-              : launch_cell<true, false, true>(p, I, T, dt, n_fail, nullptr, nullptr, st);
+        // with moments wanted the listed cells get theirs here (R after, G from before/after); the rest below
+        e = (G || R_after) ? launch_cell<true, true, true>(p, I, T, dt, n_fail, R_after, G, st)
+                           : launch_cell<true, false, true>(p, I, T, dt, n_fail, nullptr, nullptr, st);
     }
     if (e == cudaSuccess && R_after) {
-        ++*launches;
-        e = launch_cell<false, true, false>(p, I, nullptr, 0.0, nullptr, R_after, nullptr, st);
+        if (!listed) {                       // no source step anywhere: one pass over all cells
+            ++*launches;
+            e = launch_cell<false, true, false>(p, I, nullptr, 0.0, nullptr, R_after, nullptr, st);
+        } else if (p.nvac > 0) {             // the cells the source step did not visit
+            KParams pv = p;
+            pv.srclist = p.vaclist; pv.nsrc = p.nvac;
+            ++*launches;
+            e = launch_cell<false, true, true>(pv, I, nullptr, 0.0, nullptr, R_after, nullptr, st);
+        }
     }
     return e;
 }
