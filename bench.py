@@ -114,13 +114,13 @@ def measured_peak():
 # different array: corrector only), write I_out; angular: read I_in, read+write I_inout; source: read+write I.
 ALGO_BYTES = {"transport_pred": 16.0, "transport_corr": 24.0, "angular": 24.0, "source": 16.0}
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per launch of each kernel class on config 4 at full size,
-# from the `ncu --set full` capture summarised in profiles/r01_v17_kernels_full.md (transport = vacuum + general +
-# list kernels, mean of the predictor (2.65 GB) and corrector (3.63 GB) launches).  Other configs: not captured -> null.
-NCU_TRAFFIC = {4: {"transport": 3.14e9, "angular": 3.09e9, "source": 0.26e9}}
+# from the `ncu --set full` capture summarised in profiles/r01_v18_kernels_full.md (transport = vacuum + general +
+# list kernels, mean of the predictor (2.66 GB) and corrector (3.63 GB) launches).  Other configs: not captured -> null.
+NCU_TRAFFIC = {4: {"transport": 3.15e9, "angular": 3.09e9, "source": 0.51e9}}
 # Warp instructions (smsp__inst_executed.sum) per launch of each kernel class, same capture (transport: mean of
-# 879.9 M predictor and 901.4 M corrector; source: mean of the three k_cell launches).  The transport and source kernels
+# 882.4 M predictor and 907.1 M corrector; source: mean of the three k_cell launches).  The transport and source kernels
 # are bound by instruction issue, not by HBM: `roofline.issue` reports that second roof.
-NCU_WARP_INSTR = {4: {"transport": 890.7e6, "angular": 439.2e6, "source": 254.1e6}}
+NCU_WARP_INSTR = {4: {"transport": 894.8e6, "angular": 439.2e6, "source": 250.2e6}}
 ISSUE_PEAK = 148 * 4 * 1.965e9          # warp instructions / s: 148 SMs x 4 schedulers x 1 issue per clock at 1965 MHz
 
 
@@ -365,7 +365,7 @@ def main():
         roof = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak,
                 "traffic": NCU_TRAFFIC.get(args.config, {}).get(dom) if args.size is None else None,
-                "traffic_source": "profiles/r01_v17_kernels_full.md (bytes per launch)", "peak_source": which,
+                "traffic_source": "profiles/r01_v18_kernels_full.md (bytes per launch)", "peak_source": which,
                 "algorithmic_bytes_per_launch": per_unit[dom] * units,
                 "algorithmic_bytes_per_cell_dir_per_launch": per_unit[dom],
                 "kernel_ms_per_step": {k: prof[k][0] / K for k in prof},
@@ -373,7 +373,7 @@ def main():
                 "issue": ({"warp_instr_per_launch": NCU_WARP_INSTR[args.config][dom],
                            "achieved": NCU_WARP_INSTR[args.config][dom] / (dms / max(dcnt, 1) * 1e-3), "peak": ISSUE_PEAK,
                            "unit": "warp-instr/s", "frac": NCU_WARP_INSTR[args.config][dom] / (dms / max(dcnt, 1) * 1e-3) / ISSUE_PEAK,
-                           "source": "instruction count from profiles/r01_v17_kernels_full.md, time live"}
+                           "source": "instruction count from profiles/r01_v18_kernels_full.md, time live"}
                           if args.config in NCU_WARP_INSTR and args.size is None and dcnt and world == 1 else None),
                 "step_algorithmic_GBps": step_bytes / (ms / K * 1e-3) / 1e9,
                 "step_frac_of_peak": step_bytes / (ms / K * 1e-3) / 1e9 / peak}
