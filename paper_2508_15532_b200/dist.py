@@ -141,7 +141,7 @@ class SlabDomain:
         self.G = torch.zeros((4,) + self.ctx.shape, dtype=torch.float64, device=self.device)
         self.owned_units = (self.layout.k1 - self.layout.k0) * grid["n"][0] * grid["n"][1] * self.ctx.nd
 
-    def set_fields(self, f, local=False):
+    def set_fields(self, f, local=False, state=True):
         import torch
         L, dev = self.layout, self.device
         cut = (lambda a: a) if local else (lambda a: a[L.planes])
@@ -149,8 +149,9 @@ class SlabDomain:
         rho, T = np.ascontiguousarray(cut(f["rho"])), np.ascontiguousarray(cut(f["T"]))
         u4 = None if f.get("u4") is None else torch.as_tensor(np.ascontiguousarray(cut4(f["u4"])), device=dev)
         self.ctx.set_fluid(torch.as_tensor(rho, device=dev), torch.as_tensor(T, device=dev), u4)
-        self.I = self.ctx.to_device(np.ascontiguousarray(cut(f["I0"])))
-        self.T = torch.as_tensor(T, device=dev).clone()
+        if state:   # (state=False: fluid and boundary data only; the caller owns I and T)
+            self.I = self.ctx.to_device(np.ascontiguousarray(cut(f["I0"])))
+            self.T = torch.as_tensor(T, device=dev).clone()
         n1, n2, _ = self.cfg["grid"]["n"]
         for (dim, side), g in f.get("ghosts", {}).items():
             g = np.asarray(g)
