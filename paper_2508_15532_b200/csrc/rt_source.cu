@@ -31,6 +31,31 @@ __device__ __forceinline__ double warp_sum(double v) {
     return v;
 }
 
+// Sums of the ten moment components over the 32 lanes through shared memory: every lane stores its ten partial sums
+// (row c at scr[c * 33 + lane]), three lanes add up each row (11 + 11 + 10 entries, combined by two shuffles), the
+// ten totals are written behind the rows and read back by all lanes.  ~45 instructions per lane instead of the 150 of
+// ten butterfly reductions; fixed order => bit-reproducible.  scr: WSUM_DOUBLES doubles owned by the warp.
+constexpr int WSUM_DOUBLES = 10 * 33 + 10;
+__device__ __forceinline__ void warp_sum10(double M[10], double *scr, int lane) {
+#pragma unroll
+    for (int c = 0; c < 10; ++c) scr[c * 33 + lane] = M[c];
+    __syncwarp();
+    const int c = lane / 3, q = lane - 3 * c;
+    double t = 0.0;
+    if (lane < 30) {
+        const double *r = scr + c * 33 + q * 11;
+#pragma unroll
+        for (int m = 0; m < 10; ++m) t += r[m];
+        if (q < 2) t += r[10];
+    }
+    const double t1 = __shfl_down_sync(0xffffffffu, t, 1), t2 = __shfl_down_sync(0xffffffffu, t, 2);
+    if (lane < 30 && q == 0) scr[330 + c] = (t + t1) + t2;
+    __syncwarp();
+#pragma unroll
+    for (int k = 0; k < 10; ++k) M[k] = scr[330 + k];
+    __syncwarp();
+}
+
 struct TEq {
     int method;
     double a4, b1, c0;             // methods 1, 2: a4 g(T) + b1 T + c0
@@ -99,15 +124,19 @@ __device__ __forceinline__ double rotate(const double M[10], const double *__res
 #define CELL_THREADS 256
 #define CELL_MINB 3
 #endif
+#ifndef MOM_MINB      // resident CTAs per SM of the moments-only passes (no source step: fewer live values, 64 registers)
+#define MOM_MINB 4
+#endif
 template <int MAXV, bool SRC, bool MOM, bool LIST>
-__global__ void __launch_bounds__(CELL_THREADS, (MAXV > 6 ? CELL_MINB - 1 : CELL_MINB))   // 362 directions: 12 values + 24 kept coefficients per lane
+__global__ void __launch_bounds__(CELL_THREADS, (MAXV > 6 ? CELL_MINB - 1 : (SRC ? CELL_MINB : MOM_MINB)))   // 362 directions: 12 values + 24 kept coefficients per lane
 k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, double *G_out) {
-    extern __shared__ double tab[];   // nx[pitch] ny[pitch] nz[pitch] w[pitch]
+    extern __shared__ double tab[];   // nx[pitch] ny[pitch] nz[pitch] w[pitch], then one warp_sum10 scratch per warp
     for (int t = threadIdx.x; t < 3 * p.pitch; t += blockDim.x) tab[t] = p.nhat[t];
     for (int t = threadIdx.x; t < p.pitch; t += blockDim.x) tab[3 * p.pitch + t] = p.w[t];
     __syncthreads();
     const double *snx = tab, *sny = tab + p.pitch, *snz = tab + 2 * p.pitch, *sw = tab + 3 * p.pitch;
     const int lane = threadIdx.x & 31;
+    double *scr = tab + 4 * p.pitch + (threadIdx.x >> 5) * WSUM_DOUBLES;
     const long long warp0 = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5;
     const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
 
@@ -120,7 +149,7 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
             const char *nx = reinterpret_cast<const char *>(I + nc * p.pitch) + lane * 128;
             if (lane * 128 < p.pitch * 8) asm volatile("prefetch.global.L1 [%0];" ::"l"(nx));
         }
-        const int col = int(cell % p.ncol);
+        const int col = int((unsigned)cell % (unsigned)p.ncol);   // cell < 2^31 (the lists hold ints)
         const double *cen = p.cen + (long long)col * CEN_STRIDE;
         double *Ic = I + cell * p.pitch;
         // all independent loads first: the cell's intensities (needed for every cell only when moments are wanted)
@@ -168,8 +197,7 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
                     const int s = lane + 32 * v;
                     if (s < p.nd) mom_accumulate(Mb, sw[s] * val[v], snx[s], sny[s], snz[s]);
                 }
-#pragma unroll
-                for (int c = 0; c < 10; ++c) Mb[c] = warp_sum(Mb[c]);
+                warp_sum10(Mb, scr, lane);
                 if (lane < 4) Rb = rotate(Mb, ecen, L, 0, lane);
             }
             double E = 0.0, A1 = 0.0, A2 = 0.0;
@@ -237,8 +265,7 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
                 const int s = lane + 32 * v;
                 if (s < p.nd) mom_accumulate(Ma, sw[s] * val[v], snx[s], sny[s], snz[s]);
             }
-#pragma unroll
-            for (int c = 0; c < 10; ++c) Ma[c] = warp_sum(Ma[c]);
+            warp_sum10(Ma, scr, lane);
             if (lane < 16) {
                 const int mu = lane >> 2, nu = lane & 3;
                 const double Ra = rotate(Ma, ecen, L, mu, nu);
@@ -256,7 +283,7 @@ cudaError_t launch_cell(const KParams &p, double *I, double *T, double dt, int *
     long long want = (nwork + threads / 32 - 1) / (threads / 32);
     const int blocks = (int)(want < 148LL * 8 * 4 ? want : 148LL * 8 * 4);
     if (blocks == 0) return cudaSuccess;
-    const size_t smem = 4 * p.pitch * sizeof(double);
+    const size_t smem = (4 * p.pitch + (threads / 32) * WSUM_DOUBLES) * sizeof(double);
     if (p.nd <= 64) k_cell<2, SRC, MOM, LIST><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail, R, G);
     else if (p.nd <= 192) k_cell<6, SRC, MOM, LIST><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail, R, G);
     else if (p.nd <= 384) k_cell<12, SRC, MOM, LIST><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail, R, G);

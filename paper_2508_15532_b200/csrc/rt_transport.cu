@@ -446,8 +446,12 @@ k_transport_vac(const __grid_constant__ KParams p, const double *__restrict__ I_
 // General path: full 5-point stencils, both PLI states at all six faces, Eq 20 or Eq 23 per face.  Marches x3 with a
 // 5-deep register window; computes only the steps it owns (cells with a non-vacuum face, or every cell of a
 // "general" thread).
+#ifndef GEN_THREADS
+#define GEN_THREADS 128   // 128 x 4 and 256 x 2 hold the same 16 warps per SM at 128 registers; the smaller CTA is 1-2 % faster
+#define GEN_MINB 4
+#endif
 template <int LIM, bool MATTER, bool LIST>
-__global__ void __launch_bounds__(256, 2)
+__global__ void __launch_bounds__(GEN_THREADS, GEN_MINB)
 k_transport_gen(const __grid_constant__ KParams p, const double *__restrict__ I_in, const double *I_base, double *I_out,
                 const double4 *__restrict__ fc0, const double4 *__restrict__ fc1, const double4 *__restrict__ fc2,
                 const unsigned char *__restrict__ cflag, const unsigned char *__restrict__ colflag, double dt) {
@@ -644,14 +648,14 @@ template <int LIM>
 static void launch_transport_lim(const KParams &p, const double *I_in, const double *I_base, double *I_out,
                                  double *const fcoef[3], const unsigned char *cflag, const unsigned char *colflag, bool matter,
                                  double dt, cudaStream_t st) {
-    dim3 grid(((p.n1 * p.pitch + 255) / 256) * p.n2);   // walked in tiles, see tile_block()
+    dim3 grid(((p.n1 * p.pitch + GEN_THREADS - 1) / GEN_THREADS) * p.n2);   // walked in tiles, see tile_block()
     dim3 gvac(((p.n1 * p.pitch + VAC_THREADS - 1) / VAC_THREADS) * p.n2);
     const double4 *f0 = reinterpret_cast<const double4 *>(fcoef[0]), *f1 = reinterpret_cast<const double4 *>(fcoef[1]),
                   *f2 = reinterpret_cast<const double4 *>(fcoef[2]);
     if (matter) {
         if (I_base == I_in) k_transport_vac<LIM, true, true><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
         else k_transport_vac<LIM, true, false><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
-        k_transport_gen<LIM, true, false><<<grid, 256, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
+        k_transport_gen<LIM, true, false><<<grid, GEN_THREADS, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
         if (p.ngen) k_transport_gen<LIM, true, true><<<dim3((p.ngen + 127) / 128, 8), 128, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
     } else {
         if (I_base == I_in) k_transport_vac<LIM, false, true><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
