@@ -39,6 +39,8 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--size", default=None, help="override grid, e.g. 64x48x32 (debug)")
+    ap.add_argument("--transport-variant", type=int, default=0, choices=[0, 1],
+                    help="rt_options.transport_variant: 0 = x2 stencil from L1/L2 (default), 1 = staged in shared memory")
     return ap.parse_args()
 
 
@@ -124,6 +126,9 @@ NCU_WARP_INSTR = {4: {"transport": 894.8e6, "angular": 439.2e6, "source": 250.2e
 ISSUE_PEAK = 148 * 4 * 1.965e9          # warp instructions / s: 148 SMs x 4 schedulers x 1 issue per clock at 1965 MHz
 
 
+TRANSPORT_VARIANT = 0    # set from --transport-variant
+
+
 def make_config(args):
     import rt_workloads as W
     n = tuple(int(x) for x in args.size.split("x")) if args.size else None
@@ -143,7 +148,7 @@ def setup_gpu(cfg, device):
     from paper_2508_15532_b200 import rt
 
     kind, params = cfg["metric"]
-    ctx = rt.RtContext(cfg["grid"], kind, params, cfg["level"], cfg["options"], device=device)
+    ctx = rt.RtContext(cfg["grid"], kind, params, cfg["level"], dict(cfg["options"], transport_variant=TRANSPORT_VARIANT), device=device)
     f = W.fields(cfg, ctx.directions()["nhat"], ctx.geometry("e_c"))
     dev = ctx.device
     rho = torch.as_tensor(f["rho"], device=dev).contiguous()
@@ -365,6 +370,8 @@ def main_reference(args):
 
 def main():
     args = parse()
+    global TRANSPORT_VARIANT
+    TRANSPORT_VARIANT = args.transport_variant
     if args.impl == "reference":
         return main_reference(args)
     import torch
@@ -416,7 +423,7 @@ def main():
                 "data": "synthetic",
                 "config": {"workload": workload_name(r["cfg"]), "dt": r["dt"], "l2": "inputs larger than L2 (one I copy >= 1 GB vs 126 MB)"
                            if units * 8 > 2.0e8 else "inputs FIT in L2 (latency-bound config; HBM fraction not meaningful)",
-                           "multi_gpu": r["multi"],
+                           "multi_gpu": r["multi"], "transport_variant": TRANSPORT_VARIANT,
                            "finite": r["finite"]},
                 "clocks": r["clk"], "e2e": r["e2e"], "gpu_launches": r["launches"], "roofline": roof}
         if not args.no_cpu_baseline and world == 1:

@@ -41,6 +41,10 @@ enum { RT_BC_PERIODIC = 0, RT_BC_OUTFLOW = 1, RT_BC_ZERO = 2, RT_BC_FIXED = 3,
 enum { RT_MINKOWSKI_CART = 0, RT_MINK_CYL_TETRAD = 1, RT_KS_MKS = 2, RT_SNAKE = 3 };
 enum { RT_LIM_MC = 0, RT_LIM_MINMOD = 1, RT_LIM_VANLEER = 2, RT_LIM_NONE = 3 };
 enum { RT_ANG_DONOR = 0, RT_ANG_MAPR = 1 };
+/* how the vacuum (Eq 20) transport kernel gets its x2 stencil: from L1/L2 (default, the faster one on the measured
+ * configs) or from a ring of three x3-planes staged in shared memory by CTAs of 4 x2-rows (fewer L2 requests, one
+ * barrier per step).  Same arithmetic in the same order: results are bit-identical. */
+enum { RT_TRANSPORT_L2 = 0, RT_TRANSPORT_SMEM_X2 = 1 };
 /* rt_get_geometry selectors (host output, for table-level parity of the init precompute) */
 enum { RT_GEOM_G_C = 0,     /* g_{mu nu} at centres        [E3][N2][N1][4][4]            */
        RT_GEOM_E_C = 1,     /* e^mu_a at centres           [E3][N2][N1][4 mu][4 a]       */
@@ -83,6 +87,7 @@ typedef struct {
     double a_rad;      /* radiation constant in code units */
     double Y_over_rho; /* k_B / ((Gamma-1) mu m_p), so that Y = Y_over_rho * rho (L399) */
     double abar;       /* a-bar of tau = abar alpha dt (L262; 1) */
+    int transport_variant; /* RT_TRANSPORT_* (0) */
 } rt_options;
 
 /* Build the angular grid with N_d = 10 angle_level^2 + 2 directions (L207-213; angle_level = 2^generation is the

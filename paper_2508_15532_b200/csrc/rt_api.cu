@@ -89,6 +89,7 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     if (metric->kind == RT_KS_MKS && (!metric->x3_symmetric || std::fabs(metric->a) >= 1.0)) return RT_EINVAL;
     if (opt->angular_recon != RT_ANG_DONOR && opt->angular_recon != RT_ANG_MAPR) return RT_EINVAL;
     if (opt->limiter < 0 || opt->limiter > 3 || opt->source_method < 0 || opt->source_method > 3) return RT_EINVAL;
+    if (opt->transport_variant != RT_TRANSPORT_L2 && opt->transport_variant != RT_TRANSPORT_SMEM_X2) return RT_EINVAL;
     if (opt->source_method != 0 && !(opt->Y_over_rho > 0)) return RT_EINVAL;
 
     rt_ctx *c = new (std::nothrow) rt_ctx();
@@ -269,6 +270,7 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
         k.face[a] = t.face[a];
     }
     k.limiter = opt->limiter; k.method = opt->source_method;
+    k.vac_smem = opt->transport_variant == RT_TRANSPORT_SMEM_X2;
     k.n0_floor = opt->n0_floor; k.rho_floor = opt->rho_floor; k.kappa_a0 = opt->kappa_a0; k.kappa_s = opt->kappa_s;
     k.a_rad = opt->a_rad; k.Y_over_rho = opt->Y_over_rho; k.abar = opt->abar;
     k.cen = t.cen; k.ecen = t.ecen; k.angcoef = t.angcoef; k.nhat = t.nhat; k.w = t.w; k.nb = t.nb; k.mirror = t.mirror;

@@ -20,6 +20,7 @@ struct KParams {
     int bc_lo[3], bc_hi[3];
     int zlo[3], zhi[3];
     int limiter, method;
+    int vac_smem;   // rt_options.transport_variant == RT_TRANSPORT_SMEM_X2
     double n0_floor, rho_floor, kappa_a0, kappa_s, a_rad, Y_over_rho, abar;
     const double *face[3];
     const double *cen;

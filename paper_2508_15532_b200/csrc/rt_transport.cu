@@ -443,6 +443,190 @@ k_transport_vac(const __grid_constant__ KParams p, const double *__restrict__ I_
     }
 }
 
+// The same upwind path with the x2 stencil staged in shared memory.  k_transport_vac asks L2 for seven operands per
+// cell-direction and step (L1 hit rate 14 %: the transverse neighbours belong to CTAs on other SMs) and is bound by the
+// L2 -> L1 traffic that causes (6.4 GB per launch for 2 GB of compulsory DRAM traffic, lts / l1tex throughput 66-70 %).
+// Here a CTA owns YS_TY consecutive x2-rows x 32 consecutive entries of the row (one warp per row) and keeps a ring of
+// three x3-planes of that patch plus its two halo rows on each side in shared memory: the value every thread loads
+// for its own x3 window (plane k + 2) is also stored into the ring, each warp loads one halo row, and the three x2
+// operands of step k are read from the ring two steps later.  L2 requests per cell-direction and step: own + halo
+// (4 / YS_TY) + three x1 operands = 5 instead of 7.  One barrier per step (4 warps).  Threads the kernel does not
+// compute for (dead, general, matter-only columns, rows beyond n2) still load and store their row: they are the
+// neighbours' operands.
+constexpr int YS_TY = 4;
+template <int LIM, bool MATTER, bool SAME_BASE>
+__global__ void __launch_bounds__(32 * YS_TY, VAC_MINB)
+k_transport_vac_ys(const __grid_constant__ KParams p, const double *__restrict__ I_in, const double *I_base, double *I_out,
+                   const unsigned char *__restrict__ cflag, const unsigned char *__restrict__ colflag, double dt) {
+    static_assert(YS_TY == 4, "one halo row per warp: four warps, four halo rows");
+    __shared__ double tile[3][YS_TY + 4][32];
+    const int lane = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    // block -> (bx: 32-entry segment of the row, bg: group of YS_TY rows), bands of TILE_ROWS rows as in tile_block()
+    const int rowlen = p.n1 * p.pitch;
+    const int nbx = (rowlen + 31) / 32, ngy = (p.n2 + YS_TY - 1) / YS_TY;
+    constexpr int GB = TILE_ROWS / YS_TY;
+    const int lin = blockIdx.x, band = lin / (nbx * GB), rr = lin - band * nbx * GB;
+    const int th = min(GB, ngy - band * GB);
+    const int bx = rr / th, bg = band * GB + (rr - bx * th);
+    const int e0 = bx * 32 + lane, j0 = bg * YS_TY, j = j0 + ty;
+    const bool inrow = e0 < rowlen;
+    const long long kstride = (long long)p.ncol * p.pitch;
+    const int n3 = p.n3, ncol = p.ncol;
+    // loader rows: the own slot (tile row ty + 2) and one halo slot (tile rows 0, 1, YS_TY + 2, YS_TY + 3)
+    const int hr = (ty < 2) ? ty : YS_TY + ty;
+    const int jown = nb_index(j, p.n2, p.bc_lo[1], p.bc_hi[1]), jhalo = nb_index(j0 - 2 + hr, p.n2, p.bc_lo[1], p.bc_hi[1]);
+    const double *pown = (inrow && jown >= 0) ? I_in + (long long)jown * rowlen + e0 : nullptr;
+    const double *phalo = (inrow && jhalo >= 0) ? I_in + (long long)jhalo * rowlen + e0 : nullptr;
+    // role of the thread
+    bool compute = inrow && j < p.n2;
+    if (compute) {
+        const long long q = (long long)j * rowlen + e0;
+        const int cl = p.cls[q];
+        if (cl & 1) {   // dead: this kernel keeps those entries zero
+            for (int k = 0; k < n3; ++k) I_out[q + k * kstride] = 0.0;
+            compute = false;
+        } else if (cl & 2) {
+            compute = false;
+        } else if (MATTER && !(colflag[j * p.n1 + e0 / p.pitch] & 2)) {
+            compute = false;
+        }
+    }
+    ColSetup c;
+    c.col = 0; c.s = 0; c.i = 0; c.j = 0;
+    c.xl = c.xh = c.yl = c.yh = c.zf = FaceK{0.0, 0.0, true};
+    c.oxm2 = c.oxm1 = c.oxp1 = c.oxp2 = 0;
+    if (compute) col_setup(p, dt, c, e0 / p.pitch, j, e0 % p.pitch);
+    const long long pos0 = compute ? (long long)c.col * p.pitch + c.s : 0;
+    double *out = I_out + pos0;
+    const int i = c.i, s = c.s;
+    const bool xpos = c.xl.pos, ypos = c.yl.pos, zpos = c.zf.pos;
+    const int oxa = xpos ? c.oxm2 : c.oxp2, oxb = xpos ? c.oxm1 : c.oxp1, oxd = xpos ? c.oxp1 : c.oxm1;
+    const double Kxbc = xpos ? -c.xl.A : c.xh.A, Kxcd = xpos ? c.xh.A : -c.xl.A;
+    const double Kybc = ypos ? -c.yl.A : c.yh.A, Kycd = ypos ? c.yh.A : -c.yl.A;
+    const double zA = c.zf.A, zhalf = zpos ? 0.5 : -0.5;
+    // tile rows of the x2 operands (a, b: two and one cell upwind, d: one cell downwind)
+    const double *tya = &tile[0][ty + 2 + (ypos ? -2 : 2)][lane], *tyb = &tile[0][ty + 2 + (ypos ? -1 : 1)][lane],
+                 *tyd = &tile[0][ty + 2 + (ypos ? 1 : -1)][lane];
+    double *town = &tile[0][ty + 2][lane], *thalo = &tile[0][hr][lane];
+    constexpr int SLOT = (YS_TY + 4) * 32;   // doubles per ring slot
+    const double *pk = I_in + pos0;          // compute threads only
+    // own-row value of plane kk: the x3 window of a compute thread (with the x3 boundary behind it) and the ring entry
+    auto ldown = [&](int kk) -> double {
+        if (kk >= 0 && kk < n3) return pown ? __ldg(pown + kk * kstride) : 0.0;
+        return compute ? slow_ld(p, I_in, 2, i, j, kk, s) : 0.0;
+    };
+    auto ldhalo = [&](int kk) -> double { return (phalo && kk < n3) ? __ldg(phalo + kk * kstride) : 0.0; };
+    double w1 = ldown(-1), w2 = ldown(0), w3 = ldown(1), Flo;
+    {
+        const double w0 = ldown(-2);
+        const double sg = slope_k<LIM>(w2 - w1, zpos ? (w1 - w0) : (w3 - w2));
+        Flo = zA * fma(zhalf, sg, zpos ? w1 : w2);
+    }
+    // ring prologue: planes 0 and 1
+    town[0] = w2; thalo[0] = ldhalo(0);
+    town[SLOT] = w3; thalo[SLOT] = ldhalo(1);
+    __syncthreads();
+    const double *pb = I_base + pos0;
+    const unsigned *pmask = reinterpret_cast<const unsigned *>(colflag + colmask_offset(ncol, n3)) + c.col;
+    const int zlo = p.zlo[2], zhi = n3 - p.zhi[2];
+    unsigned mcur = (MATTER && compute) ? __ldg(pmask) : 0u, mnext = (MATTER && compute && n3 > 32) ? __ldg(pmask + ncol) : 0u;
+    // Prefetch plan: the rows the warp will ask for VAC_PF steps later (own row and halo row at plane k + VAC_PF + 3,
+    // the four x1-neighbour rows and the base state at plane k + VAC_PF + 1) are 18 lines of 128 bytes; lane l asks for
+    // line l, one prefetch instruction per step instead of six per lane.  pfp: the lane's line at step 0.
+    const char *pfp = nullptr;
+    int pf_kend = 0;   // the lane prefetches while k < pf_kend
+#if VAC_PF
+    {
+        const unsigned cm = __ballot_sync(0xffffffffu, compute);
+        const int lead = cm ? __ffs(cm) - 1 : 0;
+        const bool nxm2 = __any_sync(0xffffffffu, compute && xpos), nxp2 = __any_sync(0xffffffffu, compute && !xpos);
+        int off[4] = {c.oxm2, c.oxm1, c.oxp1, c.oxp2};
+#pragma unroll
+        for (int r = 0; r < 4; ++r) off[r] = __shfl_sync(0xffffffffu, off[r], lead);
+        const long long lead_el = __shfl_sync(0xffffffffu, pos0, lead) - lead;   // plane-0 element of the warp's first entry (own row)
+        if (lane < 2) {            // own row, plane k + VAC_PF + 3
+            if (pown) { pfp = reinterpret_cast<const char *>(pown - lane + (VAC_PF + 3) * kstride) + 128 * lane; pf_kend = n3 - VAC_PF - 3; }
+        } else if (lane < 4) {     // halo row
+            if (phalo) { pfp = reinterpret_cast<const char *>(phalo - lane + (VAC_PF + 3) * kstride) + 128 * (lane - 2); pf_kend = n3 - VAC_PF - 3; }
+        } else if (lane < 16) {    // x1 neighbours of the compute lanes, plane k + VAC_PF + 1
+            const int r = (lane - 4) / 3, q = (lane - 4) - 3 * r;
+            const bool need = cm != 0u && ((r == 0) ? nxm2 : (r == 3) ? nxp2 : true);
+            const int o = (r == 0) ? off[0] : (r == 1) ? off[1] : (r == 2) ? off[2] : off[3];
+            if (need) {
+                const long long el = ((lead_el + o) & ~15LL) + 16 * q + (VAC_PF + 1) * kstride;
+                pfp = reinterpret_cast<const char *>(I_in + el); pf_kend = n3 - VAC_PF - 1;
+            }
+        } else if (!SAME_BASE && lane < 18) {
+            if (cm != 0u) { pfp = reinterpret_cast<const char *>(I_base + (lead_el & ~15LL) + 16 * (lane - 16) + (VAC_PF + 1) * kstride); pf_kend = n3 - VAC_PF - 1; }
+        }
+    }
+#endif
+    const long long kbytes = kstride * (long long)sizeof(double);
+    // software pipeline: the operands of step k + 1 are requested before step k is computed
+    double qxa = 0.0, qxb = 0.0, qxd = 0.0, qbase = 0.0;
+    if (compute) {
+        qxa = __ldg(pk + oxa); qxb = __ldg(pk + oxb); qxd = __ldg(pk + oxd);
+        if (!SAME_BASE) qbase = *pb;
+    }
+    double qw4 = ldown(2), qh4 = ldhalo(2);
+    int rd = 0, wr = 2 * SLOT;   // ring offsets (doubles) of plane k and plane k + 2
+#pragma unroll 1
+    for (int k = 0; k < n3; ++k) {
+        const double xa = qxa, xb = qxb, xd = qxd, w4 = qw4, cbase = qbase;
+        const bool mat = MATTER && ((mcur >> (k & 31)) & 1u);
+        town[wr] = w4; thalo[wr] = qh4;   // plane k + 2 into the ring (read by the neighbours at step k + 2)
+        if (k + 1 < n3) {
+            qw4 = ldown(k + 3); qh4 = ldhalo(k + 3);
+            if (compute) {
+                const double *pn = pk + kstride;
+                if (!SAME_BASE) qbase = pb[kstride];
+                qxa = __ldg(pn + oxa); qxb = __ldg(pn + oxb); qxd = __ldg(pn + oxd);
+            }
+#if VAC_PF
+            if (k < pf_kend) pf_l1(pfp);
+#endif
+        }
+        pfp += kbytes;
+        if (compute) {
+            // x3: upwind state at the upper face (always formed: it is the next cell's lower flux if that cell is vacuum)
+            const double sz = slope_k<LIM>(w3 - w2, zpos ? (w2 - w1) : (w4 - w3));
+            const double Fhi = zA * fma(zhalf, sz, zpos ? w2 : w3);
+            if (!mat) {
+                const double ya = tya[rd], yb = tyb[rd], yd = tyd[rd];
+                double D = Fhi - Flo;
+                {
+                    const double d1 = xb - xa, d2 = w2 - xb, d3 = xd - w2;
+                    D = fma(Kxbc, fma(0.5, slope_k<LIM>(d1, d2), xb), D);
+                    D = fma(Kxcd, fma(0.5, slope_k<LIM>(d2, d3), w2), D);
+                }
+                {
+                    const double d1 = yb - ya, d2 = w2 - yb, d3 = yd - w2;
+                    D = fma(Kybc, fma(0.5, slope_k<LIM>(d1, d2), yb), D);
+                    D = fma(Kycd, fma(0.5, slope_k<LIM>(d2, d3), w2), D);
+                }
+                const double base = SAME_BASE ? w2 : cbase;
+                *out = base - D;      // Eq 18 (O5), dt/(n^0 n_0 sqrt(-g) dx) folded in; the x3 zero band is reset below
+            }
+            Flo = Fhi;
+            pk += kstride; pb += kstride; out += kstride;
+            if (MATTER && (k & 31) == 31) {   // next mask word (requested 32 steps ago)
+                mcur = mnext;
+                pmask += ncol;
+                mnext = (k + 33 < n3) ? __ldg(pmask + ncol) : 0u;
+            }
+        }
+        w1 = w2; w2 = w3; w3 = w4;
+        rd = (rd == 2 * SLOT) ? 0 : rd + SLOT;
+        wr = (wr == 2 * SLOT) ? 0 : wr + SLOT;
+        __syncthreads();
+    }
+    if (compute && (zlo > 0 || zhi < n3)) {   // zero band in x3 (L709): reset after the march instead of a select in every step
+        double *o = I_out + pos0;
+        for (int k = 0; k < n3; ++k)
+            if (k < zlo || k >= zhi) o[k * kstride] = 0.0;
+    }
+}
+
 // General path: full 5-point stencils, both PLI states at all six faces, Eq 20 or Eq 23 per face.  Marches x3 with a
 // 5-deep register window; computes only the steps it owns (cells with a non-vacuum face, or every cell of a
 // "general" thread).
@@ -650,16 +834,17 @@ static void launch_transport_lim(const KParams &p, const double *I_in, const dou
                                  double dt, cudaStream_t st) {
     dim3 grid(((p.n1 * p.pitch + GEN_THREADS - 1) / GEN_THREADS) * p.n2);   // walked in tiles, see tile_block()
     dim3 gvac(((p.n1 * p.pitch + VAC_THREADS - 1) / VAC_THREADS) * p.n2);
+    dim3 gys(((p.n1 * p.pitch + 31) / 32) * ((p.n2 + YS_TY - 1) / YS_TY));   // RT_TRANSPORT_SMEM_X2
     const double4 *f0 = reinterpret_cast<const double4 *>(fcoef[0]), *f1 = reinterpret_cast<const double4 *>(fcoef[1]),
                   *f2 = reinterpret_cast<const double4 *>(fcoef[2]);
     if (matter) {
-        if (I_base == I_in) k_transport_vac<LIM, true, true><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
-        else k_transport_vac<LIM, true, false><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
+        if (I_base == I_in) { if (p.vac_smem) k_transport_vac_ys<LIM, true, true><<<gys, 32 * YS_TY, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt); else k_transport_vac<LIM, true, true><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt); }
+        else { if (p.vac_smem) k_transport_vac_ys<LIM, true, false><<<gys, 32 * YS_TY, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt); else k_transport_vac<LIM, true, false><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt); }
         k_transport_gen<LIM, true, false><<<grid, GEN_THREADS, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
         if (p.ngen) k_transport_gen<LIM, true, true><<<dim3((p.ngen + 127) / 128, 8), 128, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
     } else {
-        if (I_base == I_in) k_transport_vac<LIM, false, true><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
-        else k_transport_vac<LIM, false, false><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt);
+        if (I_base == I_in) { if (p.vac_smem) k_transport_vac_ys<LIM, false, true><<<gys, 32 * YS_TY, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt); else k_transport_vac<LIM, false, true><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt); }
+        else { if (p.vac_smem) k_transport_vac_ys<LIM, false, false><<<gys, 32 * YS_TY, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt); else k_transport_vac<LIM, false, false><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt); }
         if (p.ngen) k_transport_gen<LIM, false, true><<<dim3((p.ngen + 127) / 128, 8), 128, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
     }
 }

@@ -35,7 +35,7 @@ class RtOptions(ctypes.Structure):
     _fields_ = [("limiter", ctypes.c_int), ("angular_recon", ctypes.c_int), ("source_method", ctypes.c_int),
                 ("n0_floor", ctypes.c_double), ("rho_floor", ctypes.c_double), ("kappa_a0", ctypes.c_double),
                 ("kappa_s", ctypes.c_double), ("a_rad", ctypes.c_double), ("Y_over_rho", ctypes.c_double),
-                ("abar", ctypes.c_double)]
+                ("abar", ctypes.c_double), ("transport_variant", ctypes.c_int)]
 
 
 def load_library(path=LIB_PATH):
@@ -101,7 +101,7 @@ def _stream():
 
 
 DEFAULT_OPTIONS = dict(limiter=0, angular_recon=0, source_method=2, n0_floor=0.1, rho_floor=5e-4, kappa_a0=0.0,
-                       kappa_s=0.0, a_rad=1.0, Y_over_rho=1.5, abar=1.0)
+                       kappa_s=0.0, a_rad=1.0, Y_over_rho=1.5, abar=1.0, transport_variant=0)
 
 
 class RtContext:

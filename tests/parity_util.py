@@ -13,7 +13,7 @@ def rel_err(a, b):
     return float(np.abs(a - b).max() / den) if den > 0 else float(np.abs(a).max())
 
 
-def make_pair(cfg):
+def make_pair(cfg, gpu_options=None):
     """Build (oracle, RtContext, fields, dt) for a workload config; inputs are generated once from the oracle's
     tables and handed to both sides."""
     import torch
@@ -21,7 +21,7 @@ def make_pair(cfg):
 
     kind, params = cfg["metric"]
     orc = Oracle(cfg["grid"], kind, params, cfg["level"], cfg["options"])
-    ctx = rt.RtContext(cfg["grid"], kind, params, cfg["level"], cfg["options"])
+    ctx = rt.RtContext(cfg["grid"], kind, params, cfg["level"], dict(cfg["options"], **(gpu_options or {})))   # gpu_options: kernel-variant switches the oracle does not have
     f = W.fields(cfg, orc.ang["nhat"], orc.tab["e_c"])
     orc.set_fluid(f["rho"], f["T"], f["u4"])
     dev = ctx.device

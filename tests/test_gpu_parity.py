@@ -353,3 +353,47 @@ def test_error_codes():
     with pytest.raises(rt.RtError, match="invalid argument"):
         rt.RtContext(bad, kind, params, cfg["level"], cfg["options"])
     assert lib.rt_strerror(-4) == b"call order: fluid or boundary data not set"
+
+
+# ---- RT_TRANSPORT_SMEM_X2: the vacuum transport kernel with its x2 stencil staged in shared memory ---------------
+SMEM = {"transport_variant": 1}
+
+
+@pytest.mark.parametrize("idx,n,steps", [(1, (20, 19, 1), 12),      # vacuum, FIXED / OUTFLOW ghosts, rows not a multiple of 4
+                                         (4, (24, 22, 6), 6),       # Kerr-Schild: vacuum + matter cells, masked directions
+                                         (5, (10, 9, 3), 2),        # 362 directions: row length not a multiple of 32
+                                         (6, (16, 13, 1), 10),      # snake coordinates
+                                         (2, (6, 5, 4), 3)])        # all matter: the kernel only keeps the dead entries zero
+def test_smem_variant_matches_oracle(idx, n, steps):
+    cfg = W.config(idx, n=n)
+    orc, ctx, f, dt = make_pair(cfg, SMEM)
+    _check(run_steps(orc, ctx, f, dt, steps))
+
+
+@pytest.mark.parametrize("idx,n", [(4, (20, 18, 5)), (1, (9, 7, 2)), (4, (7, 3, 9)), (5, (6, 10, 4))])
+def test_smem_variant_bit_equal_to_default(idx, n):
+    """Same arithmetic in the same order (only the way the x2 operands reach the thread differs): identical bits."""
+    import torch
+    cfg = W.config(idx, n=n)
+    res = []
+    for gpu_opt in (None, SMEM):
+        orc, ctx, f, dt = make_pair(cfg, gpu_opt)
+        rng = np.random.default_rng(5)
+        I0 = f["I0"] + rng.uniform(0.0, 1e-2, size=f["I0"].shape)          # structure in every cell, also where I0 = 0
+        I = ctx.to_device(I0); T = torch.as_tensor(f["T"], device=ctx.device).contiguous().clone()
+        R = torch.zeros((16,) + ctx.shape, dtype=torch.float64, device=ctx.device)
+        G = torch.zeros((4,) + ctx.shape, dtype=torch.float64, device=ctx.device)
+        for _ in range(3):
+            ctx.step(I, T, dt, R, G)
+        res.append((I.clone(), T.clone(), R.clone(), G.clone()))
+        ctx.close()
+    for a, b in zip(*res):
+        assert torch.isfinite(a).all() and torch.equal(a, b)
+
+
+def test_unknown_transport_variant_rejected():
+    from paper_2508_15532_b200 import rt
+    cfg = W.config(1, n=(8, 8, 1))
+    kind, params = cfg["metric"]
+    with pytest.raises(rt.RtError):
+        rt.RtContext(cfg["grid"], kind, params, cfg["level"], dict(cfg["options"], transport_variant=7))
