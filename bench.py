@@ -116,13 +116,16 @@ def measured_peak():
 # different array: corrector only), write I_out; angular: read I_in, read+write I_inout; source: read+write I.
 ALGO_BYTES = {"transport_pred": 16.0, "transport_corr": 24.0, "angular": 24.0, "source": 16.0}
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per launch of each kernel class on config 4 at full size,
-# from the `ncu --set full` capture summarised in profiles/r01_v18_kernels_full.md (transport = vacuum + general +
-# list kernels, mean of the predictor (2.66 GB) and corrector (3.63 GB) launches).  Other configs: not captured -> null.
-NCU_TRAFFIC = {4: {"transport": 3.15e9, "angular": 3.09e9, "source": 0.51e9}}
+# from the `ncu --set full` capture summarised in profiles/r01_v19_kernels_full.md (transport = vacuum + general +
+# list kernels, mean of the predictor (2.66 GB) and corrector (3.64 GB) launches).  Other configs: not captured -> null.
+NCU_TRAFFIC = {4: {"transport": 3.15e9, "angular": 3.08e9, "source": 0.51e9}}
 # Warp instructions (smsp__inst_executed.sum) per launch of each kernel class, same capture (transport: mean of
-# 882.4 M predictor and 907.1 M corrector; source: mean of the three k_cell launches).  The transport and source kernels
-# are bound by instruction issue, not by HBM: `roofline.issue` reports that second roof.
-NCU_WARP_INSTR = {4: {"transport": 894.8e6, "angular": 439.2e6, "source": 250.2e6}}
+# 883.7 M predictor and 908.4 M corrector; source: mean of the three k_cell launches): `roofline.issue`.
+NCU_WARP_INSTR = {4: {"transport": 896.0e6, "angular": 439.2e6, "source": 200.2e6}}
+# What actually limits the vacuum transport kernel: the L2 -> L1 traffic of its seven operands per
+# cell-direction (l1tex__m_xbar2l1tex_read_bytes.sum per launch of the class, mean of predictor and corrector) and the
+# L2 throughput it runs at (lts__throughput of k_transport_vac), same capture: `roofline.l2`.
+NCU_L2 = {4: {"transport": {"l2_to_l1_bytes_per_launch": 8.74e9, "lts_throughput_pct_vac_kernel": 78.2}}}
 ISSUE_PEAK = 148 * 4 * 1.965e9          # warp instructions / s: 148 SMs x 4 schedulers x 1 issue per clock at 1965 MHz
 
 
@@ -406,7 +409,7 @@ def main():
         roof = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak,
                 "traffic": NCU_TRAFFIC.get(args.config, {}).get(dom) if args.size is None else None,
-                "traffic_source": "profiles/r01_v18_kernels_full.md (bytes per launch)", "peak_source": which,
+                "traffic_source": "profiles/r01_v19_kernels_full.md (bytes per launch)", "peak_source": which,
                 "algorithmic_bytes_per_launch": per_unit[dom] * units,
                 "algorithmic_bytes_per_cell_dir_per_launch": per_unit[dom],
                 "kernel_ms_per_step": {k: prof[k][0] / K for k in prof},
@@ -414,8 +417,10 @@ def main():
                 "issue": ({"warp_instr_per_launch": NCU_WARP_INSTR[args.config][dom],
                            "achieved": NCU_WARP_INSTR[args.config][dom] / (dms / max(dcnt, 1) * 1e-3), "peak": ISSUE_PEAK,
                            "unit": "warp-instr/s", "frac": NCU_WARP_INSTR[args.config][dom] / (dms / max(dcnt, 1) * 1e-3) / ISSUE_PEAK,
-                           "source": "instruction count from profiles/r01_v18_kernels_full.md, time live"}
+                           "source": "instruction count from profiles/r01_v19_kernels_full.md, time live"}
                           if args.config in NCU_WARP_INSTR and args.size is None and dcnt and world == 1 else None),
+                "l2": (dict(NCU_L2[args.config][dom], source="profiles/r01_v19_kernels_full.md (ncu capture, not live)")
+                       if args.config in NCU_L2 and dom in NCU_L2[args.config] and args.size is None and world == 1 else None),
                 "step_algorithmic_GBps": step_bytes / (ms / K * 1e-3) / 1e9,
                 "step_frac_of_peak": step_bytes / (ms / K * 1e-3) / 1e9 / peak}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
