@@ -358,7 +358,8 @@ def main_reference(args):
     rank = int(os.environ.get("RANK", 0))
     if rank != 0:
         return
-    val, cores, sample, ms, cfg = run_oracle(args.config, max(1, min(args.steps, 3)), warmup=min(args.warmup, 1))
+    # exactly K timed steps after W warm-up steps, each step = one oracle rt_step on the bounded sample (0.1-1 s per step)
+    val, cores, sample, ms, cfg = run_oracle(args.config, max(1, args.steps), warmup=max(0, args.warmup))
     import rt_workloads as W
     full = W.config(args.config)
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
