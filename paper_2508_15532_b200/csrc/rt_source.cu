@@ -201,6 +201,9 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
                 if (lane < 4) Rb = rotate(Mb, ecen, L, 0, lane);
             }
             double E = 0.0, A1 = 0.0, A2 = 0.0;
+            const double g0 = __ldg(cen), g1 = __ldg(cen + 1), g2 = __ldg(cen + 2), g3 = __ldg(cen + 3);       // -> n_0
+            const double e0 = __ldg(cen + 4), e1 = __ldg(cen + 5), e2 = __ldg(cen + 6), e3 = __ldg(cen + 7);   // -> n^0
+            const double adt = alpha * dt;
             // kept for the update loop below: ca = n^0/d (0 marks a masked or pad entry), cb = 1/(d nbar^3)
             double ca[MAXV], cb[MAXV];
 #pragma unroll
@@ -209,11 +212,13 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
                 ca[v] = 0.0; cb[v] = 0.0;
                 if (s < p.nd) {
                     const double nx = snx[s], ny = sny[s], nz = snz[s], ws = sw[s];
-                    const double n0c = cen[0] + cen[1] * nx + cen[2] * ny + cen[3] * nz;
+                    const double n0c = g0 + g1 * nx + g2 * ny + g3 * nz;
                     if (!(n0c > -p.n0_floor)) {
-                        const double nup = cen[4] + cen[5] * nx + cen[6] * ny + cen[7] * nz;
+                        const double nup = e0 + e1 * nx + e2 * ny + e3 * nz;
                         const double nbar = uh0 - (uh1 * nx + uh2 * ny + uh3 * nz);       // Eq 5, first row
-                        const double rd = __drcp_rn(nup + nbar * alpha * dt), rn = __drcp_rn(nbar);
+                        // 1/d and 1/nbar from one reciprocal: 1/(d nbar) times nbar, times d
+                        const double d = nup + nbar * adt, r = __drcp_rn(d * nbar);
+                        const double rd = r * nbar, rn = r * d;
                         const double IbdOm = nbar * nbar * val[v] * ws;                     // Ibar dOmegabar (S17)
                         E += IbdOm;                                                         // Eq 33
                         A1 += nup * rd * IbdOm;                                             // Eq 41a
