@@ -22,7 +22,7 @@ constexpr double FOURPI = 12.566370614359172953850573533118;
 
 // T^-3.5 = (1/T)^3 sqrt(1/T): a reciprocal and a square root instead of pow()
 __device__ __forceinline__ double t_m35(double T) {
-    const double r = 1.0 / T;
+    const double r = __drcp_rn(T);
     return r * r * r * sqrt(r);
 }
 __device__ __forceinline__ double warp_sum(double v) {
@@ -61,22 +61,25 @@ struct TEq {
     double a4, b1, c0;             // methods 1, 2: a4 g(T) + b1 T + c0
     double k45, k4, k35, k1, k0;   // method 3: coefficients of Eq 46
 };
+// residual and derivative of the temperature equation; sqrt(T) and 1/sqrt(T) from one rsqrt (no division)
 __device__ __forceinline__ void teq_eval(const TEq &q, double T, double &f, double &df) {
     if (q.method == 1) {
         const double T3 = T * T * T;
         f = q.a4 * T3 * T + q.b1 * T + q.c0;
         df = 4.0 * q.a4 * T3 + q.b1;
     } else if (q.method == 2) {
-        const double r = sqrt(T);
+        const double ir = rsqrt(T), r = T * ir;
         f = q.a4 * r + q.b1 * T + q.c0;
-        df = 0.5 * q.a4 / r + q.b1;
+        df = 0.5 * q.a4 * ir + q.b1;
     } else {
-        const double r = sqrt(T), T3 = T * T * T, T35 = T3 * r, T4 = T3 * T, T45 = T4 * r;
+        const double ir = rsqrt(T), r = T * ir, T3 = T * T * T, T35 = T3 * r, T4 = T3 * T, T45 = T4 * r;
         f = -(q.k45 * T45 + q.k4 * T4 + q.k35 * T35 + q.k1 * T + q.k0);
-        df = -(4.5 * q.k45 * T35 + 4.0 * q.k4 * T3 + 3.5 * q.k35 * T3 / r + q.k1);
+        df = -(4.5 * q.k45 * T35 + 4.0 * q.k4 * T3 + 3.5 * q.k35 * T3 * ir + q.k1);
     }
 }
-// Newton-Raphson (L399) from T_-, kept inside the bracket (0, W/Y] on which the residual changes sign (S20).
+// Newton-Raphson (L399) from T_-, kept inside the bracket (0, W/Y] on which the residual changes sign (S20).  The
+// Newton step uses a reciprocal instead of a division: the iterates differ from the oracle's in the last bits, the
+// root they converge to (|dT| <= 1e-14 T) does not.
 __device__ __forceinline__ bool solve_T(const TEq &q, double Tm, double Thi, double &Tp) {
     double lo = 0.0, hi = Thi, f, df;
     if (!(Thi > 0.0)) return false;
@@ -87,7 +90,7 @@ __device__ __forceinline__ bool solve_T(const TEq &q, double Tm, double Thi, dou
     for (int it = 0; it < 100; ++it) {
         teq_eval(q, T, f, df);
         if (f < 0) lo = T; else hi = T;
-        double Tn = T - f / df;
+        double Tn = T - f * __drcp_rn(df);
         if (!(Tn > 0.0 && Tn >= lo && Tn <= hi)) Tn = 0.5 * (lo + hi);   // closed bracket (S20): a root at an end is kept
         const double d = Tn - T;
         T = Tn;
