@@ -123,15 +123,18 @@ __device__ __forceinline__ double rotate(const double M[10], const double *__res
     return r;
 }
 
-#ifndef CELL_THREADS
-#define CELL_THREADS 256
-#define CELL_MINB 3
+#ifndef CELL_THREADS   // source-step variants: 128 registers, 16 warps per SM (80 registers x 24 warps spills and is 2-3 % slower)
+#define CELL_THREADS 128
+#define CELL_MINB 4
+#endif
+#ifndef MOM_THREADS
+#define MOM_THREADS 256
 #endif
 #ifndef MOM_MINB      // resident CTAs per SM of the moments-only passes (no source step: fewer live values, 64 registers)
 #define MOM_MINB 4
 #endif
 template <int MAXV, bool SRC, bool MOM, bool LIST>
-__global__ void __launch_bounds__(CELL_THREADS, (MAXV > 6 ? CELL_MINB - 1 : (SRC ? CELL_MINB : MOM_MINB)))   // 362 directions: 12 values + 24 kept coefficients per lane
+__global__ void __launch_bounds__(SRC ? CELL_THREADS : MOM_THREADS, (SRC ? CELL_MINB : (MAXV > 6 ? MOM_MINB - 2 : MOM_MINB)))   // moments-only, 362 directions: 12 values per lane, 128 registers
 k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, double *G_out) {
     extern __shared__ double tab[];   // nx[pitch] ny[pitch] nz[pitch] w[pitch], then one warp_sum10 scratch per warp
     for (int t = threadIdx.x; t < 3 * p.pitch; t += blockDim.x) tab[t] = p.nhat[t];
@@ -286,7 +289,7 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
 
 template <bool SRC, bool MOM, bool LIST>
 cudaError_t launch_cell(const KParams &p, double *I, double *T, double dt, int *n_fail, double *R, double *G, cudaStream_t st) {
-    const int threads = CELL_THREADS;
+    const int threads = SRC ? CELL_THREADS : MOM_THREADS;
     const long long nwork = LIST ? (long long)p.nsrc : p.ncell;
     long long want = (nwork + threads / 32 - 1) / (threads / 32);
     const int blocks = (int)(want < 148LL * 8 * 4 ? want : 148LL * 8 * 4);
