@@ -316,6 +316,41 @@ def run_gpu(args, rank, world):
                 del hp
             except Exception as ex:   # e.g. out of memory at a size nobody planned for: the single-call figure stands
                 e2e["pipeline_error"] = str(ex)[:160]
+        # Coupled mode, the way the paper drives the module (L448-456): the radiation state stays on the GPU; every step the
+        # fluid state (rho, T, u^mu: what the GRMHD sector owns) comes from pinned host buffers, and the moments R, the
+        # 4-force G and the new T go back.  Extra figure beside the strict one above (which moves the intensity both ways).
+        if slab is None and world == 1:
+            try:
+                pin = lambda a: torch.empty(tuple(a.shape), dtype=torch.float64, pin_memory=True).copy_(torch.as_tensor(a))
+                hrho, hTc = pin(f["rho"]), pin(T0.cpu())
+                hu4 = None if f["u4"] is None else pin(f["u4"])
+                drho = torch.empty_like(T)
+                du4 = None if hu4 is None else torch.empty(tuple(hu4.shape), dtype=torch.float64, device=dev)
+                I.copy_(I0)
+                def three():
+                    drho.copy_(hrho, non_blocking=True); T.copy_(hTc, non_blocking=True)
+                    if du4 is not None:
+                        du4.copy_(hu4, non_blocking=True)
+                    ctx.set_fluid(drho, T, du4)
+                    ctx.step(I, T, dt, R, G)
+                    hR.copy_(R, non_blocking=True); hG.copy_(G, non_blocking=True); hTc.copy_(T, non_blocking=True)
+                    torch.cuda.synchronize()          # the host consumes R, G, T before it produces the next fluid state
+                three()
+                barrier()
+                ev0.record()
+                for _ in range(ksteps):
+                    three()
+                ev1.record()
+                barrier()
+                cms = ev0.elapsed_time(ev1)
+                if bool(torch.isfinite(hR).all().item()):
+                    e2e["coupled"] = {"value": aggregate_value(units, ksteps, world, cms), "ms_per_step": cms / ksteps,
+                                      "h2d_bytes_per_step": (hrho.numel() + hTc.numel() + (0 if hu4 is None else hu4.numel())) * 8,
+                                      "d2h_bytes_per_step": (hR.numel() + hG.numel() + hTc.numel()) * 8,
+                                      "path": "intensity resident on the GPU; per step H2D of rho, T, u4 -> rt_set_fluid -> rt_step -> "
+                                              "D2H of R, G, T, host synchronised every step"}
+            except Exception as ex:
+                e2e["coupled_error"] = str(ex)[:160]
     return dict(cfg=cfg, ctx=ctx, ms=ms, units=units, kernel_units=kernel_units, prof=prof, launches=launches, clk=clk, e2e=e2e,
                 finite=finite, dt=dt, multi=multi)
 

@@ -5,6 +5,9 @@
 #include <new>
 #include <vector>
 
+#include <cub/device/device_partition.cuh>
+#include <cub/iterator/counting_input_iterator.cuh>
+
 #include "rt_kernels.cuh"
 
 using namespace rt;
@@ -24,7 +27,8 @@ struct rt_ctx {
     DeviceTables tab;
     double *d_rho, *d_u4, *d_T, *d_Th, *d_Ih, *d_fcoef[3];
     unsigned char *d_cflag;   // per cell: any non-vacuum face
-    int *d_genlist, *d_srclist, *d_vaclist;
+    int *d_genlist, *d_srclist, *d_vaclist;   // d_srclist: [ncell] listed cells first (ascending), the rest behind them; d_vaclist points into it
+    int *d_nsel; void *d_part_tmp; size_t part_tmp_bytes;   // interaction-list partition (cub) scratch
     double *d_hI, *d_hT, *d_hR, *d_hG;   // device staging of rt_step_host (allocated on first use)
     int *d_hfail;
     double *d_mapr_xi, *d_mapr_xim, *d_mapr_a, *d_angraw;
@@ -243,7 +247,7 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     c->d_rho = c->d_u4 = c->d_T = c->d_Th = c->d_Ih = nullptr;
     c->d_fcoef[0] = c->d_fcoef[1] = c->d_fcoef[2] = nullptr;
     c->d_cflag = nullptr;
-    c->d_colflag = nullptr; c->d_cls = nullptr; c->d_genlist = nullptr; c->d_srclist = nullptr; c->d_vaclist = nullptr;
+    c->d_colflag = nullptr; c->d_cls = nullptr; c->d_genlist = nullptr; c->d_srclist = nullptr; c->d_vaclist = nullptr; c->d_nsel = nullptr; c->d_part_tmp = nullptr; c->part_tmp_bytes = 0;
     c->d_hI = c->d_hT = c->d_hR = c->d_hG = nullptr; c->d_hfail = nullptr;
     c->d_mapr_xi = c->d_mapr_xim = c->d_mapr_a = c->d_angraw = nullptr; c->d_mapr_back = c->d_mapr_nnb = nullptr; c->d_angup = nullptr;
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_cls, (size_t)ncol * pitch);
@@ -336,7 +340,7 @@ extern "C" int rt_free(rt_ctx *c) {
     if (!c) return RT_EINVAL;
     for (int a = 0; a < 3; ++a) { cudaFree(c->tab.face[a]); cudaFree(c->d_fcoef[a]); }
     cudaFree(c->tab.cen); cudaFree(c->tab.ecen); cudaFree(c->tab.angcoef); cudaFree(c->tab.nhat); cudaFree(c->tab.w);
-    cudaFree(c->tab.nb); cudaFree(c->tab.mirror); cudaFree(c->d_cflag); cudaFree(c->d_colflag); cudaFree(c->d_cls); cudaFree(c->d_genlist); cudaFree(c->d_srclist); cudaFree(c->d_vaclist); cudaFree(c->d_hI); cudaFree(c->d_hT); cudaFree(c->d_hR); cudaFree(c->d_hG); cudaFree(c->d_hfail); cudaFree(c->d_mapr_xi); cudaFree(c->d_mapr_xim); cudaFree(c->d_mapr_a);
+    cudaFree(c->tab.nb); cudaFree(c->tab.mirror); cudaFree(c->d_cflag); cudaFree(c->d_colflag); cudaFree(c->d_cls); cudaFree(c->d_genlist); cudaFree(c->d_srclist); cudaFree(c->d_nsel); cudaFree(c->d_part_tmp); cudaFree(c->d_hI); cudaFree(c->d_hT); cudaFree(c->d_hR); cudaFree(c->d_hG); cudaFree(c->d_hfail); cudaFree(c->d_mapr_xi); cudaFree(c->d_mapr_xim); cudaFree(c->d_mapr_a);
     cudaFree(c->d_angraw); cudaFree(c->d_mapr_back); cudaFree(c->d_mapr_nnb); cudaFree(c->d_angup); cudaFree(c->d_rho); cudaFree(c->d_u4); cudaFree(c->d_T); cudaFree(c->d_Th); cudaFree(c->d_Ih);
     delete c;
     return RT_OK;
@@ -457,6 +461,13 @@ extern "C" int rt_set_boundary(rt_ctx *c, int dim, int side, const double *ghost
     return RT_OK;
 }
 
+namespace {
+struct AboveFloor {   // L468 (i): cells at or above the density floor interact
+    const double *rho; double floor;
+    __device__ bool operator()(int q) const { return rho[q] >= floor; }
+};
+}  // namespace
+
 extern "C" int rt_set_fluid(rt_ctx *c, const double *rho, const double *T, const double *u4, void *stream) {
     if (!c || !rho || !T) return RT_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
@@ -472,31 +483,35 @@ extern "C" int rt_set_fluid(rt_ctx *c, const double *rho, const double *T, const
         CK(cudaStreamSynchronize(st));
         CK(cudaMemcpy(c->d_u4, h.data(), 4 * nb, cudaMemcpyHostToDevice));
     }
-    // interaction list: cells at or above the density floor (L468 (i)); below it alpha = 0 whatever T is
+    // interaction list: cells at or above the density floor (L468 (i)); below it alpha = 0 whatever T is.  Built on the
+    // device (cub partition of the cell indices: listed cells first in ascending order, the rest behind them), so that
+    // a caller who hands over a new fluid state every step (the coupled GRMHD use, L448-456) pays one 4-byte read-back.
     {
-        std::vector<double> hr((size_t)c->ncell);
-        CK(cudaStreamSynchronize(st));
-        CK(cudaMemcpy(hr.data(), c->d_rho, nb, cudaMemcpyDeviceToHost));
-        std::vector<int> sl, vl;   // vl: the complement (cells the source step cannot touch: their moments need one pass only)
-        if (c->matter && c->opt.source_method != 0)
-            for (long long q = 0; q < c->ncell; ++q) {
-                if (hr[q] >= c->opt.rho_floor) sl.push_back((int)q);
-                else vl.push_back((int)q);
-            }
-        cudaFree(c->d_srclist); cudaFree(c->d_vaclist);
-        c->d_srclist = c->d_vaclist = nullptr;
-        c->kp.nsrc = (int)sl.size();
-        c->kp.nvac = (int)vl.size();
+        c->kp.nsrc = c->kp.nvac = 0;
         c->kp.srclist = c->kp.vaclist = nullptr;
-        if (!sl.empty()) {
-            cudaError_t e = upload(&c->d_srclist, sl);
-            if (e != cudaSuccess) { g_last_cuda = (int)e; return RT_ECUDA; }
-            c->kp.srclist = c->d_srclist;
-        }
-        if (!sl.empty() && !vl.empty()) {
-            cudaError_t e = upload(&c->d_vaclist, vl);
-            if (e != cudaSuccess) { g_last_cuda = (int)e; return RT_ECUDA; }
-            c->kp.vaclist = c->d_vaclist;
+        c->d_vaclist = nullptr;
+        if (c->matter && c->opt.source_method != 0) {
+            const int n = (int)c->ncell;
+            cub::CountingInputIterator<int> idx(0);
+            AboveFloor sel{c->d_rho, c->opt.rho_floor};
+            if (!c->d_srclist) {
+                CK(cudaMalloc((void **)&c->d_srclist, (size_t)n * sizeof(int)));
+                CK(cudaMalloc((void **)&c->d_nsel, sizeof(int)));
+                CK(cub::DevicePartition::If(nullptr, c->part_tmp_bytes, idx, c->d_srclist, c->d_nsel, n, sel, st));
+                CK(cudaMalloc(&c->d_part_tmp, c->part_tmp_bytes ? c->part_tmp_bytes : 1));
+            }
+            size_t tmp = c->part_tmp_bytes;
+            CK(cub::DevicePartition::If(c->d_part_tmp, tmp, idx, c->d_srclist, c->d_nsel, n, sel, st));
+            int nsel = 0;
+            CK(cudaMemcpyAsync(&nsel, c->d_nsel, sizeof(int), cudaMemcpyDeviceToHost, st));
+            CK(cudaStreamSynchronize(st));
+            c->kp.nsrc = nsel;
+            if (nsel > 0) c->kp.srclist = c->d_srclist;
+            if (nsel > 0 && nsel < n) {   // the complement (cells the source step cannot touch: their moments need one pass only)
+                c->kp.nvac = n - nsel;
+                c->d_vaclist = c->d_srclist + nsel;
+                c->kp.vaclist = c->d_vaclist;
+            }
         }
     }
     c->fluid_set = true;
