@@ -397,3 +397,33 @@ def test_unknown_transport_variant_rejected():
     kind, params = cfg["metric"]
     with pytest.raises(rt.RtError):
         rt.RtContext(cfg["grid"], kind, params, cfg["level"], dict(cfg["options"], transport_variant=7))
+
+
+def test_set_fluid_every_step_same_bits_and_list_follows_the_density():
+    """rt_set_fluid rebuilds the interaction list on the device: calling it before every step with the same fluid changes
+    nothing, and a density that drops below the floor everywhere turns the source step off (T stays, G = 0)."""
+    import torch
+    cfg = W.config(4, n=(14, 12, 4))
+    orc, ctx, f, dt = make_pair(cfg)
+    dev = ctx.device
+    rho = torch.as_tensor(f["rho"], device=dev).contiguous()
+    u4 = torch.as_tensor(f["u4"], device=dev).contiguous()
+    res = []
+    for every in (False, True):
+        I = ctx.to_device(f["I0"]); T = torch.as_tensor(f["T"], device=dev).contiguous().clone()
+        R = torch.zeros((16,) + ctx.shape, dtype=torch.float64, device=dev)
+        G = torch.zeros((4,) + ctx.shape, dtype=torch.float64, device=dev)
+        ctx.set_fluid(rho, T, u4)
+        for _ in range(3):
+            if every:
+                ctx.set_fluid(rho, T, u4)
+            ctx.step(I, T, dt, R, G)
+        res.append((I.clone(), T.clone(), R.clone(), G.clone()))
+    for a, b in zip(*res):
+        assert torch.equal(a, b)
+    assert (res[0][3] != 0).any()                      # the torus interacts
+    T0 = torch.as_tensor(f["T"], device=dev).contiguous().clone()
+    T = T0.clone(); I = ctx.to_device(f["I0"])
+    ctx.set_fluid(torch.full_like(rho, 1e-6), T, u4)     # everything below rho_floor = 5e-4
+    ctx.step(I, T, dt, R, G)
+    assert torch.equal(T, T0) and not (G != 0).any() and torch.isfinite(R).all()
