@@ -35,6 +35,7 @@ struct rt_ctx {
     int *d_mapr_back, *d_mapr_nnb;
     unsigned char *d_angup;
     unsigned char *d_cls;     // per (column, s): dead / general class (k_classify)
+    bool u4_rest;             // d_u4 holds the tetrad rest frame (rt_set_fluid with u4 == NULL)
     unsigned char *d_colflag; // per column: bit 0 has such a cell, bit 1 has an all-vacuum cell
     KParams kp;
     long long launches;
@@ -247,7 +248,7 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     c->d_rho = c->d_u4 = c->d_T = c->d_Th = c->d_Ih = nullptr;
     c->d_fcoef[0] = c->d_fcoef[1] = c->d_fcoef[2] = nullptr;
     c->d_cflag = nullptr;
-    c->d_colflag = nullptr; c->d_cls = nullptr; c->d_genlist = nullptr; c->d_srclist = nullptr; c->d_vaclist = nullptr; c->d_nsel = nullptr; c->d_part_tmp = nullptr; c->part_tmp_bytes = 0;
+    c->u4_rest = false; c->d_colflag = nullptr; c->d_cls = nullptr; c->d_genlist = nullptr; c->d_srclist = nullptr; c->d_vaclist = nullptr; c->d_nsel = nullptr; c->d_part_tmp = nullptr; c->part_tmp_bytes = 0;
     c->d_hI = c->d_hT = c->d_hR = c->d_hG = nullptr; c->d_hfail = nullptr;
     c->d_mapr_xi = c->d_mapr_xim = c->d_mapr_a = c->d_angraw = nullptr; c->d_mapr_back = c->d_mapr_nnb = nullptr; c->d_angup = nullptr;
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_cls, (size_t)ncol * pitch);
@@ -476,7 +477,9 @@ extern "C" int rt_set_fluid(rt_ctx *c, const double *rho, const double *T, const
     CK(cudaMemcpyAsync(c->d_T, T, nb, cudaMemcpyDeviceToDevice, st));
     if (u4) {
         CK(cudaMemcpyAsync(c->d_u4, u4, 4 * nb, cudaMemcpyDeviceToDevice, st));
-    } else {   // tetrad rest frame u^mu = e^mu_0
+        c->u4_rest = false;
+    } else if (!c->u4_rest) {   // tetrad rest frame u^mu = e^mu_0 (built once: it does not depend on the call)
+        c->u4_rest = true;
         std::vector<double> h(4 * (size_t)c->ncell);
         for (long long cell = 0; cell < c->ncell; ++cell)
             for (int mu = 0; mu < 4; ++mu) h[mu * c->ncell + cell] = c->h_e[(cell % c->ncol) * 16 + 4 * mu];
