@@ -427,3 +427,28 @@ def test_set_fluid_every_step_same_bits_and_list_follows_the_density():
     ctx.set_fluid(torch.full_like(rho, 1e-6), T, u4)     # everything below rho_floor = 5e-4
     ctx.step(I, T, dt, R, G)
     assert torch.equal(T, T0) and not (G != 0).any() and torch.isfinite(R).all()
+
+
+def test_rest_frame_fluid_is_rebuilt_after_an_explicit_velocity():
+    """rt_set_fluid(u4 = NULL) builds the tetrad rest frame once and keeps it; an explicit u4 in between must not leave
+    the library with a stale copy."""
+    import torch
+    cfg = W.config(2, n=(6, 5, 4))
+    orc, ctx, f, dt = make_pair(cfg)
+    assert f["u4"] is None
+    dev = ctx.device
+    rho = torch.as_tensor(f["rho"], device=dev).contiguous()
+    def run(prep):
+        I = ctx.to_device(f["I0"] + 0.01); T = torch.as_tensor(f["T"], device=dev).contiguous().clone()
+        prep(T)
+        ctx.step(I, T, dt)
+        return I.clone(), T.clone()
+    a = run(lambda T: ctx.set_fluid(rho, T, None))
+    b = run(lambda T: (ctx.set_fluid(rho, T, None), ctx.set_fluid(rho, T, None)))             # cached second time
+    boost = torch.zeros((4,) + ctx.shape, dtype=torch.float64, device=dev)
+    boost[0] = 1.25; boost[1] = 0.75                                                            # u.u = -1, moving along x1
+    c = run(lambda T: ctx.set_fluid(rho, T, boost))
+    d = run(lambda T: ctx.set_fluid(rho, T, None))                                              # back to the rest frame
+    assert torch.equal(a[0], b[0]) and torch.equal(a[1], b[1])
+    assert not torch.equal(a[0], c[0])
+    assert torch.equal(a[0], d[0]) and torch.equal(a[1], d[1])
