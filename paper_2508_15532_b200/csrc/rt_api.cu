@@ -26,7 +26,6 @@ struct rt_ctx {
     std::vector<double> h_g, h_e, h_einv, h_sqrtg, h_omega, h_n0, h_angcoef;
     DeviceTables tab;
     double *d_rho, *d_u4, *d_T, *d_Th, *d_Ih, *d_fcoef[3];
-    unsigned char *d_cflag;   // per cell: any non-vacuum face
     int *d_genlist, *d_srclist, *d_vaclist;   // d_srclist: [ncell] listed cells first (ascending), the rest behind them; d_vaclist points into it
     int *d_nsel; void *d_part_tmp; size_t part_tmp_bytes;   // interaction-list partition (cub) scratch
     double *d_hI, *d_hT, *d_hR, *d_hG;   // device staging of rt_step_host (allocated on first use)
@@ -247,12 +246,10 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     const size_t nI = (size_t)c->ncell * pitch;
     c->d_rho = c->d_u4 = c->d_T = c->d_Th = c->d_Ih = nullptr;
     c->d_fcoef[0] = c->d_fcoef[1] = c->d_fcoef[2] = nullptr;
-    c->d_cflag = nullptr;
     c->u4_rest = false; c->d_colflag = nullptr; c->d_cls = nullptr; c->d_genlist = nullptr; c->d_srclist = nullptr; c->d_vaclist = nullptr; c->d_nsel = nullptr; c->d_part_tmp = nullptr; c->part_tmp_bytes = 0;
     c->d_hI = c->d_hT = c->d_hR = c->d_hG = nullptr; c->d_hfail = nullptr;
     c->d_mapr_xi = c->d_mapr_xim = c->d_mapr_a = c->d_angraw = nullptr; c->d_mapr_back = c->d_mapr_nnb = nullptr; c->d_angup = nullptr;
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_cls, (size_t)ncol * pitch);
-    if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_cflag, c->ncell);
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_colflag, colflag_bytes(c->ncol, n3));   // column flags, x3-chunk flags, cell-flag masks
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_rho, c->ncell * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_u4, 4 * c->ncell * sizeof(double));
@@ -341,7 +338,7 @@ extern "C" int rt_free(rt_ctx *c) {
     if (!c) return RT_EINVAL;
     for (int a = 0; a < 3; ++a) { cudaFree(c->tab.face[a]); cudaFree(c->d_fcoef[a]); }
     cudaFree(c->tab.cen); cudaFree(c->tab.ecen); cudaFree(c->tab.angcoef); cudaFree(c->tab.nhat); cudaFree(c->tab.w);
-    cudaFree(c->tab.nb); cudaFree(c->tab.mirror); cudaFree(c->d_cflag); cudaFree(c->d_colflag); cudaFree(c->d_cls); cudaFree(c->d_genlist); cudaFree(c->d_srclist); cudaFree(c->d_nsel); cudaFree(c->d_part_tmp); cudaFree(c->d_hI); cudaFree(c->d_hT); cudaFree(c->d_hR); cudaFree(c->d_hG); cudaFree(c->d_hfail); cudaFree(c->d_mapr_xi); cudaFree(c->d_mapr_xim); cudaFree(c->d_mapr_a);
+    cudaFree(c->tab.nb); cudaFree(c->tab.mirror); cudaFree(c->d_colflag); cudaFree(c->d_cls); cudaFree(c->d_genlist); cudaFree(c->d_srclist); cudaFree(c->d_nsel); cudaFree(c->d_part_tmp); cudaFree(c->d_hI); cudaFree(c->d_hT); cudaFree(c->d_hR); cudaFree(c->d_hG); cudaFree(c->d_hfail); cudaFree(c->d_mapr_xi); cudaFree(c->d_mapr_xim); cudaFree(c->d_mapr_a);
     cudaFree(c->d_angraw); cudaFree(c->d_mapr_back); cudaFree(c->d_mapr_nnb); cudaFree(c->d_angup); cudaFree(c->d_rho); cudaFree(c->d_u4); cudaFree(c->d_T); cudaFree(c->d_Th); cudaFree(c->d_Ih);
     delete c;
     return RT_OK;
@@ -533,8 +530,8 @@ extern "C" int rt_transport(rt_ctx *c, const double *I_in, const double *I_base,
     if (!c || !I_in || !I_base || !I_out || I_in == I_out) return RT_EINVAL;
     if (fixed_bc_missing(c) || (c->matter && !c->fluid_set)) return RT_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
-    if (c->matter) { ProfScope ps(c, RT_K_FACECOEF, st); CK(launch_facecoef(c->kp, c->d_T, dt, c->d_fcoef, c->d_cflag, c->d_colflag, st, &c->launches)); }
-    { ProfScope ps(c, RT_K_TRANSPORT, st); CK(launch_transport(c->kp, I_in, I_base, I_out, c->d_fcoef, c->d_cflag, c->d_colflag, c->matter, dt, st, &c->launches)); }
+    if (c->matter) { ProfScope ps(c, RT_K_FACECOEF, st); CK(launch_facecoef(c->kp, c->d_T, dt, c->d_fcoef, c->d_colflag, st, &c->launches)); }
+    { ProfScope ps(c, RT_K_TRANSPORT, st); CK(launch_transport(c->kp, I_in, I_base, I_out, c->d_fcoef, c->d_colflag, c->matter, dt, st, &c->launches)); }
     return RT_OK;
 }
 
@@ -563,8 +560,8 @@ extern "C" int rt_moments(rt_ctx *c, const double *I, double *R, void *stream) {
 // then O6 on (I*, T) with T_- = T_base
 static int stage(rt_ctx *c, const double *I_flux, const double *T_flux, const double *I_base, double *I_out, double *T_io,
                  double delta, int *n_fail, double *R, double *G, cudaStream_t st) {
-    if (c->matter) { ProfScope ps(c, RT_K_FACECOEF, st); CK(launch_facecoef(c->kp, T_flux, delta, c->d_fcoef, c->d_cflag, c->d_colflag, st, &c->launches)); }
-    { ProfScope ps(c, RT_K_TRANSPORT, st); CK(launch_transport(c->kp, I_flux, I_base, I_out, c->d_fcoef, c->d_cflag, c->d_colflag, c->matter, delta, st, &c->launches)); }
+    if (c->matter) { ProfScope ps(c, RT_K_FACECOEF, st); CK(launch_facecoef(c->kp, T_flux, delta, c->d_fcoef, c->d_colflag, st, &c->launches)); }
+    { ProfScope ps(c, RT_K_TRANSPORT, st); CK(launch_transport(c->kp, I_flux, I_base, I_out, c->d_fcoef, c->d_colflag, c->matter, delta, st, &c->launches)); }
     if (c->curved) { ProfScope ps(c, RT_K_ANGULAR, st); CK((c->opt.angular_recon == RT_ANG_MAPR ? launch_angular_mapr : launch_angular)(c->kp, I_flux, I_out, delta, st, &c->launches)); }
     if (c->opt.source_method != 0 || R || G) {
         ProfScope ps(c, RT_K_SOURCE, st);

@@ -59,10 +59,10 @@ __host__ __device__ inline size_t colflag_bytes(int ncol, int n3) {
 }
 
 // launchers (rt_transport.cu, rt_source.cu); every launch increments *launches
-cudaError_t launch_facecoef(const KParams &p, const double *T, double dt, double *fcoef[3], unsigned char *cflag, unsigned char *colflag,
+cudaError_t launch_facecoef(const KParams &p, const double *T, double dt, double *fcoef[3], unsigned char *colflag,
                             cudaStream_t st, long long *launches);
 cudaError_t launch_transport(const KParams &p, const double *I_in, const double *I_base, double *I_out,
-                             double *const fcoef[3], const unsigned char *cflag, const unsigned char *colflag, bool matter,
+                             double *const fcoef[3], const unsigned char *colflag, bool matter,
                              double dt, cudaStream_t st, long long *launches);
 cudaError_t launch_angular_mapr(const KParams &p, const double *I_in, double *I_io, double dt, cudaStream_t st, long long *launches);
 cudaError_t launch_classify(const KParams &p, unsigned char *cls, cudaStream_t st);

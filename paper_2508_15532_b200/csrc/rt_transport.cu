@@ -183,18 +183,6 @@ __device__ __forceinline__ double flux_diff(double m2, double m1, double c0, dou
     return Fhi - Flo;
 }
 
-// cell flag: 1 if any of the six faces of the cell is a non-vacuum (Eq 23) face
-__global__ void k_cellflag(KParams p, const double4 *__restrict__ fc0, const double4 *__restrict__ fc1,
-                           const double4 *__restrict__ fc2, unsigned char *__restrict__ flag) {
-    const long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (c >= p.ncell) return;
-    const int i = int(c % p.n1), j = int((c / p.n1) % p.n2), k = int(c / p.ncol);
-    const long long x = ((long long)k * p.n2 + j) * (p.n1 + 1) + i, y = ((long long)k * (p.n2 + 1) + j) * p.n1 + i;
-    const bool m = fc0[x].y >= 0 || fc0[x + 1].y >= 0 || fc1[y].y >= 0 || fc1[y + p.n1].y >= 0 || fc2[c].y >= 0 ||
-                   fc2[c + p.ncol].y >= 0;
-    flag[c] = m ? 1 : 0;
-}
-
 // generic (boundary-aware) load, kept out of line: only threads next to a ZERO / FIXED boundary come here
 __device__ __noinline__ double slow_ld(const KParams &p, const double *I, int a, int i, int j, int k, int s) {
     // reflecting boundary (x2 only): the mirror image holds the direction with n-hat^2 flipped
@@ -217,27 +205,33 @@ __device__ __forceinline__ int nb_index(int c, int N, int bc_lo, int bc_hi) {
 // flag of (col, k).  The marching kernels test a bit per step and load one word per 32 steps: a per-step flag load sat
 // in front of every step's branch and exposed its L2 latency (it was 70 % of the vacuum kernel's long-scoreboard stalls).
 constexpr int GEN_KC = 8;
-__global__ void k_colflag(KParams p, const unsigned char *__restrict__ cflag, unsigned char *__restrict__ colflag) {
-    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+// One warp per column, lane = x3 index within a 32-cell word: the cell flags (any of the six faces non-vacuum) are formed
+// from the face coefficients and go straight into the ballot that makes the mask word; no per-cell flag array.
+__global__ void k_colflag(KParams p, const double4 *__restrict__ fc0, const double4 *__restrict__ fc1,
+                          const double4 *__restrict__ fc2, unsigned char *__restrict__ colflag) {
+    const int col = (int)((blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
     if (col >= p.ncol) return;
+    const int i = col % p.n1, j = col / p.n1;
     unsigned *cmask = reinterpret_cast<unsigned *>(colflag + colmask_offset(p.ncol, p.n3));
-    int m = 0, mc = 0;
-    unsigned mw = 0;
-    for (int k = 0; k < p.n3; ++k) {
-        const int f = cflag[(long long)k * p.ncol + col];
-        m |= f ? 1 : 2;
-        mc |= f;
-        if (f) mw |= 1u << (k & 31);
-        if ((k + 1) % GEN_KC == 0 || k + 1 == p.n3) {
-            colflag[p.ncol + (long long)(k / GEN_KC) * p.ncol + col] = (unsigned char)mc;
-            mc = 0;
+    int m = 0;
+    for (int k0 = 0; k0 < p.n3; k0 += 32) {
+        const int k = k0 + lane;
+        const bool in = k < p.n3;
+        bool f = false;
+        if (in) {
+            const long long x = ((long long)k * p.n2 + j) * (p.n1 + 1) + i, y = ((long long)k * (p.n2 + 1) + j) * p.n1 + i,
+                            c = (long long)k * p.ncol + col;
+            f = fc0[x].y >= 0 || fc0[x + 1].y >= 0 || fc1[y].y >= 0 || fc1[y + p.n1].y >= 0 || fc2[c].y >= 0 || fc2[c + p.ncol].y >= 0;
         }
-        if ((k & 31) == 31 || k + 1 == p.n3) {
-            cmask[(long long)(k >> 5) * p.ncol + col] = mw;
-            mw = 0;
-        }
+        const unsigned mw = __ballot_sync(0xffffffffu, f), valid = __ballot_sync(0xffffffffu, in);
+        if (mw) m |= 1;
+        if (valid & ~mw) m |= 2;
+        if (lane == 0) cmask[(long long)(k0 >> 5) * p.ncol + col] = mw;
+        const int kc = (k0 / GEN_KC) + lane;   // lanes 0..3: the four x3 chunks of this word
+        if (lane < 32 / GEN_KC && kc * GEN_KC < p.n3)
+            colflag[p.ncol + (long long)kc * p.ncol + col] = ((mw >> (GEN_KC * lane)) & ((1u << GEN_KC) - 1u)) ? 1 : 0;
     }
-    colflag[col] = (unsigned char)m;
+    if (lane == 0) colflag[col] = (unsigned char)m;
 }
 
 // ---- spatial transport ------------------------------------------------------------------------------------------
@@ -344,7 +338,7 @@ __global__ void k_classify(const __grid_constant__ KParams p, unsigned char *__r
 template <int LIM, bool MATTER, bool SAME_BASE>
 __global__ void __launch_bounds__(VAC_THREADS, VAC_MINB)
 k_transport_vac(const __grid_constant__ KParams p, const double *__restrict__ I_in, const double *I_base, double *I_out,
-                const unsigned char *__restrict__ cflag, const unsigned char *__restrict__ colflag, double dt) {
+                const unsigned char *__restrict__ colflag, double dt) {
     int bx, by;
     tile_block(p, bx, by);
     const int e0 = bx * blockDim.x + threadIdx.x;
@@ -457,7 +451,7 @@ constexpr int YS_TY = 4;
 template <int LIM, bool MATTER, bool SAME_BASE>
 __global__ void __launch_bounds__(32 * YS_TY, VAC_MINB)
 k_transport_vac_ys(const __grid_constant__ KParams p, const double *__restrict__ I_in, const double *I_base, double *I_out,
-                   const unsigned char *__restrict__ cflag, const unsigned char *__restrict__ colflag, double dt) {
+                   const unsigned char *__restrict__ colflag, double dt) {
     static_assert(YS_TY == 4, "one halo row per warp: four warps, four halo rows");
     __shared__ double tile[3][YS_TY + 4][32];
     const int lane = threadIdx.x & 31, ty = threadIdx.x >> 5;
@@ -638,7 +632,7 @@ template <int LIM, bool MATTER, bool LIST>
 __global__ void __launch_bounds__(GEN_THREADS, GEN_MINB)
 k_transport_gen(const __grid_constant__ KParams p, const double *__restrict__ I_in, const double *I_base, double *I_out,
                 const double4 *__restrict__ fc0, const double4 *__restrict__ fc1, const double4 *__restrict__ fc2,
-                const unsigned char *__restrict__ cflag, const unsigned char *__restrict__ colflag, double dt) {
+                const unsigned char *__restrict__ colflag, double dt) {
     // LIST = false: the non-general threads of columns that hold a cell with a non-vacuum face (grid over (i, s) x j).
     // LIST = true:  the "general" (column, s) pairs, from the compact list built at rt_init (one thread per entry).
     int ci, cj, cs;
@@ -813,24 +807,23 @@ __global__ void k_angular(KParams p, const double *__restrict__ I_in, double *I_
 }  // namespace
 
 // ---- launchers ---------------------------------------------------------------------------------------------------
-cudaError_t launch_facecoef(const KParams &p, const double *T, double dt, double *fcoef[3], unsigned char *cflag, unsigned char *colflag,
+cudaError_t launch_facecoef(const KParams &p, const double *T, double dt, double *fcoef[3], unsigned char *colflag,
                             cudaStream_t st, long long *launches) {
     for (int a = 0; a < 3; ++a) {
         long long nf = (long long)(p.n1 + (a == 0)) * (p.n2 + (a == 1)) * (p.n3 + (a == 2));
         k_facecoef<<<(unsigned)((nf + 255) / 256), 256, 0, st>>>(p, T, dt, a, reinterpret_cast<double4 *>(fcoef[a]));
         ++*launches;
     }
-    k_cellflag<<<(unsigned)((p.ncell + 255) / 256), 256, 0, st>>>(p, reinterpret_cast<const double4 *>(fcoef[0]),
-                                                                  reinterpret_cast<const double4 *>(fcoef[1]),
-                                                                  reinterpret_cast<const double4 *>(fcoef[2]), cflag);
-    k_colflag<<<(p.ncol + 127) / 128, 128, 0, st>>>(p, cflag, colflag);
-    *launches += 2;
+    k_colflag<<<(unsigned)(((long long)p.ncol * 32 + 127) / 128), 128, 0, st>>>(p, reinterpret_cast<const double4 *>(fcoef[0]),
+                                                                                   reinterpret_cast<const double4 *>(fcoef[1]),
+                                                                                   reinterpret_cast<const double4 *>(fcoef[2]), colflag);
+    *launches += 1;
     return cudaGetLastError();
 }
 
 template <int LIM>
 static void launch_transport_lim(const KParams &p, const double *I_in, const double *I_base, double *I_out,
-                                 double *const fcoef[3], const unsigned char *cflag, const unsigned char *colflag, bool matter,
+                                 double *const fcoef[3], const unsigned char *colflag, bool matter,
                                  double dt, cudaStream_t st) {
     dim3 grid(((p.n1 * p.pitch + GEN_THREADS - 1) / GEN_THREADS) * p.n2);   // walked in tiles, see tile_block()
     dim3 gvac(((p.n1 * p.pitch + VAC_THREADS - 1) / VAC_THREADS) * p.n2);
@@ -838,25 +831,25 @@ static void launch_transport_lim(const KParams &p, const double *I_in, const dou
     const double4 *f0 = reinterpret_cast<const double4 *>(fcoef[0]), *f1 = reinterpret_cast<const double4 *>(fcoef[1]),
                   *f2 = reinterpret_cast<const double4 *>(fcoef[2]);
     if (matter) {
-        if (I_base == I_in) { if (p.vac_smem) k_transport_vac_ys<LIM, true, true><<<gys, 32 * YS_TY, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt); else k_transport_vac<LIM, true, true><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt); }
-        else { if (p.vac_smem) k_transport_vac_ys<LIM, true, false><<<gys, 32 * YS_TY, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt); else k_transport_vac<LIM, true, false><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt); }
-        k_transport_gen<LIM, true, false><<<grid, GEN_THREADS, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
-        if (p.ngen) k_transport_gen<LIM, true, true><<<dim3((p.ngen + 127) / 128, 8), 128, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
+        if (I_base == I_in) { if (p.vac_smem) k_transport_vac_ys<LIM, true, true><<<gys, 32 * YS_TY, 0, st>>>(p, I_in, I_base, I_out, colflag, dt); else k_transport_vac<LIM, true, true><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, colflag, dt); }
+        else { if (p.vac_smem) k_transport_vac_ys<LIM, true, false><<<gys, 32 * YS_TY, 0, st>>>(p, I_in, I_base, I_out, colflag, dt); else k_transport_vac<LIM, true, false><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, colflag, dt); }
+        k_transport_gen<LIM, true, false><<<grid, GEN_THREADS, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, colflag, dt);
+        if (p.ngen) k_transport_gen<LIM, true, true><<<dim3((p.ngen + 127) / 128, 8), 128, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, colflag, dt);
     } else {
-        if (I_base == I_in) { if (p.vac_smem) k_transport_vac_ys<LIM, false, true><<<gys, 32 * YS_TY, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt); else k_transport_vac<LIM, false, true><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt); }
-        else { if (p.vac_smem) k_transport_vac_ys<LIM, false, false><<<gys, 32 * YS_TY, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt); else k_transport_vac<LIM, false, false><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, cflag, colflag, dt); }
-        if (p.ngen) k_transport_gen<LIM, false, true><<<dim3((p.ngen + 127) / 128, 8), 128, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, cflag, colflag, dt);
+        if (I_base == I_in) { if (p.vac_smem) k_transport_vac_ys<LIM, false, true><<<gys, 32 * YS_TY, 0, st>>>(p, I_in, I_base, I_out, colflag, dt); else k_transport_vac<LIM, false, true><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, colflag, dt); }
+        else { if (p.vac_smem) k_transport_vac_ys<LIM, false, false><<<gys, 32 * YS_TY, 0, st>>>(p, I_in, I_base, I_out, colflag, dt); else k_transport_vac<LIM, false, false><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, colflag, dt); }
+        if (p.ngen) k_transport_gen<LIM, false, true><<<dim3((p.ngen + 127) / 128, 8), 128, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, colflag, dt);
     }
 }
 
 cudaError_t launch_transport(const KParams &p, const double *I_in, const double *I_base, double *I_out,
-                             double *const fcoef[3], const unsigned char *cflag, const unsigned char *colflag, bool matter,
+                             double *const fcoef[3], const unsigned char *colflag, bool matter,
                              double dt, cudaStream_t st, long long *launches) {
     switch (p.limiter) {
-        case RT_LIM_MC: launch_transport_lim<RT_LIM_MC>(p, I_in, I_base, I_out, fcoef, cflag, colflag, matter, dt, st); break;
-        case RT_LIM_MINMOD: launch_transport_lim<RT_LIM_MINMOD>(p, I_in, I_base, I_out, fcoef, cflag, colflag, matter, dt, st); break;
-        case RT_LIM_NONE: launch_transport_lim<RT_LIM_NONE>(p, I_in, I_base, I_out, fcoef, cflag, colflag, matter, dt, st); break;
-        default: launch_transport_lim<RT_LIM_VANLEER>(p, I_in, I_base, I_out, fcoef, cflag, colflag, matter, dt, st); break;
+        case RT_LIM_MC: launch_transport_lim<RT_LIM_MC>(p, I_in, I_base, I_out, fcoef, colflag, matter, dt, st); break;
+        case RT_LIM_MINMOD: launch_transport_lim<RT_LIM_MINMOD>(p, I_in, I_base, I_out, fcoef, colflag, matter, dt, st); break;
+        case RT_LIM_NONE: launch_transport_lim<RT_LIM_NONE>(p, I_in, I_base, I_out, fcoef, colflag, matter, dt, st); break;
+        default: launch_transport_lim<RT_LIM_VANLEER>(p, I_in, I_base, I_out, fcoef, colflag, matter, dt, st); break;
     }
     *launches += 1 + (matter ? 1 : 0) + (p.ngen ? 1 : 0);
     return cudaGetLastError();
