@@ -39,6 +39,7 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--size", default=None, help="override grid, e.g. 64x48x32 (debug)")
+    ap.add_argument("--transport-tile", type=str, default="0,0,0,0,0,0", help="rt_options.transport_tile: TX,TY,DCH of the vacuum-tile and of the matter-tile kernel (0 = chosen by rt_init)")
     ap.add_argument("--transport-variant", type=int, default=0, choices=[0, 1],
                     help="rt_options.transport_variant: 0 = x2 stencil from L1/L2 (default), 1 = staged in shared memory")
     return ap.parse_args()
@@ -130,6 +131,7 @@ ISSUE_PEAK = 148 * 4 * 1.965e9          # warp instructions / s: 148 SMs x 4 sch
 
 
 TRANSPORT_VARIANT = 0    # set from --transport-variant
+TRANSPORT_TILE = (0, 0, 0, 0, 0, 0)
 
 
 def make_config(args):
@@ -151,7 +153,7 @@ def setup_gpu(cfg, device):
     from paper_2508_15532_b200 import rt
 
     kind, params = cfg["metric"]
-    ctx = rt.RtContext(cfg["grid"], kind, params, cfg["level"], dict(cfg["options"], transport_variant=TRANSPORT_VARIANT), device=device)
+    ctx = rt.RtContext(cfg["grid"], kind, params, cfg["level"], dict(cfg["options"], transport_variant=TRANSPORT_VARIANT, transport_tile=TRANSPORT_TILE), device=device)
     f = W.fields(cfg, ctx.directions()["nhat"], ctx.geometry("e_c"))
     dev = ctx.device
     rho = torch.as_tensor(f["rho"], device=dev).contiguous()
@@ -409,8 +411,9 @@ def main_reference(args):
 
 def main():
     args = parse()
-    global TRANSPORT_VARIANT
+    global TRANSPORT_VARIANT, TRANSPORT_TILE
     TRANSPORT_VARIANT = args.transport_variant
+    TRANSPORT_TILE = (tuple(int(v) for v in args.transport_tile.split(",")) + (0,) * 6)[:6]
     if args.impl == "reference":
         return main_reference(args)
     import torch

@@ -93,7 +93,7 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     if (metric->kind == RT_KS_MKS && (!metric->x3_symmetric || std::fabs(metric->a) >= 1.0)) return RT_EINVAL;
     if (opt->angular_recon != RT_ANG_DONOR && opt->angular_recon != RT_ANG_MAPR) return RT_EINVAL;
     if (opt->limiter < 0 || opt->limiter > 3 || opt->source_method < 0 || opt->source_method > 3) return RT_EINVAL;
-    if (opt->transport_variant != RT_TRANSPORT_L2 && opt->transport_variant != RT_TRANSPORT_SMEM_X2) return RT_EINVAL;
+    if (opt->transport_variant != RT_TRANSPORT_TMA && opt->transport_variant != RT_TRANSPORT_L2) return RT_EINVAL;
     if (opt->source_method != 0 && !(opt->Y_over_rho > 0)) return RT_EINVAL;
 
     rt_ctx *c = new (std::nothrow) rt_ctx();
@@ -272,7 +272,6 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
         k.face[a] = t.face[a];
     }
     k.limiter = opt->limiter; k.method = opt->source_method;
-    k.vac_smem = opt->transport_variant == RT_TRANSPORT_SMEM_X2;
     k.n0_floor = opt->n0_floor; k.rho_floor = opt->rho_floor; k.kappa_a0 = opt->kappa_a0; k.kappa_s = opt->kappa_s;
     k.a_rad = opt->a_rad; k.Y_over_rho = opt->Y_over_rho; k.abar = opt->abar;
     k.cen = t.cen; k.ecen = t.ecen; k.angcoef = t.angcoef; k.nhat = t.nhat; k.w = t.w; k.nb = t.nb; k.mirror = t.mirror;
@@ -318,6 +317,8 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
         k.mapr_xi = c->d_mapr_xi; k.mapr_xim = c->d_mapr_xim; k.mapr_a = c->d_mapr_a; k.mapr_back = c->d_mapr_back;
         k.mapr_nnb = c->d_mapr_nnb; k.angraw = c->d_angraw; k.angup = c->d_angup;
     }
+    k.variant = (opt->transport_variant == RT_TRANSPORT_TMA && tile_eligible(k)) ? RT_TRANSPORT_TMA : RT_TRANSPORT_L2;
+    choose_tile(k, opt->transport_tile, k.tile);
     e = launch_classify(k, c->d_cls, 0);
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     if (e == cudaSuccess) {   // compact list of the general (column, s) pairs, in memory order
@@ -348,6 +349,13 @@ extern "C" int rt_ndir(const rt_ctx *c) { return c ? c->nd : RT_EINVAL; }
 extern "C" int rt_ndir_padded(const rt_ctx *c) { return c ? c->pitch : RT_EINVAL; }
 extern "C" long long rt_launch_count(const rt_ctx *c) { return c ? c->launches : -1; }
 extern "C" int rt_last_cuda_error(void) { return g_last_cuda; }
+
+extern "C" int rt_transport_info(const rt_ctx *c, int out[7]) {
+    if (!c || !out) return RT_EINVAL;
+    out[0] = c->kp.variant;
+    for (int q = 0; q < 6; ++q) out[1 + q] = c->kp.tile[q];
+    return RT_OK;
+}
 
 extern "C" int rt_profile_enable(rt_ctx *c, int on) {
     if (!c) return RT_EINVAL;

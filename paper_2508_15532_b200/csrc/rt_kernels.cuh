@@ -20,7 +20,8 @@ struct KParams {
     int bc_lo[3], bc_hi[3];
     int zlo[3], zhi[3];
     int limiter, method;
-    int vac_smem;   // rt_options.transport_variant == RT_TRANSPORT_SMEM_X2
+    int variant;    // RT_TRANSPORT_TMA only if tile_eligible(), else RT_TRANSPORT_L2
+    int tile[6];    // RT_TRANSPORT_TMA: TX, TY, DCH of the vacuum-tile kernel, then of the matter-tile kernel
     double n0_floor, rho_floor, kappa_a0, kappa_s, a_rad, Y_over_rho, abar;
     const double *face[3];
     const double *cen;
@@ -64,6 +65,12 @@ cudaError_t launch_facecoef(const KParams &p, const double *T, double dt, double
 cudaError_t launch_transport(const KParams &p, const double *I_in, const double *I_base, double *I_out,
                              double *const fcoef[3], const unsigned char *colflag, bool matter,
                              double dt, cudaStream_t st, long long *launches);
+// rt_transport_tile.cu: the non-"general" pairs through the TMA tile kernel
+void choose_tile(const KParams &p, const int req[6], int out[6]);
+bool tile_eligible(const KParams &p);
+cudaError_t launch_transport_tile(const KParams &p, const int tile[6], const double *I_in, const double *I_base, double *I_out,
+                                  double *const fcoef[3], const unsigned char *colflag, bool matter, double dt, cudaStream_t st,
+                                  long long *launches);
 cudaError_t launch_angular_mapr(const KParams &p, const double *I_in, double *I_io, double dt, cudaStream_t st, long long *launches);
 cudaError_t launch_classify(const KParams &p, unsigned char *cls, cudaStream_t st);
 cudaError_t launch_angular(const KParams &p, const double *I_in, double *I_io, double dt, cudaStream_t st, long long *launches);

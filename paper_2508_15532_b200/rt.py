@@ -17,7 +17,7 @@ METRIC = {"minkowski": 0, "mink_cyl": 1, "ks_mks": 2, "snake": 3}
 GEOM = dict(g_c=0, e_c=1, einv_c=2, sqrtg_c=3, omega_c=4, n0_c=5, angcoef=6)
 SYMBOLS = ["rt_init", "rt_free", "rt_ndir", "rt_ndir_padded", "rt_get_directions", "rt_get_geometry", "rt_cfl_dt",
            "rt_set_boundary", "rt_set_fluid", "rt_transport", "rt_angular_flux", "rt_source_implicit", "rt_moments",
-           "rt_step", "rt_step_host", "rt_profile_enable", "rt_profile_read", "rt_launch_count", "rt_last_cuda_error", "rt_strerror"]
+           "rt_step", "rt_step_host", "rt_profile_enable", "rt_profile_read", "rt_transport_info", "rt_launch_count", "rt_last_cuda_error", "rt_strerror"]
 
 
 class RtGrid(ctypes.Structure):
@@ -35,7 +35,7 @@ class RtOptions(ctypes.Structure):
     _fields_ = [("limiter", ctypes.c_int), ("angular_recon", ctypes.c_int), ("source_method", ctypes.c_int),
                 ("n0_floor", ctypes.c_double), ("rho_floor", ctypes.c_double), ("kappa_a0", ctypes.c_double),
                 ("kappa_s", ctypes.c_double), ("a_rad", ctypes.c_double), ("Y_over_rho", ctypes.c_double),
-                ("abar", ctypes.c_double), ("transport_variant", ctypes.c_int)]
+                ("abar", ctypes.c_double), ("transport_variant", ctypes.c_int), ("transport_tile", ctypes.c_int * 6)]
 
 
 def load_library(path=LIB_PATH):
@@ -62,6 +62,7 @@ def load_library(path=LIB_PATH):
     lib.rt_step_host.argtypes = [vp, vp, vp, vp, vp, dbl, vp, vp]
     lib.rt_profile_enable.argtypes = [vp, ci]
     lib.rt_profile_read.argtypes = [vp, vp, vp]
+    lib.rt_transport_info.argtypes = [vp, vp]
     lib.rt_launch_count.argtypes = [vp]
     lib.rt_launch_count.restype = ctypes.c_longlong
     lib.rt_strerror.argtypes = [ci]
@@ -101,7 +102,8 @@ def _stream():
 
 
 DEFAULT_OPTIONS = dict(limiter=0, angular_recon=0, source_method=2, n0_floor=0.1, rho_floor=5e-4, kappa_a0=0.0,
-                       kappa_s=0.0, a_rad=1.0, Y_over_rho=1.5, abar=1.0, transport_variant=0)
+                       kappa_s=0.0, a_rad=1.0, Y_over_rho=1.5, abar=1.0, transport_variant=0,
+                       transport_tile=(0, 0, 0, 0, 0, 0))
 
 
 class RtContext:
@@ -218,6 +220,12 @@ class RtContext:
         _check(lib().rt_profile_read(self._h, ms.ctypes.data, cnt.ctypes.data))
         names = ("facecoef", "transport", "angular", "source", "moments")
         return {n: (float(ms[i]), int(cnt[i])) for i, n in enumerate(names)}
+
+    def transport_info(self):
+        """(variant actually used, (TX, TY, DCH) of the vacuum-tile kernel + (TX, TY, DCH) of the matter-tile kernel)."""
+        out = np.zeros(7, np.int32)
+        _check(lib().rt_transport_info(self._h, out.ctypes.data))
+        return int(out[0]), tuple(int(v) for v in out[1:])
 
     def launch_count(self):
         return int(lib().rt_launch_count(self._h))

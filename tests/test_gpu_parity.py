@@ -355,7 +355,7 @@ def test_error_codes():
     assert lib.rt_strerror(-4) == b"call order: fluid or boundary data not set"
 
 
-# ---- RT_TRANSPORT_SMEM_X2: the vacuum transport kernel with its x2 stencil staged in shared memory ---------------
+# ---- RT_TRANSPORT_L2: the round-1 kernels (one thread per (column, s) loads its own operands) against the default TMA tile kernel ----
 SMEM = {"transport_variant": 1}
 
 
