@@ -39,7 +39,7 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--size", default=None, help="override grid, e.g. 64x48x32 (debug)")
-    ap.add_argument("--transport-tile", type=str, default="0,0,0,0,0,0", help="rt_options.transport_tile: TX,TY,DCH of the vacuum-tile and of the matter-tile kernel (0 = chosen by rt_init)")
+    ap.add_argument("--transport-tile", type=str, default="0,0,0", help="rt_options.transport_tile: TX,TY,DCH of the TMA tile kernel (0,0,0 = chosen by rt_init)")
     ap.add_argument("--transport-variant", type=int, default=0, choices=[0, 1],
                     help="rt_options.transport_variant: 0 = x2 stencil from L1/L2 (default), 1 = staged in shared memory")
     return ap.parse_args()
@@ -131,7 +131,7 @@ ISSUE_PEAK = 148 * 4 * 1.965e9          # warp instructions / s: 148 SMs x 4 sch
 
 
 TRANSPORT_VARIANT = 0    # set from --transport-variant
-TRANSPORT_TILE = (0, 0, 0, 0, 0, 0)
+TRANSPORT_TILE = (0, 0, 0)
 
 
 def make_config(args):
@@ -413,7 +413,7 @@ def main():
     args = parse()
     global TRANSPORT_VARIANT, TRANSPORT_TILE
     TRANSPORT_VARIANT = args.transport_variant
-    TRANSPORT_TILE = (tuple(int(v) for v in args.transport_tile.split(",")) + (0,) * 6)[:6]
+    TRANSPORT_TILE = (tuple(int(v) for v in args.transport_tile.split(",")) + (0,) * 3)[:3]
     if args.impl == "reference":
         return main_reference(args)
     import torch

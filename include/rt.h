@@ -41,12 +41,12 @@ enum { RT_BC_PERIODIC = 0, RT_BC_OUTFLOW = 1, RT_BC_ZERO = 2, RT_BC_FIXED = 3,
 enum { RT_MINKOWSKI_CART = 0, RT_MINK_CYL_TETRAD = 1, RT_KS_MKS = 2, RT_SNAKE = 3 };
 enum { RT_LIM_MC = 0, RT_LIM_MINMOD = 1, RT_LIM_VANLEER = 2, RT_LIM_NONE = 3 };
 enum { RT_ANG_DONOR = 0, RT_ANG_MAPR = 1 };
-/* how the spatial transport kernels get their stencil operands.  RT_TRANSPORT_TMA (default): a CTA owns a tile of
+/* how the vacuum (Eq 20) spatial transport gets its stencil operands.  RT_TRANSPORT_TMA (default): a CTA owns a tile of
  * columns x a chunk of directions, a producer warp streams each x3-plane of the tile with its halos once into a ring of
- * shared-memory slots (cp.async.bulk.tensor + mbarrier), the consumers read all operands from the ring.  Needs the
+ * shared-memory slots (cp.async.bulk.tensor + mbarrier), 15 consumer warps read all operands from the ring.  Needs the
  * monotonised-central limiter and a PERIODIC or OUTFLOW x3 boundary; otherwise, and with RT_TRANSPORT_L2, one thread
- * per (column, direction) loads its operands itself through L1/L2 (the round-1 kernels).  Same arithmetic in the same
- * order: results are bit-identical. */
+ * per (column, direction) loads its operands itself through L1/L2 (the round-1 kernel).  Same arithmetic in the same
+ * order: results are bit-identical.  Cells with an Eq 23 face go through k_transport_gen either way. */
 enum { RT_TRANSPORT_TMA = 0, RT_TRANSPORT_L2 = 1 };
 /* rt_get_geometry selectors (host output, for table-level parity of the init precompute) */
 enum { RT_GEOM_G_C = 0,     /* g_{mu nu} at centres        [E3][N2][N1][4][4]            */
@@ -91,9 +91,8 @@ typedef struct {
     double Y_over_rho; /* k_B / ((Gamma-1) mu m_p), so that Y = Y_over_rho * rho (L399) */
     double abar;       /* a-bar of tau = abar alpha dt (L262; 1) */
     int transport_variant; /* RT_TRANSPORT_* (0) */
-    int transport_tile[6]; /* RT_TRANSPORT_TMA tiles: columns along x1, along x2, directions per chunk (even) of the kernel for
-                              all-vacuum tiles [0..2] and of the kernel for tiles with an Eq 23 face [3..5]; a triple of 0 =
-                              chosen by rt_init for the mesh */
+    int transport_tile[3]; /* RT_TRANSPORT_TMA tile: columns along x1, along x2, directions per chunk (even); all 0 = chosen by
+                              rt_init for the mesh */
 } rt_options;
 
 /* Build the angular grid with N_d = 10 angle_level^2 + 2 directions (L207-213; angle_level = 2^generation is the
@@ -152,8 +151,8 @@ int rt_profile_enable(rt_ctx *ctx, int on);
 int rt_profile_read(rt_ctx *ctx, double *ms_host, long long *count_host);
 
 /* Which spatial transport path rt_init selected, to HOST: out[0] = RT_TRANSPORT_* actually used (RT_TRANSPORT_L2 when the
- * tile kernel's conditions do not hold), out[1..6] = the two tiles in the order of rt_options.transport_tile. */
-int rt_transport_info(const rt_ctx *ctx, int out_host[7]);
+ * tile kernel's conditions do not hold), out[1..3] = the tile in the order of rt_options.transport_tile. */
+int rt_transport_info(const rt_ctx *ctx, int out_host[4]);
 
 /* number of kernels the library launched since rt_init (for bench.py's gpu_launches) */
 long long rt_launch_count(const rt_ctx *ctx);

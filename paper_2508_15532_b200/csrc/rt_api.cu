@@ -350,10 +350,10 @@ extern "C" int rt_ndir_padded(const rt_ctx *c) { return c ? c->pitch : RT_EINVAL
 extern "C" long long rt_launch_count(const rt_ctx *c) { return c ? c->launches : -1; }
 extern "C" int rt_last_cuda_error(void) { return g_last_cuda; }
 
-extern "C" int rt_transport_info(const rt_ctx *c, int out[7]) {
+extern "C" int rt_transport_info(const rt_ctx *c, int out[4]) {
     if (!c || !out) return RT_EINVAL;
     out[0] = c->kp.variant;
-    for (int q = 0; q < 6; ++q) out[1 + q] = c->kp.tile[q];
+    for (int q = 0; q < 3; ++q) out[1 + q] = c->kp.tile[q];
     return RT_OK;
 }
 

@@ -21,7 +21,7 @@ struct KParams {
     int zlo[3], zhi[3];
     int limiter, method;
     int variant;    // RT_TRANSPORT_TMA only if tile_eligible(), else RT_TRANSPORT_L2
-    int tile[6];    // RT_TRANSPORT_TMA: TX, TY, DCH of the vacuum-tile kernel, then of the matter-tile kernel
+    int tile[3];    // RT_TRANSPORT_TMA: TX, TY, DCH
     double n0_floor, rho_floor, kappa_a0, kappa_s, a_rad, Y_over_rho, abar;
     const double *face[3];
     const double *cen;
@@ -66,11 +66,10 @@ cudaError_t launch_transport(const KParams &p, const double *I_in, const double 
                              double *const fcoef[3], const unsigned char *colflag, bool matter,
                              double dt, cudaStream_t st, long long *launches);
 // rt_transport_tile.cu: the non-"general" pairs through the TMA tile kernel
-void choose_tile(const KParams &p, const int req[6], int out[6]);
+void choose_tile(const KParams &p, const int req[3], int out[3]);
 bool tile_eligible(const KParams &p);
-cudaError_t launch_transport_tile(const KParams &p, const int tile[6], const double *I_in, const double *I_base, double *I_out,
-                                  double *const fcoef[3], const unsigned char *colflag, bool matter, double dt, cudaStream_t st,
-                                  long long *launches);
+cudaError_t launch_transport_tile(const KParams &p, const int tile[3], const double *I_in, const double *I_base, double *I_out,
+                                  const unsigned char *colflag, bool matter, double dt, cudaStream_t st, long long *launches);
 cudaError_t launch_angular_mapr(const KParams &p, const double *I_in, double *I_io, double dt, cudaStream_t st, long long *launches);
 cudaError_t launch_classify(const KParams &p, unsigned char *cls, cudaStream_t st);
 cudaError_t launch_angular(const KParams &p, const double *I_in, double *I_io, double dt, cudaStream_t st, long long *launches);

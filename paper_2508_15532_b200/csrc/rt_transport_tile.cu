@@ -29,13 +29,13 @@ namespace rt {
 namespace {
 
 constexpr int NT = 480;              // consumer threads (15 warps); warp 15 is the producer: 16 warps = 128 registers each
-constexpr int RPV = 2, RPM = 1;      // pairs per consumer thread: vacuum-tile kernel, matter-tile kernel
+constexpr int RP = 2;                // pairs per consumer thread
 #ifndef NS_X
 #define NS_X 5
 #endif
 constexpr int NS = NS_X;             // ring slots: planes k, k+1, k+2 in use, two in flight
 constexpr int SLOT_STRIDE = 24576;   // bytes between ring slots (compile-time: every operand load is LDS [R + imm])
-constexpr int BSLOT_STRIDE = RPV * NT * 8;   // base ring: own cells only
+constexpr int BSLOT_STRIDE = RP * NT * 8;   // base ring: own cells only
 
 // ---- mbarrier / TMA primitives (PTX) ------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void *q) { return (uint32_t)__cvta_generic_to_shared(q); }
@@ -86,20 +86,19 @@ struct TileParams {
     int cellB, rowB;                                   // bytes of one cell (DCH doubles), of one own row
     int oHlo, oHhi, oGxlo, oGxhi, oGylo, oGyhi;        // block offsets in a slot (own block at 0)
     int slotB, bslotB;
-    int off_ring, off_base, off_extra;
-    int split;   // the launch owns only the tiles of its kind (see the kernel)
+    int off_ring, off_base;
+    int split;   // opacities present: tiles without an all-vacuum cell are skipped (see the kernel)
 };
 
 // One x3 step of the pairs of a thread.  U = k mod NS is a compile-time constant of the unrolled march, so all ring
 // offsets are immediates.
 struct PairK { double Kxbc, Kxcd, Kybc, Kycd, zA, zhalf; };
 
-template <bool MATTER, bool SAME_BASE, int RP>
+template <bool SAME_BASE, int RP>
 __global__ void __launch_bounds__(NT + 32, 1)
 k_transport_tile(const __grid_constant__ KParams p, const __grid_constant__ TileParams tp,
                  const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapH,
                  const __grid_constant__ CUtensorMap mapG, const __grid_constant__ CUtensorMap mapD, double *I_out,
-                 const double4 *__restrict__ fc0, const double4 *__restrict__ fc1, const double4 *__restrict__ fc2,
                  const unsigned char *__restrict__ colflag, double dt) {
     extern __shared__ __align__(1024) unsigned char smem[];
     const uint32_t sbase = smem_u32(smem);
@@ -117,14 +116,27 @@ k_transport_tile(const __grid_constant__ KParams p, const __grid_constant__ Tile
     const int n3 = p.n3, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const bool perx = p.bc_lo[0] == RT_BC_PERIODIC && p.n1 >= 2, pery = p.bc_lo[1] == RT_BC_PERIODIC && p.n2 >= 2;
     if (tp.split) {
-        // Two launches share the mesh: tiles whose columns are all vacuum (column flag bit 0 clear, k_colflag) belong to the
-        // lean MATTER = false kernel, tiles with an Eq 23 face somewhere to the MATTER = true kernel; the other CTAs leave.
+        // With opacities the cells that have an Eq 23 face are recomputed afterwards by k_transport_gen; a tile without a single
+        // all-vacuum cell (column flag bit 1 clear everywhere, k_colflag) has nothing to do here.
         int has = 0;
         if ((int)threadIdx.x < tp.TX * tp.TY) {
             const int i = i0 + (int)threadIdx.x % tp.TX, j = j0 + (int)threadIdx.x / tp.TX;
-            if (i < p.n1 && j < p.n2) has = colflag[j * p.n1 + i] & 1;
+            if (i < p.n1 && j < p.n2) has = colflag[j * p.n1 + i] & 2;
         }
-        if ((__syncthreads_or(has) != 0) != MATTER) return;
+        if (__syncthreads_or(has) == 0) {   // only the dead entries (masked directions, zero bands, pad) are this kernel's: keep them zero
+            if ((int)threadIdx.x < NT)
+                for (int r = 0; r < RP; ++r) {
+                    const int q = (int)threadIdx.x + r * NT, rowpairs = tp.TX * tp.DCH;
+                    if (q >= rowpairs * tp.TY) continue;
+                    const int lj = q / rowpairs, rem = q - lj * rowpairs, c = rem / tp.DCH, d = rem - c * tp.DCH;
+                    const int i = i0 + c, j = j0 + lj, sdir = s0 + d;
+                    if (i >= p.n1 || j >= p.n2 || sdir >= p.pitch) continue;
+                    const long long e = (long long)(j * p.n1 + i) * p.pitch + sdir;
+                    if (p.cls[e] & 1)
+                        for (int k = 0; k < n3; ++k) I_out[e + k * (long long)p.ncol * p.pitch] = 0.0;
+                }
+            return;
+        }
     }
 
     // ---- producer role (one lane at a time): plane m of the ring sequence = x3-plane m - 2 of I_in; base plane k ----
@@ -180,18 +192,15 @@ k_transport_tile(const __grid_constant__ KParams p, const __grid_constant__ Tile
     // per-pair constants
     uint32_t a_own[RP], a_xa[RP], a_xb[RP], a_xd[RP], a_ya[RP], a_yb[RP], a_yd[RP], a_base[RP];
     PairK K[RP];
-    int pos0[RP], colr[RP];
-    bool wr[RP], live[RP], zpos[RP], xposr[RP], yposr[RP];
-    // matter extras in shared memory: [6][RP * NT] doubles: Zq of xl, xh, yl, yh, zf, then the two far-side operand addresses
-    double *extra = reinterpret_cast<double *>(smem + tp.off_extra);
-    int fxi[RP], fyi[RP];
+    int pos0[RP];
+    bool wr[RP], live[RP], zpos[RP];
 #pragma unroll
     for (int r = 0; r < RP; ++r) {
         const int q = t + r * NT;
-        wr[r] = live[r] = false; zpos[r] = xposr[r] = yposr[r] = true;
+        wr[r] = live[r] = false; zpos[r] = true;
         a_own[r] = a_xa[r] = a_xb[r] = a_xd[r] = a_ya[r] = a_yb[r] = a_yd[r] = ring; a_base[r] = ringB;
         K[r] = PairK{0.0, 0.0, 0.0, 0.0, 0.0, 0.5};
-        pos0[r] = 0; colr[r] = 0; fxi[r] = fyi[r] = 0;
+        pos0[r] = 0;
         if (q < npairs) {
             const int lj = q / rowpairs, rem = q - lj * rowpairs, c = rem / tp.DCH, d = rem - c * tp.DCH;
             const int i = i0 + c, j = j0 + lj, s = s0 + d;
@@ -200,12 +209,12 @@ k_transport_tile(const __grid_constant__ KParams p, const __grid_constant__ Tile
                 const int cl = p.cls[(long long)col * p.pitch + s];
                 wr[r] = !(cl & 2);
                 live[r] = cl == 0;
-                pos0[r] = col * p.pitch + s; colr[r] = col;
+                pos0[r] = col * p.pitch + s;
                 if (live[r]) {
                     ColSetup cs;
                     col_setup(p, dt, cs, i, j, s);
                     const bool xpos = cs.xl.pos, ypos = cs.yl.pos;
-                    xposr[r] = xpos; yposr[r] = ypos; zpos[r] = cs.zf.pos;
+                    zpos[r] = cs.zf.pos;
                     K[r].Kxbc = xpos ? -cs.xl.A : cs.xh.A; K[r].Kxcd = xpos ? cs.xh.A : -cs.xl.A;
                     K[r].Kybc = ypos ? -cs.yl.A : cs.yh.A; K[r].Kycd = ypos ? cs.yh.A : -cs.yl.A;
                     K[r].zA = cs.zf.A; K[r].zhalf = cs.zf.pos ? 0.5 : -0.5;
@@ -239,30 +248,22 @@ k_transport_tile(const __grid_constant__ KParams p, const __grid_constant__ Tile
                     a_xa[r] = ring + xo(xpos ? -2 : 2); a_xb[r] = ring + xo(xpos ? -1 : 1); a_xd[r] = ring + xo(xpos ? 1 : -1);
                     a_ya[r] = ring + yo(ypos ? -2 : 2); a_yb[r] = ring + yo(ypos ? -1 : 1); a_yd[r] = ring + yo(ypos ? 1 : -1);
                     a_base[r] = ringB + (lj * tp.TX + c) * tp.cellB + din;
-                    if (MATTER) {
-                        const int e = r * NT + t, st = RP * NT;
-                        extra[e] = cs.xl.Zq; extra[st + e] = cs.xh.Zq; extra[2 * st + e] = cs.yl.Zq; extra[3 * st + e] = cs.yh.Zq;
-                        extra[4 * st + e] = cs.zf.Zq;
-                        reinterpret_cast<uint2 *>(extra + 5 * st)[e] = make_uint2(ring + xo(xpos ? 2 : -2), ring + yo(ypos ? 2 : -2));
-                        fxi[r] = j * (p.n1 + 1) + i; fyi[r] = j * p.n1 + i;
-                    }
                 }
             }
         }
     }
     const long long kstride = (long long)p.ncol * p.pitch;
-    const int zlo = p.zlo[2], zhi = n3 - p.zhi[2], ncol = p.ncol;
-    const unsigned *pmask = reinterpret_cast<const unsigned *>(colflag + colmask_offset(ncol, n3));
+    const int zlo = p.zlo[2], zhi = n3 - p.zhi[2];
 
     // prologue: planes -2 .. 1 (ring sequence m = 0 .. 3) -> register windows
-    double w0[RP], w1[RP], w2[RP], w3[RP], Flo[RP];
+    double w1[RP], w2[RP], w3[RP], Flo[RP];
 #pragma unroll
     for (int m = 0; m < 4; ++m) {
         mbar_wait(bar_full + 8 * m, 0);
 #pragma unroll
         for (int r = 0; r < RP; ++r) {
             const double v = lds(a_own[r] + m * SLOT_STRIDE);
-            if (m == 0) w0[r] = v; else if (m == 1) w1[r] = v; else if (m == 2) w2[r] = v; else w3[r] = v;
+            if (m == 0) Flo[r] = v; else if (m == 1) w1[r] = v; else if (m == 2) w2[r] = v; else w3[r] = v;   // Flo: plane -2 for now
         }
         if (m < 2) {   // planes -2, -1 are not read again
             __syncwarp();
@@ -271,17 +272,10 @@ k_transport_tile(const __grid_constant__ KParams p, const __grid_constant__ Tile
     }
 #pragma unroll
     for (int r = 0; r < RP; ++r) {
-        const double sg = slope_k<RT_LIM_MC>(w2[r] - w1[r], zpos[r] ? (w1[r] - w0[r]) : (w3[r] - w2[r]));
+        const double sg = slope_k<RT_LIM_MC>(w2[r] - w1[r], zpos[r] ? (w1[r] - Flo[r]) : (w3[r] - w2[r]));
         Flo[r] = K[r].zA * fma(K[r].zhalf, sg, zpos[r] ? w1[r] : w2[r]);
     }
-    unsigned mcur[RP], mnext[RP];
-#pragma unroll
-    for (int r = 0; r < RP; ++r) {
-        mcur[r] = (MATTER && live[r]) ? __ldg(pmask + colr[r]) : 0u;
-        mnext[r] = (MATTER && live[r] && n3 > 32) ? __ldg(pmask + ncol + colr[r]) : 0u;
-    }
     double *outk = I_out;
-    const int sx = p.n2 * (p.n1 + 1), sy = (p.n2 + 1) * p.n1;
 
     for (int k0 = 0; k0 < n3; k0 += NS) {
         const uint32_t par0 = (uint32_t)((k0 / NS) & 1);   // parity of the ring round that holds plane sequence m = k0 .. k0 + NS - 1
@@ -303,45 +297,24 @@ k_transport_tile(const __grid_constant__ KParams p, const __grid_constant__ Tile
                 {
                     const double w4 = lds(a_own[r] + so);
                     const double cbase = SAME_BASE ? w2[r] : lds(a_base[r] + sb);
-                    const bool mat = MATTER && ((mcur[r] >> (k & 31)) & 1u);
                     // x3: upwind state at the upper face (always formed: it is the next cell's lower flux if that cell is vacuum)
                     const double sz = slope_k<RT_LIM_MC>(w3[r] - w2[r], zpos[r] ? (w2[r] - w1[r]) : (w4 - w3[r]));
                     const double Fhi = K[r].zA * fma(K[r].zhalf, sz, zpos[r] ? w2[r] : w3[r]);
                     const double xa = lds(a_xa[r] + sk), xb = lds(a_xb[r] + sk), xd = lds(a_xd[r] + sk);
                     const double ya = lds(a_ya[r] + sk), yb = lds(a_yb[r] + sk), yd = lds(a_yd[r] + sk);
-                    double D;
-                    if (!mat) {
-                        D = Fhi - Flo[r];
-                        {
-                            const double d1 = xb - xa, d2 = w2[r] - xb, d3 = xd - w2[r];
-                            D = fma(K[r].Kxbc, fma(0.5, slope_k<RT_LIM_MC>(d1, d2), xb), D);
-                            D = fma(K[r].Kxcd, fma(0.5, slope_k<RT_LIM_MC>(d2, d3), w2[r]), D);
-                        }
-                        {
-                            const double d1 = yb - ya, d2 = w2[r] - yb, d3 = yd - w2[r];
-                            D = fma(K[r].Kybc, fma(0.5, slope_k<RT_LIM_MC>(d1, d2), yb), D);
-                            D = fma(K[r].Kycd, fma(0.5, slope_k<RT_LIM_MC>(d2, d3), w2[r]), D);
-                        }
-                    } else {
-                        // Eq 23 faces: full five-point stencils, both PLI states (the arithmetic of k_transport_gen)
-                        const int e = r * NT + t, st = RP * NT;
-                        const uint2 far = reinterpret_cast<const uint2 *>(extra + 5 * st)[e];
-                        const bool xpos = xposr[r], ypos = yposr[r];
-                        const double xe = lds(far.x + sk), ye = lds(far.y + sk);
-                        FaceK xl, xh, yl, yh, zf;
-                        xl.A = xpos ? -K[r].Kxbc : -K[r].Kxcd; xh.A = xpos ? K[r].Kxcd : K[r].Kxbc; xl.pos = xh.pos = xpos;
-                        yl.A = ypos ? -K[r].Kybc : -K[r].Kycd; yh.A = ypos ? K[r].Kycd : K[r].Kybc; yl.pos = yh.pos = ypos;
-                        zf.A = K[r].zA; zf.pos = zpos[r];
-                        xl.Zq = extra[e]; xh.Zq = extra[st + e]; yl.Zq = extra[2 * st + e]; yh.Zq = extra[3 * st + e]; zf.Zq = extra[4 * st + e];
-                        const double4 *px = fc0 + ((long long)k * sx + fxi[r]), *py = fc1 + ((long long)k * sy + fyi[r]),
-                                      *pz = fc2 + ((long long)k * ncol + colr[r]);
-                        D = flux_diff<RT_LIM_MC, true>(w0[r], w1[r], w2[r], w3[r], w4, zf, zf, ld4(pz), ld4(pz + ncol));
-                        D += flux_diff<RT_LIM_MC, true>(xpos ? xa : xe, xpos ? xb : xd, w2[r], xpos ? xd : xb, xpos ? xe : xa, xl, xh, ld4(px), ld4(px + 1));
-                        D += flux_diff<RT_LIM_MC, true>(ypos ? ya : ye, ypos ? yb : yd, w2[r], ypos ? yd : yb, ypos ? ye : ya, yl, yh, ld4(py), ld4(py + p.n1));
+                    double D = Fhi - Flo[r];
+                    {
+                        const double d1 = xb - xa, d2 = w2[r] - xb, d3 = xd - w2[r];
+                        D = fma(K[r].Kxbc, fma(0.5, slope_k<RT_LIM_MC>(d1, d2), xb), D);
+                        D = fma(K[r].Kxcd, fma(0.5, slope_k<RT_LIM_MC>(d2, d3), w2[r]), D);
+                    }
+                    {
+                        const double d1 = yb - ya, d2 = w2[r] - yb, d3 = yd - w2[r];
+                        D = fma(K[r].Kybc, fma(0.5, slope_k<RT_LIM_MC>(d1, d2), yb), D);
+                        D = fma(K[r].Kycd, fma(0.5, slope_k<RT_LIM_MC>(d2, d3), w2[r]), D);
                     }
                     res = (band || !live[r]) ? 0.0 : cbase - D;   // Eq 18 (O5), dt / (n^0 n_0 sqrt(-g) dx) folded in
                     Flo[r] = Fhi;
-                    if (MATTER) w0[r] = w1[r];
                     w1[r] = w2[r]; w2[r] = w3[r]; w3[r] = w4;
                 }
                 if (wr[r]) outk[pos0[r]] = res;
@@ -351,13 +324,6 @@ k_transport_tile(const __grid_constant__ KParams p, const __grid_constant__ Tile
             if (lane == 0) {
                 mbar_arrive(bar_empty + 8 * uk);
                 if (!SAME_BASE) mbar_arrive(bar_emptyB + 8 * u);
-            }
-            if (MATTER && (k & 31) == 31) {
-#pragma unroll
-                for (int r = 0; r < RP; ++r) {
-                    mcur[r] = mnext[r];
-                    mnext[r] = (live[r] && k + 33 < n3) ? __ldg(pmask + (long long)((k >> 5) + 2) * ncol + colr[r]) : 0u;
-                }
             }
         }
     }
@@ -393,7 +359,7 @@ bool make_map(CUtensorMap *m, const double *I, const KParams &p, int dch, int w,
 int align_up(int v, int a) { return (v + a - 1) / a * a; }
 
 // shared-memory layout of a tile (see the kernel) for a kernel with rp pairs per thread; returns the dynamic shared memory it needs
-size_t tile_layout(const KParams &p, const int tile[3], int rp, bool same, bool matter, TileParams &t) {
+size_t tile_layout(const KParams &p, const int tile[3], bool same, TileParams &t) {
     std::memset(&t, 0, sizeof t);
     t.TX = tile[0]; t.TY = tile[1]; t.DCH = tile[2];
     t.nch = (p.pitch + t.DCH - 1) / t.DCH;
@@ -410,31 +376,30 @@ size_t tile_layout(const KParams &p, const int tile[3], int rp, bool same, bool 
     t.bslotB = t.TY * t.TX * t.cellB;
     t.off_ring = 1024;
     t.off_base = t.off_ring + NS * SLOT_STRIDE;
-    t.off_extra = t.off_base + (same ? 0 : NS * BSLOT_STRIDE);
-    return (size_t)t.off_extra + (matter ? 6 * rp * NT * sizeof(double) : 0);
+    return (size_t)t.off_base + (same ? 0 : NS * BSLOT_STRIDE);
 }
 constexpr size_t SMEM_MAX = 227 * 1024;
 
 }  // namespace
 
-// Tile shapes for a mesh: TX x TY columns x DCH directions with TX TY DCH <= rp NT pairs, for the vacuum-tile kernel
-// (out[0..2]) and the matter-tile kernel (out[3..5]).  DCH is even (TMA: the inner box extent is a multiple of 16 bytes)
-// and chosen so that ceil(pitch / DCH) chunks waste few lanes; (TX, TY) minimise the halo'd cells loaded per cell computed,
-// (TY (TX + 4) + 4 TX) / (TX TY), with the ragged tiles of this mesh counted.
-static void choose_one(const KParams &p, int rp, bool matter, int out[3]) {
+// Tile shape for a mesh: TX x TY columns x DCH directions with TX TY DCH <= RP NT pairs.  DCH is even (TMA: the inner box
+// extent is a multiple of 16 bytes) and chosen so that ceil(pitch / DCH) chunks waste few lanes; (TX, TY) minimise the halo'd
+// cells loaded per cell computed, (TY (TX + 4) + 4 TX) / (TX TY), with the ragged tiles of this mesh counted.
+void choose_tile(const KParams &p, const int req[3], int out[3]) {
+    if (req && req[0] > 0 && req[1] > 0 && req[2] > 0) { out[0] = req[0]; out[1] = req[1]; out[2] = req[2]; return; }
     double best = 1e300;
     out[0] = 2; out[1] = 1; out[2] = 8;
     for (int dch = 8; dch <= 64; dch += 2) {
         const int nch = (p.pitch + dch - 1) / dch;
         const double wd = (double)nch * dch / p.nd;   // lanes per real direction
-        const int cells = rp * NT / dch;
+        const int cells = RP * NT / dch;
         for (int ty = 1; ty <= 8; ++ty)
             for (int tx = 2; tx <= 16; ++tx) {
                 if (tx * ty > cells) continue;
                 const int tl[3] = {tx, ty, dch};
                 TileParams t;
-                if (tile_layout(p, tl, rp, false, matter, t) > SMEM_MAX || t.slotB > SLOT_STRIDE) continue;
-                const double use = (double)(tx * ty * dch) / (rp * NT);    // consumer slots in use
+                if (tile_layout(p, tl, false, t) > SMEM_MAX || t.slotB > SLOT_STRIDE) continue;
+                const double use = (double)(tx * ty * dch) / (RP * NT);    // consumer slots in use
                 const double rag = ((double)((p.n1 + tx - 1) / tx) * tx / p.n1) * ((double)((p.n2 + ty - 1) / ty) * ty / p.n2);
                 const double X = (double)(ty * (tx + 4) + 4 * tx) / (tx * ty);
                 const double cost = wd * rag / use * (1.0 + 0.12 * (X - 1.0));
@@ -442,66 +407,38 @@ static void choose_one(const KParams &p, int rp, bool matter, int out[3]) {
             }
     }
 }
-void choose_tile(const KParams &p, const int req[6], int out[6]) {
-    choose_one(p, RPV, false, out);
-    if (req && req[0] > 0 && req[1] > 0 && req[2] > 0)
-        for (int q = 0; q < 3; ++q) out[q] = req[q];
-    // the matter-tile kernel walks the same (TX, TY) tiling (the two launches split the tiles between them) with fewer
-    // directions per chunk: the largest even count its RPM pairs per thread and its shared memory allow
-    out[3] = out[0]; out[4] = out[1];
-    int dm = (req && req[5] > 0) ? req[5] : (RPM * NT / (out[0] * out[1])) & ~1;
-    for (; dm > 2; dm -= 2) {
-        const int tl[3] = {out[0], out[1], dm};
-        TileParams t;
-        if (tile_layout(p, tl, RPM, false, true, t) <= SMEM_MAX && t.slotB <= SLOT_STRIDE) break;
-    }
-    out[5] = dm;
-}
 
 bool tile_eligible(const KParams &p) {
     return p.limiter == RT_LIM_MC && (p.bc_lo[2] == RT_BC_PERIODIC || p.bc_lo[2] == RT_BC_OUTFLOW) &&
            (p.bc_hi[2] == RT_BC_PERIODIC || p.bc_hi[2] == RT_BC_OUTFLOW) && (long long)p.ncol * p.pitch < (1LL << 31) && encode_fn() != nullptr;
 }
 
-// The non-"general" pairs of the spatial transport (vacuum and Eq 23 cells) through the tile kernels: without opacities one
-// launch; with opacities two launches that split the tiles by kind (all-vacuum columns / some Eq 23 face).
-template <bool MATTER, int RP>
-static cudaError_t launch_one(const KParams &p, const int tile[3], bool split, const double *I_in, const double *I_base, double *I_out,
-                              double *const fcoef[3], const unsigned char *colflag, double dt, cudaStream_t st) {
+// The vacuum update (Eq 20 on all six faces) of the non-"general" pairs through the tile kernel.  With opacities, tiles
+// without an all-vacuum cell are skipped, and the cells that have an Eq 23 face are recomputed afterwards by
+// k_transport_gen (rt_transport.cu), which overwrites them.
+cudaError_t launch_transport_tile(const KParams &p, const int tile[3], const double *I_in, const double *I_base, double *I_out,
+                                  const unsigned char *colflag, bool matter, double dt, cudaStream_t st, long long *launches) {
     TileParams t;
     const bool same = (I_base == I_in);
-    const size_t smem = tile_layout(p, tile, RP, same, MATTER, t);
-    t.split = split ? 1 : 0;
+    const size_t smem = tile_layout(p, tile, same, t);
+    t.split = matter ? 1 : 0;
     if (smem > SMEM_MAX || t.slotB > SLOT_STRIDE || t.TX * t.TY * t.DCH > RP * NT || (t.DCH & 1) || t.TX < 2 || t.TX + 4 > 256 || t.DCH > 256)
         return cudaErrorInvalidConfiguration;
     CUtensorMap mA, mH, mG, mD;
     if (!make_map(&mA, I_in, p, t.DCH, t.TX + 4, t.TY) || !make_map(&mH, I_in, p, t.DCH, t.TX, 2) || !make_map(&mG, I_in, p, t.DCH, 2, t.TY) ||
         !make_map(&mD, I_base, p, t.DCH, t.TX, t.TY))
         return cudaErrorInvalidValue;
-    const double4 *f0 = reinterpret_cast<const double4 *>(fcoef[0]), *f1 = reinterpret_cast<const double4 *>(fcoef[1]),
-                  *f2 = reinterpret_cast<const double4 *>(fcoef[2]);
     const unsigned grid = (unsigned)(t.ntx * t.nty * t.nch);
     cudaError_t e;
     if (same) {
-        e = cudaFuncSetAttribute(k_transport_tile<MATTER, true, RP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) k_transport_tile<MATTER, true, RP><<<grid, NT + 32, smem, st>>>(p, t, mA, mH, mG, mD, I_out, f0, f1, f2, colflag, dt);
+        e = cudaFuncSetAttribute(k_transport_tile<true, RP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) k_transport_tile<true, RP><<<grid, NT + 32, smem, st>>>(p, t, mA, mH, mG, mD, I_out, colflag, dt);
     } else {
-        e = cudaFuncSetAttribute(k_transport_tile<MATTER, false, RP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) k_transport_tile<MATTER, false, RP><<<grid, NT + 32, smem, st>>>(p, t, mA, mH, mG, mD, I_out, f0, f1, f2, colflag, dt);
+        e = cudaFuncSetAttribute(k_transport_tile<false, RP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) k_transport_tile<false, RP><<<grid, NT + 32, smem, st>>>(p, t, mA, mH, mG, mD, I_out, colflag, dt);
     }
-    return e != cudaSuccess ? e : cudaGetLastError();
-}
-
-cudaError_t launch_transport_tile(const KParams &p, const int tile[6], const double *I_in, const double *I_base, double *I_out,
-                                  double *const fcoef[3], const unsigned char *colflag, bool matter, double dt, cudaStream_t st,
-                                  long long *launches) {
-    cudaError_t e = launch_one<false, RPV>(p, tile, matter, I_in, I_base, I_out, fcoef, colflag, dt, st);
     ++*launches;
-    if (e == cudaSuccess && matter) {
-        e = launch_one<true, RPM>(p, tile + 3, true, I_in, I_base, I_out, fcoef, colflag, dt, st);
-        ++*launches;
-    }
-    return e;
+    return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 }  // namespace rt

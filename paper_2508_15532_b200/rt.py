@@ -35,7 +35,7 @@ class RtOptions(ctypes.Structure):
     _fields_ = [("limiter", ctypes.c_int), ("angular_recon", ctypes.c_int), ("source_method", ctypes.c_int),
                 ("n0_floor", ctypes.c_double), ("rho_floor", ctypes.c_double), ("kappa_a0", ctypes.c_double),
                 ("kappa_s", ctypes.c_double), ("a_rad", ctypes.c_double), ("Y_over_rho", ctypes.c_double),
-                ("abar", ctypes.c_double), ("transport_variant", ctypes.c_int), ("transport_tile", ctypes.c_int * 6)]
+                ("abar", ctypes.c_double), ("transport_variant", ctypes.c_int), ("transport_tile", ctypes.c_int * 3)]
 
 
 def load_library(path=LIB_PATH):
@@ -103,7 +103,7 @@ def _stream():
 
 DEFAULT_OPTIONS = dict(limiter=0, angular_recon=0, source_method=2, n0_floor=0.1, rho_floor=5e-4, kappa_a0=0.0,
                        kappa_s=0.0, a_rad=1.0, Y_over_rho=1.5, abar=1.0, transport_variant=0,
-                       transport_tile=(0, 0, 0, 0, 0, 0))
+                       transport_tile=(0, 0, 0))
 
 
 class RtContext:
@@ -222,8 +222,8 @@ class RtContext:
         return {n: (float(ms[i]), int(cnt[i])) for i, n in enumerate(names)}
 
     def transport_info(self):
-        """(variant actually used, (TX, TY, DCH) of the vacuum-tile kernel + (TX, TY, DCH) of the matter-tile kernel)."""
-        out = np.zeros(7, np.int32)
+        """(variant actually used, (TX, TY, DCH) of the tile kernel)."""
+        out = np.zeros(4, np.int32)
         _check(lib().rt_transport_info(self._h, out.ctypes.data))
         return int(out[0]), tuple(int(v) for v in out[1:])
 
