@@ -31,6 +31,7 @@ struct KParams {
     const double *w;
     const int *nb;
     const unsigned char *cls;   // [ncol][pitch] class byte (k_classify)
+    const double *paircoef;     // [ncol][pitch][8] geometry of a (column, s) pair for the tile kernel (k_paircoef), RT_TRANSPORT_TMA only
     // MAPR tables (only when angular_recon == RT_ANG_MAPR): grid-only tables are [slot][..][pitch]
     const double *mapr_xi;    // [6][3][pitch]  log map of neighbour e in the tangent plane at n_s
     const double *mapr_xim;   // [6][3][pitch]  log map of the centre of edge e
@@ -68,6 +69,7 @@ cudaError_t launch_transport(const KParams &p, const double *I_in, const double 
 // rt_transport_tile.cu: the non-"general" pairs through the TMA tile kernel
 void choose_tile(const KParams &p, const int req[3], int out[3]);
 bool tile_eligible(const KParams &p);
+cudaError_t launch_paircoef(const KParams &p, double *out, cudaStream_t st);
 cudaError_t launch_transport_tile(const KParams &p, const int tile[3], const double *I_in, const double *I_base, double *I_out,
                                   const unsigned char *colflag, bool matter, double dt, cudaStream_t st, long long *launches);
 cudaError_t launch_angular_mapr(const KParams &p, const double *I_in, double *I_io, double dt, cudaStream_t st, long long *launches);

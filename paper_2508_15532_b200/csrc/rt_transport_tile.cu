@@ -28,14 +28,24 @@
 namespace rt {
 namespace {
 
-constexpr int NT = 480;              // consumer threads (15 warps); warp 15 is the producer: 16 warps = 128 registers each
-constexpr int RP = 2;                // pairs per consumer thread
-#ifndef NS_X
-#define NS_X 5
+#ifndef NT_X
+#define NT_X 480
 #endif
-constexpr int NS = NS_X;             // ring slots: planes k, k+1, k+2 in use, two in flight
-constexpr int SLOT_STRIDE = 24576;   // bytes between ring slots (compile-time: every operand load is LDS [R + imm])
-constexpr int BSLOT_STRIDE = RP * NT * 8;   // base ring: own cells only
+constexpr int NT = NT_X;              // consumer threads (15 warps); warp 15 is the producer: 16 warps = 128 registers each
+#ifndef RP_X
+#define RP_X 2
+#endif
+constexpr int RP = RP_X;                // pairs per consumer thread
+#ifndef NS_X
+#define NS_X 8
+#endif
+constexpr int NS = NS_X;             // ring slots: planes k, k+1, k+2 in use, five in flight (a load takes about two steps)
+#ifndef SLOT_X
+#define SLOT_X 20480
+#endif
+constexpr int SLOT_STRIDE = SLOT_X;   // bytes between ring slots (compile-time: every operand load is LDS [R + imm])
+constexpr int BSLOT_STRIDE = RP * NT * 8 + 128;   // base ring: own cells only (+ the zero word, see ZERO_OFF)
+constexpr int ZERO_OFF = SLOT_STRIDE - 8;   // a double behind each slot's data that holds 0.0: the operand of every pair that is not live
 
 // ---- mbarrier / TMA primitives (PTX) ------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void *q) { return (uint32_t)__cvta_generic_to_shared(q); }
@@ -58,6 +68,17 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         "bra WAIT_%=;\n"
         "DONE_%=:\n"
         "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+// one non-blocking probe; the blocking wait is only entered if it fails (hides the probe's latency behind the step before)
+__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
 }
 __device__ __forceinline__ void tma_box(uint32_t dst, const CUtensorMap *map, uint32_t bar, int c0, int c1, int c2, int c3) {
     asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
@@ -89,6 +110,50 @@ struct TileParams {
     int off_ring, off_base;
     int split;   // opacities present: tiles without an all-vacuum cell are skipped (see the kernel)
 };
+
+// ---- per-(column, s) table of everything geometric the tile kernel needs, built once by rt_init ----------------------------
+// [ncol * pitch][8] doubles: Q P of the faces xl, xh, yl, yh, z (n_0 gate applied), 1 / sqrt(-g_c), n^0 n_0 at the centre,
+// and a flag word (bit 0 dead, bit 1 general: the class byte of k_classify; bits 2-4: sqrt(-g) n^a_f > 0 for a = 1, 2, 3).
+// The tile kernel folds dt / (n^0 n_0 sqrt(-g_c) dx^a) in exactly as col_setup() does, so its coefficients carry the same
+// bits as those of the per-thread-load kernels; what it saves is col_setup's ~900 instructions and dependent loads per pair.
+__global__ void k_paircoef(const __grid_constant__ KParams p, double *__restrict__ out) {
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= p.n1 * p.pitch) return;
+    const int i = e / p.pitch, s = e - i * p.pitch, j = blockIdx.y, col = j * p.n1 + i;
+    double4 *o = reinterpret_cast<double4 *>(out + ((long long)col * p.pitch + s) * 8);
+    const int cl = p.cls[(long long)col * p.pitch + s];
+    double qp[5] = {0, 0, 0, 0, 0}, c8 = 1.0, den = 1.0;
+    unsigned flags = (unsigned)cl;
+    if (!(cl & 1)) {
+        const double nx = __ldg(p.nhat + s), ny = __ldg(p.nhat + p.pitch + s), nz = __ldg(p.nhat + 2 * p.pitch + s);
+        const double *cen = p.cen + (long long)col * CEN_STRIDE;
+        const double n0c = centre_n0(cen, nx, ny, nz);
+        const double nup = cen[4] + cen[5] * nx + cen[6] * ny + cen[7] * nz;
+        c8 = cen[8]; den = nup * n0c;
+        FaceC f;
+        int in;
+        f = face_coef(p.face[0] + ((long long)j * (p.n1 + 1) + i) * FACE_STRIDE, nx, ny, nz);
+        in = (i > 0) ? i - 1 : (p.bc_lo[0] == RT_BC_PERIODIC ? p.n1 - 1 : -1);
+        if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)j * p.n1 + in) * CEN_STRIDE, nx, ny, nz))) f.Q = 0.0;
+        qp[0] = f.Q * f.P; if (f.P > 0) flags |= 4u;
+        f = face_coef(p.face[0] + ((long long)j * (p.n1 + 1) + i + 1) * FACE_STRIDE, nx, ny, nz);
+        in = (i < p.n1 - 1) ? i + 1 : (p.bc_hi[0] == RT_BC_PERIODIC ? 0 : -1);
+        if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)j * p.n1 + in) * CEN_STRIDE, nx, ny, nz))) f.Q = 0.0;
+        qp[1] = f.Q * f.P;
+        f = face_coef(p.face[1] + ((long long)j * p.n1 + i) * FACE_STRIDE, nx, ny, nz);
+        in = (j > 0) ? j - 1 : (p.bc_lo[1] == RT_BC_PERIODIC ? p.n2 - 1 : -1);
+        if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)in * p.n1 + i) * CEN_STRIDE, nx, ny, nz))) f.Q = 0.0;
+        qp[2] = f.Q * f.P; if (f.P > 0) flags |= 8u;
+        f = face_coef(p.face[1] + ((long long)(j + 1) * p.n1 + i) * FACE_STRIDE, nx, ny, nz);
+        in = (j < p.n2 - 1) ? j + 1 : (p.bc_hi[1] == RT_BC_PERIODIC ? 0 : -1);
+        if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)in * p.n1 + i) * CEN_STRIDE, nx, ny, nz))) f.Q = 0.0;
+        qp[3] = f.Q * f.P;
+        f = face_coef(p.face[2] + (long long)col * FACE_STRIDE, nx, ny, nz);
+        qp[4] = f.Q * f.P; if (f.P > 0) flags |= 16u;
+    }
+    o[0] = make_double4(qp[0], qp[1], qp[2], qp[3]);
+    o[1] = make_double4(qp[4], c8, den, __longlong_as_double((long long)flags));
+}
 
 // One x3 step of the pairs of a thread.  U = k mod NS is a compile-time constant of the unrolled march, so all ring
 // offsets are immediates.
@@ -174,6 +239,10 @@ k_transport_tile(const __grid_constant__ KParams p, const __grid_constant__ Tile
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    if ((int)threadIdx.x < NS) {
+        *reinterpret_cast<double *>(smem + tp.off_ring + threadIdx.x * SLOT_STRIDE + ZERO_OFF) = 0.0;
+        if (!SAME_BASE) *reinterpret_cast<double *>(smem + tp.off_base + threadIdx.x * BSLOT_STRIDE + RP * NT * 8) = 0.0;
+    }
     __syncthreads();
 
     if (warp == NT / 32) {
@@ -198,7 +267,7 @@ k_transport_tile(const __grid_constant__ KParams p, const __grid_constant__ Tile
     for (int r = 0; r < RP; ++r) {
         const int q = t + r * NT;
         wr[r] = live[r] = false; zpos[r] = true;
-        a_own[r] = a_xa[r] = a_xb[r] = a_xd[r] = a_ya[r] = a_yb[r] = a_yd[r] = ring; a_base[r] = ringB;
+        a_own[r] = a_xa[r] = a_xb[r] = a_xd[r] = a_ya[r] = a_yb[r] = a_yd[r] = ring + ZERO_OFF; a_base[r] = ringB + RP * NT * 8;   // zero words
         K[r] = PairK{0.0, 0.0, 0.0, 0.0, 0.0, 0.5};
         pos0[r] = 0;
         if (q < npairs) {
@@ -206,18 +275,22 @@ k_transport_tile(const __grid_constant__ KParams p, const __grid_constant__ Tile
             const int i = i0 + c, j = j0 + lj, s = s0 + d;
             if (i < p.n1 && j < p.n2 && s < p.pitch) {
                 const int col = j * p.n1 + i;
-                const int cl = p.cls[(long long)col * p.pitch + s];
-                wr[r] = !(cl & 2);
-                live[r] = cl == 0;
+                const double4 *tq = reinterpret_cast<const double4 *>(p.paircoef + ((long long)col * p.pitch + s) * 8);
+                const double4 t0 = ld4(tq), t1 = ld4(tq + 1);
+                const unsigned fl = (unsigned)__double_as_longlong(t1.w);
+                wr[r] = !(fl & 2u);
+                live[r] = (fl & 3u) == 0u;
                 pos0[r] = col * p.pitch + s;
                 if (live[r]) {
-                    ColSetup cs;
-                    col_setup(p, dt, cs, i, j, s);
-                    const bool xpos = cs.xl.pos, ypos = cs.yl.pos;
-                    zpos[r] = cs.zf.pos;
-                    K[r].Kxbc = xpos ? -cs.xl.A : cs.xh.A; K[r].Kxcd = xpos ? cs.xh.A : -cs.xl.A;
-                    K[r].Kybc = ypos ? -cs.yl.A : cs.yh.A; K[r].Kycd = ypos ? cs.yh.A : -cs.yl.A;
-                    K[r].zA = cs.zf.A; K[r].zhalf = cs.zf.pos ? 0.5 : -0.5;
+                    // the folding of col_setup() / fold(): A = (Q P) * (dt / (n^0 n_0 sqrt(-g_c)) / dx^a)
+                    const double scale = dt * t1.y / t1.z;
+                    const double sx = scale * p.inv_dx[0], sy = scale * p.inv_dx[1], sz = scale * p.inv_dx[2];
+                    const double Axl = t0.x * sx, Axh = t0.y * sx, Ayl = t0.z * sy, Ayh = t0.w * sy;
+                    const bool xpos = (fl & 4u) != 0u, ypos = (fl & 8u) != 0u;
+                    zpos[r] = (fl & 16u) != 0u;
+                    K[r].Kxbc = xpos ? -Axl : Axh; K[r].Kxcd = xpos ? Axh : -Axl;
+                    K[r].Kybc = ypos ? -Ayl : Ayh; K[r].Kycd = ypos ? Ayh : -Ayl;
+                    K[r].zA = t1.x * sz; K[r].zhalf = zpos[r] ? 0.5 : -0.5;
                     const int din = d * 8;
                     auto xo = [&](int o) -> uint32_t {
                         int gi = i + o;
@@ -277,56 +350,71 @@ k_transport_tile(const __grid_constant__ KParams p, const __grid_constant__ Tile
     }
     double *outk = I_out;
 
-    for (int k0 = 0; k0 < n3; k0 += NS) {
-        const uint32_t par0 = (uint32_t)((k0 / NS) & 1);   // parity of the ring round that holds plane sequence m = k0 .. k0 + NS - 1
-#pragma unroll
-        for (int u = 0; u < NS; ++u) {
-            const int k = k0 + u;
-            if (k >= n3) break;
-            // ring sequence: operands of plane k sit at m = k + 2, the new x3-window value at m = k + 4
-            const int uo = (u + 4) % NS, uk = (u + 2) % NS;
-            const uint32_t so = (uint32_t)(uo * SLOT_STRIDE), sk = (uint32_t)(uk * SLOT_STRIDE), sb = (uint32_t)(u * BSLOT_STRIDE);
+    // One x3 step; in the unrolled march u, so, sk, sb are compile-time constants (every operand load is LDS [R + imm]).  A pair
+    // that is not live reads the zero words with zero coefficients: its result is +0.0, which is what a dead entry holds.
+    bool ready = false;   // outcome of the probe of this step's barriers, made during the step before
+    auto step = [&](int k, int u, uint32_t par0) {
+        const int uo = (u + 4) % NS, uk = (u + 2) % NS;
+        const uint32_t so = (uint32_t)(uo * SLOT_STRIDE), sk = (uint32_t)(uk * SLOT_STRIDE), sb = (uint32_t)(u * BSLOT_STRIDE);
+        if (!ready) {
             mbar_wait(bar_full + 8 * uo, par0 ^ (uint32_t)((u + 4) / NS & 1));
             if (!SAME_BASE) mbar_wait(bar_fullB + 8 * u, par0);
-            const bool band = (k < zlo || k >= zhi);
-            // straight-line code for both pairs (a pair that is not live computes on zero coefficients and address 0; only its
-            // store is predicated), so that the two dependency chains interleave
-#pragma unroll
-            for (int r = 0; r < RP; ++r) {
-                double res;
-                {
-                    const double w4 = lds(a_own[r] + so);
-                    const double cbase = SAME_BASE ? w2[r] : lds(a_base[r] + sb);
-                    // x3: upwind state at the upper face (always formed: it is the next cell's lower flux if that cell is vacuum)
-                    const double sz = slope_k<RT_LIM_MC>(w3[r] - w2[r], zpos[r] ? (w2[r] - w1[r]) : (w4 - w3[r]));
-                    const double Fhi = K[r].zA * fma(K[r].zhalf, sz, zpos[r] ? w2[r] : w3[r]);
-                    const double xa = lds(a_xa[r] + sk), xb = lds(a_xb[r] + sk), xd = lds(a_xd[r] + sk);
-                    const double ya = lds(a_ya[r] + sk), yb = lds(a_yb[r] + sk), yd = lds(a_yd[r] + sk);
-                    double D = Fhi - Flo[r];
-                    {
-                        const double d1 = xb - xa, d2 = w2[r] - xb, d3 = xd - w2[r];
-                        D = fma(K[r].Kxbc, fma(0.5, slope_k<RT_LIM_MC>(d1, d2), xb), D);
-                        D = fma(K[r].Kxcd, fma(0.5, slope_k<RT_LIM_MC>(d2, d3), w2[r]), D);
-                    }
-                    {
-                        const double d1 = yb - ya, d2 = w2[r] - yb, d3 = yd - w2[r];
-                        D = fma(K[r].Kybc, fma(0.5, slope_k<RT_LIM_MC>(d1, d2), yb), D);
-                        D = fma(K[r].Kycd, fma(0.5, slope_k<RT_LIM_MC>(d2, d3), w2[r]), D);
-                    }
-                    res = (band || !live[r]) ? 0.0 : cbase - D;   // Eq 18 (O5), dt / (n^0 n_0 sqrt(-g) dx) folded in
-                    Flo[r] = Fhi;
-                    w1[r] = w2[r]; w2[r] = w3[r]; w3[r] = w4;
-                }
-                if (wr[r]) outk[pos0[r]] = res;
-            }
-            outk += kstride;
-            __syncwarp();
-            if (lane == 0) {
-                mbar_arrive(bar_empty + 8 * uk);
-                if (!SAME_BASE) mbar_arrive(bar_emptyB + 8 * u);
-            }
         }
+        double w4[RP], cbase[RP], xa[RP], xb[RP], xd[RP], ya[RP], yb[RP], yd[RP];
+#pragma unroll
+        for (int r = 0; r < RP; ++r) {
+            w4[r] = lds(a_own[r] + so);
+            cbase[r] = SAME_BASE ? w2[r] : lds(a_base[r] + sb);
+            xa[r] = lds(a_xa[r] + sk); xb[r] = lds(a_xb[r] + sk); xd[r] = lds(a_xd[r] + sk);
+            ya[r] = lds(a_ya[r] + sk); yb[r] = lds(a_yb[r] + sk); yd[r] = lds(a_yd[r] + sk);
+        }
+        if (k + 1 < n3) {   // probe the next step's barriers now; the answer is there when the arithmetic below is done
+            const int u1 = (u + 1) % NS;
+            const uint32_t par1 = par0 ^ (uint32_t)(u + 1 == NS);
+            ready = mbar_test(bar_full + 8 * ((u1 + 4) % NS), par1 ^ (uint32_t)((u1 + 4) / NS & 1));
+            if (!SAME_BASE) ready = mbar_test(bar_fullB + 8 * u1, par1) && ready;
+        }
+#pragma unroll
+        for (int r = 0; r < RP; ++r) {
+            // x3: upwind state at the upper face (it is the next cell's lower flux)
+            const double sz = slope_k<RT_LIM_MC>(w3[r] - w2[r], zpos[r] ? (w2[r] - w1[r]) : (w4[r] - w3[r]));
+            const double Fhi = K[r].zA * fma(K[r].zhalf, sz, zpos[r] ? w2[r] : w3[r]);
+            double D = Fhi - Flo[r];
+            {
+                const double d1 = xb[r] - xa[r], d2 = w2[r] - xb[r], d3 = xd[r] - w2[r];
+                D = fma(K[r].Kxbc, fma(0.5, slope_k<RT_LIM_MC>(d1, d2), xb[r]), D);
+                D = fma(K[r].Kxcd, fma(0.5, slope_k<RT_LIM_MC>(d2, d3), w2[r]), D);
+            }
+            {
+                const double d1 = yb[r] - ya[r], d2 = w2[r] - yb[r], d3 = yd[r] - w2[r];
+                D = fma(K[r].Kybc, fma(0.5, slope_k<RT_LIM_MC>(d1, d2), yb[r]), D);
+                D = fma(K[r].Kycd, fma(0.5, slope_k<RT_LIM_MC>(d2, d3), w2[r]), D);
+            }
+            if (wr[r]) outk[pos0[r]] = cbase[r] - D;   // Eq 18 (O5), dt / (n^0 n_0 sqrt(-g) dx) folded in; the x3 zero band is reset below
+            Flo[r] = Fhi;
+            w1[r] = w2[r]; w2[r] = w3[r]; w3[r] = w4[r];
+        }
+        outk += kstride;
+        __syncwarp();
+        if (lane == 0) {
+            mbar_arrive(bar_empty + 8 * uk);
+            if (!SAME_BASE) mbar_arrive(bar_emptyB + 8 * u);
+        }
+    };
+    int k0 = 0;
+    for (; k0 + NS <= n3; k0 += NS) {   // full ring rounds, unrolled
+        const uint32_t par0 = (uint32_t)((k0 / NS) & 1);   // parity of the ring round that holds the sequence m = k0 .. k0 + NS - 1
+#pragma unroll
+        for (int u = 0; u < NS; ++u) step(k0 + u, u, par0);
     }
+#pragma unroll 1
+    for (int k = k0; k < n3; ++k) step(k, k - k0, (uint32_t)((k0 / NS) & 1));   // the last, partial round
+    if (zlo > 0 || zhi < n3)   // zero band in x3 (L709): reset after the march instead of a select in every step
+#pragma unroll
+        for (int r = 0; r < RP; ++r)
+            if (wr[r])
+                for (int k = 0; k < n3; ++k)
+                    if (k < zlo || k >= zhi) I_out[pos0[r] + k * kstride] = 0.0;
 }
 
 // ---- host side: tensor maps ------------------------------------------------------------------------------------------
@@ -398,7 +486,7 @@ void choose_tile(const KParams &p, const int req[3], int out[3]) {
                 if (tx * ty > cells) continue;
                 const int tl[3] = {tx, ty, dch};
                 TileParams t;
-                if (tile_layout(p, tl, false, t) > SMEM_MAX || t.slotB > SLOT_STRIDE) continue;
+                if (tile_layout(p, tl, false, t) > SMEM_MAX || t.slotB > ZERO_OFF) continue;
                 const double use = (double)(tx * ty * dch) / (RP * NT);    // consumer slots in use
                 const double rag = ((double)((p.n1 + tx - 1) / tx) * tx / p.n1) * ((double)((p.n2 + ty - 1) / ty) * ty / p.n2);
                 const double X = (double)(ty * (tx + 4) + 4 * tx) / (tx * ty);
@@ -406,6 +494,12 @@ void choose_tile(const KParams &p, const int req[3], int out[3]) {
                 if (cost < best) { best = cost; out[0] = tx; out[1] = ty; out[2] = dch; }
             }
     }
+}
+
+cudaError_t launch_paircoef(const KParams &p, double *out, cudaStream_t st) {
+    dim3 grid((p.n1 * p.pitch + 255) / 256, p.n2);
+    k_paircoef<<<grid, 256, 0, st>>>(p, out);
+    return cudaGetLastError();
 }
 
 bool tile_eligible(const KParams &p) {
@@ -422,7 +516,7 @@ cudaError_t launch_transport_tile(const KParams &p, const int tile[3], const dou
     const bool same = (I_base == I_in);
     const size_t smem = tile_layout(p, tile, same, t);
     t.split = matter ? 1 : 0;
-    if (smem > SMEM_MAX || t.slotB > SLOT_STRIDE || t.TX * t.TY * t.DCH > RP * NT || (t.DCH & 1) || t.TX < 2 || t.TX + 4 > 256 || t.DCH > 256)
+    if (smem > SMEM_MAX || t.slotB > ZERO_OFF || t.TX * t.TY * t.DCH > RP * NT || (t.DCH & 1) || t.TX < 2 || t.TX + 4 > 256 || t.DCH > 256)
         return cudaErrorInvalidConfiguration;
     CUtensorMap mA, mH, mG, mD;
     if (!make_map(&mA, I_in, p, t.DCH, t.TX + 4, t.TY) || !make_map(&mH, I_in, p, t.DCH, t.TX, 2) || !make_map(&mG, I_in, p, t.DCH, 2, t.TY) ||
