@@ -159,7 +159,7 @@ __global__ void k_paircoef(const __grid_constant__ KParams p, double *__restrict
 // offsets are immediates.
 struct PairK { double Kxbc, Kxcd, Kybc, Kycd, zA, zhalf; };
 
-template <bool SAME_BASE, int RP>
+template <bool SAME_BASE, bool MASK, int RP>
 __global__ void __launch_bounds__(NT + 32, 1)
 k_transport_tile(const __grid_constant__ KParams p, const __grid_constant__ TileParams tp,
                  const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapH,
@@ -279,9 +279,15 @@ k_transport_tile(const __grid_constant__ KParams p, const __grid_constant__ Tile
     PairK K[RP];
     int pos0[RP];
     bool wr[RP], live[RP], zpos[RP];
+    // MASK (opacities present): bit (k & 31) of the column's mask word = the cell has an Eq 23 face and belongs to
+    // k_transport_gen, which reads its base state from I_base: this kernel must not touch it (I_out may alias I_base)
+    const unsigned *cmask = reinterpret_cast<const unsigned *>(colflag + colmask_offset(p.ncol, n3));
+    int mcol[RP];
+    unsigned mcur[RP], mnext[RP];
 #pragma unroll
     for (int r = 0; r < RP; ++r) {
         wr[r] = live[r] = false; zpos[r] = true;
+        mcol[r] = -1; mcur[r] = mnext[r] = 0u;
         a_own[r] = a_xa[r] = a_xb[r] = a_xd[r] = a_ya[r] = a_yb[r] = a_yd[r] = ring + ZERO_OFF; a_base[r] = ringB + RP * NT * 8;   // zero words
         K[r] = PairK{0.0, 0.0, 0.0, 0.0, 0.0, 0.5};
         pos0[r] = 0;
@@ -294,6 +300,11 @@ k_transport_tile(const __grid_constant__ KParams p, const __grid_constant__ Tile
                 wr[r] = !(fl & 2u);
                 live[r] = (fl & 3u) == 0u;
                 pos0[r] = col * p.pitch + s;
+                if (MASK && wr[r]) {
+                    mcol[r] = col;
+                    mcur[r] = __ldg(cmask + col);
+                    mnext[r] = n3 > 32 ? __ldg(cmask + p.ncol + col) : 0u;
+                }
                 if (live[r]) {
                     // the folding of col_setup() / fold(): A = (Q P) * (dt / (n^0 n_0 sqrt(-g_c)) / dx^a)
                     const double scale = dt * t1.y / t1.z;
@@ -403,7 +414,8 @@ k_transport_tile(const __grid_constant__ KParams p, const __grid_constant__ Tile
                 D = fma(K[r].Kybc, fma(0.5, slope_k<RT_LIM_MC>(d1, d2), yb[r]), D);
                 D = fma(K[r].Kycd, fma(0.5, slope_k<RT_LIM_MC>(d2, d3), w2[r]), D);
             }
-            if (wr[r]) outk[pos0[r]] = cbase[r] - D;   // Eq 18 (O5), dt / (n^0 n_0 sqrt(-g) dx) folded in; the x3 zero band is reset below
+            // Eq 18 (O5), dt / (n^0 n_0 sqrt(-g) dx) folded in; the x3 zero band is reset below
+            if (wr[r] && !(MASK && live[r] && ((mcur[r] >> (k & 31)) & 1u))) outk[pos0[r]] = cbase[r] - D;   // (dead entries are always this kernel's)
             Flo[r] = Fhi;
             w1[r] = w2[r]; w2[r] = w3[r]; w3[r] = w4[r];
         }
@@ -412,6 +424,13 @@ k_transport_tile(const __grid_constant__ KParams p, const __grid_constant__ Tile
         if (lane == 0) {
             mbar_arrive(bar_empty + 8 * uk);
             if (!SAME_BASE) mbar_arrive(bar_emptyB + 8 * u);
+        }
+        if (MASK && (k & 31) == 31) {   // next mask word (requested 32 steps ago)
+#pragma unroll
+            for (int r = 0; r < RP; ++r) {
+                mcur[r] = mnext[r];
+                mnext[r] = (mcol[r] >= 0 && k + 33 < n3) ? __ldg(cmask + (long long)((k >> 5) + 2) * p.ncol + mcol[r]) : 0u;
+            }
         }
     };
     int k0 = 0;
@@ -427,7 +446,7 @@ k_transport_tile(const __grid_constant__ KParams p, const __grid_constant__ Tile
         for (int r = 0; r < RP; ++r)
             if (wr[r])
                 for (int k = 0; k < n3; ++k)
-                    if (k < zlo || k >= zhi) I_out[pos0[r] + k * kstride] = 0.0;
+                    if ((k < zlo || k >= zhi) && !(MASK && live[r] && ((__ldg(cmask + (long long)(k >> 5) * p.ncol + mcol[r]) >> (k & 31)) & 1u))) I_out[pos0[r] + k * kstride] = 0.0;
 }
 
 // ---- host side: tensor maps ------------------------------------------------------------------------------------------
@@ -538,14 +557,15 @@ cudaError_t launch_transport_tile(const KParams &p, const int tile[3], const dou
         !make_map(&mD, I_base, p, t.DCH, t.TX, t.TY))
         return cudaErrorInvalidValue;
     const unsigned grid = (unsigned)(t.ntx * t.nty * t.nch);
-    cudaError_t e;
-    if (same) {
-        e = cudaFuncSetAttribute(k_transport_tile<true, RP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) k_transport_tile<true, RP><<<grid, NT + 32, smem, st>>>(p, t, mA, mH, mG, mD, I_out, colflag, dt);
-    } else {
-        e = cudaFuncSetAttribute(k_transport_tile<false, RP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) k_transport_tile<false, RP><<<grid, NT + 32, smem, st>>>(p, t, mA, mH, mG, mD, I_out, colflag, dt);
-    }
+    cudaError_t e = cudaSuccess;
+#define RT_TILE_LAUNCH(S, M)                                                                                            \
+    do {                                                                                                                \
+        e = cudaFuncSetAttribute(k_transport_tile<S, M, RP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);  \
+        if (e == cudaSuccess) k_transport_tile<S, M, RP><<<grid, NT + 32, smem, st>>>(p, t, mA, mH, mG, mD, I_out, colflag, dt); \
+    } while (0)
+    if (same) { if (matter) RT_TILE_LAUNCH(true, true); else RT_TILE_LAUNCH(true, false); }
+    else { if (matter) RT_TILE_LAUNCH(false, true); else RT_TILE_LAUNCH(false, false); }
+#undef RT_TILE_LAUNCH
     ++*launches;
     return e != cudaSuccess ? e : cudaGetLastError();
 }
