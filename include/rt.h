@@ -96,8 +96,8 @@ typedef struct {
 } rt_options;
 
 /* Build the angular grid with N_d = 10 angle_level^2 + 2 directions (L207-213; angle_level = 2^generation is the
- * paper's rule, other levels by the extension S1), tetrads and Ricci rotation coefficients (Eq 8, 4th-order finite
- * differences, h = 1e-3), and every per-column table; upload them.  Host-side, not timed.  *out is owned by the
+ * paper's rule, other levels by the extension S1), tetrads and Ricci rotation coefficients (Eq 8, 6th-order finite
+ * differences, h = 5e-4), and every per-column table; upload them.  Host-side, not timed.  *out is owned by the
  * library until rt_free. */
 int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_level, const rt_options *opt, rt_ctx **out);
 int rt_free(rt_ctx *ctx);

@@ -21,11 +21,11 @@ Metric kinds
                e^{a-hat}_mu = [[1,0,0,0],[0,1,delta,0],[0,0,1,0],[0,0,0,1]] (rows dt, dx = dw + delta dy, dy, dz) with
                its second row's two entries transposed in print -- as printed neither the matrix nor its transpose is
                orthonormal in A1 (Eq 1 fails), the co-frame reading is.  It is the Cartesian frame, so omega = 0.
-Finite differences (S15): 4th-order central, h = 1e-3 in logical coordinates.
+Finite differences (S15): 6th-order central, h = 5e-4 in logical coordinates.
 """
 import numpy as np
 
-FD_H = 1e-3
+FD_H = 5e-4
 ETA = np.diag([-1.0, 1.0, 1.0, 1.0])
 
 
@@ -153,12 +153,13 @@ def sqrt_neg_g(kind, params, X):
 
 
 def _fd(fun, X):
-    """d fun / d x^i (i = 1..3), 4th-order central differences; returns [..., 3, (fun shape)]."""
+    """d fun / d x^i (i = 1..3), 6th-order central differences with step FD_H (reading S15 of DESIGN.md: the paper says only
+    "finite difference", L109); returns [..., 3, (fun shape)].  Truncation h^6 f^(7) / 140, round-off ~ 1.5 eps |f| / h."""
     out = []
     for i in range(3):
         d = np.zeros(3)
         d[i] = FD_H
-        f = (-fun(X + 2 * d) + 8.0 * fun(X + d) - 8.0 * fun(X - d) + fun(X - 2 * d)) / (12.0 * FD_H)
+        f = (45.0 * (fun(X + d) - fun(X - d)) - 9.0 * (fun(X + 2 * d) - fun(X - 2 * d)) + (fun(X + 3 * d) - fun(X - 3 * d))) / (60.0 * FD_H)
         out.append(f)
     return np.stack(out, axis=len(X.shape) - 1)
 

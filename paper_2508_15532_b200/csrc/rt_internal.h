@@ -31,7 +31,7 @@ struct PointGeom {
     bool dead;          // zero-area location (polar axis): tetrad undefined, no flux crosses
 };
 void eval_point(const rt_metric &m, const double x[3], PointGeom &out);
-// omega^a_{cd} (Eq 8) by 4th-order central differences, h = 1e-3 (S15)
+// omega^a_{cd} (Eq 8) by 6th-order central differences, h = 5e-4 (S15)
 void eval_omega(const rt_metric &m, const double x[3], double omega[4][4][4]);
 
 // ---- device context -----------------------------------------------------------------------------------------

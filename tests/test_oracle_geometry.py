@@ -48,7 +48,7 @@ def test_omega_antisymmetry_and_flat_values():
     X = _ks_points(a)
     om = G.ricci_rotation("ks_mks", dict(a=a, hslope=0.3), X)
     oml = np.einsum("ab,...bcd->...acd", G.ETA, om)
-    assert np.abs(oml + np.swapaxes(oml, -3, -1)).max() < 1e-7        # omega_{acd} = -omega_{dca} (to FD truncation h^4)
+    assert np.abs(oml + np.swapaxes(oml, -3, -1)).max() < 1e-10       # omega_{acd} = -omega_{dca} (6th-order FD, h = 5e-4: S15)
     assert np.abs(G.ricci_rotation("minkowski", {}, X)).max() == 0.0
     # cylindrical tetrad in flat space: only omega^R_{phi phi} = -1/R and omega^phi_{phi R} = +1/R
     X = np.array([[1.3, 0.7, 0.4]])
@@ -56,7 +56,7 @@ def test_omega_antisymmetry_and_flat_values():
     R = np.hypot(1.3, 0.7)
     ref = np.zeros((4, 4, 4))
     ref[1, 2, 2], ref[2, 2, 1] = -1 / R, 1 / R
-    assert np.abs(om - ref).max() < 1e-9
+    assert np.abs(om - ref).max() < 1e-10
 
 
 def test_angular_acceleration_is_rate_of_change_of_tetrad_components():
