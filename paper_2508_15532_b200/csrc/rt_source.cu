@@ -77,15 +77,24 @@ __device__ __forceinline__ void teq_eval(const TEq &q, double T, double &f, doub
         df = -(4.5 * q.k45 * T35 + 4.0 * q.k4 * T3 + 3.5 * q.k35 * T3 * ir + q.k1);
     }
 }
-// Newton-Raphson (L399) from T_-, kept inside the bracket (0, W/Y] on which the residual changes sign (S20).  The
-// Newton step uses a reciprocal instead of a division: the iterates differ from the oracle's in the last bits, the
-// root they converge to (|dT| <= 1e-14 T) does not.
+// Root of the temperature equation on (0, W/Y] (S20).  Existence is decided as the reading says (the residual is negative at
+// 0+ and non-negative at W/Y; otherwise the cell keeps T_- and is counted).  Method 2 (Eq 43) is a quadratic in x = sqrt(T),
+// a4 x + b1 x^2 + c0 = 0 with b1 > 0 > c0, and is solved in closed form, written so that nothing cancels:
+//     x = 2 |c0| / (a4 + sqrt(a4^2 + 4 b1 |c0|)).
+// Methods 1 and 3 (Eq 42: quartic, Eq 46: degree 9 in x) use Newton-Raphson (L399) from T_-, kept inside the bracket; the
+// Newton step multiplies by a reciprocal instead of dividing, so the iterates differ from a division-based solver's in
+// the last bits while the root they converge to (|dT| <= 1e-14 T) does not.
 __device__ __forceinline__ bool solve_T(const TEq &q, double Tm, double Thi, double &Tp) {
     double lo = 0.0, hi = Thi, f, df;
     if (!(Thi > 0.0)) return false;
     teq_eval(q, hi, f, df);
     if (!(f >= 0.0)) return false;
     if (q.method != 3 && !(q.c0 < 0.0)) return false;
+    if (q.method == 2) {
+        const double x = 2.0 * -q.c0 / (q.a4 + sqrt(fma(q.a4, q.a4, 4.0 * q.b1 * -q.c0)));
+        Tp = x * x;
+        return true;
+    }
     double T = (Tm > lo && Tm < hi) ? Tm : 0.5 * (lo + hi);
     for (int it = 0; it < 100; ++it) {
         teq_eval(q, T, f, df);

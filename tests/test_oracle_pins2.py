@@ -1,0 +1,254 @@
+"""Pins for the pieces of the oracle that round 1 left unpinned ("Oracle findings"): the n_0 sign gate of the
+spatial and the angular fluxes, the exp(-tau) and f(tau) coefficients of Eq 23 at tau ~ 1 (L266-274 with
+readings S8-S10), the MAPR candidate selection with its tie rule (reading S6) and the order of the MAPR angular update.
+CPU only; every expected value here comes from a closed form or from an independent few-line numpy computation."""
+import numpy as np
+import pytest
+
+from oracle import Oracle
+
+PER = ("periodic",) * 3
+
+
+def _n0_table(o):
+    """n_0 and n^mu per (column, s) from the oracle's centre tables (independent of rt_oracle.c)."""
+    e, g = o.tab["e_c"], o.tab["g_c"]
+    n = e[..., :, 0][..., None, :] + np.einsum("...mi,si->...sm", e[..., :, 1:], o.ang["nhat"])
+    return np.einsum("...m,...sm->...s", g[..., 0, :], n), n
+
+
+# ---- Eq 23 at tau ~ 1 ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("tau", [0.1, 1.0, 3.0])
+def test_eq23_free_streaming_term_linear_field(tau):
+    """1-D static uniform medium, I linear in x: PLI is exact (I_L = I_R at every face) and the diffusive term is the
+    same on both faces of a cell, so Eq 23 (L266-274, S8: the two weights sum to 1) leaves
+        I_new - I = -dt n^x e^{-tau} dI/dx          exactly,
+    for both signs of n^x.  A slip in the 1/2 (I_L + I_R) e^{-tau} term (factor, missing e^{-tau}, wrong sign) fails."""
+    N = 24
+    dt = 0.4 / N
+    grid = dict(n=(N, 1, 1), x0=(0.0, 0.0, 0.0), dx=(1.0 / N,) * 3, bc_lo=PER, bc_hi=PER)
+    o = Oracle(grid, "minkowski", {}, 2, dict(method=0, kappa_s=tau / dt))          # alpha = kappa_s rho, tau = alpha dt (L262)
+    o.set_fluid(np.ones((1, 1, N)), np.ones((1, 1, N)), None)
+    x = (np.arange(N) + 0.5) / N
+    slope = 0.7
+    I = np.tile((2.0 + slope * x)[None, None, :, None], (1, 1, 1, o.nd))
+    out = o.transport(I, I, dt).reshape(I.shape)
+    nx = o.ang["nhat"][:, 0]
+    assert (nx > 0.1).any() and (nx < -0.1).any()
+    ref = I - dt * nx * np.exp(-tau) * slope
+    inner = slice(3, N - 3)                                                         # away from the jump at the periodic wrap
+    assert np.abs(out[0, 0, inner] - ref[0, 0, inner]).max() < 2e-15
+    assert np.abs(out[0, 0, inner] - I[0, 0, inner]).max() > 1e-4 * np.exp(-tau)    # the term is there
+
+
+@pytest.mark.parametrize("tau", [0.1, 1.0, 3.0])
+def test_eq23_diffusive_coefficient_quadratic_field(tau):
+    """I = c x^2 on cell centres: the monotonised-central slope is the central difference (x_i >= dx), which again makes
+    I_L = I_R = c x_i x_{i+1}, so the first term of Eq 23 gives -n^x e^{-tau} 2 c x_i, and the third term (S9: coefficient
+    S+S-/(S+ - S-) = -|n^x| f(tau) / 2 on the cell-centre difference, required by Eq B9/B15-B16, L870-902) gives
+    +|n^x| f(tau) c dx: the second difference of c x^2 is 2 c dx^2.  f(tau) = sqrt((1 - e^{-tau^2}) / tau^2) (Eq 21-22, S8).
+    A factor-2 slip in either coefficient, or the anti-diffusive sign, fails."""
+    N = 32
+    dx = 1.0 / N
+    dt = 0.4 / N
+    grid = dict(n=(N, 1, 1), x0=(0.0, 0.0, 0.0), dx=(dx,) * 3, bc_lo=PER, bc_hi=PER)
+    o = Oracle(grid, "minkowski", {}, 2, dict(method=0, kappa_s=tau / dt))
+    o.set_fluid(np.ones((1, 1, N)), np.ones((1, 1, N)), None)
+    x = (np.arange(N) + 0.5) * dx
+    c = 1.3
+    I = np.tile((c * x * x)[None, None, :, None], (1, 1, 1, o.nd))
+    out = o.transport(I, I, dt).reshape(I.shape)
+    nx = o.ang["nhat"][:, 0]
+    f = np.sqrt((1.0 - np.exp(-tau * tau)) / (tau * tau))
+    ref = I[0, 0] - dt * (nx[None, :] * np.exp(-tau) * 2.0 * c * x[:, None] - np.abs(nx)[None, :] * f * c * dx)
+    inner = slice(3, N - 3)
+    assert np.abs(out[0, 0, inner] - ref[inner]).max() < 5e-15
+    # the two terms are separately visible at this resolution
+    assert dt * np.abs(nx).max() * f * c * dx > 1e-6
+
+
+# ---- n_0 sign gate (L280) ------------------------------------------------------------------------------------------------
+def _ergo_patch(level=4):
+    """Kerr-Schild a = 0.9 patch inside the ergosphere near the equator, n0_floor = 0 so that nothing but the sign of n_0
+    decides; vacuum."""
+    lo, hi = np.log(1.45), np.log(1.95)
+    grid = dict(n=(10, 1, 1), x0=(lo, 0.46, 0.0), dx=((hi - lo) / 10, 0.08, 0.1), bc_lo=("outflow", "outflow", "periodic"),
+                bc_hi=("outflow", "outflow", "periodic"), x3_symmetric=True)
+    return Oracle(grid, "ks_mks", dict(a=0.9, hslope=0.3), level, dict(method=0, n0_floor=0.0))
+
+
+def test_n0_sign_gate_blocks_the_spatial_flux():
+    """"The sign of n_0 is not allowed to change from one cell to the next" (L280, reading S14 (i)): no flux crosses a face
+    whose two cells have opposite sign(n_0) for that direction.  Inside the ergosphere n_0 turns positive towards the hole,
+    so take an unmasked cell i (n_0 < 0) whose lower neighbour has n_0 > 0, and an ingoing direction (n^1 < 0 around it): in
+    vacuum (Eq 20) the upper face takes its state from cells i+1, i+2 (and i through the slope), the lower face is gated,
+    so the update of (i, s) must not depend AT ALL on the cells below the face -- without the gate its lower flux would
+    carry I_i - slope(I_{i-1}, I_i, I_{i+1}) / 2.  Where the sign does not change, the same perturbation does change the
+    result."""
+    o = _ergo_patch()
+    n0, n = _n0_table(o)
+    n0, n1 = n0[0, 0], n[0, 0][..., 1]                     # [i, s]
+    rng = np.random.default_rng(21)
+    I = rng.uniform(0.5, 1.0, size=(1, 1, 10, o.nd))
+    dt = 1e-3
+    base = o.transport(I, I, dt).reshape(I.shape)
+    gated = ungated = 0
+    for i in range(2, 8):
+        for s in range(o.nd):
+            if not (n0[i, s] < 0 and n1[i, s] < 0 and n1[i + 1, s] < 0 and n1[i - 1, s] < 0):
+                continue
+            changes_sign = n0[i - 1, s] > 0
+            if not changes_sign and ungated >= 6:
+                continue
+            I2 = I.copy()
+            I2[0, 0, :i, s] += 0.2                         # everything below the face
+            out = o.transport(I2, I2, dt).reshape(I.shape)
+            if changes_sign:
+                assert out[0, 0, i, s] == base[0, 0, i, s]
+                gated += 1
+            else:
+                ungated += abs(out[0, 0, i, s] - base[0, 0, i, s]) > 1e-7
+    assert gated >= 3 and ungated >= 3
+
+
+def test_n0_sign_gate_blocks_the_angular_flux():
+    """The angular twin (L280: "from one [angular] cell to the next"): the flux across a geodesic-grid edge whose two cells have
+    opposite sign(n_0) is zero, so D_Omega of s does not see that neighbour; it does see a neighbour of equal sign."""
+    o = _ergo_patch()
+    n0, _ = _n0_table(o)
+    n0 = n0[0, 0]
+    nb, nnb = o.ang["nb"], o.ang["nnb"]
+    rng = np.random.default_rng(22)
+    I = rng.uniform(0.5, 1.0, size=(1, 1, 10, o.nd))
+    dt = 1e-3
+    base = o.angular_flux(I, I, dt).reshape(I.shape)
+    gated = ungated = 0
+    for i in range(10):
+        for s in range(o.nd):
+            if not n0[i, s] < 0:
+                continue
+            for t in nb[s, :nnb[s]]:
+                opposite = n0[i, t] > 0
+                if not opposite and ungated >= 40:
+                    continue
+                I2 = I.copy()
+                I2[0, 0, i, t] += 0.3
+                out = o.angular_flux(I2, I2, dt).reshape(I.shape)
+                if opposite:
+                    assert out[0, 0, i, s] == base[0, 0, i, s]
+                    gated += 1
+                else:
+                    ungated += out[0, 0, i, s] != base[0, 0, i, s]      # donor cell: seen only if the edge is upwind from t
+        if gated >= 20 and ungated >= 40:
+            break
+    assert gated >= 5 and ungated >= 10
+
+
+# ---- MAPR (reading S6) ---------------------------------------------------------------------------------------------------
+def _mapr_candidates(nh, nb, nnb, Ic, s):
+    """Independent restatement of O4': log map of the neighbours into the tangent plane at n_s, one plane per pair of
+    consecutive neighbours, solved with lstsq (the oracle uses the 2x2 normal equations)."""
+    c0 = nh[s]
+    xi, dI = [], []
+    for t in nb[s, :nnb[s]]:
+        dot = float(np.clip(c0 @ nh[t], -1, 1))
+        p = nh[t] - dot * c0
+        xi.append(np.arccos(dot) * p / np.linalg.norm(p))
+        dI.append(Ic[t] - Ic[s])
+    xi, dI = np.array(xi), np.array(dI)
+    # orthonormal basis of the tangent plane: the gradient has two components there
+    b1 = xi[0] / np.linalg.norm(xi[0])
+    b2 = np.cross(c0, b1)
+    B = np.stack([b1, b2])
+    out = []
+    for e in range(nnb[s]):
+        e2 = (e + 1) % nnb[s]
+        A = np.stack([xi[e] @ B.T, xi[e2] @ B.T])
+        g2 = np.linalg.lstsq(A, np.array([dI[e], dI[e2]]), rcond=None)[0]
+        out.append(g2 @ B)
+    return np.array(out)
+
+
+def test_mapr_picks_the_minimum_norm_plane_and_the_lowest_index_on_a_tie():
+    """The gradient the oracle returns is the candidate of smallest norm (the "minimum angle" plane, L227); when several
+    candidates have the same norm to round-off (mirror-image neighbours of a cell on a symmetry plane of the grid, or equal
+    masked neighbours) the lowest-index candidate wins, whatever the last bits say (S6)."""
+    o = Oracle(dict(n=(1, 1, 1), x0=(0, 0, 0), dx=(1, 1, 1), bc_lo=PER, bc_hi=PER), "minkowski", {}, 4, dict(method=0, ang_recon=1))
+    nh, nb, nnb = o.ang["nhat"], o.ang["nb"], o.ang["nnb"]
+    rng = np.random.default_rng(31)
+    # (a) generic fields: arg-min over the candidates
+    for s in (3, 40, 77, 120, 161):
+        Ic = rng.uniform(0.5, 1.5, size=o.nd)
+        cand = _mapr_candidates(nh, nb, nnb, Ic, s)
+        norms = (cand ** 2).sum(1)
+        assert np.sort(norms)[1] > np.sort(norms)[0] * (1 + 1e-6)          # no tie here
+        assert np.abs(o.mapr_gradient(Ic, s) - cand[norms.argmin()]).max() < 1e-11
+    # (b) structural ties: a field that depends on z only is mirror symmetric about every plane through the pole, and
+    # the grid (pole along 3-hat, a vertex at azimuth 0, S2) has the x-z plane as a mirror plane: cells with n_y = 0 see
+    # their neighbours in mirror pairs, so two candidates tie.  Perturbing the last bits must not change the winner.
+    ties = 0
+    for s in range(1, o.nd - 1):
+        if abs(nh[s, 1]) > 1e-12:
+            continue
+        Ic = 1.0 + 0.4 * nh[:, 2] + 0.3 * nh[:, 2] ** 2
+        cand = _mapr_candidates(nh, nb, nnb, Ic, s)
+        norms = (cand ** 2).sum(1)
+        m = norms.min()
+        tied = np.flatnonzero(norms <= m * (1 + 1e-9))
+        if len(tied) < 2 or np.abs(cand[tied[0]] - cand[tied[1]]).max() < 1e-6:
+            continue                                                        # no tie, or the tied planes coincide
+        ties += 1
+        for eps in (0.0, 1e-15, -1e-15):
+            Ip = Ic.copy()
+            Ip[nb[s, tied[1]]] += eps                                       # nudge one side of the mirror pair
+            assert np.abs(o.mapr_gradient(Ip, s) - cand[tied[0]]).max() < 1e-9
+    assert ties >= 3
+    # (c) equal (masked, zero) neighbours: three consecutive zeros next to a live cell give two candidates that agree on the
+    # pair they share; the winner is the lowest-index one of the minimum-norm set
+    s = 50
+    Ic = rng.uniform(0.5, 1.5, size=o.nd)
+    for q in range(3):
+        Ic[nb[s, q]] = 0.0
+    cand = _mapr_candidates(nh, nb, nnb, Ic, s)
+    norms = (cand ** 2).sum(1)
+    first = int(np.flatnonzero(norms <= norms.min() * (1 + 1e-11))[0])
+    assert np.abs(o.mapr_gradient(Ic, s) - cand[first]).max() < 1e-11
+
+
+def _cyl_angular_rate(level, ang_recon):
+    """D_Omega of the oracle for a smooth field in flat space with the rotating (cylindrical) tetrad at one point, against the
+    exact angular divergence.  Tetrad e_1 = R-hat, e_2 = phi-hat, e_3 = z-hat: the only coefficients are omega^R_{phi phi} =
+    -1/R, omega^phi_{phi R} = +1/R (pinned in test_oracle_geometry), so a direction with tetrad components (n^R, n^phi, n^z)
+    turns about the 3-axis at the rate d psi / d lambda = -n^phi / R (a^R = +n^phi n^phi / R, a^phi = -n^phi n^R / R, Eq 7
+    in the 3-vector form S4), and the exact divergence of the angular flux a F on the sphere is
+        d/d psi (psi-dot F) = -(1/R) (n^R F + n^phi dF/dpsi).
+    The conserved variable is n^0 n_0 I = -I here and the fluxes carry n_0 = -1 (Eq 18/19), so D_Omega = -div(a F): for F = 1
+    it is +n^R / R, which cancels the spatial divergence -d_a n^a = -n^R / R of the same field (the Liouville pin)."""
+    x, y = 1.3, 0.7
+    R = np.hypot(x, y)
+    grid = dict(n=(1, 1, 1), x0=(x - 0.05, y - 0.05, 0.0), dx=(0.1, 0.1, 0.1), bc_lo=PER, bc_hi=PER)
+    o = Oracle(grid, "mink_cyl", {}, level, dict(method=0, ang_recon=ang_recon))
+    nR, nP, nZ = o.ang["nhat"].T
+    F = 1.0 + 0.3 * nR + 0.25 * nP * nZ + 0.2 * nR * nP
+    dF = 0.3 * (-nP) + 0.25 * nR * nZ + 0.2 * (nR * nR - nP * nP)           # d/dpsi: n^R -> -n^phi, n^phi -> n^R
+    exact = (nR * F + nP * dF) / R
+    I = F[None, None, None, :]
+    dt = 1e-3
+    out = o.angular_flux(I, I, dt).reshape(I.shape)
+    # flat space: n^0 n_0 = -1, so I_out = I + dt D_Omega  (O4 + O5)
+    D = (out[0, 0, 0] - F) / dt
+    return float((np.abs(D - exact) * o.ang["w"]).sum() / (4 * np.pi)), float((np.abs(exact) * o.ang["w"]).sum() / (4 * np.pi))
+
+
+def test_mapr_angular_update_is_second_order_donor_cell_first_order():
+    """"A second order reconstruction in the direction space ... minimum angle plane reconstruction" (L227): the L1 error of the
+    MAPR angular update against the exact angular divergence falls ~4x per angular refinement 42 -> 162 -> 642 (ratio >= 3
+    asked), donor cell ~2x.  This also fixes the sign and normalisation of the whole angular term (Eq 19 with S4/S5) against
+    a closed form."""
+    em = [_cyl_angular_rate(lv, 1) for lv in (2, 4, 8)]
+    ed = [_cyl_angular_rate(lv, 0) for lv in (2, 4, 8)]
+    scale = em[0][1]
+    assert ed[0][0] < 0.2 * scale                                            # right sign and size already at 42 directions
+    assert ed[0][0] / ed[1][0] > 1.6 and ed[1][0] / ed[2][0] > 1.6           # first order
+    assert em[0][0] / em[1][0] > 3.0 and em[1][0] / em[2][0] > 3.0           # second order
+    assert em[2][0] < 0.25 * ed[2][0]
