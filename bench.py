@@ -30,8 +30,8 @@ UNIT = "cell-direction updates/s"
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=None, help="timed steps (default: 200 for the CUDA arm = about a second of timed region on config 4; 3 for --impl reference)")
+    ap.add_argument("--warmup", type=int, default=None, help="untimed warm-up steps (default 5; 1 for --impl reference)")
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index 1..5 (4 = Kerr-Schild, the roofline config); 6 = snake-coordinates beam (PAPER 4.6)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--multi", default="slab", choices=["slab", "replicas"],
@@ -116,18 +116,28 @@ def measured_peak():
 # what the method must move at this kernel boundary, fp64 = 8 B.  transport: read I_in, (read I_base when it is a
 # different array: corrector only), write I_out; angular: read I_in, read+write I_inout; source: read+write I.
 ALGO_BYTES = {"transport_pred": 16.0, "transport_corr": 24.0, "angular": 24.0, "source": 16.0}
-# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per launch of each kernel class on config 4 at full size,
-# from the `ncu --set full` capture summarised in profiles/r01_v20_kernels_full.md (transport = vacuum + general +
-# list kernels, mean of the predictor (2.66 GB) and corrector (3.64 GB) launches).  Other configs: not captured -> null.
-NCU_TRAFFIC = {4: {"transport": 3.15e9, "angular": 3.08e9, "source": 0.50e9}}
-# Warp instructions (smsp__inst_executed.sum) per launch of each kernel class, same capture (transport: mean of
-# 883.7 M predictor and 908.4 M corrector; source: mean of the three k_cell launches): `roofline.issue`.
-NCU_WARP_INSTR = {4: {"transport": 896.0e6, "angular": 439.2e6, "source": 167.7e6}}
-# What actually limits the vacuum transport kernel: the L2 -> L1 traffic of its seven operands per
-# cell-direction (l1tex__m_xbar2l1tex_read_bytes.sum per launch of the class, mean of predictor and corrector) and the
-# L2 throughput it runs at (lts__throughput of k_transport_vac), same capture: `roofline.l2`.
-NCU_L2 = {4: {"transport": {"l2_to_l1_bytes_per_launch": 8.74e9, "lts_throughput_pct_vac_kernel": 78.2}}}
 ISSUE_PEAK = 148 * 4 * 1.965e9          # warp instructions / s: 148 SMs x 4 schedulers x 1 issue per clock at 1965 MHz
+# Fixed byte counts of SURVEY.md 8(d) per cell-direction per rt_step: 32 B if each stage read and wrote the intensity once
+# (the fully fused ideal), 74 B for two kernels per stage.  The step's fraction of the roofline is quoted against both.
+STEP_BYTES_IDEAL, STEP_BYTES_TWO_KERNEL = 32.0, 74.0
+
+
+def ncu_metrics(cfg_index):
+    """ncu-derived per-class figures (DRAM bytes, warp instructions, L2 -> L1 bytes of one rt_step) from the newest
+    profiles/*_metrics_c<config>.json whose recorded source hash equals the hash of the library sources that are running.
+    None when no capture of THIS build is committed: nothing measured on another build is ever attached to a live time."""
+    import glob
+    from paper_2508_15532_b200.ncu_metrics import source_hash
+    cur = source_hash()
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_metrics_c%d.json" % cfg_index)), reverse=True):
+        try:
+            with open(path) as f:
+                doc = json.load(f)
+        except Exception:
+            continue
+        if doc.get("source_hash") == cur and doc.get("config") == cfg_index:
+            return doc["classes"], os.path.relpath(path, ROOT)
+    return None, None
 
 
 TRANSPORT_VARIANT = 0    # set from --transport-variant
@@ -234,6 +244,7 @@ def run_gpu(args, rank, world):
         step()
     barrier()
     I.copy_(I0); T.copy_(T0)
+    ctx._nfail.zero_()                               # failed temperature solves are counted over the timed region only
     ctx.profile_enable(True)
     ctx.profile_read()
     l0 = ctx.launch_count()
@@ -252,7 +263,16 @@ def run_gpu(args, rank, world):
     ctx.profile_enable(False)
     launches = ctx.launch_count() - l0
     finite = bool(torch.isfinite(I).all().item())
+    n_fail = ctx.n_fail()
     ms = max_over_ranks(ms, world, dev)
+    # entries that carry work: not a masked direction (n_0 > -n0_floor, L284), not in a zero band (L709)
+    n0 = ctx.geometry("n0_c")                        # [E3, N2, N1, nd]
+    g = cfg["grid"] if slab is None else slab.grid
+    live = (n0 <= -float(cfg["options"].get("n0_floor", 0.1)))
+    zl, zh = g.get("zero_lo", (0, 0, 0)), g.get("zero_hi", (0, 0, 0))
+    n1_, n2_, n3_ = g["n"]
+    live[:, :zl[1]] = False; live[:, n2_ - zh[1]:] = False; live[:, :, :zl[0]] = False; live[:, :, n1_ - zh[0]:] = False
+    live_fraction = float(live.mean()) * (n3_ - zl[2] - zh[2]) / n3_
 
     # ---- end to end through the C ABI with pinned HOST buffers (H2D + D2H inside the timed region) ----
     e2e = None
@@ -354,19 +374,27 @@ def run_gpu(args, rank, world):
             except Exception as ex:
                 e2e["coupled_error"] = str(ex)[:160]
     return dict(cfg=cfg, ctx=ctx, ms=ms, units=units, kernel_units=kernel_units, prof=prof, launches=launches, clk=clk, e2e=e2e,
-                finite=finite, dt=dt, multi=multi)
+                finite=finite, dt=dt, multi=multi, n_fail=n_fail, live_fraction=live_fraction)
 
 
 # ---- oracle legs (the only places bench.py may execute oracle/) ----------------------------------------------------
 ORACLE_SAMPLE = {1: (64, 64, 1), 2: (24, 24, 24), 3: (24, 24, 24), 4: (64, 48, 16), 5: (32, 24, 8), 6: (64, 64, 1)}
 
 
-def run_oracle(cfg_index, steps, warmup=0):
+def run_oracle(cfg_index, steps, warmup=0, threads=None):
     """The oracle as it stands on this box's host cores, on a bounded sample of the workload: the same config
-    (metric, tetrad, opacities, seeded fields, CFL rule) on a coarser grid.  returns (updates/s, cores, sample)."""
+    (metric, tetrad, opacities, seeded fields, CFL rule) on a coarser grid.  threads: OpenMP threads of the oracle's cell
+    loop (None = all cores).  returns (updates/s, cores, sample, ms per step, cfg)."""
+    import ctypes
     import numpy as np
     import rt_workloads as W
     from oracle import Oracle
+
+    ncores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    try:   # the thread count of the OpenMP runtime the oracle's library uses (the oracle itself is not touched)
+        ctypes.CDLL("libgomp.so.1").omp_set_num_threads(int(threads or ncores))
+    except OSError:
+        threads = None
 
     n = ORACLE_SAMPLE[cfg_index]
     cfg = W.config(cfg_index, n=n)
@@ -385,9 +413,9 @@ def run_oracle(cfg_index, steps, warmup=0):
         I, T, R, G, nf = orc.step(I, T, dt)
     el = time.perf_counter() - t0
     units = n[0] * n[1] * n[2] * orc.nd
-    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
-    sample = "oracle rt_step x%d on %s at %dx%dx%d x %d dirs (same config, coarser grid), OpenMP over cells" % (
-        steps, cfg["name"], n[0], n[1], n[2], orc.nd)
+    cores = int(threads or ncores)
+    sample = "oracle rt_step x%d on %s at %dx%dx%d x %d dirs (same config, coarser grid), OpenMP over cells, %d thread%s" % (
+        steps, cfg["name"], n[0], n[1], n[2], orc.nd, cores, "" if cores == 1 else "s")
     return units * steps / el, cores, sample, el / steps * 1e3, cfg
 
 
@@ -411,6 +439,10 @@ def main_reference(args):
 
 def main():
     args = parse()
+    if args.steps is None:
+        args.steps = 3 if args.impl == "reference" else 200
+    if args.warmup is None:
+        args.warmup = 1 if args.impl == "reference" else 5
     global TRANSPORT_VARIANT, TRANSPORT_TILE
     TRANSPORT_VARIANT = args.transport_variant
     TRANSPORT_TILE = (tuple(int(v) for v in args.transport_tile.split(",")) + (0,) * 3)[:3]
@@ -444,35 +476,51 @@ def main():
         per_unit = {"transport": 0.5 * (ALGO_BYTES["transport_pred"] + ALGO_BYTES["transport_corr"]),
                     "angular": ALGO_BYTES["angular"], "source": ALGO_BYTES["source"]}
         achieved = per_unit[dom] * units / (dms / max(dcnt, 1) * 1e-3) / 1e9 if dcnt else 0.0
-        step_bytes = sum(per_unit[k] * units * prof[k][1] for k in per_unit) / K
+        single = args.size is None and world == 1
+        ncu, ncu_path = ncu_metrics(args.config) if single else (None, None)
+        per_step = lambda key: (ncu[dom][key] if ncu and dom in ncu and key in ncu[dom] else None)
+        launches_per_step = max(dcnt, 1) / K
+        dom_s_per_step = dms / K * 1e-3
+        traffic = per_step("dram_bytes")
+        winstr = per_step("warp_instr")
+        l2b = per_step("l2_to_l1_bytes")
+        step_s = ms / K * 1e-3
         roof = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC.get(args.config, {}).get(dom) if args.size is None else None,
-                "traffic_source": "profiles/r01_v20_kernels_full.md (bytes per launch)", "peak_source": which,
+                # ncu figures of THIS build only (hash-matched, see ncu_metrics()); per launch of the class like `achieved`
+                "traffic": traffic / launches_per_step if traffic else None,
+                "traffic_source": ncu_path, "peak_source": which,
                 "algorithmic_bytes_per_launch": per_unit[dom] * units,
                 "algorithmic_bytes_per_cell_dir_per_launch": per_unit[dom],
                 "kernel_ms_per_step": {k: prof[k][0] / K for k in prof},
                 "kernel_launches_per_step": {k: prof[k][1] / K for k in prof},
-                "issue": ({"warp_instr_per_launch": NCU_WARP_INSTR[args.config][dom],
-                           "achieved": NCU_WARP_INSTR[args.config][dom] / (dms / max(dcnt, 1) * 1e-3), "peak": ISSUE_PEAK,
-                           "unit": "warp-instr/s", "frac": NCU_WARP_INSTR[args.config][dom] / (dms / max(dcnt, 1) * 1e-3) / ISSUE_PEAK,
-                           "source": "instruction count from profiles/r01_v20_kernels_full.md, time live"}
-                          if args.config in NCU_WARP_INSTR and args.size is None and dcnt and world == 1 else None),
-                "l2": (dict(NCU_L2[args.config][dom], source="profiles/r01_v20_kernels_full.md (ncu capture, not live)")
-                       if args.config in NCU_L2 and dom in NCU_L2[args.config] and args.size is None and world == 1 else None),
-                "step_algorithmic_GBps": step_bytes / (ms / K * 1e-3) / 1e9,
-                "step_frac_of_peak": step_bytes / (ms / K * 1e-3) / 1e9 / peak}
+                "issue": ({"warp_instr_per_step": winstr, "achieved": winstr / dom_s_per_step, "peak": ISSUE_PEAK, "unit": "warp-instr/s",
+                           "frac": winstr / dom_s_per_step / ISSUE_PEAK, "source": "instruction count from %s, time live" % ncu_path}
+                          if winstr and dcnt else None),
+                "l2": ({"l2_to_l1_bytes_per_launch": l2b / launches_per_step, "times_algorithmic": l2b / launches_per_step / (per_unit[dom] * units),
+                        "source": ncu_path} if l2b else None),
+                # the whole step against the two fixed byte counts of SURVEY.md 8(d) (a design with more kernel boundaries cannot
+                # raise its own numerator)
+                "step_frac_of_peak_32B": STEP_BYTES_IDEAL * r["units"] / step_s / 1e9 / peak,
+                "step_frac_of_peak_74B": STEP_BYTES_TWO_KERNEL * r["units"] / step_s / 1e9 / peak}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
                 "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
                 "data": "synthetic",
                 "config": {"workload": workload_name(r["cfg"]), "dt": r["dt"], "l2": "inputs larger than L2 (one I copy >= 1 GB vs 126 MB)"
                            if units * 8 > 2.0e8 else "inputs FIT in L2 (latency-bound config; HBM fraction not meaningful)",
-                           "multi_gpu": r["multi"], "transport_variant": TRANSPORT_VARIANT,
-                           "finite": r["finite"]},
+                           "multi_gpu": r["multi"], "transport_variant": TRANSPORT_VARIANT, "transport_path": list(r["ctx"].transport_info()),
+                           "finite": r["finite"], "n_fail": r["n_fail"],
+                           # share of the (cell, direction) entries that carry work (not masked, not in a zero band); the
+                           # others only ever hold 0.0 -- `value` counts every entry
+                           "live_fraction": r["live_fraction"]},
                 "clocks": r["clk"], "e2e": r["e2e"], "gpu_launches": r["launches"], "roofline": roof}
+        if r["n_fail"]:
+            raise SystemExit("bench.py: %d temperature solves failed inside the timed region" % r["n_fail"])
         if not args.no_cpu_baseline and world == 1:
             val, cores, sample, oms, _ = run_oracle(args.config, 2)
-            line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+            val1, _, sample1, _, _ = run_oracle(args.config, 1, threads=1)
+            line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                                    "single_thread": {"value": val1, "cores": 1, "sample": sample1}}
         print(json.dumps(line))
     if world > 1:
         dist.barrier()
