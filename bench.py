@@ -304,40 +304,8 @@ def run_gpu(args, rank, world):
         d2h = (hI.numel() + hT.numel() + hR.numel() + hG.numel()) * 8
         e2e = {"value": aggregate_value(units, ksteps, world, ems), "unit": UNIT, "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "steps": ksteps, "ms_per_step": ems / ksteps,
-               "path": "rt_step_host: one C-ABI call, H2D -> rt_step -> D2H back to back" if slab is None else
+               "path": "rt_step_host: one C-ABI call on pinned host buffers; inside it x3 slabs with a 4-plane halo, H2D / rt_step / D2H overlapped on three streams" if slab is None else
                        "H2D -> SlabDomain.step (rt_step + halo exchange) -> D2H"}
-        # same bytes, same result, copies overlapped with the compute: hoststep.HostPipeline streams the planes in, steps
-        # x3 slabs (deep halo) as they arrive and streams their owned planes out, on three streams (PCIe is full duplex)
-        n3 = cfg["grid"]["n"][2]
-        if slab is None and world == 1 and n3 >= 16:
-            try:
-                from paper_2508_15532_b200.hoststep import HostPipeline
-                hp = HostPipeline(cfg, n3 // 8, device=device)
-                hp.set_fields(f)
-                hI.copy_(I0); hT.copy_(T0)
-                hI2 = torch.empty(I.shape, dtype=torch.float64, pin_memory=True)
-                hT2 = torch.empty(T.shape, dtype=torch.float64, pin_memory=True)
-                bufs = [hI, hT, hI2, hT2]
-                def two():
-                    hp.step_host(bufs[0], bufs[1], bufs[2], bufs[3], hR, hG, dt)
-                    bufs[0], bufs[2] = bufs[2], bufs[0]
-                    bufs[1], bufs[3] = bufs[3], bufs[1]
-                two()
-                barrier()
-                ev0.record()
-                for _ in range(ksteps):
-                    two()
-                ev1.record()
-                barrier()
-                pms = ev0.elapsed_time(ev1)
-                if pms < ems and bool(torch.isfinite(bufs[0]).all().item()):
-                    e2e = dict(e2e, single_call={"value": e2e["value"], "ms_per_step": e2e["ms_per_step"], "path": e2e["path"]},
-                               value=aggregate_value(units, ksteps, world, pms), ms_per_step=pms / ksteps,
-                               path="hoststep.HostPipeline: %d x3 slabs with a 4-plane halo, H2D / rt_step (C ABI) / D2H "
-                                    "overlapped on three streams; bit-equal to rt_step (tests/test_gpu_dist.py)" % (n3 // 8))
-                del hp
-            except Exception as ex:   # e.g. out of memory at a size nobody planned for: the single-call figure stands
-                e2e["pipeline_error"] = str(ex)[:160]
         # Coupled mode, the way the paper drives the module (L448-456): the radiation state stays on the GPU; every step the
         # fluid state (rho, T, u^mu: what the GRMHD sector owns) comes from pinned host buffers, and the moments R, the
         # 4-force G and the new T go back.  Extra figure beside the strict one above (which moves the intensity both ways).

@@ -137,9 +137,13 @@ int rt_moments(rt_ctx *ctx, const double *I_dev, double *R_dev, void *stream);
 int rt_step(rt_ctx *ctx, double *I_inout_dev, double *T_inout_dev, double *R_out_dev, double *G_out_dev, double dt,
             int *n_fail_dev, void *stream);
 
-/* rt_step with HOST buffers (pinned memory recommended): copies I[N_c][pitch] and T[N_c] to library-owned device
- * buffers, runs rt_step, copies I, T and (if not NULL) R[16][N_c], G[4][N_c] back, all on `stream`, and synchronises the
- * stream before returning.  *n_fail_host (may be NULL) receives the number of cells whose temperature solve failed. */
+/* rt_step with HOST buffers (pinned memory, or the copies cannot overlap): I[N_c][pitch] and T[N_c] are updated in place, R[16][N_c]
+ * and G[4][N_c] (may be NULL) are written; the call returns after everything has landed on the host.  *n_fail_host (may be
+ * NULL) receives the number of cells whose temperature solve failed.  Meshes with N3 >= 16 and no FIXED boundary are cut
+ * into N3 / 8 x3-slabs with a 4-plane halo (the domain of dependence of one step): every plane crosses PCIe once, a slab is
+ * stepped by the plain rt_step as soon as its planes have arrived and its owned planes go back while later slabs arrive or
+ * compute (three internal streams, ordered after `stream`); other meshes go H2D -> rt_step -> D2H back to back.  Either way
+ * the result is rt_step's, bit for bit.  The slab contexts and device buffers are built on the first call. */
 int rt_step_host(rt_ctx *ctx, double *I_inout_host, double *T_inout_host, double *R_out_host, double *G_out_host, double dt,
                  int *n_fail_host, void *stream);
 

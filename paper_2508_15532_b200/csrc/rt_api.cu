@@ -30,6 +30,14 @@ struct rt_ctx {
     int *d_nsel; void *d_part_tmp; size_t part_tmp_bytes;   // interaction-list partition (cub) scratch
     double *d_hI, *d_hT, *d_hR, *d_hG;   // device staging of rt_step_host (allocated on first use)
     int *d_hfail;
+    // rt_step_host pipeline (x3 slabs with a 4-plane halo, each its own context over the same metric): built on first use
+    struct HostSlab { rt_ctx *sub; int k0, k1, ext_lo, ext_hi, n3l; double *I, *T, *R, *G, *rho, *u4; cudaEvent_t done; };
+    std::vector<HostSlab> hslabs;
+    cudaStream_t hs_in, hs_cmp, hs_out;
+    std::vector<cudaEvent_t> hev;      // one event per uploaded chunk
+    cudaEvent_t hev_start, hev_end[3];
+    long long fluid_version, hslab_fluid_version;
+    bool is_sub;                       // a slab context of another context's pipeline
     double *d_mapr_xi, *d_mapr_xim, *d_mapr_a, *d_angraw;
     int *d_mapr_back, *d_mapr_nnb;
     unsigned char *d_angup;
@@ -101,6 +109,8 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     if (!c) return RT_ENOMEM;
     c->grid = *grid; c->metric = *metric; c->opt = *opt; c->level = angle_level;
     c->launches = 0; c->fluid_set = false; c->profiling = false;
+    c->hs_in = c->hs_cmp = c->hs_out = nullptr; c->hev_start = nullptr; c->hev_end[0] = c->hev_end[1] = c->hev_end[2] = nullptr;
+    c->fluid_version = 0; c->hslab_fluid_version = -1; c->is_sub = false;
     if (!build_angular_grid(angle_level, c->ang)) { delete c; return RT_EINVAL; }
     const int nd = c->nd = c->ang.nd;
     const int pitch = c->pitch = (nd + 3) / 4 * 4;
@@ -343,6 +353,17 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
 
 extern "C" int rt_free(rt_ctx *c) {
     if (!c) return RT_EINVAL;
+    for (auto &h : c->hslabs) {
+        if (h.sub) rt_free(h.sub);
+        cudaFree(h.I); cudaFree(h.T); cudaFree(h.R); cudaFree(h.G); cudaFree(h.rho); cudaFree(h.u4);
+        if (h.done) cudaEventDestroy(h.done);
+    }
+    for (auto e : c->hev) cudaEventDestroy(e);
+    if (c->hev_start) cudaEventDestroy(c->hev_start);
+    for (int q = 0; q < 3; ++q) if (c->hev_end[q]) cudaEventDestroy(c->hev_end[q]);
+    if (c->hs_in) cudaStreamDestroy(c->hs_in);
+    if (c->hs_cmp) cudaStreamDestroy(c->hs_cmp);
+    if (c->hs_out) cudaStreamDestroy(c->hs_out);
     for (int a = 0; a < 3; ++a) { cudaFree(c->tab.face[a]); cudaFree(c->d_fcoef[a]); }
     cudaFree(c->tab.cen); cudaFree(c->tab.ecen); cudaFree(c->tab.angcoef); cudaFree(c->tab.nhat); cudaFree(c->tab.w);
     cudaFree(c->tab.nb); cudaFree(c->tab.mirror); cudaFree(c->d_colflag); cudaFree(c->d_cls); cudaFree(c->d_paircoef); cudaFree(c->d_genlist); cudaFree(c->d_srclist); cudaFree(c->d_nsel); cudaFree(c->d_part_tmp); cudaFree(c->d_hI); cudaFree(c->d_hT); cudaFree(c->d_hR); cudaFree(c->d_hG); cudaFree(c->d_hfail); cudaFree(c->d_mapr_xi); cudaFree(c->d_mapr_xim); cudaFree(c->d_mapr_a);
@@ -529,6 +550,7 @@ extern "C" int rt_set_fluid(rt_ctx *c, const double *rho, const double *T, const
         }
     }
     c->fluid_set = true;
+    ++c->fluid_version;
     return RT_OK;
 }
 
@@ -594,8 +616,8 @@ extern "C" int rt_step(rt_ctx *c, double *I, double *T, double *R_out, double *G
     return stage(c, c->d_Ih, c->d_Th, I, I, T, dt, n_fail, R_out, G_out, st);               // corrector
 }
 
-extern "C" int rt_step_host(rt_ctx *c, double *I_h, double *T_h, double *R_h, double *G_h, double dt, int *n_fail_h, void *stream) {
-    if (!c || !I_h || !T_h) return RT_EINVAL;
+// H2D -> rt_step -> D2H back to back on one stream (meshes too thin to cut, FIXED boundaries)
+static int step_host_simple(rt_ctx *c, double *I_h, double *T_h, double *R_h, double *G_h, double dt, int *n_fail_h, void *stream) {
     cudaStream_t st = (cudaStream_t)stream;
     const size_t nI = (size_t)c->ncell * c->pitch * sizeof(double), nC = (size_t)c->ncell * sizeof(double);
     if (!c->d_hI) {
@@ -617,4 +639,177 @@ extern "C" int rt_step_host(rt_ctx *c, double *I_h, double *T_h, double *R_h, do
     if (n_fail_h) CK(cudaMemcpyAsync(n_fail_h, c->d_hfail, sizeof(int), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     return RT_OK;
+}
+
+// ---- rt_step_host as a pipeline ---------------------------------------------------------------------------------------
+// The mesh is cut into x3 slabs with a 4-plane halo on every cut side: one rt_step (two stages x a 2-cell stencil) has a
+// domain of dependence of +-4 cells, so the plain rt_step on the extended slab (OUTFLOW on the cut faces) gives the exact
+// single-domain result on the planes the slab owns (the decomposition of DESIGN.md section 8, here on one GPU).  Every
+// plane of the input state crosses PCIe once, into a full-size device copy; a slab starts as soon as its planes are there
+// and its owned planes go back while later slabs are still arriving or computing: H2D, compute and D2H on three streams
+// (PCIe is full duplex).  Same kernels on the same values: the result equals rt_step's bit for bit.
+static const int HS_MARGIN = 4;
+
+static int hslab_build(rt_ctx *c, int nslab) {
+    const rt_grid &G = c->grid;
+    const int n3 = G.n[2];
+    const bool per = G.bc_lo[2] == RT_BC_PERIODIC;
+    const size_t plane_c = (size_t)c->ncol, plane_i = plane_c * c->pitch;
+    for (int r = 0; r < nslab; ++r) {
+        rt_ctx::HostSlab h;
+        std::memset(&h, 0, sizeof h);
+        const int base = n3 / nslab, rem = n3 % nslab;
+        h.k0 = r * base + (r < rem ? r : rem);
+        h.k1 = h.k0 + base + (r < rem ? 1 : 0);
+        const bool lo_cut = per || r > 0, hi_cut = per || r < nslab - 1;
+        h.ext_lo = lo_cut ? HS_MARGIN : 0; h.ext_hi = hi_cut ? HS_MARGIN : 0;
+        h.n3l = h.k1 - h.k0 + h.ext_lo + h.ext_hi;
+        rt_grid g = G;
+        g.n[2] = h.n3l;
+        g.x0[2] = G.x0[2] + (h.k0 - h.ext_lo) * G.dx[2];
+        g.bc_lo[2] = lo_cut ? RT_BC_OUTFLOW : G.bc_lo[2];
+        g.bc_hi[2] = hi_cut ? RT_BC_OUTFLOW : G.bc_hi[2];
+        if (per) g.bc_lo[2] = g.bc_hi[2] = RT_BC_OUTFLOW;
+        if (lo_cut) g.zero_lo[2] = 0;
+        if (hi_cut) g.zero_hi[2] = 0;
+        int rc = rt_init(&g, &c->metric, c->level, &c->opt, &h.sub);
+        if (rc != RT_OK) { c->hslabs.push_back(h); return rc; }
+        h.sub->is_sub = true;
+        cudaError_t e = cudaMalloc((void **)&h.I, h.n3l * plane_i * sizeof(double));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&h.T, h.n3l * plane_c * sizeof(double));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&h.R, 16 * h.n3l * plane_c * sizeof(double));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&h.G, 4 * h.n3l * plane_c * sizeof(double));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&h.rho, h.n3l * plane_c * sizeof(double));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&h.u4, 4 * h.n3l * plane_c * sizeof(double));
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h.done, cudaEventDisableTiming);
+        c->hslabs.push_back(h);
+        if (e != cudaSuccess) { g_last_cuda = (int)e; return e == cudaErrorMemoryAllocation ? RT_ENOMEM : RT_ECUDA; }
+    }
+    return RT_OK;
+}
+
+// local planes [0, n3l) of a slab <- global planes (k0 - ext_lo + l) mod n3 of `src`, as the fewest contiguous copies
+static cudaError_t hslab_gather(const rt_ctx::HostSlab &h, int n3, double *dst, const double *src, size_t per_plane, cudaStream_t st) {
+    int l = 0;
+    while (l < h.n3l) {
+        const int g0 = ((h.k0 - h.ext_lo + l) % n3 + n3) % n3;
+        int len = 1;
+        while (l + len < h.n3l && g0 + len < n3) ++len;
+        cudaError_t e = cudaMemcpyAsync(dst + (size_t)l * per_plane, src + (size_t)g0 * per_plane, (size_t)len * per_plane * sizeof(double),
+                                        cudaMemcpyDeviceToDevice, st);
+        if (e != cudaSuccess) return e;
+        l += len;
+    }
+    return cudaSuccess;
+}
+
+// the parent's fluid state cut into the slabs' contexts (only when it changed since the last call)
+static int hslab_fluid(rt_ctx *c, cudaStream_t st) {
+    const int n3 = c->grid.n[2];
+    const size_t pc = (size_t)c->ncol;
+    for (auto &h : c->hslabs) {
+        CK(hslab_gather(h, n3, h.rho, c->d_rho, pc, st));
+        CK(hslab_gather(h, n3, h.T, c->d_T, pc, st));
+        for (int m = 0; m < 4; ++m) CK(hslab_gather(h, n3, h.u4 + (size_t)m * h.n3l * pc, c->d_u4 + (size_t)m * c->ncell, pc, st));
+        const int rc = rt_set_fluid(h.sub, h.rho, h.T, h.u4, st);
+        if (rc != RT_OK) return rc;
+    }
+    c->hslab_fluid_version = c->fluid_version;
+    return RT_OK;
+}
+
+static int step_host_pipelined(rt_ctx *c, int nslab, double *I_h, double *T_h, double *R_h, double *G_h, double dt, int *n_fail_h, cudaStream_t cur) {
+    const int n3 = c->grid.n[2];
+    const size_t pc = (size_t)c->ncol, pi = pc * c->pitch;
+    const size_t nI = (size_t)c->ncell * c->pitch * sizeof(double), nC = (size_t)c->ncell * sizeof(double);
+    if (c->hslabs.empty()) {
+        if (!c->d_hI) {
+            CK(cudaMalloc((void **)&c->d_hI, nI));
+            CK(cudaMalloc((void **)&c->d_hT, nC));
+            CK(cudaMalloc((void **)&c->d_hfail, sizeof(int)));
+        }
+        CK(cudaStreamCreateWithFlags(&c->hs_in, cudaStreamNonBlocking));
+        CK(cudaStreamCreateWithFlags(&c->hs_cmp, cudaStreamNonBlocking));
+        CK(cudaStreamCreateWithFlags(&c->hs_out, cudaStreamNonBlocking));
+        CK(cudaEventCreateWithFlags(&c->hev_start, cudaEventDisableTiming));
+        for (int q = 0; q < 3; ++q) CK(cudaEventCreateWithFlags(&c->hev_end[q], cudaEventDisableTiming));
+        const int rc = hslab_build(c, nslab);
+        if (rc != RT_OK) return rc;
+    }
+    CK(cudaEventRecord(c->hev_start, cur));
+    CK(cudaStreamWaitEvent(c->hs_in, c->hev_start, 0));
+    CK(cudaStreamWaitEvent(c->hs_cmp, c->hev_start, 0));
+    CK(cudaStreamWaitEvent(c->hs_out, c->hev_start, 0));
+    if (c->hslab_fluid_version != c->fluid_version) {
+        const int rc = hslab_fluid(c, c->hs_cmp);
+        if (rc != RT_OK) return rc;
+    }
+    CK(cudaMemsetAsync(c->d_hfail, 0, sizeof(int), c->hs_cmp));
+    // upload order: what slab 0 needs first (under a periodic x3 its lower halo is the top of the mesh), then upwards,
+    // in chunks of a slab's worth of planes so that the first slab can start early
+    const bool per = c->grid.bc_lo[2] == RT_BC_PERIODIC;
+    const int chunk = (n3 + nslab - 1) / nslab;
+    std::vector<int> arrival(n3, -1);
+    int nchunk = 0;
+    auto upload = [&](int a, int b) -> cudaError_t {
+        cudaError_t e = cudaMemcpyAsync(c->d_hI + (size_t)a * pi, I_h + (size_t)a * pi, (size_t)(b - a) * pi * sizeof(double), cudaMemcpyHostToDevice, c->hs_in);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(c->d_hT + (size_t)a * pc, T_h + (size_t)a * pc, (size_t)(b - a) * pc * sizeof(double), cudaMemcpyHostToDevice, c->hs_in);
+        if (e != cudaSuccess) return e;
+        if ((int)c->hev.size() <= nchunk) {
+            cudaEvent_t ev;
+            e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+            if (e != cudaSuccess) return e;
+            c->hev.push_back(ev);
+        }
+        e = cudaEventRecord(c->hev[nchunk], c->hs_in);
+        for (int q = a; q < b; ++q) arrival[q] = nchunk;
+        ++nchunk;
+        return e;
+    };
+    const int top = per ? n3 - HS_MARGIN : n3;
+    if (per) CK(upload(top, n3));
+    for (int a = 0; a < top; a += chunk) CK(upload(a, a + chunk < top ? a + chunk : top));
+    for (auto &h : c->hslabs) {
+        int need = 0;
+        for (int l = 0; l < h.n3l; ++l) {
+            const int g = ((h.k0 - h.ext_lo + l) % n3 + n3) % n3;
+            if (arrival[g] > need) need = arrival[g];
+        }
+        CK(cudaStreamWaitEvent(c->hs_cmp, c->hev[need], 0));
+        CK(hslab_gather(h, n3, h.I, c->d_hI, pi, c->hs_cmp));
+        CK(hslab_gather(h, n3, h.T, c->d_hT, pc, c->hs_cmp));
+        const long long l0 = h.sub->launches;
+        const int rc = rt_step(h.sub, h.I, h.T, R_h ? h.R : nullptr, G_h ? h.G : nullptr, dt, c->d_hfail, c->hs_cmp);
+        if (rc != RT_OK) return rc;
+        c->launches += h.sub->launches - l0;
+        CK(cudaEventRecord(h.done, c->hs_cmp));
+        CK(cudaStreamWaitEvent(c->hs_out, h.done, 0));
+        const int own = h.k1 - h.k0;
+        CK(cudaMemcpyAsync(I_h + (size_t)h.k0 * pi, h.I + (size_t)h.ext_lo * pi, (size_t)own * pi * sizeof(double), cudaMemcpyDeviceToHost, c->hs_out));
+        CK(cudaMemcpyAsync(T_h + (size_t)h.k0 * pc, h.T + (size_t)h.ext_lo * pc, (size_t)own * pc * sizeof(double), cudaMemcpyDeviceToHost, c->hs_out));
+        const size_t lc = (size_t)h.n3l * pc;
+        if (R_h) for (int m = 0; m < 16; ++m)
+            CK(cudaMemcpyAsync(R_h + (size_t)m * c->ncell + (size_t)h.k0 * pc, h.R + m * lc + (size_t)h.ext_lo * pc, (size_t)own * pc * sizeof(double), cudaMemcpyDeviceToHost, c->hs_out));
+        if (G_h) for (int m = 0; m < 4; ++m)
+            CK(cudaMemcpyAsync(G_h + (size_t)m * c->ncell + (size_t)h.k0 * pc, h.G + m * lc + (size_t)h.ext_lo * pc, (size_t)own * pc * sizeof(double), cudaMemcpyDeviceToHost, c->hs_out));
+    }
+    if (n_fail_h) CK(cudaMemcpyAsync(n_fail_h, c->d_hfail, sizeof(int), cudaMemcpyDeviceToHost, c->hs_cmp));
+    cudaStream_t ss[3] = {c->hs_in, c->hs_cmp, c->hs_out};
+    for (int q = 0; q < 3; ++q) {
+        CK(cudaEventRecord(c->hev_end[q], ss[q]));
+        CK(cudaStreamWaitEvent(cur, c->hev_end[q], 0));
+    }
+    CK(cudaStreamSynchronize(cur));
+    return RT_OK;
+}
+
+extern "C" int rt_step_host(rt_ctx *c, double *I_h, double *T_h, double *R_h, double *G_h, double dt, int *n_fail_h, void *stream) {
+    if (!c || !I_h || !T_h) return RT_EINVAL;
+    if (!c->fluid_set || fixed_bc_missing(c)) return RT_ESTATE;
+    const int n3 = c->grid.n[2];
+    bool fixed = false;
+    for (int a = 0; a < 3; ++a) fixed = fixed || c->grid.bc_lo[a] == RT_BC_FIXED || c->grid.bc_hi[a] == RT_BC_FIXED;
+    const int nslab = n3 / 8;   // slabs of >= 8 owned planes: at most 8 / 8 redundant planes of compute
+    if (nslab < 2 || fixed || c->is_sub) return step_host_simple(c, I_h, T_h, R_h, G_h, dt, n_fail_h, stream);
+    return step_host_pipelined(c, nslab, I_h, T_h, R_h, G_h, dt, n_fail_h, (cudaStream_t)stream);
 }
