@@ -32,6 +32,7 @@ extern "C" {
 #define RT_ECUDA (-2)   /* a CUDA runtime call failed (rt_last_cuda_error() has the code) */
 #define RT_ENOMEM (-3)
 #define RT_ESTATE (-4)  /* call order: fluid / boundary not set */
+#define RT_ETOOBIG (-5) /* rt_transport_static: the mesh needs more scratch than RT_STATIC_SCRATCH_BYTES */
 
 enum { RT_BC_PERIODIC = 0, RT_BC_OUTFLOW = 1, RT_BC_ZERO = 2, RT_BC_FIXED = 3,
        RT_BC_REFLECT = 4 /* "symmetric" boundary (L709, DESIGN S23): ghost = mirror-image cell read in the direction with the
@@ -125,6 +126,17 @@ int rt_set_fluid(rt_ctx *ctx, const double *rho_dev, const double *T_dev, const 
 /* I_out = (n^0 n_0 I_base - dt D_x[I_in]) / (n^0 n_0), then mask + zero bands (O3 + O5).  I_out may alias I_base
  * but not I_in.  I_base may equal I_in. */
 int rt_transport(rt_ctx *ctx, const double *I_in_dev, const double *I_base_dev, double *I_out_dev, double dt, void *stream);
+/* rt_transport for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): same arguments, same result bit for bit, but the scratch of the launch (the per-face coefficients of Eq 23 and
+ * the column / cell flags; rt_transport keeps them in buffers rt_init allocated) lives in ONE file-scope device array of
+ * RT_STATIC_SCRATCH_BYTES that every GPU loading the library holds until exit.  The call makes no cudaMalloc, cudaFree or
+ * allocating library call (its first use on a device resolves the array's address with cudaGetSymbolAddress).  A mesh whose
+ * faces need more (32 bytes per face of the three dims + the flag words; about 85 000 cells fit) is refused with RT_ETOOBIG;
+ * without opacities no scratch is needed and any mesh is accepted.  The array is shared by all contexts and keeps the last
+ * call's contents (every entry that is read is rewritten first, nothing needs clearing): calls that OVERLAP on the GPU --
+ * different streams without ordering, different contexts -- race on it; serialise them. */
+#define RT_STATIC_SCRATCH_BYTES (8u << 20)
+int rt_transport_static(rt_ctx *ctx, const double *I_in_dev, const double *I_base_dev, double *I_out_dev, double dt, void *stream);
 /* I_inout -= dt D_Omega[I_in] / (n^0 n_0), then mask + zero bands (O4 + O5).  No-op when omega = 0. */
 int rt_angular_flux(rt_ctx *ctx, const double *I_in_dev, double *I_inout_dev, double dt, void *stream);
 /* Implicit source step O6 in place on (I, T); *n_fail_dev (device int, may be NULL) += cells whose solve failed. */

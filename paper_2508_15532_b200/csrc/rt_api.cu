@@ -412,6 +412,7 @@ extern "C" const char *rt_strerror(int code) {
         case RT_ECUDA: return "CUDA runtime error (see rt_last_cuda_error)";
         case RT_ENOMEM: return "out of memory";
         case RT_ESTATE: return "call order: fluid or boundary data not set";
+        case RT_ETOOBIG: return "mesh too large for the static scratch array (RT_STATIC_SCRATCH_BYTES)";
         default: return "unknown error";
     }
 }
@@ -568,6 +569,14 @@ extern "C" int rt_transport(rt_ctx *c, const double *I_in, const double *I_base,
     cudaStream_t st = (cudaStream_t)stream;
     if (c->matter) { ProfScope ps(c, RT_K_FACECOEF, st); CK(launch_facecoef(c->kp, c->d_T, dt, c->d_fcoef, c->d_colflag, st, &c->launches)); }
     { ProfScope ps(c, RT_K_TRANSPORT, st); CK(launch_transport(c->kp, I_in, I_base, I_out, c->d_fcoef, c->d_colflag, c->matter, dt, st, &c->launches)); }
+    return RT_OK;
+}
+
+extern "C" int rt_transport_static(rt_ctx *c, const double *I_in, const double *I_base, double *I_out, double dt, void *stream) {
+    if (!c || !I_in || !I_base || !I_out || I_in == I_out) return RT_EINVAL;
+    if (fixed_bc_missing(c) || (c->matter && !c->fluid_set)) return RT_ESTATE;
+    if (transport_static_bytes(c->kp, c->matter) > RT_STATIC_SCRATCH_BYTES) return RT_ETOOBIG;
+    CK(launch_transport_static(c->kp, c->d_T, I_in, I_base, I_out, c->matter, dt, (cudaStream_t)stream, &c->launches));
     return RT_OK;
 }
 

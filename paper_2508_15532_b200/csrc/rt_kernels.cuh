@@ -72,6 +72,10 @@ bool tile_eligible(const KParams &p);
 cudaError_t launch_paircoef(const KParams &p, double *out, cudaStream_t st);
 cudaError_t launch_transport_tile(const KParams &p, const int tile[3], const double *I_in, const double *I_base, double *I_out,
                                   const unsigned char *colflag, bool matter, double dt, cudaStream_t st, long long *launches);
+// rt_transport.cu: the transport launch with its scratch in a file-scope device array (rt_transport_static)
+size_t transport_static_bytes(const KParams &p, bool matter);
+cudaError_t launch_transport_static(const KParams &p, const double *T, const double *I_in, const double *I_base, double *I_out,
+                                    bool matter, double dt, cudaStream_t st, long long *launches);
 cudaError_t launch_angular_mapr(const KParams &p, const double *I_in, double *I_io, double dt, cudaStream_t st, long long *launches);
 cudaError_t launch_classify(const KParams &p, unsigned char *cls, cudaStream_t st);
 cudaError_t launch_angular(const KParams &p, const double *I_in, double *I_io, double dt, cudaStream_t st, long long *launches);

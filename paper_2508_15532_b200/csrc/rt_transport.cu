@@ -478,6 +478,63 @@ cudaError_t launch_transport(const KParams &p, const double *I_in, const double 
     return cudaGetLastError();
 }
 
+// ---- rt_transport_static: the transport launch with its per-stage scratch in a file-scope device array ------------------
+// For callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops).  The scratch of one transport launch --
+// the per-face coefficients of Eq 23 for the three dims and the column / cell flags -- lives in this array instead of the
+// context's cudaMalloc'ed buffers.  Every GPU that loads the library holds RT_STATIC_SCRATCH_BYTES until exit.  All calls
+// share it and it keeps the last call's contents: k_facecoef and k_colflag overwrite every entry the transport kernels read
+// (nothing has to start at zero), and two calls that overlap on the GPU (different streams, no ordering) race on it.
+static __device__ __align__(256) unsigned char g_static_scratch[RT_STATIC_SCRATCH_BYTES];
+
+// In host code `g_static_scratch` is a host-side stand-in, not a device address: the address the kernels get comes from
+// cudaGetSymbolAddress, resolved once per device with that device current.
+static cudaError_t static_scratch_ptr(unsigned char **out) {
+    static unsigned char *cache[64] = {nullptr};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    if (!cache[dev]) {
+        void *q = nullptr;
+        e = cudaGetSymbolAddress(&q, g_static_scratch);
+        if (e != cudaSuccess) return e;
+        cache[dev] = static_cast<unsigned char *>(q);
+    }
+    *out = cache[dev];
+    return cudaSuccess;
+}
+
+static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
+size_t transport_static_bytes(const KParams &p, bool matter) {
+    if (!matter) return 0;
+    size_t need = 0;
+    for (int a = 0; a < 3; ++a) need += align256((size_t)(p.n1 + (a == 0)) * (p.n2 + (a == 1)) * (p.n3 + (a == 2)) * sizeof(double4));
+    return need + align256(colflag_bytes(p.ncol, p.n3));
+}
+
+// cudaErrorMemoryValueTooLarge: the mesh needs more scratch than the array holds.  No cudaMalloc / cudaFree / allocating
+// library call on this path.
+cudaError_t launch_transport_static(const KParams &p, const double *T, const double *I_in, const double *I_base, double *I_out,
+                                    bool matter, double dt, cudaStream_t st, long long *launches) {
+    if (transport_static_bytes(p, matter) > RT_STATIC_SCRATCH_BYTES) return cudaErrorMemoryValueTooLarge;
+    double *fcoef[3] = {nullptr, nullptr, nullptr};
+    unsigned char *colflag = nullptr;
+    if (matter) {
+        unsigned char *base = nullptr;
+        cudaError_t e = static_scratch_ptr(&base);
+        if (e != cudaSuccess) return e;
+        size_t off = 0;
+        for (int a = 0; a < 3; ++a) {
+            fcoef[a] = reinterpret_cast<double *>(base + off);
+            off += align256((size_t)(p.n1 + (a == 0)) * (p.n2 + (a == 1)) * (p.n3 + (a == 2)) * sizeof(double4));
+        }
+        colflag = base + off;
+        e = launch_facecoef(p, T, dt, fcoef, colflag, st, launches);
+        if (e != cudaSuccess) return e;
+    }
+    return launch_transport(p, I_in, I_base, I_out, fcoef, colflag, matter, dt, st, launches);
+}
+
 cudaError_t launch_classify(const KParams &p, unsigned char *cls, cudaStream_t st) {
     dim3 grid((p.n1 * p.pitch + 255) / 256, p.n2);
     k_classify<<<grid, 256, 0, st>>>(p, cls);

@@ -16,7 +16,7 @@ BC = {"periodic": 0, "outflow": 1, "zero": 2, "fixed": 3, "reflect": 4}
 METRIC = {"minkowski": 0, "mink_cyl": 1, "ks_mks": 2, "snake": 3}
 GEOM = dict(g_c=0, e_c=1, einv_c=2, sqrtg_c=3, omega_c=4, n0_c=5, angcoef=6)
 SYMBOLS = ["rt_init", "rt_free", "rt_ndir", "rt_ndir_padded", "rt_get_directions", "rt_get_geometry", "rt_cfl_dt",
-           "rt_set_boundary", "rt_set_fluid", "rt_transport", "rt_angular_flux", "rt_source_implicit", "rt_moments",
+           "rt_set_boundary", "rt_set_fluid", "rt_transport", "rt_transport_static", "rt_angular_flux", "rt_source_implicit", "rt_moments",
            "rt_step", "rt_step_host", "rt_profile_enable", "rt_profile_read", "rt_transport_info", "rt_launch_count", "rt_last_cuda_error", "rt_strerror"]
 
 
@@ -55,6 +55,7 @@ def load_library(path=LIB_PATH):
     lib.rt_set_boundary.argtypes = [vp, ci, ci, vp]
     lib.rt_set_fluid.argtypes = [vp, vp, vp, vp, vp]
     lib.rt_transport.argtypes = [vp, vp, vp, vp, dbl, vp]
+    lib.rt_transport_static.argtypes = [vp, vp, vp, vp, dbl, vp]
     lib.rt_angular_flux.argtypes = [vp, vp, vp, dbl, vp]
     lib.rt_source_implicit.argtypes = [vp, vp, vp, dbl, vp, vp]
     lib.rt_moments.argtypes = [vp, vp, vp, vp]
@@ -186,6 +187,10 @@ class RtContext:
 
     def transport(self, I_in, I_base, I_out, dt):
         _check(lib().rt_transport(self._h, _ptr(I_in), _ptr(I_base), _ptr(I_out), float(dt), _stream()))
+
+    def transport_static(self, I_in, I_base, I_out, dt):
+        """rt_transport_static: rt_transport without any allocation (scratch in a static device array; RT_ETOOBIG beyond it)."""
+        _check(lib().rt_transport_static(self._h, _ptr(I_in), _ptr(I_base), _ptr(I_out), float(dt), _stream()))
 
     def angular_flux(self, I_in, I_inout, dt):
         _check(lib().rt_angular_flux(self._h, _ptr(I_in), _ptr(I_inout), float(dt), _stream()))
