@@ -1,4 +1,5 @@
 // C ABI of librt_b200 (include/rt.h): context, init-time precompute (a0), and the rt_* entry points.
+#include <climits>
 #include <cmath>
 #include <cstring>
 #include <limits>
@@ -117,6 +118,9 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     const int n1 = grid->n[0], n2 = grid->n[1], n3 = grid->n[2];
     const int ncol = c->ncol = n1 * n2;
     c->ncell = (long long)ncol * n3;
+    // limits of the kernels (32-bit element offsets inside an x3-plane and cell indices in the lists; one thread per
+    // direction in the angular kernels; at most 21 values per lane in the per-cell kernels): refused here, not at the first step
+    if ((long long)n1 * n2 > INT_MAX || nd > 672 || pitch > 1024 || c->ncell > INT_MAX || (long long)ncol * pitch > INT_MAX) { delete c; return RT_EINVAL; }
     c->matter = (opt->kappa_a0 != 0.0 || opt->kappa_s != 0.0);
     const double x3c = grid->x0[2] + 0.5 * grid->dx[2];
 
@@ -530,11 +534,17 @@ extern "C" int rt_set_fluid(rt_ctx *c, const double *rho, const double *T, const
             const int n = (int)c->ncell;
             cub::CountingInputIterator<int> idx(0);
             AboveFloor sel{c->d_rho, c->opt.rho_floor};
-            if (!c->d_srclist) {
-                CK(cudaMalloc((void **)&c->d_srclist, (size_t)n * sizeof(int)));
-                CK(cudaMalloc((void **)&c->d_nsel, sizeof(int)));
-                CK(cub::DevicePartition::If(nullptr, c->part_tmp_bytes, idx, c->d_srclist, c->d_nsel, n, sel, st));
-                CK(cudaMalloc(&c->d_part_tmp, c->part_tmp_bytes ? c->part_tmp_bytes : 1));
+            if (!c->d_part_tmp) {   // first use; on any failure nothing half-allocated is left behind
+                cudaError_t e = cudaMalloc((void **)&c->d_srclist, (size_t)n * sizeof(int));
+                if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_nsel, sizeof(int));
+                if (e == cudaSuccess) e = cub::DevicePartition::If(nullptr, c->part_tmp_bytes, idx, c->d_srclist, c->d_nsel, n, sel, st);
+                if (e == cudaSuccess) e = cudaMalloc(&c->d_part_tmp, c->part_tmp_bytes ? c->part_tmp_bytes : 1);
+                if (e != cudaSuccess) {
+                    cudaFree(c->d_srclist); cudaFree(c->d_nsel);
+                    c->d_srclist = nullptr; c->d_nsel = nullptr; c->d_part_tmp = nullptr;
+                    g_last_cuda = (int)e;
+                    return e == cudaErrorMemoryAllocation ? RT_ENOMEM : RT_ECUDA;
+                }
             }
             size_t tmp = c->part_tmp_bytes;
             CK(cub::DevicePartition::If(c->d_part_tmp, tmp, idx, c->d_srclist, c->d_nsel, n, sel, st));

@@ -51,10 +51,11 @@ struct KParams {
     int nvac;
 };
 
-// Layout of the column-flag buffer: [ncol] column flags, [ceil(n3/8)][ncol] x3-chunk flags, then (4-byte aligned)
+// Layout of the column-flag buffer: [ncol] column flags, then (4-byte aligned)
 // [ceil(n3/32)][ncol] 32-bit cell-flag masks (see k_colflag).
 __host__ __device__ inline size_t colmask_offset(int ncol, int n3) {
-    return (((size_t)ncol * (1 + (n3 + 7) / 8)) + 3) & ~(size_t)3;
+    (void)n3;
+    return ((size_t)ncol + 3) & ~(size_t)3;
 }
 __host__ __device__ inline size_t colflag_bytes(int ncol, int n3) {
     return colmask_offset(ncol, n3) + sizeof(unsigned) * (size_t)ncol * ((n3 + 31) / 32);

@@ -54,11 +54,9 @@ __global__ void k_facecoef(KParams p, const double *__restrict__ T, double dt, i
 
 
 // column flags: bit 0 = the column has a cell with a non-vacuum face, bit 1 = it has an all-vacuum cell
-// colflag[ncol + kc * ncol + col]: the x3 chunk [kc*GEN_KC, (kc+1)*GEN_KC) of the column has such a cell
 // column masks (32-bit words behind the flags, colmask_offset()): bit (k & 31) of word [(k >> 5) * ncol + col] = cell
 // flag of (col, k).  The marching kernels test a bit per step and load one word per 32 steps: a per-step flag load sat
 // in front of every step's branch and exposed its L2 latency (it was 70 % of the vacuum kernel's long-scoreboard stalls).
-constexpr int GEN_KC = 8;
 // One warp per column, lane = x3 index within a 32-cell word: the cell flags (any of the six faces non-vacuum) are formed
 // from the face coefficients and go straight into the ballot that makes the mask word; no per-cell flag array.
 __global__ void k_colflag(KParams p, const double4 *__restrict__ fc0, const double4 *__restrict__ fc1,
@@ -81,9 +79,6 @@ __global__ void k_colflag(KParams p, const double4 *__restrict__ fc0, const doub
         if (mw) m |= 1;
         if (valid & ~mw) m |= 2;
         if (lane == 0) cmask[(long long)(k0 >> 5) * p.ncol + col] = mw;
-        const int kc = (k0 / GEN_KC) + lane;   // lanes 0..3: the four x3 chunks of this word
-        if (lane < 32 / GEN_KC && kc * GEN_KC < p.n3)
-            colflag[p.ncol + (long long)kc * p.ncol + col] = ((mw >> (GEN_KC * lane)) & ((1u << GEN_KC) - 1u)) ? 1 : 0;
     }
     if (lane == 0) colflag[col] = (unsigned char)m;
 }

@@ -148,7 +148,14 @@ class SlabDomain:
         cut4 = (lambda a: a) if local else (lambda a: a[:, L.planes])
         rho, T = np.ascontiguousarray(cut(f["rho"])), np.ascontiguousarray(cut(f["T"]))
         u4 = None if f.get("u4") is None else torch.as_tensor(np.ascontiguousarray(cut4(f["u4"])), device=dev)
-        self.ctx.set_fluid(torch.as_tensor(rho, device=dev), torch.as_tensor(T, device=dev), u4)
+        rho_d, T_d = torch.as_tensor(rho, device=dev), torch.as_tensor(T, device=dev)
+        if local and L.world > 1:
+            # locally generated fields: the margins of the FLUID arrays must hold the neighbours' owned planes as well (they
+            # enter the face opacities and the source step of the margin cells, whose influence reaches owned planes)
+            comps = [] if u4 is None else [u4[m] for m in range(4)]
+            self._exchange(L, [rho_d, T_d] + comps, self.group)
+            T = T_d.cpu().numpy()
+        self.ctx.set_fluid(rho_d, T_d, u4)
         if state:   # (state=False: fluid and boundary data only; the caller owns I and T)
             self.I = self.ctx.to_device(np.ascontiguousarray(cut(f["I0"])))
             self.T = torch.as_tensor(T, device=dev).clone()
