@@ -39,7 +39,9 @@ enum { RT_BC_PERIODIC = 0, RT_BC_OUTFLOW = 1, RT_BC_ZERO = 2, RT_BC_FIXED = 3,
                             normal tetrad component flipped, normal fluid velocity reversed.  Only on x^2 boundaries: the
                             geodesic grid (pole along 3-hat, a vertex at azimuth 0) is mirror symmetric across 2-hat
                             only; rt_init returns RT_EINVAL for the other dims */ };
-enum { RT_MINKOWSKI_CART = 0, RT_MINK_CYL_TETRAD = 1, RT_KS_MKS = 2, RT_SNAKE = 3 };
+enum { RT_MINKOWSKI_CART = 0, RT_MINK_CYL_TETRAD = 1, RT_KS_MKS = 2, RT_SNAKE = 3,
+       RT_BL_MKS = 4 /* Boyer-Lindquist, same logical map as RT_KS_MKS, zero-angular-momentum tetrad (photon-orbit test, L563-592);
+                        the mesh must stay outside the horizon */ };
 enum { RT_LIM_MC = 0, RT_LIM_MINMOD = 1, RT_LIM_VANLEER = 2, RT_LIM_NONE = 3 };
 enum { RT_ANG_DONOR = 0, RT_ANG_MAPR = 1 };
 /* how the vacuum (Eq 20) spatial transport gets its stencil operands.  RT_TRANSPORT_TMA (default): a CTA owns a tile of
@@ -73,8 +75,8 @@ typedef struct {
 /* Metric + tetrad (L57-79, App. A).  x3_symmetric: geometry independent of x^3 (tables stored per (x1,x2) column,
  * the paper's own optimisation, L776); required for RT_KS_MKS, ignored (constant geometry) for RT_MINKOWSKI_CART. */
 typedef struct {
-    int kind;         /* RT_MINKOWSKI_CART | RT_MINK_CYL_TETRAD | RT_KS_MKS | RT_SNAKE */
-    double a, hslope; /* RT_KS_MKS: spin, theta-map parameter h: r = exp(x1), theta = pi x2 + (1-h)/2 sin(2 pi x2), phi = x3 */
+    int kind;         /* RT_MINKOWSKI_CART | RT_MINK_CYL_TETRAD | RT_KS_MKS | RT_SNAKE | RT_BL_MKS */
+    double a, hslope; /* RT_KS_MKS, RT_BL_MKS: spin, theta-map parameter h: r = exp(x1), theta = pi x2 + (1-h)/2 sin(2 pi x2), phi = x3 */
     int x3_symmetric;
     double snake_A, snake_k; /* RT_SNAKE (App A.1): flat space in (t, w, y, z), w = x - A sin(k pi y); metric Eq A1,
                                 Cartesian-aligned tetrad (Eq A2 read as the co-frame, DESIGN S27): omega = 0, n^w = n^x - delta n^y */

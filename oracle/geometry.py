@@ -16,6 +16,13 @@ Metric kinds
                theta = pi x2 + (1-h)/2 sin(2 pi x2), phi = x3 (S26).  Tetrad = A3-A4 with reading S25:
                alpha is the LAPSE (1+2r/Sigma)^(-1/2) (A5b prints its inverse; A4a and Eq 4 need the lapse),
                gamma^{ij} is the INVERSE of the 3-metric gamma_ij = g_ij (A5d as printed gives a non-unit e_r).
+  'bl_mks'     Boyer-Lindquist (t, r, theta, phi), mass 1, spin a, same logical map as 'ks_mks'; the coordinates of the
+               photon-orbit test (section 4.7: "non-horizon-penetrating coordinates ..., namely Boyer-Lindquist"; App A,
+               L816, names Kerr-Schild for the same test -- the body text is followed: only in the frame of the
+               zero-angular-momentum observers, the tetrad whose e_0 is normal to t = const (Eq 4), does a circular photon
+               orbit point exactly along phi-hat, the grid's pole, L590).  Tetrad in closed form: e_t = (1/alpha)(d_t + w d_phi),
+               e_r = sqrt(Delta/Sigma) d_r, e_theta = d_theta / sqrt(Sigma), e_phi = d_phi / sqrt(g_phiphi), with
+               alpha^2 = Sigma Delta / A, w = 2 a r / A, A = (r^2+a^2)^2 - a^2 Delta sin^2 theta.  Outside the horizon only.
   'snake'      flat space in snake coordinates (t, w, y, z), w = x - A sin(k pi y) (App A.1): metric A1
                with delta = A k pi cos(k pi y); tetrad A2 under reading S27: the printed matrix is the CO-frame
                e^{a-hat}_mu = [[1,0,0,0],[0,1,delta,0],[0,0,1,0],[0,0,0,1]] (rows dt, dx = dw + delta dy, dy, dz) with
@@ -54,6 +61,21 @@ def _ks_metric_phys(a, r, th):
     return g, Sig, H
 
 
+def _bl_metric_phys(a, r, th):
+    """Boyer-Lindquist covariant metric in (t, r, theta, phi), M = 1; also Sigma, Delta, A."""
+    s2 = np.sin(th) ** 2
+    Sig = r * r + a * a * np.cos(th) ** 2
+    Del = r * r - 2.0 * r + a * a
+    A = (r * r + a * a) ** 2 - a * a * Del * s2
+    g = np.zeros(r.shape + (4, 4))
+    g[..., 0, 0] = -(1.0 - 2.0 * r / Sig)
+    g[..., 0, 3] = g[..., 3, 0] = -2.0 * a * r * s2 / Sig
+    g[..., 1, 1] = Sig / Del
+    g[..., 2, 2] = Sig
+    g[..., 3, 3] = A * s2 / Sig
+    return g, Sig, Del, A
+
+
 def _snake_delta(params, X):
     """delta = A k pi cos(k pi y) (below Eq A1); y is the second logical coordinate."""
     A, k = params["A"], params["k"]
@@ -72,9 +94,9 @@ def metric(kind, params, X):
         g[..., 2, 1] = d
         g[..., 2, 2] = 1.0 + d * d
         return g
-    if kind == "ks_mks":
+    if kind in ("ks_mks", "bl_mks"):
         r, th, drdx, dthdx = _ks_map(params, X)
-        g, _, _ = _ks_metric_phys(params["a"], r, th)
+        g = _ks_metric_phys(params["a"], r, th)[0] if kind == "ks_mks" else _bl_metric_phys(params["a"], r, th)[0]
         J = np.ones(r.shape + (4,))
         J[..., 1] = drdx
         J[..., 2] = dthdx
@@ -106,6 +128,27 @@ def tetrad(kind, params, X):
         einv = np.broadcast_to(np.eye(4), shp + (4, 4)).copy()   # Eq A2 read as the co-frame (S27)
         einv[..., 1, 2] = d
         return np.linalg.inv(einv), einv
+    if kind == "bl_mks":
+        r, th, drdx, dthdx = _ks_map(params, X)
+        a = params["a"]
+        g, Sig, Del, A = _bl_metric_phys(a, r, th)
+        alpha = np.sqrt(Sig * Del / A)          # lapse of the t = const slices
+        w = 2.0 * a * r / A                     # frame dragging: the ZAMO's d phi / d t
+        e = np.zeros(shp + (4, 4))
+        einv = np.zeros(shp + (4, 4))
+        with np.errstate(divide="ignore", invalid="ignore"):
+            gpp = np.sqrt(g[..., 3, 3])
+            e[..., 0, 0] = 1.0 / alpha
+            e[..., 3, 0] = w / alpha
+            e[..., 1, 1] = np.sqrt(Del / Sig) / drdx
+            e[..., 2, 2] = 1.0 / np.sqrt(Sig) / dthdx
+            e[..., 3, 3] = 1.0 / gpp
+            einv[..., 0, 0] = alpha
+            einv[..., 1, 1] = np.sqrt(Sig / Del) * drdx
+            einv[..., 2, 2] = np.sqrt(Sig) * dthdx
+            einv[..., 3, 0] = -w * gpp
+            einv[..., 3, 3] = gpp
+        return e, einv
     if kind == "ks_mks":
         r, th, drdx, dthdx = _ks_map(params, X)
         g, Sig, H = _ks_metric_phys(params["a"], r, th)

@@ -50,7 +50,7 @@ double snake_delta(const rt_metric &mt, double y) { return mt.snake_A * mt.snake
 // covariant metric in logical coordinates
 void metric_at(const rt_metric &mt, const double x[3], double g[4][4]) {
     zero44(g);
-    if (mt.kind != RT_KS_MKS) {
+    if (mt.kind != RT_KS_MKS && mt.kind != RT_BL_MKS) {
         g[0][0] = -1; g[1][1] = g[2][2] = g[3][3] = 1;
         if (mt.kind == RT_SNAKE) {   // x = w + A sin(k pi y):  dx = dw + delta dy  =>  ds^2 = -dt^2 + (dw + delta dy)^2 + dy^2 + dz^2
             const double dl = snake_delta(mt, x[1]);
@@ -65,6 +65,15 @@ void metric_at(const rt_metric &mt, const double x[3], double g[4][4]) {
     const double J1 = r, J2 = PI + PI * (1.0 - h) * std::cos(2 * PI * x[1]);
     const double st = std::sin(th), ct = std::cos(th), s2 = st * st;
     const double Sig = r * r + a * a * ct * ct, H = 2.0 * r / Sig;
+    if (mt.kind == RT_BL_MKS) {   // Boyer-Lindquist (section 4.7); the Gram-Schmidt below gives the zero-angular-momentum frame
+        const double Del = r * r - 2.0 * r + a * a;
+        g[0][0] = -1.0 + H;
+        g[0][3] = g[3][0] = -a * H * s2;
+        g[1][1] = Sig / Del * J1 * J1;
+        g[2][2] = Sig * J2 * J2;
+        g[3][3] = s2 * (r * r + a * a + a * a * H * s2);
+        return;
+    }
     g[0][0] = -1.0 + H;
     g[0][1] = g[1][0] = H * J1;
     g[0][3] = g[3][0] = -a * H * s2;

@@ -13,7 +13,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "librt_b200.so")
 
 BC = {"periodic": 0, "outflow": 1, "zero": 2, "fixed": 3, "reflect": 4}
-METRIC = {"minkowski": 0, "mink_cyl": 1, "ks_mks": 2, "snake": 3}
+METRIC = {"minkowski": 0, "mink_cyl": 1, "ks_mks": 2, "snake": 3, "bl_mks": 4}
 GEOM = dict(g_c=0, e_c=1, einv_c=2, sqrtg_c=3, omega_c=4, n0_c=5, angcoef=6)
 SYMBOLS = ["rt_init", "rt_free", "rt_ndir", "rt_ndir_padded", "rt_get_directions", "rt_get_geometry", "rt_cfl_dt",
            "rt_set_boundary", "rt_set_fluid", "rt_transport", "rt_transport_static", "rt_angular_flux", "rt_source_implicit", "rt_moments",

@@ -15,11 +15,12 @@ import math
 
 import numpy as np
 
-FULL_SIZES = {1: (64, 64, 1), 2: (64, 64, 64), 3: (128, 128, 128), 4: (128, 96, 64), 5: (192, 128, 96), 6: (128, 128, 1)}
-LEVELS = {1: 2, 2: 4, 3: 4, 4: 4, 5: 6, 6: 4}
-NSTEPS = {1: 100, 2: 200, 3: 500, 4: 50, 5: 20, 6: 400}
+FULL_SIZES = {1: (64, 64, 1), 2: (64, 64, 64), 3: (128, 128, 128), 4: (128, 96, 64), 5: (192, 128, 96), 6: (128, 128, 1),
+              7: (512, 1, 256)}
+LEVELS = {1: 2, 2: 4, 3: 4, 4: 4, 5: 6, 6: 4, 7: 8}
+NSTEPS = {1: 100, 2: 200, 3: 500, 4: 50, 5: 20, 6: 400, 7: 1000}
 NAMES = {1: "flat_beam_2d", 2: "flat_thermal_relaxation", 3: "scattering_diffusion",
-         4: "kerr_schild_torus", 5: "coupled_accretion_step", 6: "snake_beam"}
+         4: "kerr_schild_torus", 5: "coupled_accretion_step", 6: "snake_beam", 7: "bl_photon_orbit"}
 
 
 def config(idx, n=None, level=None):
@@ -71,6 +72,19 @@ def config(idx, n=None, level=None):
         c["metric"] = ("snake", dict(A=0.1, k=2.0))
         c["options"] = dict(method=0, kappa_a0=0.0, kappa_s=0.0)
         c["dt"] = 0.2 / N      # |n^w| <= 1 + A k pi = 1.63
+    elif idx == 7:
+        # PAPER.md 4.7 (L563-592): beams on the two circular photon orbits of a Kerr hole, a = +0.5, equatorial (r, phi) mesh of
+        # 512 x 256, G3 = 642 directions with the pole along phi-hat, Boyer-Lindquist coordinates.  One x2 cell centred on the
+        # equator (theta = pi/2 at x2 = 1/2) with OUTFLOW on both sides stands for the paper's 2-D mesh; r in [2, 5] is
+        # log-spaced (outside the horizon, r_h = 1.87; the orbits sit at 2.347 and 3.532, Eq 53)
+        a = 0.5
+        x1lo, x1hi = math.log(2.0), math.log(5.0)
+        c["grid"] = dict(n=n, x0=(x1lo, 0.5 - 0.01 * n[1], 0.0), dx=((x1hi - x1lo) / n[0], 0.02, 2.0 * math.pi / n[2]),
+                         bc_lo=("outflow", "outflow", "periodic"), bc_hi=("outflow", "outflow", "periodic"), x3_symmetric=True)
+        c["metric"] = ("bl_mks", dict(a=a, hslope=0.3))
+        c["options"] = dict(method=0, kappa_a0=0.0, kappa_s=0.0)
+        c["dt"] = None
+        c["orbits"] = tuple(2.0 * (1.0 + math.cos(2.0 / 3.0 * math.acos(sg * a))) for sg in (-1.0, 1.0))   # Eq 53: co-, counter-rotating
     else:
         raise ValueError(idx)
     return c
@@ -118,6 +132,21 @@ def fields(cfg, nhat, e_c=None):
             g[:, k * n2 + j0:k * n2 + j1, s_star] = 1.0
         out["ghosts"][(0, 0)] = g
         out["beam_dir"] = s_star
+    elif idx == 7:
+        # "initializing a small strip of cells along these radii, namely in the three cells closest to the circular orbit
+        # radius" (L573): the co-rotating beam in the grid's pole direction +phi-hat (the first direction), the counter-
+        # rotating one in -phi-hat (the last), each over an arc of phi an eighth of the circle long
+        out["I0"] = np.zeros(shp + (nd,))
+        out["rho"] = np.zeros(shp)
+        out["T"] = np.ones(shp)
+        r = np.exp(ax[0])
+        arc = max(1, n3 // 8)
+        out["strips"] = []
+        for rph, s_dir, k0 in ((cfg["orbits"][0], 0, n3 // 16), (cfg["orbits"][1], nd - 1, n3 // 2)):
+            ic = int(np.argmin(np.abs(r - rph)))
+            i0, i1 = max(0, ic - 1), min(n1, ic + 2)
+            out["I0"][k0:k0 + arc, :, i0:i1, s_dir] = 1.0
+            out["strips"].append(dict(r=rph, s=s_dir, i=(i0, i1), k=(k0, k0 + arc)))
     elif idx == 2:
         out["I0"] = np.zeros(shp + (nd,))
         out["rho"] = np.ones(shp)

@@ -124,3 +124,85 @@ def test_steady_source_inverse_square_paper_setup():
     slope = float(torch.linalg.lstsq(B, mean_E.log()[:, None]).solution[0, 0])
     assert abs(slope + 2.0) < 0.08, slope
     ctx.close()
+
+
+# ---- section 4.7: beams on the circular photon orbits of a Kerr hole (L563-592, Eq 53) ---------------------------------
+def test_bl_photon_orbit_matches_the_oracle():
+    """Boyer-Lindquist metric kind (RT_BL_MKS): geometry tables of the two independent implementations (closed-form tetrad of
+    the zero-angular-momentum frame vs the library's Gram-Schmidt) and six steps of the beam set-up on a small mesh."""
+    import rt_workloads as W
+    from parity_util import make_pair, run_steps
+    cfg = W.config(7, n=(24, 1, 16), level=2)
+    orc, ctx, f, dt = make_pair(cfg)
+    for name in ("g_c", "e_c", "einv_c", "sqrtg_c"):
+        assert rel_err(ctx.geometry(name), orc.tab[name]) < 1e-13, name
+    assert rel_err(ctx.geometry("omega_c"), orc.tab["omega_c"]) < 1e-10
+    out = run_steps(orc, ctx, f, dt, 6)
+    for k in ("I", "R"):
+        assert rel_err(*out[k]) <= TOL, k
+    assert out["I"][1].max() > 0.1
+    ctx.close()
+
+
+def test_bl_photon_orbits_paper_setup_one_full_orbit():
+    """The paper's set-up (a = +0.5, 512 x 256 in (r, phi), G3 = 642 directions, pole along phi-hat, strips three cells wide
+    on the radii of Eq 53) followed for one full co-rotating orbit, T = 2 pi (a + r1^{3/2}) = 25.7 M (3700 steps).  Both beams
+    must keep circling at the geodesic angular velocity Omega = 1 / (a +- r^{3/2}) on their radius: "a circular component
+    traveling around the black hole as expected" (L586).  The orbits are unstable ("the portions of the beam inside the
+    circular orbit radius fall inwards, and those outside ... escape outwards"), so a little energy leaks from the packet."""
+    import math
+    import torch
+    import rt_workloads as W
+    from paper_2508_15532_b200 import rt
+    cfg = W.config(7)
+    n1, _, n3 = cfg["grid"]["n"]
+    kind, params = cfg["metric"]
+    ctx = rt.RtContext(cfg["grid"], kind, params, cfg["level"], cfg["options"])
+    assert ctx.nd == 642
+    f = W.fields(cfg, ctx.directions()["nhat"], ctx.geometry("e_c"))
+    dev = ctx.device
+    ctx.set_fluid(torch.as_tensor(f["rho"], device=dev), torch.as_tensor(f["T"], device=dev), None)
+    dt = min(ctx.cfl_dt())
+    I = ctx.to_device(f["I0"]); T = torch.as_tensor(f["T"], device=dev).clone()
+    R = torch.zeros((16,) + ctx.shape, dtype=torch.float64, device=dev)
+    a = params["a"]
+    dx1, dx3 = cfg["grid"]["dx"][0], cfg["grid"]["dx"][2]
+    r = np.exp(cfg["grid"]["x0"][0] + dx1 * (np.arange(n1) + 0.5))
+    phi = dx3 * (np.arange(n3) + 0.5)
+    r1, r2 = cfg["orbits"]
+    assert abs(r1 - 2.3473) < 1e-4 and abs(r2 - 3.5321) < 1e-4              # Eq 53 (the paper prints 2.34, 3.53)
+    period = 2 * math.pi * (a + r1 ** 1.5)
+    ctx.step(I, T, 0.0 * dt, R, None)                                       # moments of the initial state
+    E0 = -R[0].cpu().numpy()[:, 0, :]
+
+    def packet(E, st, t):
+        sg = 1.0 if st["s"] == 0 else -1.0
+        Om = 1.0 / (a + sg * st["r"] ** 1.5)                                # d phi / d t of the circular photon orbit
+        phic = (0.5 * (phi[st["k"][0]] + phi[st["k"][1] - 1]) + Om * t) % (2 * math.pi)
+        dphi = (phi - phic + math.pi) % (2 * math.pi) - math.pi
+        win, band = np.abs(dphi) < 0.6, np.abs(r - st["r"]) < 0.6
+        Ew = E[win][:, band]
+        rc = (Ew.sum(0) * r[band]).sum() / Ew.sum()
+        pc = (Ew.sum(1) * dphi[win]).sum() / Ew.sum()
+        ipk = np.unravel_index(np.argmax(Ew), Ew.shape)
+        return Ew.sum(), (rc - st["r"]) / (st["r"] * dx1), pc / dx3, r[band][ipk[1]]
+
+    e_start = [packet(E0, st, 0.0)[0] for st in f["strips"]]
+    t, nst = 0.0, int(math.ceil(period / dt))
+    for q in range(4):
+        for _ in range(nst // 4):
+            ctx.step(I, T, dt, R, None)
+        t += dt * (nst // 4)
+        torch.cuda.synchronize()
+        E = -R[0].cpu().numpy()[:, 0, :]
+        assert np.isfinite(E).all()
+        for st, e0 in zip(f["strips"], e_start):
+            e, roff, poff, rpk = packet(E, st, t)
+            cell = st["r"] * dx1
+            print("t = %.2f  orbit r = %.4f: packet energy %.3f of start, r-centroid %+.2f cells, phi %+.2f cells, peak at r = %.4f"
+                  % (t, st["r"], e / e0, roff, poff, rpk))
+            assert abs(rpk - st["r"]) < 1.5 * cell                          # the crest stays on the circle of Eq 53
+            assert abs(roff) < 2.5 and abs(poff) < 1.5                      # ... and moves at the geodesic angular velocity
+            assert e > 0.85 * e0
+    assert float(I.min()) > -1e-12
+    ctx.close()

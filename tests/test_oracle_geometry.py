@@ -1,4 +1,6 @@
 """Pins for O2 (oracle/geometry.py) and the sign conventions of O4: exact facts only.  CPU only."""
+import os
+
 import numpy as np
 import pytest
 
@@ -150,3 +152,49 @@ def test_snake_metric_tetrad_and_zero_connection():
     # n^w = n^x - delta n^y: a ray along y-hat moves backwards in w where delta > 0
     delta = P["A"] * P["k"] * np.pi * np.cos(P["k"] * np.pi * X[:, 1])
     assert np.abs(e[:, 1, 2] + delta).max() < 1e-14
+
+
+def _radial_acceleration_of_phi_hat(a, r, sign):
+    """a^r-hat of the direction n-hat = +-phi-hat from the oracle's Ricci rotation coefficients in Boyer-Lindquist
+    coordinates on the equator: a^i = -(omega^i_cd - n^i omega^0_cd) n^c n^d  (Eq 7-8 in the 3-vector form, S4)."""
+    P = dict(a=a, hslope=0.3)
+    om = G.ricci_rotation("bl_mks", P, np.array([[np.log(r), 0.5, 0.0]]))[0]
+    n = np.array([1.0, 0.0, 0.0, sign])
+    acc = -(np.einsum("icd,c,d->i", om, n, n) - n * np.einsum("cd,c,d->", om[0], n, n))
+    assert abs(acc[2]) < 1e-12 and abs(acc[3]) < 1e-12        # stays in the equatorial plane, stays unit
+    return acc[1]
+
+
+@pytest.mark.parametrize("a", [0.5, -0.5, 0.7, -0.7, 0.95, -0.95])
+def test_bl_tetrad_and_circular_photon_orbits_eq53(a):
+    """Section 4.7 (L563-592).  In the frame of the zero-angular-momentum observers (e_0 normal to t = const, Eq 4) a photon
+    on a circular orbit moves along +-phi-hat for ever, i.e. the angular acceleration that drives the angular fluxes
+    (Eq 7-8 -> Eq 19) vanishes for n-hat = +-phi-hat exactly at the radii of Eq 53 (L569), r = 2 [1 + cos(2/3 arccos(-+a))]
+    -- the paper's spins are +-0.5, +-0.7, +-0.95 (L586) -- and changes sign there: inside the direction turns inwards,
+    outside outwards ("we expect to switch from escaping to infalling radiation as we cross the circular orbit radius").
+    This pins the oracle's omega in a curved space-time against a number the paper prints (r1 ~ 2.34, r2 ~ 3.53, L648)."""
+    P = dict(a=a, hslope=0.3)
+    rh = 1 + np.sqrt(1 - a * a)
+    X = np.stack([np.log(np.linspace(rh + 0.2, 8.0, 7)), np.linspace(0.2, 0.8, 7), np.zeros(7)], -1)
+    g = G.metric("bl_mks", P, X)
+    e, einv = G.tetrad("bl_mks", P, X)
+    assert np.abs(np.einsum("...ma,...mn,...nb->...ab", e, g, e) - G.ETA).max() < 1e-13        # Eq 1
+    gi = np.linalg.inv(g)
+    assert np.abs(e[..., :, 0] + gi[..., 0, :] / np.sqrt(-gi[..., 0, 0])[..., None]).max() < 1e-13   # Eq 4
+    assert np.abs(np.einsum("...am,...mb->...ab", einv, e) - np.eye(4)).max() < 1e-13
+    for sign, r_eq53 in ((+1.0, 2 * (1 + np.cos(2 / 3 * np.arccos(-a)))), (-1.0, 2 * (1 + np.cos(2 / 3 * np.arccos(+a))))):
+        lo, hi = max(rh + 0.05, r_eq53 - 0.5), r_eq53 + 0.5
+        flo, fhi = _radial_acceleration_of_phi_hat(a, lo, sign), _radial_acceleration_of_phi_hat(a, hi, sign)
+        assert flo < 0 < fhi                                                        # infalling inside, escaping outside
+        for _ in range(60):
+            mid = 0.5 * (lo + hi)
+            if _radial_acceleration_of_phi_hat(a, mid, sign) < 0:
+                lo = mid
+            else:
+                hi = mid
+        assert abs(0.5 * (lo + hi) - r_eq53) < 1e-8
+    if a == 0.5:                                                                    # the values the paper prints (L648)
+        gold = dict((l.split()[0], float(l.split()[1])) for l in open(os.path.join(os.path.dirname(__file__), "golden", "paper_values.txt"))
+                    if l.strip() and not l.startswith("#"))
+        assert abs(2 * (1 + np.cos(2 / 3 * np.arccos(-a))) - gold["photon_r1_a0.5"]) < 0.01
+        assert abs(2 * (1 + np.cos(2 / 3 * np.arccos(+a))) - gold["photon_r2_a0.5"]) < 0.01
