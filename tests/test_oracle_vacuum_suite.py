@@ -78,3 +78,57 @@ def test_steady_point_source_decays_as_inverse_square():
     mean_E = np.array([E[(d >= a) & (d < b)].mean() for a, b in zip(edges[:-1], edges[1:])])
     slope = np.polyfit(np.log(0.5 * (edges[:-1] + edges[1:])), np.log(mean_E), 1)[0]
     assert abs(slope + 2.0) < 0.3
+
+
+# ---- section 4.4: two-dimensional hohlraum (L498-531) --------------------------------------------------------------------
+def hohlraum_exact(x, y, t, nmu=600, npsi=1200):
+    """E / (4 pi I_wall) at (x, y) and time t for the walls x = 0 and y = 0 radiating isotropically into the vacuum quadrant
+    since t = 0: the fraction of the sphere of directions whose backward ray reaches a wall within the path length t (the
+    rays are straight, the walls fill the whole boundary of the quadrant, so a ray with n^x > 0 or n^y > 0 always ends on a
+    radiating wall, after the distance min(x / n^x, y / n^y) over the positive components).  Midpoint quadrature in
+    (cos zeta, psi) about the z axis, independent of the geodesic grid.  This is the solution the paper's Eq 49 writes in
+    closed form (its Eq 50 is garbled in PAPER.md, L521, so the integral itself is used)."""
+    mu = (np.arange(nmu) + 0.5) / nmu * 2 - 1
+    psi = (np.arange(npsi) + 0.5) / npsi * 2 * np.pi
+    s = np.sqrt(1 - mu * mu)[:, None]
+    nx, ny = s * np.cos(psi)[None, :], s * np.sin(psi)[None, :]
+    with np.errstate(divide="ignore", invalid="ignore"):
+        dx_ = np.where(nx > 0, x / nx, np.inf)
+        dy_ = np.where(ny > 0, y / ny, np.inf)
+    return float((np.minimum(dx_, dy_) <= t).mean())
+
+
+def hohlraum_grid(N, level):
+    grid = dict(n=(N, N, 1), x0=(0.0, 0.0, 0.0), dx=(20.0 / N, 20.0 / N, 20.0 / N), bc_lo=("fixed", "fixed", "periodic"),
+                bc_hi=("outflow", "outflow", "periodic"))
+    return grid, 0.4 * 20.0 / N
+
+
+def test_hohlraum_matches_the_first_principles_solution():
+    """[0, 20]^2, walls at x = 0 and y = 0 held at unit isotropic intensity (FIXED ghosts), vacuum inside, t = 6.7 (L498-510):
+    the energy density in the region of interest [0, 10]^2 follows the exact solution; the residual is the angular
+    discretisation (162 directions here) plus the smearing of the two fronts at x = t and y = t."""
+    N, level = 32, 4
+    grid, dt = hohlraum_grid(N, level)
+    o = Oracle(grid, "minkowski", {}, level, dict(method=0))
+    wall = np.ones((2, N, o.nd))
+    o.set_boundary(0, 0, wall)
+    o.set_boundary(1, 0, wall)
+    I = np.zeros((1, N, N, o.nd))
+    T = np.ones((1, N, N))
+    nst = int(round(6.7 / dt))
+    for _ in range(nst):
+        I, T, R, G, nf = o.step(I, T, dt)
+    t = nst * dt
+    E = (I.reshape(1, N, N, o.nd) * o.ang["w"]).sum(-1)[0] / (4 * np.pi)         # [j, i]
+    xc = (np.arange(N) + 0.5) * 20.0 / N
+    half = N // 2
+    ex = np.array([[hohlraum_exact(xc[i], xc[j], t) for i in range(half)] for j in range(half)])
+    err = np.abs(E[:half, :half] - ex)
+    assert 0.70 < ex[0, 0] < 0.75 and abs(E[0, 0] - ex[0, 0]) < 0.03      # next to both walls: just under three quarters of the sphere
+    print("hohlraum: mean |err| %.4f  max %.4f" % (err.mean(), err.max()))
+    assert err.mean() < 0.012 and err.max() < 0.06
+    assert np.abs(E - E.T).max() < 1e-12 * 1 + 0.02                        # x <-> y symmetry up to the grid's own asymmetry
+    # a wrong front speed or a one-sided wall would not fit: the solution for t/2 is far away
+    ex_half = np.array([[hohlraum_exact(xc[i], xc[j], 0.5 * t) for i in range(half)] for j in range(half)])
+    assert np.abs(E[:half, :half] - ex_half).mean() > 0.08
