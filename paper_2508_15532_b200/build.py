@@ -9,7 +9,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librt_b200.so")
-SOURCES = ["rt_api.cu", "rt_transport.cu", "rt_transport_tile.cu", "rt_source.cu", "rt_angular_mapr.cu", "rt_geodesic.cpp", "rt_geometry.cpp"]
+SOURCES = ["rt_api.cu", "rt_transport.cu", "rt_transport_tile.cu", "rt_source.cu", "rt_moments_mma.cu", "rt_angular_mapr.cu", "rt_geodesic.cpp", "rt_geometry.cpp"]
 HEADERS = ["rt_internal.h", "rt_kernels.cuh", "rt_transport_dev.cuh", os.path.join("..", "..", "include", "rt.h")]
 
 

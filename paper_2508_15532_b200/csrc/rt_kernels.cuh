@@ -84,6 +84,8 @@ cudaError_t launch_angular(const KParams &p, const double *I_in, double *I_io, d
 // G_nu = -(R^0_nu after - before)/dt.
 cudaError_t launch_source(const KParams &p, double *I, double *T, double dt, int *n_fail, double *R_after, double *G,
                           cudaStream_t st, long long *launches);
+// rt_moments_mma.cu: R^mu_nu of all cells (list == nullptr) or of list[0 .. n) on the fp64 tensor pipe
+cudaError_t launch_moments_mma(const KParams &p, const double *I, double *R, const int *list, int n, cudaStream_t st);
 cudaError_t launch_moments(const KParams &p, const double *I, double *R, cudaStream_t st, long long *launches);
 
 }  // namespace rt

@@ -327,15 +327,13 @@ cudaError_t launch_source(const KParams &p, double *I, double *T, double dt, int
         e = (G || R_after) ? launch_cell<true, true, true>(p, I, T, dt, n_fail, R_after, G, st)
                            : launch_cell<true, false, true>(p, I, T, dt, n_fail, nullptr, nullptr, st);
     }
-    if (e == cudaSuccess && R_after) {
+    if (e == cudaSuccess && R_after) {   // cells the source step did not visit: the tensor-pipe moments pass (rt_moments_mma.cu)
         if (!listed) {                       // no source step anywhere: one pass over all cells
             ++*launches;
-            e = launch_cell<false, true, false>(p, I, nullptr, 0.0, nullptr, R_after, nullptr, st);
-        } else if (p.nvac > 0) {             // the cells the source step did not visit
-            KParams pv = p;
-            pv.srclist = p.vaclist; pv.nsrc = p.nvac;
+            e = launch_moments_mma(p, I, R_after, nullptr, 0, st);
+        } else if (p.nvac > 0) {
             ++*launches;
-            e = launch_cell<false, true, true>(pv, I, nullptr, 0.0, nullptr, R_after, nullptr, st);
+            e = launch_moments_mma(p, I, R_after, p.vaclist, p.nvac, st);
         }
     }
     return e;
@@ -343,7 +341,7 @@ cudaError_t launch_source(const KParams &p, double *I, double *T, double dt, int
 
 cudaError_t launch_moments(const KParams &p, const double *I, double *R, cudaStream_t st, long long *launches) {
     ++*launches;
-    return launch_cell<false, true, false>(p, const_cast<double *>(I), nullptr, 0.0, nullptr, R, nullptr, st);
+    return launch_moments_mma(p, I, R, nullptr, 0, st);
 }
 
 }  // namespace rt
