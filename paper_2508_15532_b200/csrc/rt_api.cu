@@ -43,7 +43,7 @@ struct rt_ctx {
     int *d_mapr_back, *d_mapr_nnb;
     unsigned char *d_angup;
     unsigned char *d_cls;     // per (column, s): dead / general class (k_classify)
-    double *d_paircoef;       // per (column, s): geometry table of the tile kernel (k_paircoef)
+    double *d_paircoef, *d_paircoefz;   // per (column, s): geometry tables of the tile kernels (k_paircoef)
     bool u4_rest;             // d_u4 holds the tetrad rest frame (rt_set_fluid with u4 == NULL)
     unsigned char *d_colflag; // per column: bit 0 has such a cell, bit 1 has an all-vacuum cell
     KParams kp;
@@ -262,7 +262,7 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     const size_t nI = (size_t)c->ncell * pitch;
     c->d_rho = c->d_u4 = c->d_T = c->d_Th = c->d_Ih = nullptr;
     c->d_fcoef[0] = c->d_fcoef[1] = c->d_fcoef[2] = nullptr;
-    c->u4_rest = false; c->d_colflag = nullptr; c->d_cls = nullptr; c->d_paircoef = nullptr; c->d_genlist = nullptr; c->d_srclist = nullptr; c->d_vaclist = nullptr; c->d_nsel = nullptr; c->d_part_tmp = nullptr; c->part_tmp_bytes = 0;
+    c->u4_rest = false; c->d_colflag = nullptr; c->d_cls = nullptr; c->d_paircoef = nullptr; c->d_paircoefz = nullptr; c->d_genlist = nullptr; c->d_srclist = nullptr; c->d_vaclist = nullptr; c->d_nsel = nullptr; c->d_part_tmp = nullptr; c->part_tmp_bytes = 0;
     c->d_hI = c->d_hT = c->d_hR = c->d_hG = nullptr; c->d_hfail = nullptr;
     c->d_mapr_xi = c->d_mapr_xim = c->d_mapr_a = c->d_angraw = nullptr; c->d_mapr_back = c->d_mapr_nnb = nullptr; c->d_angup = nullptr;
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_cls, (size_t)ncol * pitch);
@@ -338,8 +338,10 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     e = launch_classify(k, c->d_cls, 0);
     if (e == cudaSuccess && k.variant == RT_TRANSPORT_TMA) {
         e = cudaMalloc((void **)&c->d_paircoef, (size_t)ncol * pitch * 8 * sizeof(double));
-        k.paircoef = c->d_paircoef;
-        if (e == cudaSuccess) e = launch_paircoef(k, c->d_paircoef, 0);
+        if (e == cudaSuccess && c->matter) e = cudaMalloc((void **)&c->d_paircoefz, (size_t)ncol * pitch * 8 * sizeof(double));
+        k.paircoef = c->d_paircoef; k.paircoefz = c->d_paircoefz;
+        choose_tile_gen(k, k.tile_gen);
+        if (e == cudaSuccess) e = launch_paircoef(k, c->d_paircoef, c->d_paircoefz, 0);
     }
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     if (e == cudaSuccess) {   // compact list of the general (column, s) pairs, in memory order
@@ -371,7 +373,7 @@ extern "C" int rt_free(rt_ctx *c) {
     if (c->hs_out) cudaStreamDestroy(c->hs_out);
     for (int a = 0; a < 3; ++a) { cudaFree(c->tab.face[a]); cudaFree(c->d_fcoef[a]); }
     cudaFree(c->tab.cen); cudaFree(c->tab.ecen); cudaFree(c->tab.angcoef); cudaFree(c->tab.nhat); cudaFree(c->tab.w);
-    cudaFree(c->tab.nb); cudaFree(c->tab.mirror); cudaFree(c->d_colflag); cudaFree(c->d_cls); cudaFree(c->d_paircoef); cudaFree(c->d_genlist); cudaFree(c->d_srclist); cudaFree(c->d_nsel); cudaFree(c->d_part_tmp); cudaFree(c->d_hI); cudaFree(c->d_hT); cudaFree(c->d_hR); cudaFree(c->d_hG); cudaFree(c->d_hfail); cudaFree(c->d_mapr_xi); cudaFree(c->d_mapr_xim); cudaFree(c->d_mapr_a);
+    cudaFree(c->tab.nb); cudaFree(c->tab.mirror); cudaFree(c->d_colflag); cudaFree(c->d_cls); cudaFree(c->d_paircoef); cudaFree(c->d_paircoefz); cudaFree(c->d_genlist); cudaFree(c->d_srclist); cudaFree(c->d_nsel); cudaFree(c->d_part_tmp); cudaFree(c->d_hI); cudaFree(c->d_hT); cudaFree(c->d_hR); cudaFree(c->d_hG); cudaFree(c->d_hfail); cudaFree(c->d_mapr_xi); cudaFree(c->d_mapr_xim); cudaFree(c->d_mapr_a);
     cudaFree(c->d_angraw); cudaFree(c->d_mapr_back); cudaFree(c->d_mapr_nnb); cudaFree(c->d_angup); cudaFree(c->d_rho); cudaFree(c->d_u4); cudaFree(c->d_T); cudaFree(c->d_Th); cudaFree(c->d_Ih);
     delete c;
     return RT_OK;

@@ -21,7 +21,8 @@ struct KParams {
     int zlo[3], zhi[3];
     int limiter, method;
     int variant;    // RT_TRANSPORT_TMA only if tile_eligible(), else RT_TRANSPORT_L2
-    int tile[3];    // RT_TRANSPORT_TMA: TX, TY, DCH
+    int tile[3];    // RT_TRANSPORT_TMA: TX, TY, DCH of the vacuum tile kernel
+    int tile_gen[3];   // ... of the Eq 23 tile kernel (one pair per thread)
     double n0_floor, rho_floor, kappa_a0, kappa_s, a_rad, Y_over_rho, abar;
     const double *face[3];
     const double *cen;
@@ -31,7 +32,8 @@ struct KParams {
     const double *w;
     const int *nb;
     const unsigned char *cls;   // [ncol][pitch] class byte (k_classify)
-    const double *paircoef;     // [ncol][pitch][8] geometry of a (column, s) pair for the tile kernel (k_paircoef), RT_TRANSPORT_TMA only
+    const double *paircoef;     // [ncol][pitch][8] geometry of a (column, s) pair for the tile kernels (k_paircoef), RT_TRANSPORT_TMA only
+    const double *paircoefz;    // [ncol][pitch][8] the Q Z products of the five faces (Eq 23's advective term), only with opacities
     // MAPR tables (only when angular_recon == RT_ANG_MAPR): grid-only tables are [slot][..][pitch]
     const double *mapr_xi;    // [6][3][pitch]  log map of neighbour e in the tangent plane at n_s
     const double *mapr_xim;   // [6][3][pitch]  log map of the centre of edge e
@@ -70,7 +72,10 @@ cudaError_t launch_transport(const KParams &p, const double *I_in, const double 
 // rt_transport_tile.cu: the non-"general" pairs through the TMA tile kernel
 void choose_tile(const KParams &p, const int req[3], int out[3]);
 bool tile_eligible(const KParams &p);
-cudaError_t launch_paircoef(const KParams &p, double *out, cudaStream_t st);
+cudaError_t launch_paircoef(const KParams &p, double *out, double *outz, cudaStream_t st);
+void choose_tile_gen(const KParams &p, int out[3]);
+cudaError_t launch_transport_tile_gen(const KParams &p, const double *I_in, const double *I_base, double *I_out, double *const fcoef[3],
+                                      const unsigned char *colflag, double dt, cudaStream_t st, long long *launches);
 cudaError_t launch_transport_tile(const KParams &p, const int tile[3], const double *I_in, const double *I_base, double *I_out,
                                   const unsigned char *colflag, bool matter, double dt, cudaStream_t st, long long *launches);
 // rt_transport.cu: the transport launch with its scratch in a file-scope device array (rt_transport_static)

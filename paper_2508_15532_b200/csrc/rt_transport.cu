@@ -444,7 +444,7 @@ static void launch_transport_lim(const KParams &p, const double *I_in, const dou
             if (I_base == I_in) k_transport_vac<LIM, true, true><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, colflag, dt);
             else k_transport_vac<LIM, true, false><<<gvac, VAC_THREADS, 0, st>>>(p, I_in, I_base, I_out, colflag, dt);
         }
-        k_transport_gen<LIM, true, false><<<grid, GEN_THREADS, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, colflag, dt);
+        if (!tiled) k_transport_gen<LIM, true, false><<<grid, GEN_THREADS, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, colflag, dt);
         if (p.ngen) k_transport_gen<LIM, true, true><<<dim3((p.ngen + 127) / 128, 8), 128, 0, st>>>(p, I_in, I_base, I_out, f0, f1, f2, colflag, dt);
     } else {
         if (!tiled) {
@@ -459,8 +459,9 @@ cudaError_t launch_transport(const KParams &p, const double *I_in, const double 
                              double *const fcoef[3], const unsigned char *colflag, bool matter,
                              double dt, cudaStream_t st, long long *launches) {
     const bool tiled = p.variant == RT_TRANSPORT_TMA;
-    if (tiled) {   // the vacuum update of every non-"general" pair in the tile kernel; cells with an Eq 23 face are overwritten below
+    if (tiled) {   // the non-"general" pairs through the two tile kernels: vacuum cells, then the cells with an Eq 23 face
         cudaError_t e = launch_transport_tile(p, p.tile, I_in, I_base, I_out, colflag, matter, dt, st, launches);
+        if (e == cudaSuccess && matter) e = launch_transport_tile_gen(p, I_in, I_base, I_out, fcoef, colflag, dt, st, launches);
         if (e != cudaSuccess) return e;
     }
     switch (p.limiter) {
@@ -469,7 +470,7 @@ cudaError_t launch_transport(const KParams &p, const double *I_in, const double 
         case RT_LIM_NONE: launch_transport_lim<RT_LIM_NONE>(p, I_in, I_base, I_out, fcoef, colflag, matter, tiled, dt, st); break;
         default: launch_transport_lim<RT_LIM_VANLEER>(p, I_in, I_base, I_out, fcoef, colflag, matter, tiled, dt, st); break;
     }
-    *launches += (tiled ? 0 : 1) + (matter ? 1 : 0) + (p.ngen ? 1 : 0);
+    *launches += (tiled ? 0 : 1 + (matter ? 1 : 0)) + (p.ngen ? 1 : 0);
     return cudaGetLastError();
 }
 

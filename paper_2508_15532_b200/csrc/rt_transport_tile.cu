@@ -108,6 +108,7 @@ struct TileParams {
     int oHlo, oHhi, oGxlo, oGxhi, oGylo, oGyhi;        // block offsets in a slot (own block at 0)
     int slotB, bslotB;
     int off_ring, off_base;
+    int slotStride, bslotStride, zeroOff, bzeroOff;   // run-time ring geometry (k_transport_tile_gen; the vacuum kernel's is compile-time)
     int split;   // opacities present: tiles without an all-vacuum cell are skipped (see the kernel)
 };
 
@@ -116,13 +117,13 @@ struct TileParams {
 // and a flag word (bit 0 dead, bit 1 general: the class byte of k_classify; bits 2-4: sqrt(-g) n^a_f > 0 for a = 1, 2, 3).
 // The tile kernel folds dt / (n^0 n_0 sqrt(-g_c) dx^a) in exactly as col_setup() does, so its coefficients carry the same
 // bits as those of the per-thread-load kernels; what it saves is col_setup's ~900 instructions and dependent loads per pair.
-__global__ void k_paircoef(const __grid_constant__ KParams p, double *__restrict__ out) {
+__global__ void k_paircoef(const __grid_constant__ KParams p, double *__restrict__ out, double *__restrict__ outz) {
     const int e = blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= p.n1 * p.pitch) return;
     const int i = e / p.pitch, s = e - i * p.pitch, j = blockIdx.y, col = j * p.n1 + i;
     double4 *o = reinterpret_cast<double4 *>(out + ((long long)col * p.pitch + s) * 8);
     const int cl = p.cls[(long long)col * p.pitch + s];
-    double qp[5] = {0, 0, 0, 0, 0}, c8 = 1.0, den = 1.0;
+    double qp[5] = {0, 0, 0, 0, 0}, qz[5] = {0, 0, 0, 0, 0}, c8 = 1.0, den = 1.0;
     unsigned flags = (unsigned)cl;
     if (!(cl & 1)) {
         const double nx = __ldg(p.nhat + s), ny = __ldg(p.nhat + p.pitch + s), nz = __ldg(p.nhat + 2 * p.pitch + s);
@@ -135,24 +136,29 @@ __global__ void k_paircoef(const __grid_constant__ KParams p, double *__restrict
         f = face_coef(p.face[0] + ((long long)j * (p.n1 + 1) + i) * FACE_STRIDE, nx, ny, nz);
         in = (i > 0) ? i - 1 : (p.bc_lo[0] == RT_BC_PERIODIC ? p.n1 - 1 : -1);
         if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)j * p.n1 + in) * CEN_STRIDE, nx, ny, nz))) f.Q = 0.0;
-        qp[0] = f.Q * f.P; if (f.P > 0) flags |= 4u;
+        qp[0] = f.Q * f.P; qz[0] = f.Q * f.Z; if (f.P > 0) flags |= 4u;
         f = face_coef(p.face[0] + ((long long)j * (p.n1 + 1) + i + 1) * FACE_STRIDE, nx, ny, nz);
         in = (i < p.n1 - 1) ? i + 1 : (p.bc_hi[0] == RT_BC_PERIODIC ? 0 : -1);
         if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)j * p.n1 + in) * CEN_STRIDE, nx, ny, nz))) f.Q = 0.0;
-        qp[1] = f.Q * f.P;
+        qp[1] = f.Q * f.P; qz[1] = f.Q * f.Z;
         f = face_coef(p.face[1] + ((long long)j * p.n1 + i) * FACE_STRIDE, nx, ny, nz);
         in = (j > 0) ? j - 1 : (p.bc_lo[1] == RT_BC_PERIODIC ? p.n2 - 1 : -1);
         if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)in * p.n1 + i) * CEN_STRIDE, nx, ny, nz))) f.Q = 0.0;
-        qp[2] = f.Q * f.P; if (f.P > 0) flags |= 8u;
+        qp[2] = f.Q * f.P; qz[2] = f.Q * f.Z; if (f.P > 0) flags |= 8u;
         f = face_coef(p.face[1] + ((long long)(j + 1) * p.n1 + i) * FACE_STRIDE, nx, ny, nz);
         in = (j < p.n2 - 1) ? j + 1 : (p.bc_hi[1] == RT_BC_PERIODIC ? 0 : -1);
         if (in >= 0 && sign_differs(n0c, centre_n0(p.cen + ((long long)in * p.n1 + i) * CEN_STRIDE, nx, ny, nz))) f.Q = 0.0;
-        qp[3] = f.Q * f.P;
+        qp[3] = f.Q * f.P; qz[3] = f.Q * f.Z;
         f = face_coef(p.face[2] + (long long)col * FACE_STRIDE, nx, ny, nz);
-        qp[4] = f.Q * f.P; if (f.P > 0) flags |= 16u;
+        qp[4] = f.Q * f.P; qz[4] = f.Q * f.Z; if (f.P > 0) flags |= 16u;
     }
     o[0] = make_double4(qp[0], qp[1], qp[2], qp[3]);
     o[1] = make_double4(qp[4], c8, den, __longlong_as_double((long long)flags));
+    if (outz) {   // sqrt(-g) n_0 n^0 at the five faces: the advective term of Eq 23 (only with opacities)
+        double4 *oz = reinterpret_cast<double4 *>(outz + ((long long)col * p.pitch + s) * 8);
+        oz[0] = make_double4(qz[0], qz[1], qz[2], qz[3]);
+        oz[1] = make_double4(qz[4], 0.0, 0.0, 0.0);
+    }
 }
 
 // One x3 step of the pairs of a thread.  U = k mod NS is a compile-time constant of the unrolled march, so all ring
@@ -449,6 +455,232 @@ k_transport_tile(const __grid_constant__ KParams p, const __grid_constant__ Tile
                     if ((k < zlo || k >= zhi) && !(MASK && live[r] && ((__ldg(cmask + (long long)(k >> 5) * p.ncol + mcol[r]) >> (k & 31)) & 1u))) I_out[pos0[r] + k * kstride] = 0.0;
 }
 
+// ---- the Eq 23 cells through the same ring --------------------------------------------------------------------------------
+// Cells with a non-vacuum face (mask bit of k_colflag) of the non-"general" pairs: full five-point stencils in all three
+// dims, both PLI states at the six faces, Eq 20 or Eq 23 per face from the per-face coefficients of k_facecoef -- the
+// arithmetic of k_transport_gen (rt_transport.cu), in the same order, with the thirteen operands taken from the ring instead
+// of thirteen global loads.  One pair per thread (the Eq 23 path holds ten face coefficients and a five-deep x3 window);
+// tiles without such a cell leave at once; steps whose cell is all-vacuum only shift the window.
+#ifndef NTG_X
+#define NTG_X 480
+#endif
+constexpr int NTG = NTG_X;   // consumer threads of k_transport_tile_gen (+ one producer warp)
+template <bool SAME_BASE>
+__global__ void __launch_bounds__(NTG + 32, 1)
+k_transport_tile_gen(const __grid_constant__ KParams p, const __grid_constant__ TileParams tp,
+                     const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapH,
+                     const __grid_constant__ CUtensorMap mapG, const __grid_constant__ CUtensorMap mapD, double *I_out,
+                     const double4 *__restrict__ fc0, const double4 *__restrict__ fc1, const double4 *__restrict__ fc2,
+                     const unsigned char *__restrict__ colflag, double dt) {
+    constexpr int RP = 1;
+    extern __shared__ __align__(1024) unsigned char smem[];
+    const uint32_t sbase = smem_u32(smem);
+    // barriers: full[NS], empty[NS], fullB[NS], emptyB[NS]
+    const uint32_t bar_full = sbase, bar_empty = sbase + 8 * NS, bar_fullB = sbase + 16 * NS, bar_emptyB = sbase + 24 * NS;
+    const uint32_t ring = sbase + tp.off_ring, ringB = sbase + tp.off_base;
+
+    // block -> (direction chunk fastest, then tiles in bands of 6 tile rows with x2 fastest inside a band)
+    const int ch = blockIdx.x % tp.nch, tile = blockIdx.x / tp.nch;
+    constexpr int BAND = 6;
+    const int band = tile / (tp.ntx * BAND), rr = tile - band * tp.ntx * BAND;
+    const int th = min(BAND, tp.nty - band * BAND);
+    const int tx = rr / th, ty = band * BAND + (rr - tx * th);
+    const int i0 = tx * tp.TX, j0 = ty * tp.TY, s0 = ch * tp.DCH;
+    const int n3 = p.n3, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const bool perx = p.bc_lo[0] == RT_BC_PERIODIC && p.n1 >= 2, pery = p.bc_lo[1] == RT_BC_PERIODIC && p.n2 >= 2;
+    {
+        int has = 0;
+        if ((int)threadIdx.x < tp.TX * tp.TY) {
+            const int i = i0 + (int)threadIdx.x % tp.TX, j = j0 + (int)threadIdx.x / tp.TX;
+            if (i < p.n1 && j < p.n2) has = colflag[j * p.n1 + i] & 1;
+        }
+        if (__syncthreads_or(has) == 0) return;
+    }
+
+    // ---- producer role (one lane at a time): plane m of the ring sequence = x3-plane m - 2 of I_in; base plane k ----
+    const bool hlo = j0 >= 1, hhi = j0 + tp.TY < p.n2;
+    const bool gxlo = perx && i0 < 2, gxhi = perx && i0 + tp.TX >= p.n1 - 1;
+    const bool gylo = pery && j0 < 2, gyhi = pery && j0 + tp.TY >= p.n2 - 1;
+    const uint32_t bA = (uint32_t)(tp.TY * tp.rowB), bH = (uint32_t)(2 * tp.TX * tp.cellB), bG = (uint32_t)(2 * tp.TY * tp.cellB);
+    const uint32_t bytes = bA + (hlo ? bH : 0) + (hhi ? bH : 0) + (gxlo ? bG : 0) + (gxhi ? bG : 0) + (gylo ? bH : 0) + (gyhi ? bH : 0);
+    const uint32_t bytesB = (uint32_t)(tp.TY * tp.TX * tp.cellB);
+    auto issue_plane = [&](int m) {   // caller: one lane; the slot's previous plane has been released (or m < NS)
+        const int slot = m % NS;
+        if (m >= NS) mbar_wait(bar_empty + 8 * slot, ((m / NS) & 1) ^ 1);
+        const int ks = plane_src(m - 2, n3, p.bc_lo[2], p.bc_hi[2]);
+        const uint32_t dst = ring + slot * tp.slotStride, bar = bar_full + 8 * slot;
+        mbar_expect_tx(bar, bytes);
+        tma_box(dst, &mapA, bar, s0, i0 - 2, j0, ks);
+        if (hlo) tma_box(dst + tp.oHlo, &mapH, bar, s0, i0, j0 - 2, ks);
+        if (hhi) tma_box(dst + tp.oHhi, &mapH, bar, s0, i0, j0 + tp.TY, ks);
+        if (gxlo) tma_box(dst + tp.oGxlo, &mapG, bar, s0, p.n1 - 2, j0, ks);
+        if (gxhi) tma_box(dst + tp.oGxhi, &mapG, bar, s0, 0, j0, ks);
+        if (gylo) tma_box(dst + tp.oGylo, &mapH, bar, s0, i0, p.n2 - 2, ks);
+        if (gyhi) tma_box(dst + tp.oGyhi, &mapH, bar, s0, i0, 0, ks);
+    };
+    auto issue_base = [&](int k) {
+        const int slot = k % NS;
+        if (k >= NS) mbar_wait(bar_emptyB + 8 * slot, ((k / NS) & 1) ^ 1);
+        mbar_expect_tx(bar_fullB + 8 * slot, bytesB);
+        tma_box(ringB + slot * tp.bslotStride, &mapD, bar_fullB + 8 * slot, s0, i0, j0, k);
+    };
+
+    // the geometry rows of this thread's pair, requested first
+    const int rowpairs = tp.TX * tp.DCH, npairs = rowpairs * tp.TY;
+    const int q_ = (int)threadIdx.x;
+    const int lj = q_ / rowpairs, rem_ = q_ - lj * rowpairs, c = rem_ / tp.DCH, d = rem_ - c * tp.DCH;
+    const int i = i0 + c, j = j0 + lj, s = s0 + d;
+    const bool pvalid = q_ < NTG && q_ < npairs && i < p.n1 && j < p.n2 && s < p.pitch;
+    const int col = pvalid ? j * p.n1 + i : 0;
+    const long long trow = pvalid ? (long long)col * p.pitch + s : 0;
+    const double4 *tq = reinterpret_cast<const double4 *>(p.paircoef + trow * 8), *tz = reinterpret_cast<const double4 *>(p.paircoefz + trow * 8);
+    const double4 t0 = ld4(tq), t1 = ld4(tq + 1), z0 = ld4(tz), z1 = ld4(tz + 1);
+    const unsigned *cmask = reinterpret_cast<const unsigned *>(colflag + colmask_offset(p.ncol, n3));
+    unsigned mcur = pvalid ? __ldg(cmask + col) : 0u, mnext = (pvalid && n3 > 32) ? __ldg(cmask + p.ncol + col) : 0u;
+
+    if (threadIdx.x == NTG) {
+        for (int q = 0; q < NS; ++q) {
+            mbar_init(bar_full + 8 * q, 1); mbar_init(bar_empty + 8 * q, NTG / 32);
+            mbar_init(bar_fullB + 8 * q, 1); mbar_init(bar_emptyB + 8 * q, NTG / 32);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if ((int)threadIdx.x < NS) {
+        *reinterpret_cast<double *>(smem + tp.off_ring + threadIdx.x * tp.slotStride + tp.zeroOff) = 0.0;
+        if (!SAME_BASE) *reinterpret_cast<double *>(smem + tp.off_base + threadIdx.x * tp.bslotStride + tp.bzeroOff) = 0.0;
+    }
+    __syncthreads();
+
+    if (warp == NTG / 32) {
+        // ===== producer warp: one lane streams the planes; base plane k goes out just before ring plane k + 4, which the
+        // consumers need together with it =====
+        if (lane == 0)
+            for (int m = 0; m < n3 + 4; ++m) {
+                if (!SAME_BASE && m >= 4) issue_base(m - 4);
+                issue_plane(m);
+            }
+        return;
+    }
+
+    const int t = threadIdx.x;
+    const unsigned fl = (unsigned)__double_as_longlong(t1.w);
+    const bool live = pvalid && (fl & 3u) == 0u;          // dead entries belong to the vacuum kernel, general pairs to the list kernel
+    if (!live) mcur = mnext = 0u;
+    uint32_t a_own = ring + tp.zeroOff, a_x[4], a_y[4], a_base = ringB + tp.bzeroOff;
+#pragma unroll
+    for (int o = 0; o < 4; ++o) a_x[o] = a_y[o] = ring + tp.zeroOff;
+    FaceK xl, xh, yl, yh, zf;
+    xl = xh = yl = yh = zf = FaceK{0.0, 0.0, true};
+    if (live) {
+        const double scale = dt * t1.y / t1.z;              // the folding of col_setup() / fold()
+        const double sx = scale * p.inv_dx[0], sy = scale * p.inv_dx[1], sz = scale * p.inv_dx[2];
+        const bool xpos = (fl & 4u) != 0u, ypos = (fl & 8u) != 0u, zpos = (fl & 16u) != 0u;
+        xl = FaceK{t0.x * sx, z0.x * sx, xpos}; xh = FaceK{t0.y * sx, z0.y * sx, xpos};
+        yl = FaceK{t0.z * sy, z0.z * sy, ypos}; yh = FaceK{t0.w * sy, z0.w * sy, ypos};
+        zf = FaceK{t1.x * sz, z1.x * sz, zpos};
+        const int din = d * 8;
+        auto xo = [&](int o) -> uint32_t {
+            int gi = i + o;
+            if (gi < 0 || gi >= p.n1) {
+                const int bc = gi < 0 ? p.bc_lo[0] : p.bc_hi[0];
+                if (bc == RT_BC_OUTFLOW) gi = gi < 0 ? 0 : p.n1 - 1;        // the edge cell itself
+                else if (bc == RT_BC_PERIODIC && perx)
+                    return (gi < 0 ? tp.oGxlo + (gi + 2) * tp.cellB : tp.oGxhi + (gi - p.n1) * tp.cellB) + lj * 2 * tp.cellB + din;
+                else gi = i;   // a single periodic column wraps onto itself ("general" pairs do not come here)
+            }
+            return lj * tp.rowB + (gi - i0 + 2) * tp.cellB + din;
+        };
+        auto yo = [&](int o) -> uint32_t {
+            int gj = j + o;
+            if (gj < 0 || gj >= p.n2) {
+                const int bc = gj < 0 ? p.bc_lo[1] : p.bc_hi[1];
+                if (bc == RT_BC_OUTFLOW) gj = gj < 0 ? 0 : p.n2 - 1;
+                else if (bc == RT_BC_PERIODIC && pery)
+                    return (gj < 0 ? tp.oGylo + (gj + 2) * tp.TX * tp.cellB : tp.oGyhi + (gj - p.n2) * tp.TX * tp.cellB) + c * tp.cellB + din;
+                else gj = j;
+            }
+            const int lr = gj - j0;
+            if (lr < 0) return tp.oHlo + ((lr + 2) * tp.TX + c) * tp.cellB + din;
+            if (lr >= tp.TY) return tp.oHhi + ((lr - tp.TY) * tp.TX + c) * tp.cellB + din;
+            return lr * tp.rowB + (c + 2) * tp.cellB + din;
+        };
+        a_own = ring + xo(0);
+        a_x[0] = ring + xo(-2); a_x[1] = ring + xo(-1); a_x[2] = ring + xo(1); a_x[3] = ring + xo(2);
+        a_y[0] = ring + yo(-2); a_y[1] = ring + yo(-1); a_y[2] = ring + yo(1); a_y[3] = ring + yo(2);
+        a_base = ringB + (lj * tp.TX + c) * tp.cellB + din;
+    }
+    const long long kstride = (long long)p.ncol * p.pitch;
+    const int zlo = p.zlo[2], zhi = n3 - p.zhi[2], ncol = p.ncol, n1 = p.n1;
+    const int sxf = p.n2 * (n1 + 1), syf = (p.n2 + 1) * n1;
+    const double4 *px = fc0 + ((long long)j * (n1 + 1) + i), *py = fc1 + ((long long)j * n1 + i), *pz = fc2 + col;
+    if (!pvalid) { px = fc0; py = fc1; pz = fc2; }
+
+    // prologue: planes -2 .. 1 (ring sequence m = 0 .. 3) -> the x3 window
+    double w0, w1, w2, w3;
+#pragma unroll
+    for (int m = 0; m < 4; ++m) {
+        mbar_wait(bar_full + 8 * m, 0);
+        const double v = lds(a_own + m * tp.slotStride);
+        if (m == 0) w0 = v; else if (m == 1) w1 = v; else if (m == 2) w2 = v; else w3 = v;
+        if (m < 2) {   // planes -2, -1 are not read again
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_empty + 8 * m);
+        }
+    }
+    double *outk = I_out + (live ? trow : 0);
+
+    // The march is NOT unrolled over the ring (the body is ~400 instructions: eight copies overflow the instruction cache and
+    // spill); the slot offsets are run-time values, three adds per step.
+    bool ready = false;
+    int u = 0;                     // k mod NS
+    uint32_t par0 = 0;             // parity of the ring round that holds the sequence m = k - u .. k - u + NS - 1
+#pragma unroll 1
+    for (int k = 0; k < n3; ++k) {
+        const int uo = u + 4 < NS ? u + 4 : u + 4 - NS, uk = u + 2 < NS ? u + 2 : u + 2 - NS;
+        const uint32_t so = (uint32_t)(uo * tp.slotStride), sk = (uint32_t)(uk * tp.slotStride), sb = (uint32_t)(u * tp.bslotStride);
+        if (!ready) {
+            mbar_wait(bar_full + 8 * uo, par0 ^ (uint32_t)(u + 4 >= NS));
+            if (!SAME_BASE) mbar_wait(bar_fullB + 8 * u, par0);
+        }
+        const double w4 = lds(a_own + so);
+        const bool mat = (mcur >> (k & 31)) & 1u;
+        const bool matn = ((k & 31) == 31 ? mnext : (mcur >> ((k & 31) + 1))) & 1u;
+        if (matn && k + 1 < n3) {   // the per-face coefficients of the next step: towards L1 now (no registers held)
+            pf_l1(px + sxf); pf_l1(py + syf); pf_l1(py + syf + n1); pf_l1(pz + 2 * ncol);
+        }
+        if (mat) {
+            const double4 fzl = ld4(pz), fzh = ld4(pz + ncol), fxl = ld4(px), fxh = ld4(px + 1), fyl = ld4(py), fyh = ld4(py + n1);
+            const double xm2 = lds(a_x[0] + sk), xm1 = lds(a_x[1] + sk), xp1 = lds(a_x[2] + sk), xp2 = lds(a_x[3] + sk);
+            const double ym2 = lds(a_y[0] + sk), ym1 = lds(a_y[1] + sk), yp1 = lds(a_y[2] + sk), yp2 = lds(a_y[3] + sk);
+            const double cbase = SAME_BASE ? w2 : lds(a_base + sb);
+            double D = flux_diff<RT_LIM_MC, true>(w0, w1, w2, w3, w4, zf, zf, fzl, fzh);
+            D += flux_diff<RT_LIM_MC, true>(xm2, xm1, w2, xp1, xp2, xl, xh, fxl, fxh);
+            D += flux_diff<RT_LIM_MC, true>(ym2, ym1, w2, yp1, yp2, yl, yh, fyl, fyh);
+            *outk = (k < zlo || k >= zhi) ? 0.0 : cbase - D;      // Eq 18 (O5), dt / (n^0 n_0 sqrt(-g) dx) folded in
+        }
+        const int u1 = u + 1 < NS ? u + 1 : 0;
+        const uint32_t par1 = par0 ^ (uint32_t)(u + 1 == NS);
+        if (k + 1 < n3) {   // probe the next step's barriers; the answer is there when it is needed
+            const int uo1 = u1 + 4 < NS ? u1 + 4 : u1 + 4 - NS;
+            ready = mbar_test(bar_full + 8 * uo1, par1 ^ (uint32_t)(u1 + 4 >= NS));
+            if (!SAME_BASE) ready = mbar_test(bar_fullB + 8 * u1, par1) && ready;
+        }
+        w0 = w1; w1 = w2; w2 = w3; w3 = w4;
+        outk += kstride; px += sxf; py += syf; pz += ncol;
+        __syncwarp();
+        if (lane == 0) {
+            mbar_arrive(bar_empty + 8 * uk);
+            if (!SAME_BASE) mbar_arrive(bar_emptyB + 8 * u);
+        }
+        if ((k & 31) == 31) {   // next mask word (requested 32 steps ago)
+            mcur = mnext;
+            mnext = (live && k + 33 < n3) ? __ldg(cmask + (long long)((k >> 5) + 2) * ncol + col) : 0u;
+        }
+        u = u1; par0 = par1;
+    }
+    (void)t;
+}
+
 // ---- host side: tensor maps ------------------------------------------------------------------------------------------
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                                   const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -498,6 +730,17 @@ size_t tile_layout(const KParams &p, const int tile[3], bool same, TileParams &t
     t.off_base = t.off_ring + NS * SLOT_STRIDE;
     return (size_t)t.off_base + (same ? 0 : NS * BSLOT_STRIDE);
 }
+// the same for k_transport_tile_gen: its own, smaller ring (strides fitted to the tile), so that most of the SM's shared
+// memory stays L1 cache for the per-face coefficient loads
+size_t tile_layout_gen(const KParams &p, const int tile[3], bool same, TileParams &t) {
+    tile_layout(p, tile, same, t);
+    t.zeroOff = t.slotB;
+    t.slotStride = align_up(t.slotB + 8, 1024);
+    t.bzeroOff = t.bslotB;
+    t.bslotStride = align_up(t.bslotB + 8, 128);
+    t.off_base = t.off_ring + NS * t.slotStride;
+    return (size_t)t.off_base + (same ? 0 : NS * t.bslotStride);
+}
 constexpr size_t SMEM_MAX = 227 * 1024;
 
 }  // namespace
@@ -505,21 +748,20 @@ constexpr size_t SMEM_MAX = 227 * 1024;
 // Tile shape for a mesh: TX x TY columns x DCH directions with TX TY DCH <= RP NT pairs.  DCH is even (TMA: the inner box
 // extent is a multiple of 16 bytes) and chosen so that ceil(pitch / DCH) chunks waste few lanes; (TX, TY) minimise the halo'd
 // cells loaded per cell computed, (TY (TX + 4) + 4 TX) / (TX TY), with the ragged tiles of this mesh counted.
-void choose_tile(const KParams &p, const int req[3], int out[3]) {
-    if (req && req[0] > 0 && req[1] > 0 && req[2] > 0) { out[0] = req[0]; out[1] = req[1]; out[2] = req[2]; return; }
+static void choose_tile_rp(const KParams &p, int rp, int out[3], int dch_min = 8, int nt = NT) {
     double best = 1e300;
     out[0] = 2; out[1] = 1; out[2] = 8;
-    for (int dch = 8; dch <= 64; dch += 2) {
+    for (int dch = dch_min; dch <= 64; dch += 2) {
         const int nch = (p.pitch + dch - 1) / dch;
         const double wd = (double)nch * dch / p.nd;   // lanes per real direction
-        const int cells = RP * NT / dch;
+        const int cells = rp * nt / dch;
         for (int ty = 1; ty <= 8; ++ty)
             for (int tx = 2; tx <= 16; ++tx) {
                 if (tx * ty > cells) continue;
                 const int tl[3] = {tx, ty, dch};
                 TileParams t;
                 if (tile_layout(p, tl, false, t) > SMEM_MAX || t.slotB > ZERO_OFF) continue;
-                const double use = (double)(tx * ty * dch) / (RP * NT);    // consumer slots in use
+                const double use = (double)(tx * ty * dch) / (rp * nt);    // consumer slots in use
                 const double rag = ((double)((p.n1 + tx - 1) / tx) * tx / p.n1) * ((double)((p.n2 + ty - 1) / ty) * ty / p.n2);
                 const double X = (double)(ty * (tx + 4) + 4 * tx) / (tx * ty);
                 // short box rows (under 192 bytes) cost TMA throughput: measured 3 % at 80-byte rows against 192-byte rows
@@ -530,11 +772,18 @@ void choose_tile(const KParams &p, const int req[3], int out[3]) {
     }
 }
 
-cudaError_t launch_paircoef(const KParams &p, double *out, cudaStream_t st) {
+cudaError_t launch_paircoef(const KParams &p, double *out, double *outz, cudaStream_t st) {
     dim3 grid((p.n1 * p.pitch + 255) / 256, p.n2);
-    k_paircoef<<<grid, 256, 0, st>>>(p, out);
+    k_paircoef<<<grid, 256, 0, st>>>(p, out, outz);
     return cudaGetLastError();
 }
+
+void choose_tile(const KParams &p, const int req[3], int out[3]) {
+    if (req && req[0] > 0 && req[1] > 0 && req[2] > 0) { out[0] = req[0]; out[1] = req[1]; out[2] = req[2]; return; }
+    choose_tile_rp(p, RP, out);
+}
+// (at least 16 directions per chunk: a warp then spans at most two cells and its per-face coefficient loads are near-broadcasts)
+void choose_tile_gen(const KParams &p, int out[3]) { choose_tile_rp(p, 1, out, 16, NTG); }
 
 bool tile_eligible(const KParams &p) {
     return p.limiter == RT_LIM_MC && (p.bc_lo[2] == RT_BC_PERIODIC || p.bc_lo[2] == RT_BC_OUTFLOW) &&
@@ -566,6 +815,33 @@ cudaError_t launch_transport_tile(const KParams &p, const int tile[3], const dou
     if (same) { if (matter) RT_TILE_LAUNCH(true, true); else RT_TILE_LAUNCH(true, false); }
     else { if (matter) RT_TILE_LAUNCH(false, true); else RT_TILE_LAUNCH(false, false); }
 #undef RT_TILE_LAUNCH
+    ++*launches;
+    return e != cudaSuccess ? e : cudaGetLastError();
+}
+
+// The Eq 23 cells of the non-"general" pairs through k_transport_tile_gen (it overwrites what the vacuum kernel left alone).
+cudaError_t launch_transport_tile_gen(const KParams &p, const double *I_in, const double *I_base, double *I_out, double *const fcoef[3],
+                                      const unsigned char *colflag, double dt, cudaStream_t st, long long *launches) {
+    TileParams t;
+    const bool same = (I_base == I_in);
+    const size_t smem = tile_layout_gen(p, p.tile_gen, same, t);
+    if (smem > SMEM_MAX || t.TX * t.TY * t.DCH > NTG || (t.DCH & 1) || t.TX < 2 || t.TX + 4 > 256 || t.DCH > 256)
+        return cudaErrorInvalidConfiguration;
+    CUtensorMap mA, mH, mG, mD;
+    if (!make_map(&mA, I_in, p, t.DCH, t.TX + 4, t.TY) || !make_map(&mH, I_in, p, t.DCH, t.TX, 2) || !make_map(&mG, I_in, p, t.DCH, 2, t.TY) ||
+        !make_map(&mD, I_base, p, t.DCH, t.TX, t.TY))
+        return cudaErrorInvalidValue;
+    const double4 *f0 = reinterpret_cast<const double4 *>(fcoef[0]), *f1 = reinterpret_cast<const double4 *>(fcoef[1]),
+                  *f2 = reinterpret_cast<const double4 *>(fcoef[2]);
+    const unsigned grid = (unsigned)(t.ntx * t.nty * t.nch);
+    cudaError_t e;
+    if (same) {
+        e = cudaFuncSetAttribute(k_transport_tile_gen<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) k_transport_tile_gen<true><<<grid, NTG + 32, smem, st>>>(p, t, mA, mH, mG, mD, I_out, f0, f1, f2, colflag, dt);
+    } else {
+        e = cudaFuncSetAttribute(k_transport_tile_gen<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) k_transport_tile_gen<false><<<grid, NTG + 32, smem, st>>>(p, t, mA, mH, mG, mD, I_out, f0, f1, f2, colflag, dt);
+    }
     ++*launches;
     return e != cudaSuccess ? e : cudaGetLastError();
 }
