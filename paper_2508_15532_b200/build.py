@@ -20,17 +20,16 @@ def stale():
     return any(os.path.getmtime(os.path.join(CSRC, f)) > t for f in SOURCES + HEADERS)
 
 
-def build(force=False, verbose=False, out=LIB, defines=()):
-    """`defines` (tuning macros such as VAC_PF=3) and `out` are for kernel tuning runs; the product build uses neither."""
-    if out == LIB and not defines and not (force or stale()):
+def build(force=False, verbose=False):
+    if not (force or stale()):
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-shared",
-           "-Xcompiler", "-fPIC", "--fmad=true", "-o", out] + ["-D" + d for d in defines] + [os.path.join(CSRC, f) for f in SOURCES]
+           "-Xcompiler", "-fPIC", "--fmad=true", "-o", LIB] + [os.path.join(CSRC, f) for f in SOURCES]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     subprocess.check_call(cmd)
-    return out
+    return LIB
 
 
 if __name__ == "__main__":

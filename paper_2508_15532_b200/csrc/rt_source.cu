@@ -132,16 +132,10 @@ __device__ __forceinline__ double rotate(const double M[10], const double *__res
     return r;
 }
 
-#ifndef CELL_THREADS   // source-step variants: 128 registers, 16 warps per SM (80 registers x 24 warps spills and is 2-3 % slower)
-#define CELL_THREADS 128
-#define CELL_MINB 4
-#endif
-#ifndef MOM_THREADS
-#define MOM_THREADS 256
-#endif
-#ifndef MOM_MINB      // resident CTAs per SM of the moments-only passes (no source step: fewer live values, 64 registers)
-#define MOM_MINB 4
-#endif
+// source-step variants: 128 registers, 16 warps per SM (80 registers x 24 warps spills and is 2-3 % slower)
+constexpr int CELL_THREADS = 128, CELL_MINB = 4;
+// moments-only instantiation (kept for completeness; the moments-only passes run in rt_moments_mma.cu)
+constexpr int MOM_THREADS = 256, MOM_MINB = 4;
 template <int MAXV, bool SRC, bool MOM, bool LIST>
 __global__ void __launch_bounds__(SRC ? CELL_THREADS : MOM_THREADS, (SRC ? CELL_MINB : (MAXV > 6 ? MOM_MINB - 2 : MOM_MINB)))   // moments-only, 362 directions: 12 values per lane, 128 registers
 k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, double *G_out) {

@@ -93,18 +93,11 @@ __global__ void k_colflag(KParams p, const double4 *__restrict__ fc0, const doub
 // so that the CTAs resident at the same time cover a compact (x1, x2) patch and their transverse neighbours are
 // read from L2 instead of DRAM (row-major order re-reads ~4 halo rows per wave of ~5 rows).
 // how many x3-planes beyond its two-plane register pipeline the angular kernel prefetches (0 = off)
-#ifndef ANG_PF
-#define ANG_PF 2
-#endif
+constexpr int ANG_PF = 2;
 // how many x3-planes beyond the register pipeline the vacuum kernel prefetches its operands (0 = off)
-#ifndef VAC_PF
-#define VAC_PF 2
-#endif
+constexpr int VAC_PF = 2;
 constexpr int TILE_ROWS = 24;
-#ifndef VAC_THREADS
-#define VAC_THREADS 128
-#define VAC_MINB 5
-#endif
+constexpr int VAC_THREADS = 128, VAC_MINB = 5;
 __device__ __forceinline__ void tile_block(const KParams &p, int &bx, int &by) {
     const int nbx = (p.n1 * p.pitch + (int)blockDim.x - 1) / (int)blockDim.x;
     const int lin = blockIdx.x, band = lin / (nbx * TILE_ROWS), r = lin - band * nbx * TILE_ROWS;
@@ -187,7 +180,6 @@ k_transport_vac(const __grid_constant__ KParams p, const double *__restrict__ I_
             qxa = __ldg(pn + oxa); qxb = __ldg(pn + oxb); qxd = __ldg(pn + oxd);
             qya = __ldg(pn + oya); qyb = __ldg(pn + oyb); qyd = __ldg(pn + oyd);
             qw4 = (k + 3 < n3) ? __ldg(pn + 2 * kstride) : slow_ld(p, I_in, 2, i, j, k + 3, s);
-#if VAC_PF
             if (k + VAC_PF + 1 < n3) {   // operands of step k + 1 + VAC_PF: pulled towards the SM now (no registers held)
                 const double *pf = pn + VAC_PF * kstride;
                 pf_l1(pf + oxa); pf_l1(pf + oxb); pf_l1(pf + oxd);
@@ -195,7 +187,6 @@ k_transport_vac(const __grid_constant__ KParams p, const double *__restrict__ I_
                 if (k + VAC_PF + 3 < n3) pf_l1(pf + 2 * kstride);
                 if (!SAME_BASE) pf_l1(pb + (VAC_PF + 1) * kstride);
             }
-#endif
         }
         // x3: upwind state at the upper face (always formed: it is the next cell's lower flux if that cell is vacuum)
         const double sz = slope_k<LIM>(w3 - w2, zpos ? (w2 - w1) : (w4 - w3));
@@ -234,10 +225,7 @@ k_transport_vac(const __grid_constant__ KParams p, const double *__restrict__ I_
 // General path: full 5-point stencils, both PLI states at all six faces, Eq 20 or Eq 23 per face.  Marches x3 with a
 // 5-deep register window; computes only the steps it owns (cells with a non-vacuum face, or every cell of a
 // "general" thread).
-#ifndef GEN_THREADS
-#define GEN_THREADS 128   // 128 x 4 and 256 x 2 hold the same 16 warps per SM at 128 registers; the smaller CTA is 1-2 % faster
-#define GEN_MINB 4
-#endif
+constexpr int GEN_THREADS = 128, GEN_MINB = 4;   // 128 x 4 and 256 x 2 hold the same 16 warps per SM at 128 registers; the smaller CTA is 1-2 % faster
 template <int LIM, bool MATTER, bool LIST>
 __global__ void __launch_bounds__(GEN_THREADS, GEN_MINB)
 k_transport_gen(const __grid_constant__ KParams p, const double *__restrict__ I_in, const double *I_base, double *I_out,
@@ -390,12 +378,10 @@ __global__ void k_angular(KParams p, const double *__restrict__ I_in, double *I_
                 if (inrow) vn1 = __ldg(pin + 3 * kstride);
                 if (upd) ion1 = pio[3 * kstride];
             }
-#if ANG_PF
             if (k + 2 + ANG_PF + 1 < n3) {   // planes further ahead: towards the SM now, no registers held
                 if (inrow) { pf_l1(pin + (2 + ANG_PF) * kstride); pf_l1(pin + (3 + ANG_PF) * kstride); }
                 if (upd) { pf_l1(pio + (2 + ANG_PF) * kstride); pf_l1(pio + (3 + ANG_PF) * kstride); }
             }
-#endif
         }
         __syncthreads();
         if (live) {

@@ -28,22 +28,10 @@
 namespace rt {
 namespace {
 
-#ifndef NT_X
-#define NT_X 480
-#endif
-constexpr int NT = NT_X;              // consumer threads (15 warps); warp 15 is the producer: 16 warps = 128 registers each
-#ifndef RP_X
-#define RP_X 2
-#endif
-constexpr int RP = RP_X;                // pairs per consumer thread
-#ifndef NS_X
-#define NS_X 8
-#endif
-constexpr int NS = NS_X;             // ring slots: planes k, k+1, k+2 in use, five in flight (a load takes about two steps)
-#ifndef SLOT_X
-#define SLOT_X 20480
-#endif
-constexpr int SLOT_STRIDE = SLOT_X;   // bytes between ring slots (compile-time: every operand load is LDS [R + imm])
+constexpr int NT = 480;               // consumer threads (15 warps); warp 15 is the producer: 16 warps = 128 registers each
+constexpr int RP = 2;                   // pairs per consumer thread
+constexpr int NS = 8;                // ring slots: planes k, k+1, k+2 in use, five in flight (a load takes about two steps)
+constexpr int SLOT_STRIDE = 20480;   // bytes between ring slots (compile-time: every operand load is LDS [R + imm])
 constexpr int BSLOT_STRIDE = RP * NT * 8 + 128;   // base ring: own cells only (+ the zero word, see ZERO_OFF)
 constexpr int ZERO_OFF = SLOT_STRIDE - 8;   // a double behind each slot's data that holds 0.0: the operand of every pair that is not live
 
@@ -461,10 +449,7 @@ k_transport_tile(const __grid_constant__ KParams p, const __grid_constant__ Tile
 // arithmetic of k_transport_gen (rt_transport.cu), in the same order, with the thirteen operands taken from the ring instead
 // of thirteen global loads.  One pair per thread (the Eq 23 path holds ten face coefficients and a five-deep x3 window);
 // tiles without such a cell leave at once; steps whose cell is all-vacuum only shift the window.
-#ifndef NTG_X
-#define NTG_X 480
-#endif
-constexpr int NTG = NTG_X;   // consumer threads of k_transport_tile_gen (+ one producer warp)
+constexpr int NTG = 480;     // consumer threads of k_transport_tile_gen (+ one producer warp)
 template <bool SAME_BASE>
 __global__ void __launch_bounds__(NTG + 32, 1)
 k_transport_tile_gen(const __grid_constant__ KParams p, const __grid_constant__ TileParams tp,
