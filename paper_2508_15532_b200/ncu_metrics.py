@@ -18,7 +18,7 @@ ROOT = os.path.dirname(HERE)
 
 # kernel name (substring) -> class of rt_profile_read
 CLASSES = (("k_facecoef", "facecoef"), ("k_colflag", "facecoef"), ("k_transport", "transport"), ("k_angular", "angular"),
-           ("k_cell<", "source"), ("k_cell", "source"))
+           ("k_cell", "source"), ("k_moments", "source"))
 METRICS = {"dram_bytes": ("dram__bytes_read.sum", "dram__bytes_write.sum"), "warp_instr": ("smsp__inst_executed.sum",),
            "l2_to_l1_bytes": ("l1tex__m_xbar2l1tex_read_bytes.sum",), "time_us": ("gpu__time_duration.sum",)}
 UNIT_SCALE = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "inst": 1.0, "us": 1.0, "ms": 1e3, "ns": 1e-3, "": 1.0}
