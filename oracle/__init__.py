@@ -9,8 +9,9 @@ may import this package.  It imports nothing from the CUDA package and shares no
   geometry.py   O2  metric / tetrad / Ricci rotation coefficients (numpy)
   rt_oracle.c   O3-O8 stepping (plain C, sequential sums), built on demand with gcc
 
-Parity status: everything is pinned except MAPR angular reconstruction (ang_recon=1): "parity unpinned"
-beyond exactness for tangent-plane-linear fields.
+Parity status: every function is pinned.  MAPR angular reconstruction (ang_recon=1) is a reading of a method the paper only
+names: its stated properties (second order, linear exactness, conservation, arg-min and tie rules) are pinned; its
+identity with the cited Christov & Popov method (not in the container) cannot be checked.
 """
 import ctypes
 import os

@@ -16,7 +16,10 @@
  *
  * Layout: intensity I[cell][s], cell = (k*N2 + j)*N1 + i, s fastest, pitch = nd (no padding).
  * Geometry tables: index gc = (kg*N2 + j)*N1 + i with kg = (n3g == 1 ? 0 : k)  (x3-symmetric storage).
- * Parity status: MAPR (ang_recon = 1) is "parity unpinned" beyond linear exactness (S6).
+ * Parity status: every function is pinned (tests/test_oracle_*.py).  MAPR (ang_recon = 1) is a READING of a method the paper
+ * only names (L227, S6): its stated properties -- second-order convergence, linear exactness, reduction to donor cell,
+ * per-cell conservation, the arg-min and tie rules -- are pinned (tests/test_oracle_pins2.py, test_oracle_transport.py);
+ * that its candidate planes are those of the cited Christov & Popov paper (not in the container) cannot be checked.
  */
 #include <math.h>
 #include <stdlib.h>
