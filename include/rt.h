@@ -121,8 +121,8 @@ int rt_cfl_dt(const rt_ctx *ctx, double out_host[2]);
 int rt_set_boundary(rt_ctx *ctx, int dim, int side, const double *ghost_dev);
 /* Fluid state: rho[N_c], T[N_c], u4[4][N_c] coordinate-frame u^mu (NULL = tetrad rest frame e_0).  Copied into
  * library-owned buffers on `stream`; T is the temperature used for the transport opacities of rt_transport.  Also
- * rebuilds the interaction list (cells with rho >= rho_floor, L468) on the device; the call synchronises `stream` once to
- * read the list length back (4 bytes), so it may be called every step (coupled GRMHD use, L448-456). */
+ * rebuilds the interaction list (cells with rho >= rho_floor, L468) on the device; nothing is read back and the stream is not
+ * synchronised, so the call may be made every step (coupled GRMHD use, L448-456). */
 int rt_set_fluid(rt_ctx *ctx, const double *rho_dev, const double *T_dev, const double *u4_dev, void *stream);
 
 /* I_out = (n^0 n_0 I_base - dt D_x[I_in]) / (n^0 n_0), then mask + zero bands (O3 + O5).  I_out may alias I_base

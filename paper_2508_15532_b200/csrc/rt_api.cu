@@ -27,7 +27,7 @@ struct rt_ctx {
     std::vector<double> h_g, h_e, h_einv, h_sqrtg, h_omega, h_n0, h_angcoef;
     DeviceTables tab;
     double *d_rho, *d_u4, *d_T, *d_Th, *d_Ih, *d_fcoef[3];
-    int *d_genlist, *d_srclist, *d_vaclist;   // d_srclist: [ncell] listed cells first (ascending), the rest behind them; d_vaclist points into it
+    int *d_genlist, *d_srclist;   // d_srclist: [ncell] listed cells first (ascending), the rest behind them; d_nsel: how many are listed
     int *d_nsel; void *d_part_tmp; size_t part_tmp_bytes;   // interaction-list partition (cub) scratch
     double *d_hI, *d_hT, *d_hR, *d_hG;   // device staging of rt_step_host (allocated on first use)
     int *d_hfail;
@@ -262,7 +262,7 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     const size_t nI = (size_t)c->ncell * pitch;
     c->d_rho = c->d_u4 = c->d_T = c->d_Th = c->d_Ih = nullptr;
     c->d_fcoef[0] = c->d_fcoef[1] = c->d_fcoef[2] = nullptr;
-    c->u4_rest = false; c->d_colflag = nullptr; c->d_cls = nullptr; c->d_paircoef = nullptr; c->d_paircoefz = nullptr; c->d_genlist = nullptr; c->d_srclist = nullptr; c->d_vaclist = nullptr; c->d_nsel = nullptr; c->d_part_tmp = nullptr; c->part_tmp_bytes = 0;
+    c->u4_rest = false; c->d_colflag = nullptr; c->d_cls = nullptr; c->d_paircoef = nullptr; c->d_paircoefz = nullptr; c->d_genlist = nullptr; c->d_srclist = nullptr; c->d_nsel = nullptr; c->d_part_tmp = nullptr; c->part_tmp_bytes = 0;
     c->d_hI = c->d_hT = c->d_hR = c->d_hG = nullptr; c->d_hfail = nullptr;
     c->d_mapr_xi = c->d_mapr_xim = c->d_mapr_a = c->d_angraw = nullptr; c->d_mapr_back = c->d_mapr_nnb = nullptr; c->d_angup = nullptr;
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_cls, (size_t)ncol * pitch);
@@ -503,6 +503,13 @@ extern "C" int rt_set_boundary(rt_ctx *c, int dim, int side, const double *ghost
 }
 
 namespace {
+// tetrad rest frame u^mu = e^mu_0 of every cell (rt_set_fluid with u4 == NULL)
+__global__ void k_rest_frame(const double *__restrict__ ecen, double *__restrict__ u4, long long ncell, int ncol) {
+    const long long cell = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (cell >= ncell) return;
+    const double *e = ecen + (cell % ncol) * 16;
+    for (int mu = 0; mu < 4; ++mu) u4[mu * ncell + cell] = e[4 * mu];
+}
 struct AboveFloor {   // L468 (i): cells at or above the density floor interact
     const double *rho; double floor;
     __device__ bool operator()(int q) const { return rho[q] >= floor; }
@@ -518,21 +525,17 @@ extern "C" int rt_set_fluid(rt_ctx *c, const double *rho, const double *T, const
     if (u4) {
         CK(cudaMemcpyAsync(c->d_u4, u4, 4 * nb, cudaMemcpyDeviceToDevice, st));
         c->u4_rest = false;
-    } else if (!c->u4_rest) {   // tetrad rest frame u^mu = e^mu_0 (built once: it does not depend on the call)
+    } else if (!c->u4_rest) {   // tetrad rest frame u^mu = e^mu_0 (built once, on the device: it does not depend on the call)
         c->u4_rest = true;
-        std::vector<double> h(4 * (size_t)c->ncell);
-        for (long long cell = 0; cell < c->ncell; ++cell)
-            for (int mu = 0; mu < 4; ++mu) h[mu * c->ncell + cell] = c->h_e[(cell % c->ncol) * 16 + 4 * mu];
-        CK(cudaStreamSynchronize(st));
-        CK(cudaMemcpy(c->d_u4, h.data(), 4 * nb, cudaMemcpyHostToDevice));
+        k_rest_frame<<<(unsigned)((c->ncell + 255) / 256), 256, 0, st>>>(c->tab.ecen, c->d_u4, c->ncell, c->ncol);
+        CK(cudaGetLastError());
     }
-    // interaction list: cells at or above the density floor (L468 (i)); below it alpha = 0 whatever T is.  Built on the
-    // device (cub partition of the cell indices: listed cells first in ascending order, the rest behind them), so that
-    // a caller who hands over a new fluid state every step (the coupled GRMHD use, L448-456) pays one 4-byte read-back.
+    // interaction list: cells at or above the density floor (L468 (i)); below it alpha = 0 whatever T is.  Built on the device
+    // (cub partition of the cell indices: listed cells first in ascending order, the rest behind them); its length STAYS on
+    // the device, so a caller who hands over a new fluid state every step (the coupled GRMHD use, L448-456) pays no
+    // read-back and no synchronisation here.
     {
-        c->kp.nsrc = c->kp.nvac = 0;
-        c->kp.srclist = c->kp.vaclist = nullptr;
-        c->d_vaclist = nullptr;
+        c->kp.srclist = nullptr; c->kp.nsel = nullptr;
         if (c->matter && c->opt.source_method != 0) {
             const int n = (int)c->ncell;
             cub::CountingInputIterator<int> idx(0);
@@ -551,16 +554,7 @@ extern "C" int rt_set_fluid(rt_ctx *c, const double *rho, const double *T, const
             }
             size_t tmp = c->part_tmp_bytes;
             CK(cub::DevicePartition::If(c->d_part_tmp, tmp, idx, c->d_srclist, c->d_nsel, n, sel, st));
-            int nsel = 0;
-            CK(cudaMemcpyAsync(&nsel, c->d_nsel, sizeof(int), cudaMemcpyDeviceToHost, st));
-            CK(cudaStreamSynchronize(st));
-            c->kp.nsrc = nsel;
-            if (nsel > 0) c->kp.srclist = c->d_srclist;
-            if (nsel > 0 && nsel < n) {   // the complement (cells the source step cannot touch: their moments need one pass only)
-                c->kp.nvac = n - nsel;
-                c->d_vaclist = c->d_srclist + nsel;
-                c->kp.vaclist = c->d_vaclist;
-            }
+            c->kp.srclist = c->d_srclist; c->kp.nsel = c->d_nsel;
         }
     }
     c->fluid_set = true;

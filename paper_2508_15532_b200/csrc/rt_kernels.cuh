@@ -47,10 +47,12 @@ struct KParams {
     const double *ghost[3][2];
     const int *mirror;        // [pitch] RT_BC_REFLECT (x2 only): index of the direction with n-hat^2 flipped
     const double *rho, *u4;  // library-owned fluid copies
-    const int *srclist;      // cells with rho >= rho_floor (the only ones the source step can touch), built by rt_set_fluid
-    int nsrc;
-    const int *vaclist;      // the other cells (only when both lists are non-empty)
-    int nvac;
+    // interaction list (rt_set_fluid, cub partition): srclist[0 .. *nsel) = cells with rho >= rho_floor in ascending order (the only
+    // ones the source step can touch), srclist[*nsel .. ncell) = the others.  The length stays on the DEVICE (no read-back, no
+    // synchronisation in rt_set_fluid): list kernels read *nsel and run grid-stride.  srclist == nullptr: no list (no opacity or
+    // no source step).
+    const int *srclist;
+    const int *nsel;
 };
 
 // Layout of the column-flag buffer: [ncol] column flags, then (4-byte aligned)
@@ -90,7 +92,7 @@ cudaError_t launch_angular(const KParams &p, const double *I_in, double *I_io, d
 cudaError_t launch_source(const KParams &p, double *I, double *T, double dt, int *n_fail, double *R_after, double *G,
                           cudaStream_t st, long long *launches);
 // rt_moments_mma.cu: R^mu_nu of all cells (list == nullptr) or of list[0 .. n) on the fp64 tensor pipe
-cudaError_t launch_moments_mma(const KParams &p, const double *I, double *R, const int *list, int n, cudaStream_t st);
+cudaError_t launch_moments_mma(const KParams &p, const double *I, double *R, bool complement, cudaStream_t st);
 cudaError_t launch_moments(const KParams &p, const double *I, double *R, cudaStream_t st, long long *launches);
 
 }  // namespace rt

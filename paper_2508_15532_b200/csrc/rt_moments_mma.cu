@@ -57,7 +57,10 @@ k_moments_mma(const __grid_constant__ KParams p, const double *__restrict__ I, d
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int g = lane >> 2, t = lane & 3;
     double *mo = mout + warp * 80;
-    const long long nwork = LIST ? (long long)p.nsrc : p.ncell;
+    // LIST: the complement of the interaction list, srclist[*nsel .. ncell) (the length lives on the device)
+    const long long noff = LIST ? (long long)__ldg(p.nsel) : 0;
+    const int *list = LIST ? p.srclist + noff : nullptr;
+    const long long nwork = p.ncell - noff;
     const long long ngroups = (nwork + 7) / 8;
     const long long gw = (long long)blockIdx.x * MM_WARPS + warp, gstride = (long long)gridDim.x * MM_WARPS;
     const int npair = p.pitch / 8;
@@ -69,7 +72,7 @@ k_moments_mma(const __grid_constant__ KParams p, const double *__restrict__ I, d
     auto lookup = [&](long long grp_, bool &valid_) -> long long {
         const long long wi = grp_ * 8 + g;
         valid_ = grp_ < ngroups && wi < nwork;
-        return valid_ ? (LIST ? (long long)__ldg(p.srclist + wi) : wi) : 0;
+        return valid_ ? (LIST ? (long long)__ldg(list + wi) : wi) : 0;
     };
     bool valid;
     long long cell = lookup(gw, valid);
@@ -121,7 +124,7 @@ k_moments_mma(const __grid_constant__ KParams p, const double *__restrict__ I, d
             const int cl = lane & 7, nu = lane >> 3;
             const long long wj = grp * 8 + cl;
             if (wj < nwork) {
-                const long long cj = LIST ? (long long)p.srclist[wj] : wj;
+                const long long cj = LIST ? (long long)list[wj] : wj;
                 const int col = int((unsigned)cj % (unsigned)p.ncol);
                 const double *ecen = p.ecen + (long long)col * 16, *L = p.cen + (long long)col * CEN_STRIDE + 28;
                 const double *M = mo + cl * 10;
@@ -143,20 +146,16 @@ k_moments_mma(const __grid_constant__ KParams p, const double *__restrict__ I, d
 
 }  // namespace
 
-// R^mu_nu of all cells (list == nullptr) or of the cells in list[0 .. n)
-cudaError_t launch_moments_mma(const KParams &p, const double *I, double *R, const int *list, int n, cudaStream_t st) {
-    const long long nwork = list ? (long long)n : p.ncell;
-    if (nwork == 0) return cudaSuccess;
+// R^mu_nu of all cells, or (complement) of the cells behind the interaction list
+cudaError_t launch_moments_mma(const KParams &p, const double *I, double *R, bool complement, cudaStream_t st) {
     const size_t smem = ((size_t)(p.pitch / 4) * 64 + MM_WARPS * 80) * sizeof(double);
-    const long long groups = (nwork + 7) / 8;
+    const long long groups = (p.ncell + 7) / 8;
     long long blocks = (groups + MM_WARPS - 1) / MM_WARPS;
     if (blocks > 148LL * 8) blocks = 148LL * 8;
     cudaError_t e;
-    if (list) {
-        KParams q = p;
-        q.srclist = list; q.nsrc = n;
+    if (complement) {
         e = cudaFuncSetAttribute(k_moments_mma<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) k_moments_mma<true><<<(unsigned)blocks, 32 * MM_WARPS, smem, st>>>(q, I, R);
+        if (e == cudaSuccess) k_moments_mma<true><<<(unsigned)blocks, 32 * MM_WARPS, smem, st>>>(p, I, R);
     } else {
         e = cudaFuncSetAttribute(k_moments_mma<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e == cudaSuccess) k_moments_mma<false><<<(unsigned)blocks, 32 * MM_WARPS, smem, st>>>(p, I, R);

@@ -150,7 +150,7 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
     const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
 
     // LIST: the warp index runs over the compact list of cells above the density floor (built by rt_set_fluid)
-    const long long nwork = LIST ? (long long)p.nsrc : p.ncell;
+    const long long nwork = LIST ? (long long)__ldg(p.nsel) : p.ncell;
     for (long long widx = warp0; widx < nwork; widx += nwarps) {
         const long long cell = LIST ? (long long)p.srclist[widx] : widx;
         if (!SRC && widx + nwarps < nwork) {   // moments-only passes stream: next cell of this warp, one 128-byte line per lane, into L2/L1
@@ -293,7 +293,8 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
 template <bool SRC, bool MOM, bool LIST>
 cudaError_t launch_cell(const KParams &p, double *I, double *T, double dt, int *n_fail, double *R, double *G, cudaStream_t st) {
     const int threads = SRC ? CELL_THREADS : MOM_THREADS;
-    const long long nwork = LIST ? (long long)p.nsrc : p.ncell;
+    // a list's length is only known on the device: a fixed grid, the kernel strides over whatever the list holds
+    const long long nwork = p.ncell;
     long long want = (nwork + threads / 32 - 1) / (threads / 32);
     const int blocks = (int)(want < 148LL * 8 * 4 ? want : 148LL * 8 * 4);
     if (blocks == 0) return cudaSuccess;
@@ -314,7 +315,7 @@ cudaError_t launch_source(const KParams &p, double *I, double *T, double dt, int
                           cudaStream_t st, long long *launches) {
     cudaError_t e = cudaSuccess;
     if (G) e = cudaMemsetAsync(G, 0, 4 * p.ncell * sizeof(double), st);
-    const bool listed = p.method != 0 && p.nsrc > 0;
+    const bool listed = p.method != 0 && p.srclist != nullptr;   // (the list may still be empty: its kernels then find nothing to do)
     if (e == cudaSuccess && listed) {
         ++*launches;
         // with moments wanted the listed cells get theirs here (R after, G from before/after); the rest below
@@ -322,20 +323,15 @@ cudaError_t launch_source(const KParams &p, double *I, double *T, double dt, int
                            : launch_cell<true, false, true>(p, I, T, dt, n_fail, nullptr, nullptr, st);
     }
     if (e == cudaSuccess && R_after) {   // cells the source step did not visit: the tensor-pipe moments pass (rt_moments_mma.cu)
-        if (!listed) {                       // no source step anywhere: one pass over all cells
-            ++*launches;
-            e = launch_moments_mma(p, I, R_after, nullptr, 0, st);
-        } else if (p.nvac > 0) {
-            ++*launches;
-            e = launch_moments_mma(p, I, R_after, p.vaclist, p.nvac, st);
-        }
+        ++*launches;
+        e = launch_moments_mma(p, I, R_after, listed, st);   // listed: the complement of the list; else every cell
     }
     return e;
 }
 
 cudaError_t launch_moments(const KParams &p, const double *I, double *R, cudaStream_t st, long long *launches) {
     ++*launches;
-    return launch_moments_mma(p, I, R, nullptr, 0, st);
+    return launch_moments_mma(p, I, R, false, st);
 }
 
 }  // namespace rt
