@@ -446,8 +446,9 @@ k_transport_tile(const __grid_constant__ KParams p, const __grid_constant__ Tile
 // ---- the Eq 23 cells through the same ring --------------------------------------------------------------------------------
 // Cells with a non-vacuum face (mask bit of k_colflag) of the non-"general" pairs: full five-point stencils in all three
 // dims, both PLI states at the six faces, Eq 20 or Eq 23 per face from the per-face coefficients of k_facecoef -- the
-// arithmetic of k_transport_gen (rt_transport.cu), in the same order, with the thirteen operands taken from the ring instead
-// of thirteen global loads.  One pair per thread (the Eq 23 path holds ten face coefficients and a five-deep x3 window);
+// arithmetic of k_transport_gen (rt_transport.cu) with the thirteen operands taken from the ring instead of thirteen global
+// loads, except that the x3 face flux and slope a step has formed are carried to the next step instead of being formed again
+// (the results agree with k_transport_gen's to rounding).  One pair per thread (the Eq 23 path holds ten face coefficients and a five-deep x3 window);
 // tiles without such a cell leave at once; steps whose cell is all-vacuum only shift the window.
 constexpr int NTG = 480;     // consumer threads of k_transport_tile_gen (+ one producer warp)
 template <bool SAME_BASE>
@@ -613,6 +614,8 @@ k_transport_tile_gen(const __grid_constant__ KParams p, const __grid_constant__ 
         }
     }
     double *outk = I_out + (live ? trow : 0);
+    double dz2 = w3 - w2, s0z = slope_mc(w2 - w1, dz2), Fzl = 0.0;   // x3 carries: I_{k+1} - I_k, slope of cell k, flux through its low face
+    bool zcarry = false;
 
     // The march is NOT unrolled over the ring (the body is ~400 instructions: eight copies overflow the instruction cache and
     // spill); the slot offsets are run-time values, three adds per step.
@@ -633,16 +636,24 @@ k_transport_tile_gen(const __grid_constant__ KParams p, const __grid_constant__ 
         if (matn && k + 1 < n3) {   // the per-face coefficients of the next step: towards L1 now (no registers held)
             pf_l1(px + sxf); pf_l1(py + syf); pf_l1(py + syf + n1); pf_l1(pz + 2 * ncol);
         }
+        // x3: the slope of cell k + 1 is formed every step and carried (it is the next step's own slope)
+        const double dz3 = w4 - w3, spz = slope_mc(dz2, dz3);
         if (mat) {
-            const double4 fzl = ld4(pz), fzh = ld4(pz + ncol), fxl = ld4(px), fxh = ld4(px + 1), fyl = ld4(py), fyh = ld4(py + n1);
+            const double4 fzh = ld4(pz + ncol), fxl = ld4(px), fxh = ld4(px + 1), fyl = ld4(py), fyh = ld4(py + n1);
             const double xm2 = lds(a_x[0] + sk), xm1 = lds(a_x[1] + sk), xp1 = lds(a_x[2] + sk), xp2 = lds(a_x[3] + sk);
             const double ym2 = lds(a_y[0] + sk), ym1 = lds(a_y[1] + sk), yp1 = lds(a_y[2] + sk), yp2 = lds(a_y[3] + sk);
             const double cbase = SAME_BASE ? w2 : lds(a_base + sb);
-            double D = flux_diff<RT_LIM_MC, true>(w0, w1, w2, w3, w4, zf, zf, fzl, fzh);
+            // x3: the flux through the low face is the one the step before sent through its high face (same thread, same
+            // folded coefficients: the geometry does not depend on x3); formed afresh only at the start of a run of such cells
+            if (!zcarry) Fzl = face_flux<true>(zf, w1 + 0.5 * slope_mc(w1 - w0, w2 - w1), w2 - 0.5 * s0z, w1, w2, ld4(pz));
+            const double Fzh = face_flux<true>(zf, w2 + 0.5 * s0z, w3 - 0.5 * spz, w2, w3, fzh);
+            double D = Fzh - Fzl;
             D += flux_diff<RT_LIM_MC, true>(xm2, xm1, w2, xp1, xp2, xl, xh, fxl, fxh);
             D += flux_diff<RT_LIM_MC, true>(ym2, ym1, w2, yp1, yp2, yl, yh, fyl, fyh);
             *outk = (k < zlo || k >= zhi) ? 0.0 : cbase - D;      // Eq 18 (O5), dt / (n^0 n_0 sqrt(-g) dx) folded in
+            Fzl = Fzh;
         }
+        zcarry = mat;
         const int u1 = u + 1 < NS ? u + 1 : 0;
         const uint32_t par1 = par0 ^ (uint32_t)(u + 1 == NS);
         if (k + 1 < n3) {   // probe the next step's barriers; the answer is there when it is needed
@@ -650,7 +661,7 @@ k_transport_tile_gen(const __grid_constant__ KParams p, const __grid_constant__ 
             ready = mbar_test(bar_full + 8 * uo1, par1 ^ (uint32_t)(u1 + 4 >= NS));
             if (!SAME_BASE) ready = mbar_test(bar_fullB + 8 * u1, par1) && ready;
         }
-        w0 = w1; w1 = w2; w2 = w3; w3 = w4;
+        w0 = w1; w1 = w2; w2 = w3; w3 = w4; dz2 = dz3; s0z = spz;
         outk += kstride; px += sxf; py += syf; pz += ncol;
         __syncwarp();
         if (lane == 0) {

@@ -53,10 +53,16 @@ def test_slabs_reproduce_the_single_domain(idx, n, world, bc3):
         whole = getattr(one, name)
         parts = torch.cat([d.owned(getattr(d, name), lead) for d in doms], dim=lead)
         assert parts.shape == whole.shape, name
-        assert torch.equal(parts, whole), (name, float((parts - whole).abs().max()))
+        if bc3 is None:
+            assert torch.equal(parts, whole), (name, float((parts - whole).abs().max()))
+        else:
+            # a ZERO ghost in x3 keeps the whole domain on the per-thread-load kernels while the slabs below the top one (their
+            # upper x3 side is an interior cut) run the tile kernels: same scheme, face fluxes combined in another order
+            scale = float(one.R.abs().max()) / dt if name == "G" else float(whole.abs().max())
+            assert float((parts - whole).abs().max()) <= 1e-13 * scale, name
     # and the margins hold the neighbours' owned planes after the exchange
     for d in doms:
-        assert torch.equal(d.I, one.I[torch.as_tensor(d.layout.planes, device=one.I.device)])
+        assert torch.equal(d.I, torch.cat([dd.owned(dd.I, 0) for dd in doms], dim=0)[torch.as_tensor(d.layout.planes, device=one.I.device)])
 
 
 @pytest.mark.parametrize("idx,n", [(4, (14, 12, 32)), (4, (12, 10, 19)), (3, (9, 8, 24)), (2, (6, 5, 8))])

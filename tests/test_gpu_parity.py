@@ -371,8 +371,10 @@ def test_smem_variant_matches_oracle(idx, n, steps):
 
 
 @pytest.mark.parametrize("idx,n", [(4, (20, 18, 5)), (1, (9, 7, 2)), (4, (7, 3, 9)), (5, (6, 10, 4))])
-def test_smem_variant_bit_equal_to_default(idx, n):
-    """Same arithmetic in the same order (only the way the x2 operands reach the thread differs): identical bits."""
+def test_smem_variant_equal_to_default(idx, n):
+    """Vacuum cells: same arithmetic in the same order (only the way the operands reach the thread differs), identical bits.
+    Cells with an Eq 23 face: the tile kernel forms every face flux once and applies the cell factor last, the round-1
+    kernel folds it into the face coefficients, so they agree to rounding, far inside the parity tolerance."""
     import torch
     cfg = W.config(idx, n=n)
     res = []
@@ -386,9 +388,16 @@ def test_smem_variant_bit_equal_to_default(idx, n):
         for _ in range(3):
             ctx.step(I, T, dt, R, G)
         res.append((I.clone(), T.clone(), R.clone(), G.clone()))
+        matter = bool(cfg["options"].get("kappa_a0", 0.0) or cfg["options"].get("kappa_s", 0.0))
         ctx.close()
-    for a, b in zip(*res):
-        assert torch.isfinite(a).all() and torch.equal(a, b)
+    rmax = float(res[0][2].abs().max())
+    for name, a, b in zip("ITRG", *res):
+        assert torch.isfinite(a).all()
+        if matter:
+            scale = rmax / dt if name == "G" else float(a.abs().max())     # G = -(R after - R before) / dt
+            assert float((a - b).abs().max()) <= 1e-13 * max(scale, 1e-300), name
+        else:
+            assert torch.equal(a, b), name
 
 
 def test_unknown_transport_variant_rejected():
