@@ -91,8 +91,8 @@ cudaError_t launch_angular(const KParams &p, const double *I_in, double *I_io, d
 // G_nu = -(R^0_nu after - before)/dt.
 cudaError_t launch_source(const KParams &p, double *I, double *T, double dt, int *n_fail, double *R_after, double *G,
                           cudaStream_t st, long long *launches);
-// rt_moments_mma.cu: R^mu_nu of all cells (list == nullptr) or of list[0 .. n) on the fp64 tensor pipe
-cudaError_t launch_moments_mma(const KParams &p, const double *I, double *R, bool complement, cudaStream_t st);
+// rt_moments_mma.cu: R^mu_nu on the fp64 tensor pipe; part: 0 all cells, 1 interaction list, 2 its complement; gmode: see the kernel
+cudaError_t launch_moments_mma(const KParams &p, const double *I, double *R, double *G, int part, int gmode, double dt, cudaStream_t st);
 cudaError_t launch_moments(const KParams &p, const double *I, double *R, cudaStream_t st, long long *launches);
 
 }  // namespace rt

@@ -1,4 +1,4 @@
-// Moments-only pass of librt_b200 (sm_100a) on the fp64 tensor pipe: R^mu_nu of cells the source step does not visit.
+// Moments pass of librt_b200 (sm_100a) on the fp64 tensor pipe: R^mu_nu (and the 4-force G_nu around a source step).
 //
 // PAPER.md Eq 13 (L141): R^mu_nu = sum_s w_s I_s n^mu n_nu.  In the tetrad frame the ten independent sums
 //     M^{ab}(cell) = sum_s I(cell, s) W(s, ab),      W(s, ab) = w_s nhat^a_s nhat^b_s     (nhat^0 = 1)
@@ -6,10 +6,10 @@
 // unit applies (the paper itself singles this reduction out, L776).  One warp takes 8 cells at a time and runs
 // mma.sync.m8n8k4.f64 over the direction axis (A = 8 cells x 4 directions straight from global memory, one 16-byte load per
 // lane per two k-steps; B = W in fragment order from shared memory; two 8-wide column tiles hold the 10 components), then
-// rotates M to R^mu_nu = e^mu_a M^{ab} (e^lam_b g_{lam nu}) with the per-column rows, as k_cell does.  About 40
-// warp-instructions per cell instead of k_cell<MOM>'s ~350: the pass becomes a stream over the intensity.
-// The sums run in a fixed order, so the result is bit-reproducible; it differs from k_cell<MOM>'s (another order) in the
-// last bits, inside the 1e-10 parity budget like every other reduction here.
+// rotates M to R^mu_nu = e^mu_a M^{ab} (e^lam_b g_{lam nu}) with the per-column rows.  About 40 warp-instructions per
+// cell instead of the ~350 of a lane-per-direction accumulation with warp reductions (round 1): the pass is a stream over
+// the intensity.  The sums run in a fixed order, so the result is bit-reproducible; it differs from the oracle's sequential
+// sum in the last bits, inside the 1e-10 parity budget like every other reduction here.
 #include "rt_kernels.cuh"
 
 namespace rt {
@@ -21,7 +21,7 @@ __device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
-// component c of the ten: 00 01 02 03 11 12 13 22 23 33 (the order of k_cell's mom_accumulate)
+// component c of the ten: 00 01 02 03 11 12 13 22 23 33 
 __device__ __forceinline__ double wcomp(int c, double w, double nx, double ny, double nz) {
     switch (c) {
         case 0: return w;
@@ -39,9 +39,14 @@ __device__ __forceinline__ double mget(const double *M, int a, int b) {
 
 // Direction order of the contraction: k-step 2 jj takes the directions 8 jj + 2 t, k-step 2 jj + 1 the directions
 // 8 jj + 2 t + 1 (t = lane % 4), so that a lane's two A values are adjacent in memory; a tail of (pitch % 8) / 4 single steps.
+// part: 0 = every cell, 1 = the cells of the interaction list, 2 = the others (LIST kernels only).
+// gmode: 0 = R only; 1 = R^0_nu into G (the moments BEFORE a source step; R untouched); 2 = R (if given), and
+// G_nu = -(R^0_nu - G_nu) / dt (Eq 36 / 48: G holds the moments before, left there by a gmode-1 pass over the same cells; a cell
+// the source step did not change gets exactly 0: both passes add the same numbers in the same order).
 template <bool LIST>
 __global__ void __launch_bounds__(32 * MM_WARPS, 2)
-k_moments_mma(const __grid_constant__ KParams p, const double *__restrict__ I, double *__restrict__ R) {
+k_moments_mma(const __grid_constant__ KParams p, const double *__restrict__ I, double *__restrict__ R, double *__restrict__ G,
+              int part, int gmode, double inv_dt) {
     extern __shared__ double sm[];
     const int nks = p.pitch / 4;                       // k-steps (pitch is a multiple of 4)
     double *bfrag = sm;                                // [nks][2 tiles][32 lanes]
@@ -57,10 +62,10 @@ k_moments_mma(const __grid_constant__ KParams p, const double *__restrict__ I, d
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int g = lane >> 2, t = lane & 3;
     double *mo = mout + warp * 80;
-    // LIST: the complement of the interaction list, srclist[*nsel .. ncell) (the length lives on the device)
-    const long long noff = LIST ? (long long)__ldg(p.nsel) : 0;
-    const int *list = LIST ? p.srclist + noff : nullptr;
-    const long long nwork = p.ncell - noff;
+    // LIST: the interaction list srclist[0 .. *nsel) or its complement srclist[*nsel .. ncell) (the length lives on the device)
+    const long long nsel = LIST ? (long long)__ldg(p.nsel) : 0;
+    const int *list = LIST ? p.srclist + (part == 2 ? nsel : 0) : nullptr;
+    const long long nwork = LIST ? (part == 2 ? p.ncell - nsel : nsel) : p.ncell;
     const long long ngroups = (nwork + 7) / 8;
     const long long gw = (long long)blockIdx.x * MM_WARPS + warp, gstride = (long long)gridDim.x * MM_WARPS;
     const int npair = p.pitch / 8;
@@ -134,8 +139,14 @@ k_moments_mma(const __grid_constant__ KParams p, const double *__restrict__ I, d
                 for (int a2 = 0; a2 < 4; ++a2) T[a2] = mget(M, a2, 0) * l0 + mget(M, a2, 1) * l1 + mget(M, a2, 2) * l2 + mget(M, a2, 3) * l3;
 #pragma unroll
                 for (int mu = 0; mu < 4; ++mu) {
+                    if (mu > 0 && gmode == 1) break;
                     const double2 ea = __ldg(reinterpret_cast<const double2 *>(ecen + 4 * mu)), eb = __ldg(reinterpret_cast<const double2 *>(ecen + 4 * mu + 2));
-                    R[(long long)(4 * mu + nu) * p.ncell + cj] = ea.x * T[0] + ea.y * T[1] + eb.x * T[2] + eb.y * T[3];
+                    const double r = ea.x * T[0] + ea.y * T[1] + eb.x * T[2] + eb.y * T[3];
+                    if (gmode != 1 && R) R[(long long)(4 * mu + nu) * p.ncell + cj] = r;
+                    if (mu == 0 && gmode != 0) {
+                        double *g = G + (long long)nu * p.ncell + cj;
+                        *g = (gmode == 1) ? r : -(r - *g) * inv_dt;
+                    }
                 }
             }
         }
@@ -146,19 +157,20 @@ k_moments_mma(const __grid_constant__ KParams p, const double *__restrict__ I, d
 
 }  // namespace
 
-// R^mu_nu of all cells, or (complement) of the cells behind the interaction list
-cudaError_t launch_moments_mma(const KParams &p, const double *I, double *R, bool complement, cudaStream_t st) {
+// Moments of every cell (part 0), of the listed cells (1) or of the others (2); see the kernel for gmode
+cudaError_t launch_moments_mma(const KParams &p, const double *I, double *R, double *G, int part, int gmode, double dt, cudaStream_t st) {
     const size_t smem = ((size_t)(p.pitch / 4) * 64 + MM_WARPS * 80) * sizeof(double);
     const long long groups = (p.ncell + 7) / 8;
     long long blocks = (groups + MM_WARPS - 1) / MM_WARPS;
     if (blocks > 148LL * 8) blocks = 148LL * 8;
+    const double inv_dt = gmode == 2 ? 1.0 / dt : 0.0;
     cudaError_t e;
-    if (complement) {
+    if (part != 0) {
         e = cudaFuncSetAttribute(k_moments_mma<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) k_moments_mma<true><<<(unsigned)blocks, 32 * MM_WARPS, smem, st>>>(p, I, R);
+        if (e == cudaSuccess) k_moments_mma<true><<<(unsigned)blocks, 32 * MM_WARPS, smem, st>>>(p, I, R, G, part, gmode, inv_dt);
     } else {
         e = cudaFuncSetAttribute(k_moments_mma<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) k_moments_mma<false><<<(unsigned)blocks, 32 * MM_WARPS, smem, st>>>(p, I, R);
+        if (e == cudaSuccess) k_moments_mma<false><<<(unsigned)blocks, 32 * MM_WARPS, smem, st>>>(p, I, R, G, part, gmode, inv_dt);
     }
     return e != cudaSuccess ? e : cudaGetLastError();
 }

@@ -1,17 +1,16 @@
-// Cell-local kernels of librt_b200 (sm_100a): implicit radiation-fluid source step (O6) fused with the moment
-// reduction (O7) and the 4-force (Eq 36/48).
+// Cell-local kernel of librt_b200 (sm_100a): the implicit radiation-fluid source step (O6).
 //
 // PAPER.md: fluid-frame boost Eq 5 (L85) with I/nu^4 and nu^2 dOmega invariance (S17); angular sums Eq 33, 41
 // (L344, L388-390); temperature equations Eq 42 / 43 / 46 (L396-426; S19: A' = alpha_- dt A); intensity update
-// Eq 35 (L352) with the coefficients the T-equation was built from (S19b); density floor L468; moments Eq 13
-// (L141); G_nu = -(R^0_nu after - before)/dt (Eq 36, 48).
+// Eq 35 (L352) with the coefficients the T-equation was built from (S19b); density floor L468.
+// The moments (Eq 13) and the 4-force G_nu = -(R^0_nu after - before)/dt (Eq 36, 48) come from the tensor-pipe pass of
+// rt_moments_mma.cu, run before and after this kernel on the same cells (launch_source below).
 //
-// Design: one warp per cell; the cell's N_d intensities live in registers (MAXV per lane, s = lane + 32 v, so
-// every load/store is a 256-byte coalesced row); all angular sums are butterfly warp reductions (fixed order =>
-// bit-reproducible); the scalar temperature solve runs redundantly on all lanes (no divergence, no broadcast).
-// Moments are accumulated in the TETRAD frame, M^{ab} = sum_s w_s I_s n^a n^b (10 sums with constant n-hat), and
-// rotated once per cell: R^mu_nu = e^mu_a M^{ab} (e^lam_b g_{lam nu}).
+// Design: a warp takes CB cells of the interaction list per trip; a cell's N_d intensities live in registers (MAXV per
+// lane, s = lane + 32 v, so every load/store is a 256-byte coalesced row); the angular sums are added in a fixed order
+// (bit-reproducible); see k_cell_batch.
 #include <cmath>
+#include <type_traits>
 
 #include "rt_kernels.cuh"
 
@@ -24,36 +23,6 @@ constexpr double FOURPI = 12.566370614359172953850573533118;
 __device__ __forceinline__ double t_m35(double T) {
     const double r = __drcp_rn(T);
     return r * r * r * sqrt(r);
-}
-__device__ __forceinline__ double warp_sum(double v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
-
-// Sums of the ten moment components over the 32 lanes through shared memory: every lane stores its ten partial sums
-// (row c at scr[c * 33 + lane]), three lanes add up each row (11 + 11 + 10 entries, combined by two shuffles), the
-// ten totals are written behind the rows and read back by all lanes.  ~45 instructions per lane instead of the 150 of
-// ten butterfly reductions; fixed order => bit-reproducible.  scr: WSUM_DOUBLES doubles owned by the warp.
-constexpr int WSUM_DOUBLES = 10 * 33 + 10;
-__device__ __forceinline__ void warp_sum10(double M[10], double *scr, int lane) {
-#pragma unroll
-    for (int c = 0; c < 10; ++c) scr[c * 33 + lane] = M[c];
-    __syncwarp();
-    const int c = lane / 3, q = lane - 3 * c;
-    double t = 0.0;
-    if (lane < 30) {
-        const double *r = scr + c * 33 + q * 11;
-#pragma unroll
-        for (int m = 0; m < 10; ++m) t += r[m];
-        if (q < 2) t += r[10];
-    }
-    const double t1 = __shfl_down_sync(0xffffffffu, t, 1), t2 = __shfl_down_sync(0xffffffffu, t, 2);
-    if (lane < 30 && q == 0) scr[330 + c] = (t + t1) + t2;
-    __syncwarp();
-#pragma unroll
-    for (int k = 0; k < 10; ++k) M[k] = scr[330 + k];
-    __syncwarp();
 }
 
 struct TEq {
@@ -109,135 +78,135 @@ __device__ __forceinline__ bool solve_T(const TEq &q, double Tm, double Thi, dou
     return true;
 }
 
-// 10 independent components of M^{ab}: 00 01 02 03 11 12 13 22 23 33
-__device__ __forceinline__ void mom_accumulate(double M[10], double wI, double nx, double ny, double nz) {
-    M[0] += wI;
-    M[1] += wI * nx; M[2] += wI * ny; M[3] += wI * nz;
-    M[4] += wI * nx * nx; M[5] += wI * nx * ny; M[6] += wI * nx * nz;
-    M[7] += wI * ny * ny; M[8] += wI * ny * nz; M[9] += wI * nz * nz;
-}
-__device__ __forceinline__ double mom_get(const double M[10], int a, int b) {
-    if (a > b) { int t = a; a = b; b = t; }
-    const int base[4] = {0, 4, 7, 9};
-    return M[base[a] + (b - a)];
-}
-// R^mu_nu for (mu, nu) from tetrad-frame M, e^mu_a (ecen) and L[b][nu] (cen + 28)
-__device__ __forceinline__ double rotate(const double M[10], const double *__restrict__ ecen, const double *__restrict__ L, int mu, int nu) {
-    double r = 0.0;
-    for (int a = 0; a < 4; ++a) {
-        double t = 0.0;
-        for (int b = 0; b < 4; ++b) t += mom_get(M, a, b) * L[4 * b + nu];
-        r += ecen[4 * mu + a] * t;
-    }
-    return r;
-}
+constexpr int CELL_THREADS = 128, CELL_MINB = 4;   // 128 registers, 16 warps per SM
 
-// source-step variants: 128 registers, 16 warps per SM (80 registers x 24 warps spills and is 2-3 % slower)
-constexpr int CELL_THREADS = 128, CELL_MINB = 4;
-// moments-only instantiation (kept for completeness; the moments-only passes run in rt_moments_mma.cu)
-constexpr int MOM_THREADS = 256, MOM_MINB = 4;
-template <int MAXV, bool SRC, bool MOM, bool LIST>
-__global__ void __launch_bounds__(SRC ? CELL_THREADS : MOM_THREADS, (SRC ? CELL_MINB : (MAXV > 6 ? MOM_MINB - 2 : MOM_MINB)))   // moments-only, 362 directions: 12 values per lane, 128 registers
-k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, double *G_out) {
-    extern __shared__ double tab[];   // nx[pitch] ny[pitch] nz[pitch] w[pitch], then one warp_sum10 scratch per warp
+// ---- the source step, CB cells per warp trip -----------------------------------------------------------------------------
+// With one cell per warp trip (round 1) about half of the ~760 instructions per cell (162 directions) were scalar work every
+// lane repeats (fluid-frame velocity, opacities, the temperature solve with its dependent reciprocal chain), and the warp's
+// instruction stream was one long dependent chain.  Here a warp takes CB listed cells per trip:
+//   phase 0  lane l does the scalar set-up of cell l mod CB (loads, opacities, u-hat): once per trip, not once per cell;
+//   phase 1  cell by cell, lanes over directions: nbar, d, the three angular sums of Eq 33 / 41 as per-lane partials, and the
+//            two coefficients of Eq 35 (n^0 I / d stays in the value's register, 1 / (d nbar^3) goes to shared memory);
+//            the CB cells' loops are independent instruction streams the scheduler can overlap;
+//   sums     the 3 CB rows of partials are added through shared memory in a fixed order (two lanes per row);
+//   phase 2  lane l solves the temperature equation of cell l mod CB: ONE solve stream for the CB cells;
+//   phase 3  cell by cell: Eq 35, store.
+template <int MAXV>
+struct CellBatch { static constexpr int CB = MAXV <= 3 ? 8 : (24 / MAXV > 0 ? 24 / MAXV : 1); };
+
+template <int MAXV>
+__global__ void __launch_bounds__(CELL_THREADS, CELL_MINB)
+k_cell_batch(KParams p, double *I, double *T, double dt, int *n_fail) {
+    constexpr int CB = CellBatch<MAXV>::CB;
+    constexpr int PART = CB * 3 * 33 + CB * 3;                                   // partial sums [CB * 3][33], totals [CB * 3]
+    constexpr int SCR = MAXV * 32 * CB + PART;
+    extern __shared__ double tab[];   // nx[pitch] ny[pitch] nz[pitch] w[pitch], then one scratch area per warp
     for (int t = threadIdx.x; t < 3 * p.pitch; t += blockDim.x) tab[t] = p.nhat[t];
     for (int t = threadIdx.x; t < p.pitch; t += blockDim.x) tab[3 * p.pitch + t] = p.w[t];
     __syncthreads();
     const double *snx = tab, *sny = tab + p.pitch, *snz = tab + 2 * p.pitch, *sw = tab + 3 * p.pitch;
     const int lane = threadIdx.x & 31;
-    double *scr = tab + 4 * p.pitch + (threadIdx.x >> 5) * WSUM_DOUBLES;
+    double *cbs = tab + 4 * p.pitch + (threadIdx.x >> 5) * SCR;   // [CB][MAXV * 32]: 1 / (d nbar^3) of every direction
+    double *part = cbs + MAXV * 32 * CB;
     const long long warp0 = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5;
     const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
+    const long long nwork = (long long)__ldg(p.nsel);
+    const int myc = lane % CB;   // the cell of the trip whose scalars this lane holds
 
-    // LIST: the warp index runs over the compact list of cells above the density floor (built by rt_set_fluid)
-    const long long nwork = LIST ? (long long)__ldg(p.nsel) : p.ncell;
-    for (long long widx = warp0; widx < nwork; widx += nwarps) {
-        const long long cell = LIST ? (long long)p.srclist[widx] : widx;
-        if (!SRC && widx + nwarps < nwork) {   // moments-only passes stream: next cell of this warp, one 128-byte line per lane, into L2/L1
-            const long long nc = LIST ? (long long)p.srclist[widx + nwarps] : widx + nwarps;
-            const char *nx = reinterpret_cast<const char *>(I + nc * p.pitch) + lane * 128;
-            if (lane * 128 < p.pitch * 8) asm volatile("prefetch.global.L1 [%0];" ::"l"(nx));
-        }
-        const int col = int((unsigned)cell % (unsigned)p.ncol);   // cell < 2^31 (the lists hold ints)
-        const double *cen = p.cen + (long long)col * CEN_STRIDE;
-        double *Ic = I + cell * p.pitch;
-        // all independent loads first: the cell's intensities (needed for every cell only when moments are wanted)
-        // and its fluid state
-        double val[MAXV];
-        if (MOM) {
-#pragma unroll
-            for (int v = 0; v < MAXV; ++v) {
-                const int s = lane + 32 * v;
-                val[v] = (s < p.nd) ? Ic[s] : 0.0;
-            }
-        }
-        double alpha = 0.0, aa = 0.0, as = 0.0, rho = 0.0, Tm = 0.0, u0 = 1.0, u1 = 0.0, u2 = 0.0, u3 = 0.0;
-        if (SRC) {
-            rho = p.rho[cell];
-            Tm = T[cell];
-            u0 = p.u4[cell]; u1 = p.u4[p.ncell + cell]; u2 = p.u4[2 * p.ncell + cell]; u3 = p.u4[3 * p.ncell + cell];
+    for (long long w0 = warp0 * CB; w0 < nwork; w0 += nwarps * CB) {
+        const int ncb = (int)((nwork - w0) < CB ? (nwork - w0) : CB);
+        // ---- phase 0: scalars of cell myc ----
+        const bool have = myc < ncb;
+        const long long mycell = have ? (long long)__ldg(p.srclist + w0 + myc) : 0;
+        double rho = 0.0, Tm = 1.0, aa = 0.0, as = 0.0, alpha = 0.0, uh0 = 1.0, uh1 = 0.0, uh2 = 0.0, uh3 = 0.0;
+        if (have) {
+            rho = p.rho[mycell];
+            Tm = T[mycell];
+            const double u0 = p.u4[mycell], u1 = p.u4[p.ncell + mycell], u2 = p.u4[2 * p.ncell + mycell], u3 = p.u4[3 * p.ncell + mycell];
+            const double *cen = p.cen + (long long)((unsigned)mycell % (unsigned)p.ncol) * CEN_STRIDE;
+            uh0 = cen[12] * u0 + cen[13] * u1 + cen[14] * u2 + cen[15] * u3;
+            uh1 = cen[16] * u0 + cen[17] * u1 + cen[18] * u2 + cen[19] * u3;
+            uh2 = cen[20] * u0 + cen[21] * u1 + cen[22] * u2 + cen[23] * u3;
+            uh3 = cen[24] * u0 + cen[25] * u1 + cen[26] * u2 + cen[27] * u3;
             if (rho >= p.rho_floor) {
                 aa = (p.kappa_a0 != 0.0) ? p.kappa_a0 * rho * rho * t_m35(Tm) : 0.0;
                 as = p.kappa_s * rho;
             }
             alpha = aa + as;
         }
-        const bool interact = SRC && p.method != 0 && alpha != 0.0;
-        if (!interact && !MOM) continue;
-        if (!MOM) {
+        const bool interact = have && p.method != 0 && alpha != 0.0;
+        const double adt = alpha * dt;
+
+        // ---- phase 1: per cell, lanes over directions ----
+        double val[CB][MAXV];          // I, then n^0 I / d for the cells that interact
+        unsigned livebits = 0u;        // bit c * MAXV + v: direction v of cell c is updated (not masked, not a pad entry)
+#pragma unroll
+        for (int c = 0; c < CB; ++c) {
+            const long long cell = __shfl_sync(0xffffffffu, mycell, c);
+            const bool inter_c = __shfl_sync(0xffffffffu, (int)interact, c) != 0;
+            const bool there = c < ncb;
+            const double *Ic = I + cell * p.pitch;
 #pragma unroll
             for (int v = 0; v < MAXV; ++v) {
                 const int s = lane + 32 * v;
-                val[v] = (s < p.nd) ? Ic[s] : 0.0;
+                val[c][v] = (there && s < p.nd) ? Ic[s] : 0.0;
             }
-        }
-        const double *ecen = p.ecen + (long long)col * 16, *L = cen + 28;
-        double Rb = 0.0;          // lanes 0..3: R^0_nu before the source step
-        bool updated = false;
-        if (interact) {
-            const double uh0 = cen[12] * u0 + cen[13] * u1 + cen[14] * u2 + cen[15] * u3;
-            const double uh1 = cen[16] * u0 + cen[17] * u1 + cen[18] * u2 + cen[19] * u3;
-            const double uh2 = cen[20] * u0 + cen[21] * u1 + cen[22] * u2 + cen[23] * u3;
-            const double uh3 = cen[24] * u0 + cen[25] * u1 + cen[26] * u2 + cen[27] * u3;
-            if (MOM && G_out) {   // moments before the update (only where the update can change them)
-                double Mb[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+            double E = 0.0, A1 = 0.0, A2 = 0.0;
+            if (inter_c) {
+                const double b0 = __shfl_sync(0xffffffffu, uh0, c), b1 = __shfl_sync(0xffffffffu, uh1, c);
+                const double b2 = __shfl_sync(0xffffffffu, uh2, c), b3 = __shfl_sync(0xffffffffu, uh3, c);
+                const double adt_c = __shfl_sync(0xffffffffu, adt, c);
+                const double *cen = p.cen + (long long)((unsigned)cell % (unsigned)p.ncol) * CEN_STRIDE;
+                const double g0 = __ldg(cen), g1 = __ldg(cen + 1), g2 = __ldg(cen + 2), g3 = __ldg(cen + 3);       // -> n_0
+                const double e0 = __ldg(cen + 4), e1 = __ldg(cen + 5), e2 = __ldg(cen + 6), e3 = __ldg(cen + 7);   // -> n^0
 #pragma unroll
                 for (int v = 0; v < MAXV; ++v) {
                     const int s = lane + 32 * v;
-                    if (s < p.nd) mom_accumulate(Mb, sw[s] * val[v], snx[s], sny[s], snz[s]);
-                }
-                warp_sum10(Mb, scr, lane);
-                if (lane < 4) Rb = rotate(Mb, ecen, L, 0, lane);
-            }
-            double E = 0.0, A1 = 0.0, A2 = 0.0;
-            const double g0 = __ldg(cen), g1 = __ldg(cen + 1), g2 = __ldg(cen + 2), g3 = __ldg(cen + 3);       // -> n_0
-            const double e0 = __ldg(cen + 4), e1 = __ldg(cen + 5), e2 = __ldg(cen + 6), e3 = __ldg(cen + 7);   // -> n^0
-            const double adt = alpha * dt;
-            // kept for the update loop below: ca = n^0/d (0 marks a masked or pad entry), cb = 1/(d nbar^3)
-            double ca[MAXV], cb[MAXV];
-#pragma unroll
-            for (int v = 0; v < MAXV; ++v) {
-                const int s = lane + 32 * v;
-                ca[v] = 0.0; cb[v] = 0.0;
-                if (s < p.nd) {
-                    const double nx = snx[s], ny = sny[s], nz = snz[s], ws = sw[s];
-                    const double n0c = g0 + g1 * nx + g2 * ny + g3 * nz;
-                    if (!(n0c > -p.n0_floor)) {
-                        const double nup = e0 + e1 * nx + e2 * ny + e3 * nz;
-                        const double nbar = uh0 - (uh1 * nx + uh2 * ny + uh3 * nz);       // Eq 5, first row
-                        // 1/d and 1/nbar from one reciprocal: 1/(d nbar) times nbar, times d
-                        const double d = nup + nbar * adt, r = __drcp_rn(d * nbar);
-                        const double rd = r * nbar, rn = r * d;
-                        const double IbdOm = nbar * nbar * val[v] * ws;                     // Ibar dOmegabar (S17)
-                        E += IbdOm;                                                         // Eq 33
-                        A1 += nup * rd * IbdOm;                                             // Eq 41a
-                        A2 += ws * rn * rd;                                                 // Eq 41b
-                        ca[v] = nup * rd;
-                        cb[v] = rd * (rn * rn * rn);
+                    double cb = 0.0, ca = 0.0;
+                    if (s < p.nd) {
+                        const double nx = snx[s], ny = sny[s], nz = snz[s], ws = sw[s];
+                        const double n0c = g0 + g1 * nx + g2 * ny + g3 * nz;
+                        if (!(n0c > -p.n0_floor)) {
+                            const double nup = e0 + e1 * nx + e2 * ny + e3 * nz;
+                            const double nbar = b0 - (b1 * nx + b2 * ny + b3 * nz);        // Eq 5, first row
+                            // 1/d and 1/nbar from one reciprocal: 1/(d nbar) times nbar, times d
+                            const double d = nup + nbar * adt_c, r = __drcp_rn(d * nbar);
+                            const double rd = r * nbar, rn = r * d;
+                            const double IbdOm = nbar * nbar * val[c][v] * ws;               // Ibar dOmegabar (S17)
+                            E += IbdOm;                                                     // Eq 33
+                            A1 += nup * rd * IbdOm;                                         // Eq 41a
+                            A2 += ws * rn * rd;                                             // Eq 41b
+                            ca = nup * rd;                                                  // n^0 / d
+                            cb = rd * (rn * rn * rn);                                       // 1 / (d nbar^3)
+                            livebits |= 1u << (c * MAXV + v);
+                        }
                     }
+                    val[c][v] = ca * val[c][v];
+                    cbs[(c * MAXV + v) * 32 + lane] = cb;
                 }
             }
-            E = warp_sum(E); A1 = warp_sum(A1); A2 = warp_sum(A2) * (dt / FOURPI);
+            part[(c * 3 + 0) * 33 + lane] = E; part[(c * 3 + 1) * 33 + lane] = A1; part[(c * 3 + 2) * 33 + lane] = A2;
+        }
+        __syncwarp();
+        // ---- the 3 CB sums: LPR lanes per row, each over its entries in index order, then one exchange ----
+        {
+            constexpr int LPR = (6 * CB <= 32) ? 2 : 1, NPL = 32 / LPR;
+            double t = 0.0;
+            if (lane < 3 * CB * LPR) {
+                const double *r = part + (lane / LPR) * 33 + (lane % LPR) * NPL;
+#pragma unroll
+                for (int m = 0; m < NPL; ++m) t += r[m];
+            }
+            if (LPR == 2) t += __shfl_xor_sync(0xffffffffu, t, 1);   // (the even lane adds first half + second half)
+            if (lane < 3 * CB * LPR && (lane % LPR) == 0) part[CB * 3 * 33 + lane / LPR] = t;
+        }
+        __syncwarp();
+        // ---- phase 2: lane l solves the temperature equation of cell l mod CB ----
+        bool ok = false;
+        double Tp = Tm, scale = 1.0, Sdt = 0.0;
+        if (interact) {
+            const double *tot = part + CB * 3 * 33 + myc * 3;
+            const double E = tot[0], A1 = tot[1], A2 = tot[2] * (dt / FOURPI);
             const double Y = p.Y_over_rho * rho, W = E + Y * Tm, Nbar = p.kappa_a0 * rho * rho;
             TEq q;
             q.method = p.method;
@@ -252,86 +221,90 @@ k_cell(KParams p, double *I, double *T, double dt, int *n_fail, double *R_out, d
                 q.k1 = -Y * Nbar * dt;
                 q.k0 = W * Nbar * dt;
             }
-            double Tp;
-            if (solve_T(q, Tm, W / Y, Tp)) {
+            ok = solve_T(q, Tm, W / Y, Tp);
+            if (ok) {
                 const double Ep = W - Y * Tp;                                               // Eq 39
                 const double emis = (p.method == 1) ? aa * p.a_rad * Tp * Tp * Tp * Tp : Nbar * p.a_rad * sqrt(Tp);
-                const double scale = (p.method == 3) ? alpha / (as + Nbar * t_m35(Tp)) : 1.0;
-                const double Sdt = (emis + as * Ep) * (dt / FOURPI);
-#pragma unroll
-                for (int v = 0; v < MAXV; ++v) {
-                    if (ca[v] != 0.0) {   // (n^0/d > 0 for every unmasked direction)
-                        // Eq 35 divided by nbar^4 (L432): I+ = [n^0/d] I- + [nbar dt/(4 pi d)] S / nbar^4
-                        val[v] = scale * (ca[v] * val[v] + Sdt * cb[v]);
-                        Ic[lane + 32 * v] = val[v];
-                    }
-                }
-                if (lane == 0) T[cell] = Tp;
-                updated = true;
-            } else if (lane == 0 && n_fail) {
+                scale = (p.method == 3) ? alpha / (as + Nbar * t_m35(Tp)) : 1.0;
+                Sdt = (emis + as * Ep) * (dt / FOURPI);
+                if (lane < CB) T[mycell] = Tp;
+            } else if (lane < CB && n_fail) {
                 atomicAdd(n_fail, 1);
             }
         }
-        if (MOM) {
-            double Ma[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+        __syncwarp();
+
+        // ---- phase 3: Eq 35 divided by nbar^4 (L432): I+ = [n^0/d] I- + [nbar dt/(4 pi d)] S / nbar^4 ----
 #pragma unroll
-            for (int v = 0; v < MAXV; ++v) {
-                const int s = lane + 32 * v;
-                if (s < p.nd) mom_accumulate(Ma, sw[s] * val[v], snx[s], sny[s], snz[s]);
-            }
-            warp_sum10(Ma, scr, lane);
-            if (lane < 16) {
-                const int mu = lane >> 2, nu = lane & 3;
-                const double Ra = rotate(Ma, ecen, L, mu, nu);
-                if (R_out) R_out[lane * p.ncell + cell] = Ra;
-                if (G_out && mu == 0) G_out[nu * p.ncell + cell] = updated ? -(Ra - Rb) / dt : 0.0;
+        for (int c = 0; c < CB; ++c) {
+            if (c >= ncb) break;
+            const long long cell = __shfl_sync(0xffffffffu, mycell, c);
+            const bool ok_c = __shfl_sync(0xffffffffu, (int)ok, c) != 0;
+            double *Ic = I + cell * p.pitch;
+            if (ok_c) {
+                const double sc = __shfl_sync(0xffffffffu, scale, c), sd = __shfl_sync(0xffffffffu, Sdt, c);
+#pragma unroll
+                for (int v = 0; v < MAXV; ++v) {
+                    if ((livebits >> (c * MAXV + v)) & 1u) {
+                        val[c][v] = sc * (val[c][v] + sd * cbs[(c * MAXV + v) * 32 + lane]);
+                        Ic[lane + 32 * v] = val[c][v];
+                    }
+                }
             }
         }
+        __syncwarp();
     }
 }
 
-template <bool SRC, bool MOM, bool LIST>
-cudaError_t launch_cell(const KParams &p, double *I, double *T, double dt, int *n_fail, double *R, double *G, cudaStream_t st) {
-    const int threads = SRC ? CELL_THREADS : MOM_THREADS;
-    // a list's length is only known on the device: a fixed grid, the kernel strides over whatever the list holds
-    const long long nwork = p.ncell;
-    long long want = (nwork + threads / 32 - 1) / (threads / 32);
-    const int blocks = (int)(want < 148LL * 8 * 4 ? want : 148LL * 8 * 4);
-    if (blocks == 0) return cudaSuccess;
-    const size_t smem = (4 * p.pitch + (threads / 32) * WSUM_DOUBLES) * sizeof(double);
-    if (p.nd <= 64) k_cell<2, SRC, MOM, LIST><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail, R, G);
-    else if (p.nd <= 192) k_cell<6, SRC, MOM, LIST><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail, R, G);
-    else if (p.nd <= 384) k_cell<12, SRC, MOM, LIST><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail, R, G);
-    else if (p.nd <= 672) k_cell<21, SRC, MOM, LIST><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail, R, G);
-    else return cudaErrorInvalidValue;
-    return cudaGetLastError();
+cudaError_t launch_cell_batch(const KParams &p, double *I, double *T, double dt, int *n_fail, cudaStream_t st) {
+    const int threads = CELL_THREADS, warps = threads / 32;
+    auto go = [&](auto maxv_tag) -> cudaError_t {
+        constexpr int MAXV = decltype(maxv_tag)::value;
+        constexpr int CB = CellBatch<MAXV>::CB;
+        constexpr int PART = CB * 3 * 33 + CB * 3;
+        const size_t scr = MAXV * 32 * CB + PART;
+        const size_t smem = (4 * p.pitch + warps * scr) * sizeof(double);
+        // a list's length is only known on the device: a fixed grid, the kernel strides over whatever the list holds
+        long long want = (p.ncell + (long long)warps * CB - 1) / ((long long)warps * CB);
+        const int blocks = (int)(want < 148LL * 8 * 4 ? want : 148LL * 8 * 4);
+        if (blocks == 0) return cudaSuccess;
+        cudaError_t e = cudaFuncSetAttribute(k_cell_batch<MAXV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        k_cell_batch<MAXV><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail);
+        return cudaGetLastError();
+    };
+    if (p.nd <= 64) return go(std::integral_constant<int, 2>());
+    if (p.nd <= 192) return go(std::integral_constant<int, 6>());
+    if (p.nd <= 384) return go(std::integral_constant<int, 12>());
+    if (p.nd <= 672) return go(std::integral_constant<int, 21>());
+    return cudaErrorInvalidValue;
 }
 
 }  // namespace
 
-// Source step on the cells of the interaction list, with their moments (R after, G from before / after) when wanted;
-// G is zero elsewhere; R of the cells not on the list comes from a second, source-free pass over the complement list.
+// Source step on the cells of the interaction list.  Moments, where wanted, come from the tensor-pipe pass (rt_moments_mma.cu)
+// run over the same intensities: R^0_nu of the listed cells before the step (parked in G), R of the listed cells after it with
+// G_nu = -(R^0_nu after - before) / dt (Eq 36, 48), and R of the cells the step does not visit; G is zero there.
 cudaError_t launch_source(const KParams &p, double *I, double *T, double dt, int *n_fail, double *R_after, double *G,
                           cudaStream_t st, long long *launches) {
     cudaError_t e = cudaSuccess;
     if (G) e = cudaMemsetAsync(G, 0, 4 * p.ncell * sizeof(double), st);
     const bool listed = p.method != 0 && p.srclist != nullptr;   // (the list may still be empty: its kernels then find nothing to do)
     if (e == cudaSuccess && listed) {
-        ++*launches;
-        // with moments wanted the listed cells get theirs here (R after, G from before/after); the rest below
-        e = (G || R_after) ? launch_cell<true, true, true>(p, I, T, dt, n_fail, R_after, G, st)
-                           : launch_cell<true, false, true>(p, I, T, dt, n_fail, nullptr, nullptr, st);
+        if (G) { ++*launches; e = launch_moments_mma(p, I, nullptr, G, 1, 1, dt, st); }
+        if (e == cudaSuccess) { ++*launches; e = launch_cell_batch(p, I, T, dt, n_fail, st); }
+        if (e == cudaSuccess && (G || R_after)) { ++*launches; e = launch_moments_mma(p, I, R_after, G, 1, G ? 2 : 0, dt, st); }
     }
-    if (e == cudaSuccess && R_after) {   // cells the source step did not visit: the tensor-pipe moments pass (rt_moments_mma.cu)
+    if (e == cudaSuccess && R_after) {   // cells the source step did not visit (all of them without a list)
         ++*launches;
-        e = launch_moments_mma(p, I, R_after, listed, st);   // listed: the complement of the list; else every cell
+        e = launch_moments_mma(p, I, R_after, nullptr, listed ? 2 : 0, 0, dt, st);
     }
     return e;
 }
 
 cudaError_t launch_moments(const KParams &p, const double *I, double *R, cudaStream_t st, long long *launches) {
     ++*launches;
-    return launch_moments_mma(p, I, R, false, st);
+    return launch_moments_mma(p, I, R, nullptr, 0, 0, 1.0, st);
 }
 
 }  // namespace rt
