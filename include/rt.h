@@ -96,6 +96,13 @@ typedef struct {
     int transport_variant; /* RT_TRANSPORT_* (0) */
     int transport_tile[3]; /* RT_TRANSPORT_TMA tile: columns along x1, along x2, directions per chunk (even); all 0 = chosen by
                               rt_init for the mesh */
+    /* L215: the geodesic grid "can be deformed in advance by performing a Lorentz transformation of its directions" and
+     * "oriented along a pre-defined direction".  grid_axis: direction (tetrad components 1-3, any length) the grid's pole is
+     * turned to; grid_boost: velocity (c = 1, |beta| < 1) of the frame in which the grid is the regular one -- the cells crowd
+     * around +beta.  Zero vectors = the regular grid with its pole along tetrad axis 3 (S2).  Numbering and neighbour lists do
+     * not change; areas, edges and the angular coefficients are those of the deformed cells.  A grid without the x-z mirror
+     * symmetry cannot serve RT_BC_REFLECT (rt_init returns RT_EINVAL). */
+    double grid_axis[3], grid_boost[3];
 } rt_options;
 
 /* Build the angular grid with N_d = 10 angle_level^2 + 2 directions (L207-213; angle_level = 2^generation is the

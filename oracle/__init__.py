@@ -113,7 +113,8 @@ class Oracle:
         self.kind, self.params = metric_kind, dict(metric_params or {})
         self.opt = dict(DEFAULT_OPTIONS)
         self.opt.update(options or {})
-        self.ang = geodesic.build(level)
+        # (angular-grid options stay on the Python side: the C core only sees the tables)
+        self.ang = geodesic.build(level, boost=self.opt.pop("grid_boost", None), axis=self.opt.pop("grid_axis", None))
         self.nd = self.ang["nd"]
         self.tab = geometry.build_tables(self.grid, self.kind, self.params)
         n = self.grid["n"]

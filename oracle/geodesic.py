@@ -116,8 +116,44 @@ def _tri_solid_angle(a, b, c):
     return 2.0 * np.arctan2(num, den)
 
 
-def build(level):
+def _orient(n, axis):
+    """Rotation that takes the grid's pole (0,0,1) to the unit vector along `axis` about the axis perpendicular to both (L215:
+    "It can also be easily oriented along a pre-defined direction"); the opposite pole is reached by a half turn about x."""
+    a = np.asarray(axis, dtype=float)
+    a = a / np.linalg.norm(a)
+    z = np.array([0.0, 0.0, 1.0])
+    k = np.cross(z, a)
+    sn, cs = np.linalg.norm(k), float(np.dot(z, a))
+    if sn < 1e-15:
+        return n.copy() if cs > 0 else n * np.array([1.0, -1.0, -1.0])
+    k = k / sn
+    # Rodrigues: v cos + (k x v) sin + k (k.v)(1 - cos)
+    return n * cs + np.cross(k, n) * sn + np.outer(n @ k, k) * (1.0 - cs)
+
+
+def _aberrate(n, beta):
+    """Directions n of a frame that moves with velocity beta (c = 1) seen from the frame it moves in: the Lorentz
+    transformation of the null vector (1, n) (L215: "the grid can be deformed in advance by performing a Lorentz
+    transformation of its directions").  k'^0 = gamma (1 + beta.n), k' = n + [gamma + (gamma - 1) (beta.n) / beta^2] beta ... written
+    with gamma^2 / (gamma + 1) = (gamma - 1) / beta^2 so that beta -> 0 is regular."""
+    b = np.asarray(beta, dtype=float)
+    b2 = float(b @ b)
+    assert b2 < 1.0
+    gam = 1.0 / np.sqrt(1.0 - b2)
+    bn = n @ b
+    k0 = gam * (1.0 + bn)
+    ks = n + np.outer(gam + gam * gam / (gam + 1.0) * bn, b)
+    return ks / k0[:, None]
+
+
+def build(level, boost=None, axis=None):
     """Return the tables of the geodesic grid with N_d = 10 level^2 + 2 cells.
+
+    axis: direction the grid's pole is turned to (None = tetrad axis 3, S2); boost: velocity of the frame in which the grid is
+    the regular one (None = no deformation).  Both act on the cell centres of the regular grid IN ITS CANONICAL ORDER (the
+    numbering and the neighbour lists do not change: a Lorentz transformation maps circles on the sphere to circles, so the
+    Delaunay triangulation of the deformed centres is the same set of triangles); the Voronoi cells, their areas and edges
+    are then those of the deformed centres.
 
     dict: nd, nhat[nd,3], w[nd], nnb[nd], nb[nd,6] (-1 padded, counter-clockwise seen from outside,
     starting at the lowest neighbour index), dlam[nd,6], emid[nd,6,3], eun[nd,6,3].
@@ -139,6 +175,10 @@ def build(level):
     rank = np.empty(nd, dtype=int)
     rank[order] = np.arange(nd)
     nhat = _unit(verts[order])
+    if axis is not None and np.any(np.asarray(axis) != 0):
+        nhat = _unit(_orient(nhat, axis))
+    if boost is not None and np.any(np.asarray(boost) != 0):
+        nhat = _unit(_aberrate(nhat, boost))
     tris = [tuple(rank[list(t)]) for t in tris]
 
     # circumcentre of each Delaunay triangle = a Voronoi corner

@@ -113,7 +113,7 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     c->launches = 0; c->fluid_set = false; c->profiling = false;
     c->hs_in = c->hs_cmp = c->hs_out = nullptr; c->hev_start = nullptr; c->hev_end[0] = c->hev_end[1] = c->hev_end[2] = nullptr;
     c->fluid_version = 0; c->hslab_fluid_version = -1; c->is_sub = false;
-    if (!build_angular_grid(angle_level, c->ang)) { delete c; return RT_EINVAL; }
+    if (!build_angular_grid(angle_level, opt->grid_axis, opt->grid_boost, c->ang)) { delete c; return RT_EINVAL; }
     const int nd = c->nd = c->ang.nd;
     const int pitch = c->pitch = (nd + 3) / 4 * 4;
     const int n1 = grid->n[0], n2 = grid->n[1], n3 = grid->n[2];

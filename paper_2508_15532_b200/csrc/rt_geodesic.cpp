@@ -99,9 +99,32 @@ double tri_solid_angle(V3 a, V3 b, V3 c) {  // Van Oosterom & Strackee, unit vec
     return 2.0 * std::atan2(std::fabs(dot(a, cross(b, c))), 1.0 + dot(a, b) + dot(b, c) + dot(c, a));
 }
 
+// L215: "to account for strong anisotropies of the radiation because of the Lorentz boost, the grid can be deformed in advance by
+// performing a Lorentz transformation of its directions.  It can also be easily oriented along a pre-defined direction".
+// Both act on the cell centres of the regular grid in its canonical order; numbering and neighbour lists stay (a Lorentz
+// transformation maps circles on the sphere to circles: the Delaunay triangles of the deformed centres are the same).
+// turn the pole (0,0,1) to `axis` about the direction perpendicular to both
+V3 orient(V3 v, const double axis[3]) {
+    V3 a = unit({axis[0], axis[1], axis[2]});
+    const V3 z = {0, 0, 1};
+    V3 k = cross(z, a);
+    const double sn = norm(k), cs = dot(z, a);
+    if (sn < 1e-15) return cs > 0 ? v : V3{v.x, -v.y, -v.z};
+    k = (1.0 / sn) * k;
+    return cs * v + sn * cross(k, v) + ((1.0 - cs) * dot(k, v)) * k;   // Rodrigues
+}
+// direction of the null vector (1, n) of a frame moving with velocity beta, seen from the frame it moves in
+V3 aberrate(V3 n, const double beta[3]) {
+    const V3 b = {beta[0], beta[1], beta[2]};
+    const double gam = 1.0 / std::sqrt(1.0 - dot(b, b)), bn = dot(b, n);
+    const double k0 = gam * (1.0 + bn);
+    const V3 ks = n + (gam + gam * gam / (gam + 1.0) * bn) * b;
+    return (1.0 / k0) * ks;
+}
+
 }  // namespace
 
-bool build_angular_grid(int level, AngularGrid &g) {
+bool build_angular_grid(int level, const double axis[3], const double boost[3], AngularGrid &g) {
     if (level < 1 || level > 64) return false;
     int a = 0, m = level;
     while (m % 2 == 0) { m /= 2; ++a; }
@@ -133,6 +156,12 @@ bool build_angular_grid(int level, AngularGrid &g) {
     for (int i = 0; i < nd; ++i) rank[order[i]] = i;
     std::vector<V3> n(nd);
     for (int i = 0; i < nd; ++i) n[i] = unit(mesh.v[order[i]]);
+    if (axis && (axis[0] != 0 || axis[1] != 0 || axis[2] != 0))
+        for (int i = 0; i < nd; ++i) n[i] = unit(orient(n[i], axis));
+    if (boost && (boost[0] != 0 || boost[1] != 0 || boost[2] != 0)) {
+        if (!(boost[0] * boost[0] + boost[1] * boost[1] + boost[2] * boost[2] < 1.0)) return false;
+        for (int i = 0; i < nd; ++i) n[i] = unit(aberrate(n[i], boost));
+    }
     std::vector<Tri> tris;
     for (const Tri &t : mesh.t) {
         Tri r = {rank[t[0]], rank[t[1]], rank[t[2]]};

@@ -20,7 +20,8 @@ struct AngularGrid {
     std::vector<double> emid;  // [nd][6][3] edge centre
     std::vector<double> eun;   // [nd][6][3] outward unit normal of the edge, tangent at emid
 };
-bool build_angular_grid(int level, AngularGrid &g);
+// axis: direction the pole is turned to, boost: velocity of the frame in which the grid is regular (L215); zero vectors / NULL = none
+bool build_angular_grid(int level, const double axis[3], const double boost[3], AngularGrid &g);
 
 // ---- geometry at one point (PAPER.md 2.1, Eq 1-4, Eq 8, App. A) ----------------------------------------------
 struct PointGeom {

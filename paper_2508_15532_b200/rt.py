@@ -35,7 +35,8 @@ class RtOptions(ctypes.Structure):
     _fields_ = [("limiter", ctypes.c_int), ("angular_recon", ctypes.c_int), ("source_method", ctypes.c_int),
                 ("n0_floor", ctypes.c_double), ("rho_floor", ctypes.c_double), ("kappa_a0", ctypes.c_double),
                 ("kappa_s", ctypes.c_double), ("a_rad", ctypes.c_double), ("Y_over_rho", ctypes.c_double),
-                ("abar", ctypes.c_double), ("transport_variant", ctypes.c_int), ("transport_tile", ctypes.c_int * 3)]
+                ("abar", ctypes.c_double), ("transport_variant", ctypes.c_int), ("transport_tile", ctypes.c_int * 3),
+                ("grid_axis", ctypes.c_double * 3), ("grid_boost", ctypes.c_double * 3)]
 
 
 def load_library(path=LIB_PATH):
@@ -124,6 +125,9 @@ class RtContext:
         od = dict(DEFAULT_OPTIONS)
         for k, v in (options or {}).items():
             od[{"method": "source_method", "ang_recon": "angular_recon"}.get(k, k)] = v
+        for k in ("grid_axis", "grid_boost", "transport_tile"):   # vectors: tuples -> ctypes arrays
+            if k in od and not isinstance(od[k], ctypes.Array):
+                od[k] = ((ctypes.c_int if k == "transport_tile" else ctypes.c_double) * 3)(*od[k])
         o = RtOptions(**od)
         self._h = ctypes.c_void_p()
         _check(lib().rt_init(ctypes.byref(g), ctypes.byref(m), int(level), ctypes.byref(o), ctypes.byref(self._h)))
