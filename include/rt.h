@@ -41,7 +41,8 @@ enum { RT_BC_PERIODIC = 0, RT_BC_OUTFLOW = 1, RT_BC_ZERO = 2, RT_BC_FIXED = 3,
                             only; rt_init returns RT_EINVAL for the other dims */ };
 enum { RT_MINKOWSKI_CART = 0, RT_MINK_CYL_TETRAD = 1, RT_KS_MKS = 2, RT_SNAKE = 3,
        RT_BL_MKS = 4 /* Boyer-Lindquist, same logical map as RT_KS_MKS, zero-angular-momentum tetrad (photon-orbit test, L563-592);
-                        the mesh must stay outside the horizon */ };
+                        the mesh must stay outside the horizon */,
+       RT_USER = 5 /* metric (and, optionally, tetrad) from the caller's host functions, called by rt_init only */ };
 enum { RT_LIM_MC = 0, RT_LIM_MINMOD = 1, RT_LIM_VANLEER = 2, RT_LIM_NONE = 3 };
 enum { RT_ANG_DONOR = 0, RT_ANG_MAPR = 1 };
 /* how the vacuum (Eq 20) spatial transport gets its stencil operands.  RT_TRANSPORT_TMA (default): a CTA owns a tile of
@@ -75,11 +76,21 @@ typedef struct {
 /* Metric + tetrad (L57-79, App. A).  x3_symmetric: geometry independent of x^3 (tables stored per (x1,x2) column,
  * the paper's own optimisation, L776); required for RT_KS_MKS, ignored (constant geometry) for RT_MINKOWSKI_CART. */
 typedef struct {
-    int kind;         /* RT_MINKOWSKI_CART | RT_MINK_CYL_TETRAD | RT_KS_MKS | RT_SNAKE | RT_BL_MKS */
+    int kind;         /* RT_MINKOWSKI_CART | RT_MINK_CYL_TETRAD | RT_KS_MKS | RT_SNAKE | RT_BL_MKS | RT_USER */
     double a, hslope; /* RT_KS_MKS, RT_BL_MKS: spin, theta-map parameter h: r = exp(x1), theta = pi x2 + (1-h)/2 sin(2 pi x2), phi = x3 */
     int x3_symmetric;
     double snake_A, snake_k; /* RT_SNAKE (App A.1): flat space in (t, w, y, z), w = x - A sin(k pi y); metric Eq A1,
                                 Cartesian-aligned tetrad (Eq A2 read as the co-frame, DESIGN S27): omega = 0, n^w = n^x - delta n^y */
+    /* RT_USER (L57-79: any stationary metric with an orthonormal tetrad whose e_0 is normal to t = const, Eq 4).  HOST functions,
+     * called only inside rt_init, at cell centres, face centres and the finite-difference points of Eq 8 (x = logical x1, x2,
+     * x3; must not depend on x3, x3_symmetric = 1 is required):
+     *   g_fn  fills the covariant metric g[mu][nu] (symmetric, signature - + + +); required;
+     *   e_fn  fills e[mu][a] = e^mu_a-hat (orthonormal, e_0 along -grad t: Eq 4); NULL = the library builds the tetrad as for
+     *         RT_KS_MKS (e_0 from Eq 4, then Gram-Schmidt of d_3, d_2, d_1 in the 3-metric);
+     *   user  is handed back to both.  A point with sqrt(-g) = 0 (coordinate axis) is a zero-area location: no flux crosses it. */
+    void (*g_fn)(const double x[3], double g[4][4], void *user);
+    void (*e_fn)(const double x[3], double e[4][4], void *user);
+    void *user;
 } rt_metric;
 
 typedef struct {

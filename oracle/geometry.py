@@ -101,13 +101,45 @@ def metric(kind, params, X):
         J[..., 1] = drdx
         J[..., 2] = dthdx
         return g * J[..., :, None] * J[..., None, :]
+    if kind == "user":   # the caller's metric: params["g"](x[3]) -> g[4, 4], point by point
+        flat = X.reshape(-1, 3)
+        return np.array([np.asarray(params["g"](x), dtype=np.float64) for x in flat]).reshape(X.shape[:-1] + (4, 4))
     raise ValueError(kind)
+
+
+def _tetrad_from_metric(g):
+    """Tetrad of a stationary metric g[..., 4, 4] when the caller gives none (L57-79): e_0 is the unit normal of the t = const
+    slices (Eq 4: e^mu_0 = -g^{0 mu} / sqrt(-g^{00})); the three space-like legs are the coordinate vectors d_3, d_2, d_1 made
+    orthonormal in that order (d_3 keeps its direction: with x3 = phi this is the locally non-rotating frame of A3-A4).
+    einv[a][mu] = eta_ab g_{mu nu} e^nu_b."""
+    gi = np.linalg.inv(g)
+    e = np.zeros(g.shape)
+    e[..., :, 0] = -gi[..., 0, :] / np.sqrt(-gi[..., 0, 0])[..., None]
+    legs = {}
+    for a in (3, 2, 1):
+        v = np.zeros(g.shape[:-1])
+        v[..., a] = 1.0
+        for b in range(3, a, -1):
+            pr = np.einsum("...i,...ij,...j->...", v[..., 1:], g[..., 1:, 1:], legs[b][..., 1:])
+            v = v - pr[..., None] * legs[b]
+        nrm = np.sqrt(np.einsum("...i,...ij,...j->...", v[..., 1:], g[..., 1:, 1:], v[..., 1:]))
+        legs[a] = v / nrm[..., None]
+        e[..., :, a] = legs[a]
+    einv = np.einsum("ab,...mn,...nb->...am", ETA, g, e)
+    return e, einv
 
 
 def tetrad(kind, params, X):
     """(e[..., mu, a], einv[..., a, mu]) at logical points X[..., 3]."""
     X = np.asarray(X, dtype=np.float64)
     shp = X.shape[:-1]
+    if kind == "user":
+        g = metric(kind, params, X)
+        if params.get("e") is None:
+            return _tetrad_from_metric(g)
+        flat = X.reshape(-1, 3)
+        e = np.array([np.asarray(params["e"](x), dtype=np.float64) for x in flat]).reshape(shp + (4, 4))
+        return e, np.einsum("ab,...mn,...nb->...am", ETA, g, e)
     if kind == "minkowski":
         e = np.broadcast_to(np.eye(4), shp + (4, 4)).copy()
         return e, e.copy()

@@ -99,7 +99,8 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
         if ((grid->bc_lo[a] == RT_BC_PERIODIC) != (grid->bc_hi[a] == RT_BC_PERIODIC)) return RT_EINVAL;
         if (grid->zero_lo[a] < 0 || grid->zero_hi[a] < 0) return RT_EINVAL;
     }
-    if (metric->kind < 0 || metric->kind > RT_BL_MKS) return RT_EINVAL;
+    if (metric->kind < 0 || metric->kind > RT_USER) return RT_EINVAL;
+    if (metric->kind == RT_USER && (!metric->g_fn || !metric->x3_symmetric)) return RT_EINVAL;
     if ((metric->kind == RT_KS_MKS || metric->kind == RT_BL_MKS) && (!metric->x3_symmetric || std::fabs(metric->a) >= 1.0)) return RT_EINVAL;
     if (metric->kind == RT_BL_MKS && !(std::exp(grid->x0[0]) > 1.0 + std::sqrt(1.0 - metric->a * metric->a))) return RT_EINVAL;   // outside the horizon only
     if (opt->angular_recon != RT_ANG_DONOR && opt->angular_recon != RT_ANG_MAPR) return RT_EINVAL;

@@ -50,6 +50,7 @@ double snake_delta(const rt_metric &mt, double y) { return mt.snake_A * mt.snake
 // covariant metric in logical coordinates
 void metric_at(const rt_metric &mt, const double x[3], double g[4][4]) {
     zero44(g);
+    if (mt.kind == RT_USER) { mt.g_fn(x, g, mt.user); return; }
     if (mt.kind != RT_KS_MKS && mt.kind != RT_BL_MKS) {
         g[0][0] = -1; g[1][1] = g[2][2] = g[3][3] = 1;
         if (mt.kind == RT_SNAKE) {   // x = w + A sin(k pi y):  dx = dw + delta dy  =>  ds^2 = -dt^2 + (dw + delta dy)^2 + dy^2 + dz^2
@@ -123,22 +124,26 @@ void eval_point(const rt_metric &mt, const double x[3], PointGeom &o) {
         o.sqrtg = 0.0;
         return;
     }
-    // e_0 from Eq 4
-    const double lapse_inv = std::sqrt(-ginv[0][0]);
-    for (int mu = 0; mu < 4; ++mu) o.e[mu][0] = -ginv[0][mu] / lapse_inv;
-    // Gram-Schmidt of d_3, d_2, d_1 with the spatial metric
-    double leg[4][4] = {{0}};  // leg[a][mu]
-    for (int a = 3; a >= 1; --a) {
-        double v[4] = {0, 0, 0, 0};
-        v[a] = 1.0;
-        for (int b = 3; b > a; --b) {
-            double pr = gdot(o.g, v, leg[b]);
-            for (int mu = 1; mu < 4; ++mu) v[mu] -= pr * leg[b][mu];
+    if (mt.kind == RT_USER && mt.e_fn) {
+        mt.e_fn(x, o.e, mt.user);   // the caller's tetrad
+    } else {
+        // e_0 from Eq 4
+        const double lapse_inv = std::sqrt(-ginv[0][0]);
+        for (int mu = 0; mu < 4; ++mu) o.e[mu][0] = -ginv[0][mu] / lapse_inv;
+        // Gram-Schmidt of d_3, d_2, d_1 with the spatial metric
+        double leg[4][4] = {{0}};  // leg[a][mu]
+        for (int a = 3; a >= 1; --a) {
+            double v[4] = {0, 0, 0, 0};
+            v[a] = 1.0;
+            for (int b = 3; b > a; --b) {
+                double pr = gdot(o.g, v, leg[b]);
+                for (int mu = 1; mu < 4; ++mu) v[mu] -= pr * leg[b][mu];
+            }
+            double nrm = std::sqrt(gdot(o.g, v, v));
+            for (int mu = 1; mu < 4; ++mu) leg[a][mu] = v[mu] / nrm;
         }
-        double nrm = std::sqrt(gdot(o.g, v, v));
-        for (int mu = 1; mu < 4; ++mu) leg[a][mu] = v[mu] / nrm;
+        for (int a = 1; a < 4; ++a) for (int mu = 0; mu < 4; ++mu) o.e[mu][a] = leg[a][mu];
     }
-    for (int a = 1; a < 4; ++a) for (int mu = 0; mu < 4; ++mu) o.e[mu][a] = leg[a][mu];
     // e^a_mu = eta^{ab} g_{mu nu} e^nu_b
     for (int a = 0; a < 4; ++a)
         for (int mu = 0; mu < 4; ++mu) {

@@ -13,7 +13,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "librt_b200.so")
 
 BC = {"periodic": 0, "outflow": 1, "zero": 2, "fixed": 3, "reflect": 4}
-METRIC = {"minkowski": 0, "mink_cyl": 1, "ks_mks": 2, "snake": 3, "bl_mks": 4}
+METRIC = {"minkowski": 0, "mink_cyl": 1, "ks_mks": 2, "snake": 3, "bl_mks": 4, "user": 5}
 GEOM = dict(g_c=0, e_c=1, einv_c=2, sqrtg_c=3, omega_c=4, n0_c=5, angcoef=6)
 SYMBOLS = ["rt_init", "rt_free", "rt_ndir", "rt_ndir_padded", "rt_get_directions", "rt_get_geometry", "rt_cfl_dt",
            "rt_set_boundary", "rt_set_fluid", "rt_transport", "rt_transport_static", "rt_angular_flux", "rt_source_implicit", "rt_moments",
@@ -26,9 +26,23 @@ class RtGrid(ctypes.Structure):
                 ("zero_lo", ctypes.c_int * 3), ("zero_hi", ctypes.c_int * 3)]
 
 
+# RT_USER host callbacks: void fn(const double x[3], double out[4][4], void *user)
+METRIC_FN = ctypes.CFUNCTYPE(None, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), ctypes.c_void_p)
+
+
 class RtMetric(ctypes.Structure):
     _fields_ = [("kind", ctypes.c_int), ("a", ctypes.c_double), ("hslope", ctypes.c_double), ("x3_symmetric", ctypes.c_int),
-                ("snake_A", ctypes.c_double), ("snake_k", ctypes.c_double)]
+                ("snake_A", ctypes.c_double), ("snake_k", ctypes.c_double),
+                ("g_fn", METRIC_FN), ("e_fn", METRIC_FN), ("user", ctypes.c_void_p)]
+
+
+def _metric_callback(fn):
+    """Python callable x[3] -> array [4,4]  ->  C callback of rt_metric (argument marshalling only)."""
+    def cb(x, out, _user):
+        a = np.asarray(fn(np.array([x[0], x[1], x[2]])), dtype=np.float64).reshape(16)
+        for q in range(16):
+            out[q] = a[q]
+    return METRIC_FN(cb)
 
 
 class RtOptions(ctypes.Structure):
@@ -122,6 +136,9 @@ class RtContext:
         g.zero_lo[:] = grid.get("zero_lo", (0, 0, 0)); g.zero_hi[:] = grid.get("zero_hi", (0, 0, 0))
         mp = dict(metric_params or {})
         m = RtMetric(METRIC[metric_kind], mp.get("a", 0.0), mp.get("hslope", 0.3), 1, mp.get("A", 0.0), mp.get("k", 0.0))
+        if metric_kind == "user":   # params: g = callable x[3] -> g[4,4]; e = callable x[3] -> e[mu, a] or None (library tetrad)
+            self._cb = (_metric_callback(mp["g"]), _metric_callback(mp["e"]) if mp.get("e") is not None else METRIC_FN())
+            m.g_fn, m.e_fn = self._cb
         od = dict(DEFAULT_OPTIONS)
         for k, v in (options or {}).items():
             od[{"method": "source_method", "ang_recon": "angular_recon"}.get(k, k)] = v

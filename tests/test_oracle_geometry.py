@@ -198,3 +198,38 @@ def test_bl_tetrad_and_circular_photon_orbits_eq53(a):
                     if l.strip() and not l.startswith("#"))
         assert abs(2 * (1 + np.cos(2 / 3 * np.arccos(-a))) - gold["photon_r1_a0.5"]) < 0.01
         assert abs(2 * (1 + np.cos(2 / 3 * np.arccos(+a))) - gold["photon_r2_a0.5"]) < 0.01
+
+
+def test_generic_tetrad_of_a_user_metric_reproduces_the_papers_closed_forms():
+    """The tetrad the 'user' metric kind builds when the caller gives none (e_0 from Eq 4, Gram-Schmidt of d_3, d_2, d_1) is, for
+    the Kerr-Schild metric, the closed form A3-A4 of the paper (L814-850) and, for Boyer-Lindquist, the zero-angular-momentum
+    frame; for any metric it is orthonormal, g_{mu nu} e^mu_a e^nu_b = eta_ab, with e_0 normal to t = const."""
+    rng = np.random.default_rng(11)
+    X = np.stack([rng.uniform(0.9, 3.0, 40), rng.uniform(0.05, 0.95, 40), rng.uniform(0, 6, 40)], -1)
+    for kind in ("ks_mks", "bl_mks"):
+        params = dict(a=0.7, hslope=0.3)
+        g = G.metric(kind, params, X)
+        e_ref, einv_ref = G.tetrad(kind, params, X)
+        e, einv = G._tetrad_from_metric(g)
+        assert np.abs(e - e_ref).max() < 1e-12 and np.abs(einv - einv_ref).max() < 1e-11
+    # an arbitrary stationary metric with lapse, shift and a non-diagonal 3-metric
+    A = rng.normal(size=(6, 3, 3)) * 0.2 + np.eye(3)
+    gam = np.einsum("nij,nkj->nik", A, A)
+    beta = rng.normal(size=(6, 3)) * 0.2
+    lapse = rng.uniform(0.5, 1.5, 6)
+    g = np.zeros((6, 4, 4))
+    g[:, 1:, 1:] = gam
+    g[:, 0, 1:] = g[:, 1:, 0] = np.einsum("nij,nj->ni", gam, beta)
+    g[:, 0, 0] = -lapse ** 2 + np.einsum("ni,nij,nj->n", beta, gam, beta)
+    e, einv = G._tetrad_from_metric(g)
+    eta = np.diag([-1.0, 1, 1, 1])
+    assert np.abs(np.einsum("nma,nmk,nkb->nab", e, g, e) - eta).max() < 1e-13
+    assert np.abs(np.einsum("nam,nmb->nab", einv, e) - np.eye(4)).max() < 1e-13
+    # Eq 4: e_0 = (1, -beta^i) / lapse; the space-like legs have no time component, d_3 keeps its direction
+    assert np.abs(e[:, 0, 0] - 1 / lapse).max() < 1e-13 and np.abs(e[:, 1:, 0] + beta / lapse[:, None]).max() < 1e-13
+    assert np.abs(e[:, 0, 1:]).max() == 0.0 and np.abs(e[:, 1:3, 3]).max() == 0.0
+    # through the 'user' kind: the same numbers
+    prm = dict(g=lambda x: g[int(round(x[0]))], e=None)
+    Xi = np.stack([np.arange(6.0), np.zeros(6), np.zeros(6)], -1)
+    e2, einv2 = G.tetrad("user", prm, Xi)
+    assert np.array_equal(e2, e) and np.array_equal(einv2, einv)
