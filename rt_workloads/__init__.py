@@ -186,3 +186,28 @@ def fields(cfg, nhat, e_c=None):
         if idx == 5:
             out["B"] = 1e-2 * np.stack([_smooth_field(rng, X) for _ in range(3)])   # generated, unused (GRMHD sector)
     return out
+
+
+def novikov_thorne_T(r, a, alpha=0.05):
+    """PAPER.md Eq 54-55 (L598-608) in code units: the Novikov-Thorne disk temperature up to the constant (4e7 K) (M / 3 Msun)^-1/4,
+    T ~ alpha^-1/4 r^-3/8 A^-1/2 B^1/2 E^1/4, with A, B, E as printed (Eq 55a-c).  Input data of the radiating-disk workload."""
+    r = np.asarray(r, dtype=np.float64)
+    A = 1.0 + a * a / r ** 2 + 2.0 * a * a / r ** 3
+    B = 1.0 + np.sqrt(a * a / r ** 3)
+    E = 1.0 + 4.0 * a * a / r ** 2 - 4.0 * a * a / r ** 3 + 3.0 * a ** 4 / r ** 4
+    return alpha ** -0.25 * r ** -0.375 * A ** -0.5 * B ** 0.5 * E ** 0.25
+
+
+def radiating_disk(cfg, a_rad=1.0, r_in=6.0, r_out=10.0):
+    """PAPER.md 4.8 (L594-617): "a strip of cells along the equator" between r = 6 and 10 that radiates isotropically in the
+    tetrad frame with I = a_rad T^4 / (4 pi) (Eq 56), T from Eq 54.  For a Kerr-Schild config of this module (logical x1 = ln r,
+    x2 = theta map) returns (j0, j1, i0, i1, I_disk[i1 - i0]): the rows next to the equator, the radial cells of the strip and
+    the intensity each of them is held at (the caller re-imposes it after every step)."""
+    g = cfg["grid"]
+    n1, n2 = g["n"][0], g["n"][1]
+    r = np.exp(g["x0"][0] + (np.arange(n1) + 0.5) * g["dx"][0])
+    sel = np.where((r >= r_in) & (r <= r_out))[0]
+    i0, i1 = int(sel[0]), int(sel[-1]) + 1
+    j0, j1 = (n2 // 2 - 1, n2 // 2 + 1) if n2 % 2 == 0 else (n2 // 2, n2 // 2 + 1)
+    T = novikov_thorne_T(r[i0:i1], cfg["metric"][1]["a"])
+    return j0, j1, i0, i1, a_rad * T ** 4 / (4.0 * math.pi)

@@ -249,3 +249,67 @@ def test_hohlraum_paper_setup():
             print("hohlraum 64 x 64 x 642 at t = %.2f: mean |E - exact| / (4 pi I_wall) = %.4f, max %.4f" % (t, err.mean(), err.max()))
             assert err.mean() < 0.006 and err.max() < 0.04
         ctx.close()
+
+
+# ---- section 4.5: tetrad choices; section 4.8: radiating disk ---------------------------------------------------------
+def test_spherical_tetrad_beam_matches_the_oracle():
+    """The beam of section 4.5 in the spherical tetrad (Eq 52), handed to the library as an RT_USER tetrad: parity with the
+    oracle; the physics (same straight line as in the Cartesian and cylindrical tetrads) is pinned on the oracle side
+    (tests/test_oracle_vacuum_suite.py)."""
+    import torch
+    from paper_2508_15532_b200 import rt
+    from test_oracle_vacuum_suite import tetrad_beam_setup
+    grid, params, N = tetrad_beam_setup("user")
+    orc = Oracle(grid, "user", params, 4, dict(method=0))
+    ctx = rt.RtContext(grid, "user", params, 4, dict(method=0))
+    one = torch.ones(ctx.shape, dtype=torch.float64, device=ctx.device)
+    ctx.set_fluid(torch.zeros_like(one), one, None)
+    rng = np.random.default_rng(4)
+    I_o = np.zeros((1, N, N, orc.nd))
+    I_o[0, 10:16, 3:7, :] = rng.uniform(0.0, 1.0, size=(6, 4, orc.nd))          # every direction, so every coefficient matters
+    I_o[0, 12:14, 4:6, 40] = 2.0
+    T_o = np.ones((1, N, N))
+    I_g = ctx.to_device(I_o); T_g = one.clone()
+    dt = 0.4 * grid["dx"][0]
+    assert dt <= min(ctx.cfl_dt())
+    for _ in range(12):
+        I_o, T_o, R_o, G_o, nf = orc.step(I_o, T_o, dt)
+        ctx.step(I_g, T_g, dt, None, None)
+    torch.cuda.synchronize()
+    assert rel_err(ctx.to_host(I_g), np.asarray(I_o).reshape(1, N, N, orc.nd)) <= TOL
+    ctx.close()
+
+
+def test_radiating_disk_matches_the_oracle_and_lights_the_space_above_it():
+    """Section 4.8 (L594-617): Novikov-Thorne strip on the equator of a Kerr-Schild mesh, a = 0.9375, vacuum, the strip re-imposed
+    by the caller after every step (the library owns no source but the fluid's).  Parity with the oracle step by step, then:
+    the radiation leaves the disk on both sides symmetrically and reaches cells the disk does not touch."""
+    import torch
+    import rt_workloads as W
+    from parity_util import make_pair
+    cfg = W.config(5, n=(28, 16, 6))
+    cfg["level"] = 4
+    cfg["options"] = dict(method=0, kappa_a0=0.0, kappa_s=0.0)
+    orc, ctx, f, dt = make_pair(cfg)
+    j0, j1, i0, i1, Id = W.radiating_disk(cfg)
+    assert i1 - i0 >= 3 and Id.min() > 0 and Id[0] > Id[-1]                  # hotter inside
+    I_o = np.zeros(ctx.shape + (orc.nd,)); T_o = np.ones(ctx.shape)
+    I_g = ctx.to_device(I_o); T_g = torch.ones(ctx.shape, dtype=torch.float64, device=ctx.device)
+    Id_g = torch.as_tensor(Id, device=ctx.device)
+    def impose():
+        I_o[:, j0:j1, i0:i1, :] = Id[None, None, :, None]
+        I_g[:, j0:j1, i0:i1, :ctx.nd] = Id_g[None, None, :, None]
+    impose()
+    for _ in range(8):
+        I_o, T_o, R_o, G_o, nf = orc.step(I_o, T_o, dt)
+        I_o = np.asarray(I_o).reshape(ctx.shape + (orc.nd,))
+        ctx.step(I_g, T_g, dt, None, None)
+        impose()
+    torch.cuda.synchronize()
+    Ig = ctx.to_host(I_g)
+    assert rel_err(Ig, I_o) <= TOL
+    E = (Ig * orc.ang["w"]).sum(-1)                                          # [k, j, i]
+    assert E[:, j0 - 2, i0:i1].min() > 0 and E[:, j1 + 1, i0:i1].min() > 0     # light above and below the strip
+    # north-south symmetry of the mesh, the metric and the source
+    assert np.abs(E[:, :j0, :] - E[:, :j1 - 1:-1, :][:, :j0, :]).max() <= 1e-9 * E.max()
+    ctx.close()

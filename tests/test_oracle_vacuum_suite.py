@@ -132,3 +132,73 @@ def test_hohlraum_matches_the_first_principles_solution():
     # a wrong front speed or a one-sided wall would not fit: the solution for t/2 is far away
     ex_half = np.array([[hohlraum_exact(xc[i], xc[j], 0.5 * t) for i in range(half)] for j in range(half)])
     assert np.abs(E[:half, :half] - ex_half).mean() > 0.08
+
+
+# ---- section 4.5: comparison of tetrad choices (L533-555) ---------------------------------------------------------------
+def spherical_tetrad(x):
+    """Flat space in Cartesian logical coordinates (x1, x2, x3) = (x, z, y); tetrad along the spherical unit vectors with the
+    polar axis along x2: e_1 = r-hat, e_2 = theta-hat, e_3 = phi-hat (Eq 52; its printed matrix is garbled, the text fixes the
+    meaning: "a tetrad aligned along the spherical unit vectors r-hat, theta-hat and phi-hat", L545).  Returned as e[mu, a]."""
+    X, Z, Y = x
+    rho = np.hypot(X, Y)
+    r = np.sqrt(rho * rho + Z * Z)
+    st, ct, cp, sp = rho / r, Z / r, X / rho, Y / rho
+    e = np.zeros((4, 4))
+    e[0, 0] = 1.0
+    # Cartesian components (x, y, z) -> logical slots (1, 3, 2)
+    e[1, 1], e[3, 1], e[2, 1] = st * cp, st * sp, ct             # r-hat
+    e[1, 2], e[3, 2], e[2, 2] = ct * cp, ct * sp, -st            # theta-hat
+    e[1, 3], e[3, 3], e[2, 3] = -sp, cp, 0.0                     # phi-hat
+    return e
+
+
+def tetrad_beam_setup(kind):
+    N = 40
+    grid = dict(n=(N, N, 1), x0=(1.0, 1.0, -0.075), dx=(0.15, 0.15, 0.15), bc_lo=("outflow", "outflow", "periodic"),
+                bc_hi=("outflow", "outflow", "periodic"), x3_symmetric=True)
+    params = {} if kind != "user" else dict(g=lambda x: np.diag([-1.0, 1.0, 1.0, 1.0]), e=spherical_tetrad)
+    return grid, params, N
+
+
+def _beam_run(kind, nst=40):
+    grid, params, N = tetrad_beam_setup(kind)
+    o = Oracle(grid, kind, params, 4, dict(method=0))
+    xc = 1.0 + (np.arange(N) + 0.5) * 0.15
+    # the beam: the grid direction closest to 45 degrees in the (x1, x2) plane, written in each cell's own tetrad
+    e = o.tab["e_c"]                                           # [1, N, N, mu, a]
+    d = np.array([0.0, 1.0, 1.0, 0.0]) / np.sqrt(2.0)
+    I = np.zeros((1, N, N, o.nd))
+    aim = np.zeros(2)                                          # mean Cartesian direction of the angular cells that were lit
+    for j in (12, 13):
+        for i in (4, 5):
+            dh = np.linalg.solve(e[0, j, i], d)[1:]            # tetrad components of the Cartesian direction
+            s = int(np.argmax(o.ang["nhat"] @ dh))
+            I[0, j, i, s] = 2.0
+            aim += (e[0, j, i] @ np.concatenate([[1.0], o.ang["nhat"][s]]))[1:3] / 4
+    T = np.ones((1, N, N))
+    dt = 0.4 * 0.15
+    E0 = None
+    for _ in range(nst):
+        I, T, R, G, nf = o.step(I, T, dt)
+    I = I.reshape(1, N, N, o.nd)
+    E = (I * o.ang["w"]).sum(-1)[0]
+    cx, cz = (E.sum(0) * xc).sum() / E.sum(), (E.sum(1) * xc).sum() / E.sum()
+    return np.array([cx, cz]), aim, nst * dt, o
+
+
+def test_beam_follows_the_same_straight_line_in_three_tetrads():
+    """Cartesian, cylindrical (Eq 51) and spherical (Eq 52) tetrads in flat space: the beam leaves the source at 45 degrees and
+    its energy centroid lies, after the same time, at the same place to a fraction of a cell -- on the straight line, a distance
+    c t from the source up to the angular cell's width ("we can accurately model the direction of the beam in each case,
+    although the cylindrical- and spherical-aligned tetrads show some bending", L555)."""
+    start = np.array([1.0 + 5 * 0.15, 1.0 + 13 * 0.15])
+    res = {k: _beam_run(k) for k in ("minkowski", "mink_cyl", "user")}
+    assert np.abs(res["user"][3].tab["omega_c"]).max() > 0.05 and np.abs(res["minkowski"][3].tab["omega_c"]).max() == 0.0
+    t = res["minkowski"][2]
+    for k, (c, aim, _, _) in res.items():
+        disp = c - start
+        ang, want = np.degrees(np.arctan2(disp[1], disp[0])), np.degrees(np.arctan2(aim[1], aim[0]))
+        print(k, "centroid", c, "moved at %.1f deg, lit cells point at %.1f deg" % (ang, want), "path %.3f of c t = %.3f" % (np.hypot(*disp), t))
+        assert abs(want - 45.0) < 15.0                                   # one of the grid's directions next to the diagonal (L539)
+        assert abs(ang - want) < (0.5 if k == "minkowski" else 6.0), (k, ang, want)
+        assert 0.9 * t < np.hypot(*disp) < 1.02 * t, (k, disp)
