@@ -10,7 +10,8 @@ R, G inside the timed region).  `roofline` = dominant kernel, algorithmic bytes 
 `cpu_baseline` = the oracle timed on a bounded sample on this box's cores (a baseline, not the target).
 N > 1: the mesh grows with N along x3 and is cut into slabs, one per rank, with a 4-plane halo
 exchanged point to point once per step (inside the timed region); value = owned cell-directions of all ranks * steps /
-max-over-ranks time ("weak").  --multi replicas: N independent copies instead.
+max-over-ranks time ("weak").  --multi slab-strong: the config's own mesh cut into N slabs ("strong"; every rank still carries
+its 8 halo planes, so thin slabs pay for them).  --multi replicas: N independent copies instead.
 """
 import argparse
 import json
@@ -34,8 +35,9 @@ def parse():
     ap.add_argument("--warmup", type=int, default=None, help="untimed warm-up steps (default 5; 1 for --impl reference)")
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index 1..5 (4 = Kerr-Schild, the roofline config); 6 = snake-coordinates beam (PAPER 4.6)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--multi", default="slab", choices=["slab", "replicas"],
-                    help="N > 1: slab decomposition along x3 with halo exchange (default) or independent replicas")
+    ap.add_argument("--multi", default="slab", choices=["slab", "slab-strong", "replicas"],
+                    help="N > 1: slab decomposition along x3 with halo exchange -- the mesh grows with N (slab, weak scaling, default) or "
+                         "stays the config's (slab-strong: strong scaling, 8 halo planes per rank on fewer owned ones) -- or independent replicas")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--size", default=None, help="override grid, e.g. 64x48x32 (debug)")
@@ -189,7 +191,7 @@ def setup_slab(args, cfg, rank, world, device):
     from paper_2508_15532_b200.dist import SlabDomain
 
     n = cfg["grid"]["n"]
-    gcfg = W.config(args.config, n=(n[0], n[1], n[2] * world))
+    gcfg = W.config(args.config, n=(n[0], n[1], n[2] * (1 if args.multi == "slab-strong" else world)))
     slab = SlabDomain(gcfg, rank, world, device=device)
     gen = dict(gcfg, grid=dict(slab.grid), seed=gcfg["seed"] + rank)
     f = W.fields(gen, slab.ctx.directions()["nhat"], slab.ctx.geometry("e_c"))
@@ -211,11 +213,12 @@ def run_gpu(args, rank, world):
     torch.cuda.set_device(local)
     cfg = make_config(args)
     slab, multi = None, "single GPU"
-    if world > 1 and args.multi == "slab":
+    if world > 1 and args.multi in ("slab", "slab-strong"):
         try:
             slab, cfg, dt = setup_slab(args, cfg, rank, world, device)
-            multi = ("slab decomposition along x3 (weak: %d planes per rank), deep halo: 4 planes of I and T per neighbour "
-                     "per step over %s send/recv, %d planes computed per rank" % (slab.layout.k1 - slab.layout.k0, dist.get_backend(), slab.layout.n3_local))
+            multi = ("slab decomposition along x3 (%s: %d planes per rank), deep halo: 4 planes of I and T per neighbour "
+                     "per step over %s send/recv, %d planes computed per rank" % ("strong, the config's mesh" if args.multi == "slab-strong" else "weak",
+                                                                                 slab.layout.k1 - slab.layout.k0, dist.get_backend(), slab.layout.n3_local))
         except Exception as e:   # e.g. slabs thinner than the halo: fall back to independent replicas, and say so
             slab, multi = None, "replicas only (slab decomposition unavailable: %s)" % str(e)[:120]
     elif world > 1:
@@ -233,6 +236,11 @@ def run_gpu(args, rank, world):
         units = ctx.ncell * ctx.nd                   # cell-direction updates per step
         step = lambda: ctx.step(I, T, dt, R, G)
     kernel_units = ctx.ncell * ctx.nd                # what one launch processes (incl. halo planes)
+    units_total = units * world
+    if slab is not None:                             # slabs may own different numbers of planes
+        ut = torch.tensor([float(units)], dtype=torch.float64, device=dev)
+        dist.all_reduce(ut)
+        units_total = int(ut.item())
     I0, T0 = I.clone(), T.clone()
 
     def barrier():
@@ -302,7 +310,7 @@ def run_gpu(args, rank, world):
         ems = max_over_ranks(ems, world, dev)
         h2d = (hI.numel() + hT.numel()) * 8
         d2h = (hI.numel() + hT.numel() + hR.numel() + hG.numel()) * 8
-        e2e = {"value": aggregate_value(units, ksteps, world, ems), "unit": UNIT, "h2d_bytes_per_step": h2d,
+        e2e = {"value": units_total * ksteps / (ems * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "steps": ksteps, "ms_per_step": ems / ksteps,
                "path": "rt_step_host: one C-ABI call on pinned host buffers; inside it x3 slabs with a 4-plane halo, H2D / rt_step / D2H overlapped on three streams" if slab is None else
                        "H2D -> SlabDomain.step (rt_step + halo exchange) -> D2H"}
@@ -341,7 +349,7 @@ def run_gpu(args, rank, world):
                                               "D2H of R, G, T, host synchronised every step"}
             except Exception as ex:
                 e2e["coupled_error"] = str(ex)[:160]
-    return dict(cfg=cfg, ctx=ctx, ms=ms, units=units, kernel_units=kernel_units, prof=prof, launches=launches, clk=clk, e2e=e2e,
+    return dict(cfg=cfg, ctx=ctx, ms=ms, units=units, units_total=units_total, slab=slab is not None, kernel_units=kernel_units, prof=prof, launches=launches, clk=clk, e2e=e2e,
                 finite=finite, dt=dt, multi=multi, n_fail=n_fail, live_fraction=live_fraction)
 
 
@@ -435,7 +443,7 @@ def main():
     r = run_gpu(args, rank, world)
     if rank == 0:
         ms, K = r["ms"], args.steps
-        value = aggregate_value(r["units"], K, world, ms)
+        value = r["units_total"] * K / (ms * 1e-3)   # whole job: the units all ranks own, over the max-over-ranks time
         units = r["kernel_units"]                 # per-launch units of the roofline figures
         peak, which = measured_peak()
         prof = r["prof"]
@@ -472,7 +480,8 @@ def main():
                 "step_frac_of_peak_32B": STEP_BYTES_IDEAL * r["units"] / step_s / 1e9 / peak,
                 "step_frac_of_peak_74B": STEP_BYTES_TWO_KERNEL * r["units"] / step_s / 1e9 / peak}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
-                "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                "ms_per_step": ms / K, "higher_is_better": True, "scaling": "strong" if (world > 1 and args.multi == "slab-strong" and r["slab"]) else "weak",
+                "vs_baseline": None, "dtype": "f64",
                 "data": "synthetic",
                 "config": {"workload": workload_name(r["cfg"]), "dt": r["dt"], "l2": "inputs larger than L2 (one I copy >= 1 GB vs 126 MB)"
                            if units * 8 > 2.0e8 else "inputs FIT in L2 (latency-bound config; HBM fraction not meaningful)",
