@@ -114,6 +114,9 @@ typedef struct {
      * not change; areas, edges and the angular coefficients are those of the deformed cells.  A grid without the x-z mirror
      * symmetry cannot serve RT_BC_REFLECT (rt_init returns RT_EINVAL). */
     double grid_axis[3], grid_boost[3];
+    int angflux_split;     /* 0: the angular flux of Eq 19 is upwinded on the total normal velocity of the edge (reading S5, the
+                              default); 1: term by term as printed (L239), the zeta-hat and psi-hat parts of the velocity each
+                              upwinded on its own sign.  Donor-cell reconstruction only (rt_init returns RT_EINVAL with MAPR). */
 } rt_options;
 
 /* Build the angular grid with N_d = 10 angle_level^2 + 2 directions (L207-213; angle_level = 2^generation is the

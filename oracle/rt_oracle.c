@@ -50,6 +50,7 @@ typedef struct {
     const double *rho, *u4;     /* rho[Nc]; u4[4][Nc] coordinate-frame u^mu */
     const double *ghost[3][2];  /* BC_FIXED: [2 layers][face cells][nd], layer 0 next to the interior */
     const int *mirror[3];       /* BC_REFLECT: mirror[a][s] = the direction with n-hat^a flipped (a permutation) */
+    int angflux_split;          /* 0: Eq 19 upwinded on the total normal velocity (S5); 1: term by term as printed (L239) */
 } orc_problem;
 
 static const double FOURPI = 12.566370614359172953850573533118;
@@ -242,16 +243,32 @@ static double div_x(const orc_problem *P, const double *I, const double *T, int 
 
 /* normal angular velocity V_e = a(m_e).u_e = -u_i omega^i_{cd} m^c m^d, m^c = (1, m_e) (O4, S4) and
  * n_0 at the edge centre, for edge e of direction s in the cell with geometry index gc */
+static void edge_coeff2(const orc_problem *P, long gc, int s, int e, double *V, double *n0e, double Vsplit[2]);
 static void edge_coeff(const orc_problem *P, long gc, int s, int e, double *V, double *n0e) {
+    double Vs[2];
+    edge_coeff2(P, gc, s, e, V, n0e, Vs);
+}
+/* the same, and the two terms of Eq 19 as printed (L239): the normal velocity split along the unit vectors of the tetrad-frame
+ * angles, V_zeta = (a.e_zeta)(u.e_zeta), V_psi = (a.e_psi)(u.e_psi), n-hat = (sin zeta cos psi, sin zeta sin psi, cos zeta);
+ * V = V_zeta + V_psi since u is tangent to the sphere at the edge centre */
+static void edge_coeff2(const orc_problem *P, long gc, int s, int e, double *V, double *n0e, double Vsplit[2]) {
     const double *m3 = P->emid + 3 * (6 * s + e), *u3 = P->eun + 3 * (6 * s + e);
     double m[4] = {1.0, m3[0], m3[1], m3[2]};
     const double *om = P->omega_c + 64 * gc;
-    double v = 0.0;
+    double v = 0.0, a3[3];
     for (int ii = 1; ii < 4; ++ii) {
         double q = 0.0;
         for (int c = 0; c < 4; ++c)
             for (int d = 0; d < 4; ++d) q += om[(ii * 4 + c) * 4 + d] * m[c] * m[d];
+        a3[ii - 1] = -q;              /* a^i up to its component along m, which no tangent vector sees */
         v -= u3[ii - 1] * q;
+    }
+    {
+        double sz = sqrt(m3[0] * m3[0] + m3[1] * m3[1]);
+        double cp = sz > 0 ? m3[0] / sz : 1.0, sp = sz > 0 ? m3[1] / sz : 0.0;
+        double ez[3] = {m3[2] * cp, m3[2] * sp, -sz}, ep[3] = {-sp, cp, 0.0};
+        Vsplit[0] = (a3[0] * ez[0] + a3[1] * ez[1] + a3[2] * ez[2]) * (u3[0] * ez[0] + u3[1] * ez[1] + u3[2] * ez[2]);
+        Vsplit[1] = (a3[0] * ep[0] + a3[1] * ep[1] + a3[2] * ep[2]) * (u3[0] * ep[0] + u3[1] * ep[1] + u3[2] * ep[2]);
     }
     *V = v;
     double n[4];
@@ -311,8 +328,8 @@ static double div_omega(const orc_problem *P, const double *Ic, int i, int j, in
     if (P->ang_recon == 1) mapr_gradient(P, Ic, s, gs);
     for (int e = 0; e < P->nnb[s]; ++e) {
         int t = P->nb[6 * s + e];
-        double V, n0e, n0t;
-        edge_coeff(P, gc, s, e, &V, &n0e);
+        double V, n0e, n0t, Vs[2];
+        edge_coeff2(P, gc, s, e, &V, &n0e, Vs);
         centre_n0(P, i, j, k, t, &up0, &n0t);
         if (sgn(n0s) != sgn(n0t)) continue;               /* L280 applied to angular neighbours */
         double IL = Ic[s], IR = Ic[t];                    /* donor cell (L227) */
@@ -325,6 +342,8 @@ static double div_omega(const orc_problem *P, const double *Ic, int i, int j, in
             IR = mapr_edge_value(P, Ic, t, et, gt);
         }
         double F = n0e * V * (V > 0 ? IL : IR);           /* Eq 19 upwinded on the total normal velocity (S5) */
+        if (P->angflux_split)                             /* ... or each of its two terms on its own (L239, as printed) */
+            F = n0e * (Vs[0] * (Vs[0] > 0 ? IL : IR) + Vs[1] * (Vs[1] > 0 ? IL : IR));
         sum += P->dlam[6 * s + e] * F;
     }
     return sum / P->w[s];
@@ -556,8 +575,9 @@ void orc_cfl(const orc_problem *P, double out[2]) {
                         if (n[1 + a] != 0.0) dts = fmin(dts, 0.5 * P->dx[a] * n[0] / fabs(n[1 + a]));
                     double rate = 0.0;
                     for (int e = 0; e < P->nnb[s]; ++e) {
-                        double V, n0e;
-                        edge_coeff(P, gc, s, e, &V, &n0e);
+                        double V, n0e, Vs[2];
+                        edge_coeff2(P, gc, s, e, &V, &n0e, Vs);
+                        if (P->angflux_split) V = fmax(Vs[0], 0.0) + fmax(Vs[1], 0.0);   /* what leaves through this edge */
                         if (V > 0) rate += V * fabs(n0e) * P->dlam[6 * s + e] / P->w[s];
                     }
                     if (rate > 0) dta = fmin(dta, 0.5 * fabs(n[0] * n0) / rate);

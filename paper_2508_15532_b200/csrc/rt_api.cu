@@ -101,6 +101,7 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     }
     if (metric->kind < 0 || metric->kind > RT_USER) return RT_EINVAL;
     if (metric->kind == RT_USER && (!metric->g_fn || !metric->x3_symmetric)) return RT_EINVAL;
+    if (opt->angflux_split && opt->angular_recon != 0) return RT_EINVAL;
     if ((metric->kind == RT_KS_MKS || metric->kind == RT_BL_MKS) && (!metric->x3_symmetric || std::fabs(metric->a) >= 1.0)) return RT_EINVAL;
     if (metric->kind == RT_BL_MKS && !(std::exp(grid->x0[0]) > 1.0 + std::sqrt(1.0 - metric->a * metric->a))) return RT_EINVAL;   // outside the horizon only
     if (opt->angular_recon != RT_ANG_DONOR && opt->angular_recon != RT_ANG_MAPR) return RT_EINVAL;
@@ -177,25 +178,38 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
                 for (int e = 0; e < A.nnb[s]; ++e) {
                     const double *m3 = &A.emid[3 * (6 * s + e)], *u3 = &A.eun[3 * (6 * s + e)];
                     const double m[4] = {1.0, m3[0], m3[1], m3[2]};
-                    double V = 0.0;
+                    double V = 0.0, a3[3];
                     for (int ii = 1; ii < 4; ++ii) {
                         double q = 0.0;
                         for (int cc = 0; cc < 4; ++cc) for (int d = 0; d < 4; ++d) q += om[ii][cc][d] * m[cc] * m[d];
+                        a3[ii - 1] = -q;
                         V -= u3[ii - 1] * q;                                     // a(m_e) . u_e  (Eq 7-8, S4)
+                    }
+                    // Eq 19 as printed (L239): the zeta-hat and psi-hat parts of the normal velocity, upwinded one by one
+                    double Vout = V > 0 ? V : 0.0, Vin = V > 0 ? 0.0 : V;        // what multiplies the own / the neighbour's value
+                    if (opt->angflux_split) {
+                        const double sz = std::sqrt(m3[0] * m3[0] + m3[1] * m3[1]);
+                        const double cp = sz > 0 ? m3[0] / sz : 1.0, sp = sz > 0 ? m3[1] / sz : 0.0;
+                        const double ez[3] = {m3[2] * cp, m3[2] * sp, -sz}, ep[3] = {-sp, cp, 0.0};
+                        const double Vz = (a3[0] * ez[0] + a3[1] * ez[1] + a3[2] * ez[2]) * (u3[0] * ez[0] + u3[1] * ez[1] + u3[2] * ez[2]);
+                        const double Vp = (a3[0] * ep[0] + a3[1] * ep[1] + a3[2] * ep[2]) * (u3[0] * ep[0] + u3[1] * ep[1] + u3[2] * ep[2]);
+                        Vout = std::fmax(Vz, 0.0) + std::fmax(Vp, 0.0);
+                        Vin = std::fmin(Vz, 0.0) + std::fmin(Vp, 0.0);
                     }
                     omax = std::fmax(omax, std::fabs(V));
                     const double n0e = ce[0] + ce[1] * m3[0] + ce[2] * m3[1] + ce[3] * m3[2];
                     const int t = A.nb[6 * s + e];
                     const double n0s = c->h_n0[col * nd + s], n0t = c->h_n0[col * nd + t];
                     const bool gate = ((n0s > 0) - (n0s < 0)) != ((n0t > 0) - (n0t < 0));   // L280
-                    const double coef = gate ? 0.0 : A.dlam[6 * s + e] * n0e * V / A.w[s];  // Eq 19 / Eq 18
+                    const double c0 = gate ? 0.0 : A.dlam[6 * s + e] * n0e / A.w[s];
+                    const double coef = c0 * V;                                 // Eq 19 / Eq 18
                     c->h_angcoef[(col * 6 + e) * nd + s] = coef;
                     if (mapr) {
                         angraw[(col * 6 + e) * pitch + s] = coef;
                         if (V > 0) angup[col * pitch + s] |= (unsigned char)(1u << e);
                     }
-                    if (V > 0) self += coef;                                    // upwind: own value (S5)
-                    else angc[(col * ANG_SLOTS + e) * pitch + s] = coef;        // upwind: neighbour's value
+                    self += c0 * Vout;                                          // upwind: own value (S5)
+                    angc[(col * ANG_SLOTS + e) * pitch + s] = c0 * Vin;         // upwind: neighbour's value
                 }
                 angc[(col * ANG_SLOTS + 6) * pitch + s] = self;
             }
@@ -481,6 +495,20 @@ extern "C" int rt_cfl_dt(const rt_ctx *c, double out[2]) {
                         double qq = 0.0;
                         for (int cc = 0; cc < 4; ++cc) for (int d = 0; d < 4; ++d) qq += om[(ii * 4 + cc) * 4 + d] * m[cc] * m[d];
                         V -= u3[ii - 1] * qq;
+                    }
+                    if (c->opt.angflux_split) {   // what leaves through this edge when the two terms are upwinded one by one
+                        double a3[3];
+                        for (int ii = 1; ii < 4; ++ii) {
+                            double qq = 0.0;
+                            for (int cc = 0; cc < 4; ++cc) for (int d = 0; d < 4; ++d) qq += om[(ii * 4 + cc) * 4 + d] * m[cc] * m[d];
+                            a3[ii - 1] = -qq;
+                        }
+                        const double sz = std::sqrt(m3[0] * m3[0] + m3[1] * m3[1]);
+                        const double cp = sz > 0 ? m3[0] / sz : 1.0, sp = sz > 0 ? m3[1] / sz : 0.0;
+                        const double ez[3] = {m3[2] * cp, m3[2] * sp, -sz}, ep[3] = {-sp, cp, 0.0};
+                        const double Vz = (a3[0] * ez[0] + a3[1] * ez[1] + a3[2] * ez[2]) * (u3[0] * ez[0] + u3[1] * ez[1] + u3[2] * ez[2]);
+                        const double Vp = (a3[0] * ep[0] + a3[1] * ep[1] + a3[2] * ep[2]) * (u3[0] * ep[0] + u3[1] * ep[1] + u3[2] * ep[2]);
+                        V = std::fmax(Vz, 0.0) + std::fmax(Vp, 0.0);
                     }
                     if (V > 0) {
                         const double *g0 = &c->h_g[col * 16];

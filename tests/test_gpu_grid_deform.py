@@ -57,3 +57,33 @@ def test_a_grid_without_the_mirror_plane_cannot_reflect():
         Oracle(grid, kind, params, 2, dict(cfg["options"], grid_boost=(0.0, 0.3, 0.0)))
     with pytest.raises(rt.RtError):
         rt.RtContext(cfg["grid"], kind, params, 2, dict(cfg["options"], grid_boost=(0.0, 0.8, 0.7)))     # |beta| >= 1
+
+
+# ---- Eq 19 term by term (rt_options.angflux_split, L239 as printed) ----------------------------------------------------------
+@pytest.mark.parametrize("idx,n,steps,kw", [(4, (16, 12, 6), 3, dict(angflux_split=1)),
+                                            (5, (8, 6, 4), 2, dict(angflux_split=1, grid_boost=(0.2, 0.0, 0.3)))])
+def test_steps_with_the_split_angular_flux_match_the_oracle(idx, n, steps, kw):
+    cfg = W.config(idx, n=n)
+    cfg["options"] = dict(cfg["options"], **kw)
+    orc, ctx, f, dt = make_pair(cfg)
+    assert abs(min(ctx.cfl_dt()) - min(orc.cfl())) <= 1e-9 * min(orc.cfl())       # the outflow-rate bound follows the option
+    out = run_steps(orc, ctx, f, dt, steps)
+    for k in ("I", "T", "R"):
+        assert rel_err(*out[k]) <= TOL, k
+    assert out["nfail"][0] == out["nfail"][1]
+    ctx.close()
+    # and it is not the default flux in disguise
+    cfg0 = W.config(idx, n=n)
+    cfg0["options"] = dict(cfg0["options"], **{k: v for k, v in kw.items() if k != "angflux_split"})
+    orc0, ctx0, f0, dt0 = make_pair(cfg0)
+    out0 = run_steps(orc0, ctx0, f0, dt, steps)
+    assert rel_err(out0["I"][0], out["I"][0]) > 1e-6
+    ctx0.close()
+
+
+def test_split_angular_flux_is_donor_cell_only():
+    from paper_2508_15532_b200 import rt
+    cfg = W.config(4, n=(8, 6, 2))
+    kind, params = cfg["metric"]
+    with pytest.raises(rt.RtError):
+        rt.RtContext(cfg["grid"], kind, params, 2, dict(cfg["options"], angflux_split=1, ang_recon=1))

@@ -252,3 +252,49 @@ def test_mapr_angular_update_is_second_order_donor_cell_first_order():
     assert ed[0][0] / ed[1][0] > 1.6 and ed[1][0] / ed[2][0] > 1.6           # first order
     assert em[0][0] / em[1][0] > 3.0 and em[1][0] / em[2][0] > 3.0           # second order
     assert em[2][0] < 0.25 * ed[2][0]
+
+
+# ---- Eq 19 as printed: the two terms of the angular flux upwinded one by one (option angflux_split, S5 / L239) -----------------
+def _split_pair(split):
+    from oracle import Oracle
+    import rt_workloads as W
+    cfg = W.config(4, n=(10, 8, 2))
+    kind, params = cfg["metric"]
+    o = Oracle(cfg["grid"], kind, params, 4, dict(method=0, angflux_split=split))
+    return cfg, o
+
+
+def test_split_angular_flux_conserves_and_reduces_to_the_default_where_it_must():
+    """(i) flux form: what leaves a cell through an edge enters its neighbour, term by term, so sum_s dOmega_s n^0 n_0 dI_s = 0
+    over the unmasked directions of a cell whose neighbours are all unmasked; (ii) an intensity that is uniform over the sphere
+    has I_L = I_R on every edge: the split and the default flux are the same number; (iii) on a generic field they differ (the
+    option is live), by less than the flux itself."""
+    import numpy as np
+    cfg, o1 = _split_pair(1)
+    _, o0 = _split_pair(0)
+    n = cfg["grid"]["n"]
+    shp = (n[2], n[1], n[0], o1.nd)
+    rng = np.random.default_rng(8)
+    dt = 1e-3
+    # (ii)
+    Iu = np.broadcast_to(rng.uniform(1, 2, size=shp[:3])[..., None], shp).copy()
+    a, b = Iu.copy(), Iu.copy()
+    a = np.asarray(o1.angular_flux(Iu, a, dt)).reshape(shp); b = np.asarray(o0.angular_flux(Iu, b, dt)).reshape(shp)
+    assert np.abs(a - b).max() <= 1e-15 * np.abs(b).max()
+    # (iii), (i)
+    I = rng.uniform(1, 2, size=shp)
+    a = np.asarray(o1.angular_flux(I, I.copy(), dt)).reshape(shp); b = np.asarray(o0.angular_flux(I, I.copy(), dt)).reshape(shp)
+    d1, d0 = a - I, b - I
+    e, g = o1.tab["e_c"][0], o1.tab["g_c"][0]                      # [j, i, mu, a]
+    nh = np.concatenate([np.ones((o1.nd, 1)), o1.ang["nhat"]], 1)
+    nmu = np.einsum("jima,sa->jism", e, nh)
+    n0 = np.einsum("jim,jism->jis", g[..., 0, :], nmu)
+    wgt = o1.ang["w"] * nmu[..., 0] * n0                           # dOmega n^0 n_0
+    unmasked = (n0 <= -0.1).all(-1)                                # cells with no masked direction: no sink, no gated edge
+    unmasked[:2] = unmasked[-2:] = False                          # (and outside the polar zero band)
+    assert unmasked.sum() > 10
+    diff = np.abs(d1 - d0)[:, unmasked].max()
+    assert 1e-3 * np.abs(d0[:, unmasked]).max() < diff < np.abs(d0[:, unmasked]).max()
+    for d in (d1, d0):
+        tot = (d * wgt[None]).sum(-1)[:, unmasked]
+        assert np.abs(tot).max() <= 1e-12 * np.abs(d * wgt[None]).sum(-1)[:, unmasked].max() + 1e-18
