@@ -12,8 +12,8 @@
 // (TY (TX + 4) + 4 TX) / (TX TY) (2.3-2.7 for the tiles used), and the march has no global loads, no prefetches and no
 // 64-bit address arithmetic left except the store.
 //
-// Thread mapping: the tile's (column, s) pairs are numbered q = (lj TX + c) DCH + d; consumer thread t owns pairs t and
-// t + NT.  As in rt_transport.cu everything geometric of a pair (folded face coefficients, upwind sides, operand offsets
+// Thread mapping: the tile's (column, s) pairs are numbered q = (lj TX + c) DCH + d; consumer thread t owns the pairs
+// t, t + NT, .. (RP of them; RP = 1 as built).  As in rt_transport.cu everything geometric of a pair (folded face coefficients, upwind sides, operand offsets
 // inside a slot) is formed once (the geometry is x3-independent) and lives in registers for the whole march, and the x3
 // stencil is a register window.  Pairs of the "general" class (sign change of n^a inside the cell, ZERO / FIXED /
 // REFLECT ghosts) stay with the list kernel of rt_transport.cu; the arithmetic is the same, in the same order, as in
@@ -28,8 +28,9 @@
 namespace rt {
 namespace {
 
-constexpr int NT = 480;               // consumer threads (15 warps); warp 15 is the producer: 16 warps = 128 registers each
-constexpr int RP = 2;                   // pairs per consumer thread
+constexpr int NT = 736;               // consumer threads (23 warps) + warp 23, the producer: 24 warps of <= 85 registers.  One pair per thread and
+                                      // 23 warps beat two pairs per thread and 15 warps of 128 registers by 4-5 % (the kernel is issue-bound: more warps to pick from)
+constexpr int RP = 1;                   // pairs per consumer thread (the kernel is written for any RP)
 constexpr int NS = 8;                // ring slots: planes k, k+1, k+2 in use, five in flight (a load takes about two steps)
 constexpr int SLOT_STRIDE = 20480;   // bytes between ring slots (compile-time: every operand load is LDS [R + imm])
 constexpr int BSLOT_STRIDE = RP * NT * 8 + 128;   // base ring: own cells only (+ the zero word, see ZERO_OFF)
