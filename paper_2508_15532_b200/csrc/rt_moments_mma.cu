@@ -44,7 +44,7 @@ __device__ __forceinline__ double mget(const double *M, int a, int b) {
 // G_nu = -(R^0_nu - G_nu) / dt (Eq 36 / 48: G holds the moments before, left there by a gmode-1 pass over the same cells; a cell
 // the source step did not change gets exactly 0: both passes add the same numbers in the same order).
 template <bool LIST>
-__global__ void __launch_bounds__(32 * MM_WARPS, 2)
+__global__ void __launch_bounds__(32 * MM_WARPS, 4)
 k_moments_mma(const __grid_constant__ KParams p, const double *__restrict__ I, double *__restrict__ R, double *__restrict__ G,
               int part, int gmode, double inv_dt) {
     extern __shared__ double sm[];
@@ -72,8 +72,9 @@ k_moments_mma(const __grid_constant__ KParams p, const double *__restrict__ I, d
     // Software pipeline over (group, batch): the loads run a batch of NB pairs (NB x 512 bytes per warp) ahead of the MMAs that
     // consume them, double-buffered, and the last batch of a group already fetches the first batch of the warp's next group
     // (whose cell indices were looked up at the start of this one).  Without this every loop trip exposed a full memory latency
-    // (long-scoreboard stalls of 41 cycles per issue, 3 TB/s).
-    constexpr int NB = 8;
+    // (long-scoreboard stalls of 41 cycles per issue, 3 TB/s).  Four blocks of 64 registers per SM (32 warps) with a short batch
+    // beat two blocks of 128 registers with NB = 8 by 13 % (measured: 16 warps do not cover the latency, however deep the batch).
+    constexpr int NB = 2;
     auto lookup = [&](long long grp_, bool &valid_) -> long long {
         const long long wi = grp_ * 8 + g;
         valid_ = grp_ < ngroups && wi < nwork;
