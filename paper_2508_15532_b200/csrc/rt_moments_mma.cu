@@ -43,8 +43,9 @@ __device__ __forceinline__ double mget(const double *M, int a, int b) {
 // gmode: 0 = R only; 1 = R^0_nu into G (the moments BEFORE a source step; R untouched); 2 = R (if given), and
 // G_nu = -(R^0_nu - G_nu) / dt (Eq 36 / 48: G holds the moments before, left there by a gmode-1 pass over the same cells; a cell
 // the source step did not change gets exactly 0: both passes add the same numbers in the same order).
-template <bool LIST>
-__global__ void __launch_bounds__(32 * MM_WARPS, 4)
+// WIDE: rows of more than 256 directions (see NB below)
+template <bool LIST, bool WIDE>
+__global__ void __launch_bounds__(32 * MM_WARPS, WIDE ? 2 : 4)
 k_moments_mma(const __grid_constant__ KParams p, const double *__restrict__ I, double *__restrict__ R, double *__restrict__ G,
               int part, int gmode, double inv_dt) {
     extern __shared__ double sm[];
@@ -72,9 +73,10 @@ k_moments_mma(const __grid_constant__ KParams p, const double *__restrict__ I, d
     // Software pipeline over (group, batch): the loads run a batch of NB pairs (NB x 512 bytes per warp) ahead of the MMAs that
     // consume them, double-buffered, and the last batch of a group already fetches the first batch of the warp's next group
     // (whose cell indices were looked up at the start of this one).  Without this every loop trip exposed a full memory latency
-    // (long-scoreboard stalls of 41 cycles per issue, 3 TB/s).  Four blocks of 64 registers per SM (32 warps) with a short batch
-    // beat two blocks of 128 registers with NB = 8 by 13 % (measured: 16 warps do not cover the latency, however deep the batch).
-    constexpr int NB = 2;
+    // (long-scoreboard stalls of 41 cycles per issue, 3 TB/s).  Which side of the trade wins depends on the row length (measured):
+    // at 162 directions four blocks of 64 registers per SM (32 warps) with a short batch beat two blocks of 128 registers with
+    // NB = 8 by 13 %; at 362 directions (a group is 23 KB, the B fragments 47 KB per block) the deep batch wins by 40 %.
+    constexpr int NB = WIDE ? 8 : 2;
     auto lookup = [&](long long grp_, bool &valid_) -> long long {
         const long long wi = grp_ * 8 + g;
         valid_ = grp_ < ngroups && wi < nwork;
@@ -165,14 +167,16 @@ cudaError_t launch_moments_mma(const KParams &p, const double *I, double *R, dou
     long long blocks = (groups + MM_WARPS - 1) / MM_WARPS;
     if (blocks > 148LL * 8) blocks = 148LL * 8;
     const double inv_dt = gmode == 2 ? 1.0 / dt : 0.0;
-    cudaError_t e;
-    if (part != 0) {
-        e = cudaFuncSetAttribute(k_moments_mma<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) k_moments_mma<true><<<(unsigned)blocks, 32 * MM_WARPS, smem, st>>>(p, I, R, G, part, gmode, inv_dt);
-    } else {
-        e = cudaFuncSetAttribute(k_moments_mma<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) k_moments_mma<false><<<(unsigned)blocks, 32 * MM_WARPS, smem, st>>>(p, I, R, G, part, gmode, inv_dt);
-    }
+    cudaError_t e = cudaSuccess;
+#define RT_MM_LAUNCH(L, W)                                                                                              \
+    do {                                                                                                                \
+        e = cudaFuncSetAttribute(k_moments_mma<L, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);          \
+        if (e == cudaSuccess) k_moments_mma<L, W><<<(unsigned)blocks, 32 * MM_WARPS, smem, st>>>(p, I, R, G, part, gmode, inv_dt); \
+    } while (0)
+    const bool wide = p.pitch > 256;
+    if (part != 0) { if (wide) RT_MM_LAUNCH(true, true); else RT_MM_LAUNCH(true, false); }
+    else { if (wide) RT_MM_LAUNCH(false, true); else RT_MM_LAUNCH(false, false); }
+#undef RT_MM_LAUNCH
     return e != cudaSuccess ? e : cudaGetLastError();
 }
 
