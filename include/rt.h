@@ -117,6 +117,10 @@ typedef struct {
     int angflux_split;     /* 0: the angular flux of Eq 19 is upwinded on the total normal velocity of the edge (reading S5, the
                               default); 1: term by term as printed (L239), the zeta-hat and psi-hat parts of the velocity each
                               upwinded on its own sign.  Donor-cell reconstruction only (rt_init returns RT_EINVAL with MAPR). */
+    int source_literal;    /* 0: the intensity update (Eq 35) uses the coefficients the temperature equation was built from, so
+                              that the updated intensities add up to E_+ of Eq 39 (reading S19b, the default); 1: "the opacities
+                              must be updated and are therefore recalculated for the new value of T_+" (L432) taken literally for
+                              source Methods 2 and 3: every opacity of Eq 35 at T_+ (energy then balances to O(alpha_+ - alpha_-)) */
 } rt_options;
 
 /* Build the angular grid with N_d = 10 angle_level^2 + 2 directions (L207-213; angle_level = 2^generation is the

@@ -44,7 +44,7 @@ class _Problem(ctypes.Structure):
         ("kappa_s", ctypes.c_double), ("a_rad", ctypes.c_double), ("Y_over_rho", ctypes.c_double),
         ("abar", ctypes.c_double),
         ("rho", _dp), ("u4", _dp), ("ghost", (_dp * 2) * 3), ("mirror", _ip * 3),
-        ("angflux_split", ctypes.c_int),
+        ("angflux_split", ctypes.c_int), ("source_literal", ctypes.c_int),
     ]
 
 
@@ -98,7 +98,7 @@ def mirror_map(nhat, a):
 
 
 DEFAULT_OPTIONS = dict(limiter=0, ang_recon=0, method=2, n0_floor=0.1, rho_floor=5e-4, kappa_a0=0.0,
-                       kappa_s=0.0, a_rad=1.0, Y_over_rho=1.5, abar=1.0, angflux_split=0)
+                       kappa_s=0.0, a_rad=1.0, Y_over_rho=1.5, abar=1.0, angflux_split=0, source_literal=0)
 
 
 class Oracle:

@@ -51,6 +51,9 @@ typedef struct {
     const double *ghost[3][2];  /* BC_FIXED: [2 layers][face cells][nd], layer 0 next to the interior */
     const int *mirror[3];       /* BC_REFLECT: mirror[a][s] = the direction with n-hat^a flipped (a permutation) */
     int angflux_split;          /* 0: Eq 19 upwinded on the total normal velocity (S5); 1: term by term as printed (L239) */
+    int source_literal;         /* 0: Eq 35 with the coefficients the temperature equation was built from (S19b, conservative);
+                                   1: "the opacities must be updated and are therefore recalculated for the new value of T_+" (L432)
+                                   taken literally for Methods 2 and 3: every opacity of Eq 35 at T_+ */
 } orc_problem;
 
 static const double FOURPI = 12.566370614359172953850573533118;
@@ -488,6 +491,11 @@ int orc_source(const orc_problem *P, double *I, double *T, double dt) {
                 else emis = Nbar * P->a_rad * sqrt(Tp);                                      /* alpha_P(T+) a T+^4 */
                 if (P->method == 3) scale = alpha / (as + Nbar * pow(Tp, -3.5));             /* alpha_- / alpha_+ */
                 double S = emis + as * Ep;
+                double alpha_upd = alpha;                                                     /* the opacity inside d_s of Eq 35 */
+                if (P->source_literal && P->method != 1) {                                   /* L432, literal (S19b) */
+                    alpha_upd = as + Nbar * pow(Tp, -3.5);
+                    scale = 1.0;
+                }
                 for (int s = 0; s < nd; ++s) {
                     double nu0, nd0;
                     centre_n0(P, i, j, k, s, &nu0, &nd0);
@@ -495,7 +503,7 @@ int orc_source(const orc_problem *P, double *I, double *T, double dt) {
                     const double *nh = P->nhat + 3 * s;
                     double nbar = uh[0] - (uh[1] * nh[0] + uh[2] * nh[1] + uh[3] * nh[2]);
                     double n4 = nbar * nbar * nbar * nbar;
-                    double d = nu0 + nbar * alpha * dt;
+                    double d = nu0 + nbar * alpha_upd * dt;
                     double Ibar = n4 * Ic[s];
                     double Ip = scale * (nu0 / d * Ibar + nbar * dt / (FOURPI * d) * S);     /* Eq 35 */
                     Ic[s] = Ip / n4;                                                          /* L432 */

@@ -302,7 +302,7 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
         k.zlo[a] = grid->zero_lo[a]; k.zhi[a] = grid->zero_hi[a];
         k.face[a] = t.face[a];
     }
-    k.limiter = opt->limiter; k.method = opt->source_method;
+    k.limiter = opt->limiter; k.method = opt->source_method; k.source_literal = opt->source_literal;
     k.n0_floor = opt->n0_floor; k.rho_floor = opt->rho_floor; k.kappa_a0 = opt->kappa_a0; k.kappa_s = opt->kappa_s;
     k.a_rad = opt->a_rad; k.Y_over_rho = opt->Y_over_rho; k.abar = opt->abar;
     k.cen = t.cen; k.ecen = t.ecen; k.angcoef = t.angcoef; k.nhat = t.nhat; k.w = t.w; k.nb = t.nb; k.mirror = t.mirror;

@@ -19,7 +19,7 @@ struct KParams {
     double inv_dx[3];
     int bc_lo[3], bc_hi[3];
     int zlo[3], zhi[3];
-    int limiter, method;
+    int limiter, method, source_literal;
     int variant;    // RT_TRANSPORT_TMA only if tile_eligible(), else RT_TRANSPORT_L2
     int tile[3];    // RT_TRANSPORT_TMA: TX, TY, DCH of the vacuum tile kernel
     int tile_gen[3];   // ... of the Eq 23 tile kernel (one pair per thread)

@@ -94,7 +94,9 @@ constexpr int CELL_THREADS = 128, CELL_MINB = 4;   // 128 registers, 16 warps pe
 template <int MAXV>
 struct CellBatch { static constexpr int CB = MAXV <= 3 ? 8 : (24 / MAXV > 0 ? 24 / MAXV : 1); };
 
-template <int MAXV>
+// LITERAL: rt_options.source_literal with Method 2 or 3 -- Eq 35 with every opacity at T_+ (L432 taken literally, S19b's option):
+// phase 3 forms d_s again with alpha(T_+) (an instantiation of its own: the default path pays nothing for the option)
+template <int MAXV, bool LITERAL>
 __global__ void __launch_bounds__(CELL_THREADS, CELL_MINB)
 k_cell_batch(KParams p, double *I, double *T, double dt, int *n_fail) {
     constexpr int CB = CellBatch<MAXV>::CB;
@@ -203,7 +205,7 @@ k_cell_batch(KParams p, double *I, double *T, double dt, int *n_fail) {
         __syncwarp();
         // ---- phase 2: lane l solves the temperature equation of cell l mod CB ----
         bool ok = false;
-        double Tp = Tm, scale = 1.0, Sdt = 0.0;
+        double Tp = Tm, scale = 1.0, Sdt = 0.0, adtp = 0.0;
         if (interact) {
             const double *tot = part + CB * 3 * 33 + myc * 3;
             const double E = tot[0], A1 = tot[1], A2 = tot[2] * (dt / FOURPI);
@@ -225,7 +227,8 @@ k_cell_batch(KParams p, double *I, double *T, double dt, int *n_fail) {
             if (ok) {
                 const double Ep = W - Y * Tp;                                               // Eq 39
                 const double emis = (p.method == 1) ? aa * p.a_rad * Tp * Tp * Tp * Tp : Nbar * p.a_rad * sqrt(Tp);
-                scale = (p.method == 3) ? alpha / (as + Nbar * t_m35(Tp)) : 1.0;
+                scale = (p.method == 3 && !LITERAL) ? alpha / (as + Nbar * t_m35(Tp)) : 1.0;
+                if (LITERAL) adtp = (as + Nbar * t_m35(Tp)) * dt;
                 Sdt = (emis + as * Ep) * (dt / FOURPI);
                 if (lane < CB) T[mycell] = Tp;
             } else if (lane < CB && n_fail) {
@@ -243,11 +246,33 @@ k_cell_batch(KParams p, double *I, double *T, double dt, int *n_fail) {
             double *Ic = I + cell * p.pitch;
             if (ok_c) {
                 const double sc = __shfl_sync(0xffffffffu, scale, c), sd = __shfl_sync(0xffffffffu, Sdt, c);
+                if (LITERAL) {
+                    // val holds (n^0 / d_-) I_-: times d_- / d_+, and the source term with 1 / (d_+ nbar^3)
+                    const double b0 = __shfl_sync(0xffffffffu, uh0, c), b1 = __shfl_sync(0xffffffffu, uh1, c);
+                    const double b2 = __shfl_sync(0xffffffffu, uh2, c), b3 = __shfl_sync(0xffffffffu, uh3, c);
+                    const double am = __shfl_sync(0xffffffffu, adt, c), ap = __shfl_sync(0xffffffffu, adtp, c);
+                    const double *cen = p.cen + (long long)((unsigned)cell % (unsigned)p.ncol) * CEN_STRIDE;
+                    const double e0 = __ldg(cen + 4), e1 = __ldg(cen + 5), e2 = __ldg(cen + 6), e3 = __ldg(cen + 7);
 #pragma unroll
-                for (int v = 0; v < MAXV; ++v) {
-                    if ((livebits >> (c * MAXV + v)) & 1u) {
-                        val[c][v] = sc * (val[c][v] + sd * cbs[(c * MAXV + v) * 32 + lane]);
-                        Ic[lane + 32 * v] = val[c][v];
+                    for (int v = 0; v < MAXV; ++v) {
+                        if ((livebits >> (c * MAXV + v)) & 1u) {
+                            const int s = lane + 32 * v;
+                            const double nx = snx[s], ny = sny[s], nz = snz[s];
+                            const double nup = e0 + e1 * nx + e2 * ny + e3 * nz;
+                            const double nbar = b0 - (b1 * nx + b2 * ny + b3 * nz);
+                            const double dm = nup + nbar * am, dp = nup + nbar * ap, r = __drcp_rn(dp * nbar);
+                            const double rd = r * nbar, rn = r * dp;
+                            val[c][v] = val[c][v] * (dm * rd) + sd * (rd * (rn * rn * rn));
+                            Ic[s] = val[c][v];
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int v = 0; v < MAXV; ++v) {
+                        if ((livebits >> (c * MAXV + v)) & 1u) {
+                            val[c][v] = sc * (val[c][v] + sd * cbs[(c * MAXV + v) * 32 + lane]);
+                            Ic[lane + 32 * v] = val[c][v];
+                        }
                     }
                 }
             }
@@ -268,9 +293,12 @@ cudaError_t launch_cell_batch(const KParams &p, double *I, double *T, double dt,
         long long want = (p.ncell + (long long)warps * CB - 1) / ((long long)warps * CB);
         const int blocks = (int)(want < 148LL * 8 * 4 ? want : 148LL * 8 * 4);
         if (blocks == 0) return cudaSuccess;
-        cudaError_t e = cudaFuncSetAttribute(k_cell_batch<MAXV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        const bool literal = p.source_literal && p.method != 1;   // (Method 1 does not update its opacities, L432)
+        cudaError_t e = literal ? cudaFuncSetAttribute(k_cell_batch<MAXV, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
+                                : cudaFuncSetAttribute(k_cell_batch<MAXV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        k_cell_batch<MAXV><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail);
+        if (literal) k_cell_batch<MAXV, true><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail);
+        else k_cell_batch<MAXV, false><<<blocks, threads, smem, st>>>(p, I, T, dt, n_fail);
         return cudaGetLastError();
     };
     if (p.nd <= 64) return go(std::integral_constant<int, 2>());

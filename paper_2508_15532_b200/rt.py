@@ -50,7 +50,7 @@ class RtOptions(ctypes.Structure):
                 ("n0_floor", ctypes.c_double), ("rho_floor", ctypes.c_double), ("kappa_a0", ctypes.c_double),
                 ("kappa_s", ctypes.c_double), ("a_rad", ctypes.c_double), ("Y_over_rho", ctypes.c_double),
                 ("abar", ctypes.c_double), ("transport_variant", ctypes.c_int), ("transport_tile", ctypes.c_int * 3),
-                ("grid_axis", ctypes.c_double * 3), ("grid_boost", ctypes.c_double * 3), ("angflux_split", ctypes.c_int)]
+                ("grid_axis", ctypes.c_double * 3), ("grid_boost", ctypes.c_double * 3), ("angflux_split", ctypes.c_int), ("source_literal", ctypes.c_int)]
 
 
 def load_library(path=LIB_PATH):

@@ -461,3 +461,22 @@ def test_rest_frame_fluid_is_rebuilt_after_an_explicit_velocity():
     assert torch.equal(a[0], b[0]) and torch.equal(a[1], b[1])
     assert not torch.equal(a[0], c[0])
     assert torch.equal(a[0], d[0]) and torch.equal(a[1], d[1])
+
+
+# ---- rt_options.source_literal: Eq 35 with every opacity at T_+ (L432 taken literally, S19b's option) -------------------------------
+@pytest.mark.parametrize("idx,n,method", [(2, (6, 5, 4), 2), (2, (6, 5, 4), 3), (4, (16, 12, 4), 2), (4, (12, 10, 4), 3), (5, (8, 6, 4), 2),
+                                          (2, (6, 5, 4), 1)])
+def test_literal_opacity_update_matches_oracle(idx, n, method):
+    cfg = W.config(idx, n=n)
+    cfg["options"] = dict(cfg["options"], method=method, source_literal=1)
+    orc, ctx, f, dt = make_pair(cfg)
+    out = run_steps(orc, ctx, f, dt, 3)
+    _check(out)
+    ctx.close()
+    if method != 1:   # and it is not the default update in disguise
+        cfg0 = W.config(idx, n=n)
+        cfg0["options"] = dict(cfg0["options"], method=method)
+        orc0, ctx0, f0, _ = make_pair(cfg0)
+        out0 = run_steps(orc0, ctx0, f0, dt, 3)
+        assert rel_err(out0["I"][0], out["I"][0]) > 1e-7
+        ctx0.close()

@@ -298,3 +298,49 @@ def test_split_angular_flux_conserves_and_reduces_to_the_default_where_it_must()
     for d in (d1, d0):
         tot = (d * wgt[None]).sum(-1)[:, unmasked]
         assert np.abs(tot).max() <= 1e-12 * np.abs(d * wgt[None]).sum(-1)[:, unmasked].max() + 1e-18
+
+
+# ---- L432 taken literally: every opacity of Eq 35 at T_+ (option source_literal, S19b) -----------------------------------------
+def _relax_cell(method, literal, kappa_a0, kappa_s, dt, T0=1.4):
+    from oracle import Oracle
+    import numpy as np
+    grid = dict(n=(2, 2, 2), x0=(0, 0, 0), dx=(1.0,) * 3, bc_lo=("periodic",) * 3, bc_hi=("periodic",) * 3)
+    o = Oracle(grid, "minkowski", {}, 2, dict(method=method, kappa_a0=kappa_a0, kappa_s=kappa_s, source_literal=literal))
+    rng = np.random.default_rng(5)
+    I = rng.uniform(0.02, 0.06, size=(2, 2, 2, o.nd))
+    T = np.full((2, 2, 2), T0)
+    o.set_fluid(np.ones((2, 2, 2)), T, None)
+    I1, T1, nf = o.source_implicit(I.copy(), T.copy(), dt)
+    assert nf == 0
+    w = o.ang["w"]
+    E0, E1 = (I * w).sum(-1), (np.asarray(I1).reshape(I.shape) * w).sum(-1)
+    Y = 1.5
+    # energy the gas gave up against energy the radiation gained (Eq 39: they are equal for the conservative reading)
+    return np.asarray(I1).reshape(I.shape), np.asarray(T1).reshape(T.shape), np.abs((E1 - E0) + Y * (np.asarray(T1).reshape(T.shape) - T)).max(), np.abs(E1 - E0).max()
+
+
+def test_literal_opacity_update_is_the_default_where_the_opacity_does_not_change_and_second_order_close_elsewhere():
+    import numpy as np
+    # Method 1 keeps its opacities (L432 names Methods 2 and 3 only); pure scattering has no temperature in its opacity
+    for method, ka, ks in ((1, 3.0, 0.5), (2, 0.0, 2.0), (3, 0.0, 2.0)):
+        a = _relax_cell(method, 0, ka, ks, 0.05)
+        b = _relax_cell(method, 1, ka, ks, 0.05)
+        assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]), method
+    for method in (2, 3):
+        mis = []
+        for dt in (0.02, 0.01, 0.005):
+            I0, T0, bal0, dE0 = _relax_cell(method, 0, 3.0, 0.5, dt)
+            I1, T1, bal1, dE1 = _relax_cell(method, 1, 3.0, 0.5, dt)
+            assert np.array_equal(T0, T1)                        # the temperature equation is the same
+            assert np.isfinite(I1).all() and I1.min() > 0 and np.abs(I1 - I0).max() > 1e-7
+            if method == 2:
+                assert bal0 <= 1e-13 * dE0 + 1e-16               # conservative reading: Eq 39 to round-off
+            assert bal1 > 1e-9 * dE1                               # the literal update does not close the balance ...
+            mis.append(bal1 / dE1)
+        if method == 2:
+            # ... by O(alpha_+ - alpha_-) = O(dt) of the exchanged energy (which is itself O(dt)): halves with dt
+            assert 1.8 < mis[0] / mis[1] < 2.3 and 1.8 < mis[1] / mis[2] < 2.3, mis
+        else:
+            # Method 3's temperature equation was derived for the update scaled by alpha_- / alpha_+ (S19b); without the factor the
+            # un-interacted part is off by that ratio: the same order as the exchanged energy, at every dt
+            assert 0.1 < mis[2] < 1.0 and abs(mis[0] / mis[2] - 1.0) < 0.2, mis
