@@ -11,7 +11,8 @@ R, G inside the timed region).  `roofline` = dominant kernel, algorithmic bytes 
 N > 1: the mesh grows with N along x3 and is cut into slabs, one per rank, with a 4-plane halo
 exchanged point to point once per step (inside the timed region); value = owned cell-directions of all ranks * steps /
 max-over-ranks time ("weak").  --multi slab-strong: the config's own mesh cut into N slabs ("strong"; every rank still carries
-its 8 halo planes, so thin slabs pay for them).  --multi replicas: N independent copies instead.
+its 8 halo planes, so thin slabs pay for them).  --multi box [--pgrid P2xP3]: the config's own mesh in x2 x x3 boxes.  --multi
+replicas: N independent copies instead.
 """
 import argparse
 import json
@@ -35,9 +36,11 @@ def parse():
     ap.add_argument("--warmup", type=int, default=None, help="untimed warm-up steps (default 5; 1 for --impl reference)")
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index 1..5 (4 = Kerr-Schild, the roofline config); 6 = snake-coordinates beam (PAPER 4.6)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--multi", default="slab", choices=["slab", "slab-strong", "replicas"],
+    ap.add_argument("--pgrid", default=None, help="--multi box: process grid P2xP3 along x2 and x3 (default: the most square factorisation of N)")
+    ap.add_argument("--multi", default="slab", choices=["slab", "slab-strong", "box", "replicas"],
                     help="N > 1: slab decomposition along x3 with halo exchange -- the mesh grows with N (slab, weak scaling, default) or "
-                         "stays the config's (slab-strong: strong scaling, 8 halo planes per rank on fewer owned ones) -- or independent replicas")
+                         "stays the config's (slab-strong: strong scaling, 8 halo planes per rank on fewer owned ones; box: the config's mesh cut "
+                         "along x2 and x3, dist.BoxDomain) -- or independent replicas")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--size", default=None, help="override grid, e.g. 64x48x32 (debug)")
@@ -203,6 +206,43 @@ def setup_slab(args, cfg, rank, world, device):
     return slab, gcfg, float(t.item())
 
 
+def setup_box(args, cfg, rank, world, device):
+    """N > 1, --multi box: the config's own mesh cut into P2 x P3 boxes along x2 and x3 (strong scaling), 4-cell halos on both axes,
+    exchanged axis by axis once per step.  Every rank generates the global seeded fields and keeps its box.  returns (BoxDomain, dt)."""
+    import torch
+    import torch.distributed as dist
+    import rt_workloads as W
+    from paper_2508_15532_b200.dist import BoxDomain
+    if args.pgrid:
+        p2, p3 = (int(x) for x in args.pgrid.lower().split("x"))
+    else:
+        p2 = max(d for d in range(1, int(world ** 0.5) + 1) if world % d == 0)
+        p3 = world // p2
+    if p2 * p3 != world:
+        raise ValueError("--pgrid %dx%d does not match %d ranks" % (p2, p3, world))
+    box = BoxDomain(cfg, rank, p2, p3, device=device)
+    kind, params = cfg["metric"]
+    f = W.fields(cfg, box.ctx.directions()["nhat"], _global_e_c(cfg, kind, params))
+    box.set_fields(f)
+    dt = cfg["dt"] if cfg["dt"] is not None else min(box.ctx.cfl_dt())
+    t = torch.tensor([dt], dtype=torch.float64, device=box.device)
+    dist.all_reduce(t, op=dist.ReduceOp.MIN)
+    return box, float(t.item())
+
+
+def _global_e_c(cfg, kind, params):
+    """tetrad at the cell centres of the GLOBAL mesh (input of the field generator; the oracle's geometry module is a table builder
+    the generators already rely on in the tests -- here a throw-away one-plane context of the library gives the same table)"""
+    from paper_2508_15532_b200 import rt
+    g = dict(cfg["grid"])
+    n = g["n"]
+    g["n"] = (n[0], n[1], min(n[2], 8))
+    probe = rt.RtContext(g, kind, params, cfg["level"], cfg["options"])
+    e = probe.geometry("e_c")
+    probe.close()
+    return e
+
+
 def run_gpu(args, rank, world):
     import numpy as np
     import torch
@@ -221,6 +261,15 @@ def run_gpu(args, rank, world):
                                                                                  slab.layout.k1 - slab.layout.k0, dist.get_backend(), slab.layout.n3_local))
         except Exception as e:   # e.g. slabs thinner than the halo: fall back to independent replicas, and say so
             slab, multi = None, "replicas only (slab decomposition unavailable: %s)" % str(e)[:120]
+    elif world > 1 and args.multi == "box":
+        try:
+            slab, dt = setup_box(args, cfg, rank, world, device)
+            L = slab.layout
+            multi = ("box decomposition %d x %d along x2, x3 (strong, the config's mesh: %d rows x %d planes owned, %d x %d computed per rank), "
+                     "4-cell halos exchanged axis by axis once per step over %s send/recv"
+                     % (L.p2, L.p3, L.L2.k1 - L.L2.k0, L.L3.k1 - L.L3.k0, L.L2.n3_local, L.L3.n3_local, dist.get_backend()))
+        except Exception as e:
+            slab, multi = None, "replicas only (box decomposition unavailable: %s)" % str(e)[:120]
     elif world > 1:
         multi = "replicas only (--multi replicas)"
     if slab is not None:
@@ -496,7 +545,7 @@ def main():
                 "step_frac_of_peak_32B": STEP_BYTES_IDEAL * r["units"] / step_s / 1e9 / peak,
                 "step_frac_of_peak_74B": STEP_BYTES_TWO_KERNEL * r["units"] / step_s / 1e9 / peak}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
-                "ms_per_step": ms / K, "higher_is_better": True, "scaling": "strong" if (world > 1 and args.multi == "slab-strong" and r["slab"]) else "weak",
+                "ms_per_step": ms / K, "higher_is_better": True, "scaling": "strong" if (world > 1 and args.multi in ("slab-strong", "box") and r["slab"]) else "weak",
                 "vs_baseline": None, "dtype": "f64",
                 "data": "synthetic",
                 "config": {"workload": workload_name(r["cfg"]), "dt": r["dt"], "l2": "inputs larger than L2 (one I copy >= 1 GB vs 126 MB)"

@@ -210,3 +210,192 @@ def exchange_local(domains):
             getattr(d, name)[L.recv_lo() if side == "lo" else L.recv_hi()].copy_(v)
     if torch.cuda.is_available():
         torch.cuda.synchronize()
+
+
+# ---- two-dimensional decomposition: x2 x x3 boxes ------------------------------------------------------------------------------------
+# The same deep-halo scheme along two axes: a rank owns a box of rows (x2) and planes (x3) and carries MARGIN of each on every cut side.
+# Thin x3 slabs pay 8 / n3_local redundant planes; cutting x2 as well keeps both factors small on many ranks (8 ranks on a 96 x 64
+# (x2, x3) mesh: 2 x 4 boxes compute (48 + 4..8) x (16 + 8) instead of 96 x (8 + 8): 1.6x the owned cells instead of 2x).  The halo is
+# exchanged axis by axis -- x3 first (contiguous planes, all local rows), then x2 (rows of all local planes, margins included, packed
+# by `.contiguous()`) -- so the corner blocks arrive through the second phase.  rank = r3 * p2 + r2.
+class BoxLayout:
+    def __init__(self, n2, n3, periodic2, periodic3, rank, p2, p3, margin=MARGIN):
+        if p2 < 1 or p3 < 1 or not (0 <= rank < p2 * p3):
+            raise ValueError("bad rank / process grid")
+        self.p2, self.p3, self.rank, self.world = p2, p3, rank, p2 * p3
+        self.r2, self.r3 = rank % p2, rank // p2
+        self.L2 = SlabLayout(n2, periodic2, self.r2, p2, margin)
+        self.L3 = SlabLayout(n3, periodic3, self.r3, p3, margin)
+
+    def peer(self, axis, r):
+        """global rank of the box at position r along `axis` (2 or 3) in my row / column of the process grid"""
+        return self.r3 * self.p2 + r if axis == 2 else r * self.p2 + self.r2
+
+
+def _axis_slice(t, axis, sl):
+    idx = [slice(None)] * t.dim()
+    idx[axis] = sl
+    return t[tuple(idx)]
+
+
+def exchange_axis(layout, tensors, axes, left, right, group=None):
+    """`exchange` along an arbitrary tensor axis: tensors[i]'s decomposed axis is axes[i]; left / right are the neighbours' global
+    ranks.  Non-leading axes give strided pieces: sent from a packed copy, received into a buffer and copied in."""
+    import torch
+    import torch.distributed as dist
+    if layout.world == 1:
+        return
+    stage = dist.get_backend(group) == "gloo" and any(t.is_cuda for t in tensors)
+    ops, landed = [], []
+    for t, ax in zip(tensors, axes):
+        def send(sl, peer):
+            piece = _axis_slice(t, ax, sl).contiguous()
+            ops.append(dist.P2POp(dist.isend, piece.cpu() if stage else piece, peer, group))
+
+        def recv(sl, peer):
+            view = _axis_slice(t, ax, sl)
+            buf = torch.empty(view.shape, dtype=t.dtype, device="cpu" if stage else t.device)
+            landed.append((view, buf))
+            ops.append(dist.P2POp(dist.irecv, buf, peer, group))
+
+        if layout.lo_cut:
+            send(layout.send_lo(), left)
+        if layout.hi_cut:
+            send(layout.send_hi(), right)
+        if layout.hi_cut:
+            recv(layout.recv_hi(), right)
+        if layout.lo_cut:
+            recv(layout.recv_lo(), left)
+    for req in dist.batch_isend_irecv(ops):
+        req.wait()
+    for view, buf in landed:
+        view.copy_(buf)
+
+
+def exchange_box(layout, tensors, axes3, axes2, group=None):
+    """Halo update of a BoxLayout: x3 first, then x2 (whose pieces span the x3 margins: corners)."""
+    L = layout
+    if L.p3 > 1:
+        exchange_axis(L.L3, tensors, axes3, None if L.L3.left is None else L.peer(3, L.L3.left),
+                      None if L.L3.right is None else L.peer(3, L.L3.right), group)
+    if L.p2 > 1:
+        exchange_axis(L.L2, tensors, axes2, None if L.L2.left is None else L.peer(2, L.L2.left),
+                      None if L.L2.right is None else L.peer(2, L.L2.right), group)
+
+
+def _cut_grid(g, grid, layout, dim):
+    """the part of local_grid() that concerns one dim, for a 1-D layout along it"""
+    n = list(g["n"]); n[dim] = layout.n3_local; g["n"] = tuple(n)
+    x0 = list(g["x0"]); x0[dim] = grid["x0"][dim] + (layout.k0 - layout.ext_lo) * grid["dx"][dim]; g["x0"] = tuple(x0)
+    bl, bh = list(g["bc_lo"]), list(g["bc_hi"])
+    if layout.world > 1:
+        bl[dim] = "outflow" if layout.lo_cut else grid["bc_lo"][dim]
+        bh[dim] = "outflow" if layout.hi_cut else grid["bc_hi"][dim]
+        if layout.periodic:
+            bl[dim] = bh[dim] = "outflow"
+    g["bc_lo"], g["bc_hi"] = tuple(bl), tuple(bh)
+    zl, zh = list(g.get("zero_lo", (0, 0, 0))), list(g.get("zero_hi", (0, 0, 0)))
+    if layout.lo_cut:
+        zl[dim] = 0
+    if layout.hi_cut:
+        zh[dim] = 0
+    g["zero_lo"], g["zero_hi"] = tuple(zl), tuple(zh)
+    return g
+
+
+def local_grid_box(grid, layout):
+    g = dict(grid)
+    g.setdefault("zero_lo", (0, 0, 0)); g.setdefault("zero_hi", (0, 0, 0))
+    g = _cut_grid(g, grid, layout.L3, 2)
+    return _cut_grid(g, grid, layout.L2, 1)
+
+
+class BoxDomain:
+    """One rank's box of a mesh decomposed along x2 and x3 (see BoxLayout): library context on the extended box + the halo exchange.
+    Same interface as SlabDomain (global fields are cut here)."""
+
+    def __init__(self, cfg, rank, p2, p3, device="cuda:0", group=None):
+        import torch
+        from . import rt
+        grid = cfg["grid"]
+        self.layout = BoxLayout(grid["n"][1], grid["n"][2], grid["bc_lo"][1] == "periodic", grid["bc_lo"][2] == "periodic", rank, p2, p3)
+        self.group = group
+        kind, params = cfg["metric"]
+        self.cfg, self.grid = cfg, local_grid_box(grid, self.layout)
+        self.ctx = rt.RtContext(self.grid, kind, params, cfg["level"], cfg["options"], device=device)
+        self.device = self.ctx.device
+        self.I = self.T = None
+        self.R = torch.zeros((16,) + self.ctx.shape, dtype=torch.float64, device=self.device)
+        self.G = torch.zeros((4,) + self.ctx.shape, dtype=torch.float64, device=self.device)
+        L2, L3 = self.layout.L2, self.layout.L3
+        self.owned_units = (L3.k1 - L3.k0) * (L2.k1 - L2.k0) * grid["n"][0] * self.ctx.nd
+
+    def _cut(self, a, lead=0):
+        """global [.., N3, N2, ...] -> this box's planes and rows (x3 at axis `lead`)"""
+        L2, L3 = self.layout.L2, self.layout.L3
+        a = np.take(a, L3.planes, axis=lead)
+        return np.ascontiguousarray(np.take(a, L2.planes, axis=lead + 1))
+
+    def set_fields(self, f):
+        import torch
+        dev, L2, L3 = self.device, self.layout.L2, self.layout.L3
+        rho, T = self._cut(f["rho"]), self._cut(f["T"])
+        u4 = None if f.get("u4") is None else torch.as_tensor(self._cut(f["u4"], 1), device=dev)
+        self.ctx.set_fluid(torch.as_tensor(rho, device=dev), torch.as_tensor(T, device=dev), u4)
+        self.I = self.ctx.to_device(self._cut(f["I0"]))
+        self.T = torch.as_tensor(T, device=dev).clone()
+        n1, n2, n3 = self.cfg["grid"]["n"]
+        for (dim, side), g in f.get("ghosts", {}).items():
+            g = np.asarray(g)
+            nd = g.shape[-1]
+            if dim == 0:      # [layer][k * N2 + j]
+                g = g.reshape(2, n3, n2, nd)[:, L3.planes][:, :, L2.planes].reshape(2, -1, nd)
+            elif dim == 1:    # [layer][k * N1 + i]: belongs to the boxes at that physical end of x2
+                if (side == 0 and L2.lo_cut) or (side == 1 and L2.hi_cut):
+                    continue
+                g = g.reshape(2, n3, n1, nd)[:, L3.planes].reshape(2, -1, nd)
+            else:             # [layer][j * N1 + i]
+                if (side == 0 and L3.lo_cut) or (side == 1 and L3.hi_cut):
+                    continue
+                g = g.reshape(2, n2, n1, nd)[:, L2.planes].reshape(2, -1, nd)
+            gd = torch.zeros(g.shape[:2] + (self.ctx.pitch,), dtype=torch.float64, device=dev)
+            gd[..., :self.ctx.nd] = torch.as_tensor(np.ascontiguousarray(g), device=dev)
+            self.ctx.set_boundary(dim, side, gd)
+
+    def exchange_halo(self):
+        exchange_box(self.layout, [self.I, self.T], [0, 0], [1, 1], self.group)
+
+    def step(self, dt, moments=True):
+        self.ctx.step(self.I, self.T, dt, self.R if moments else None, self.G if moments else None)
+        self.exchange_halo()
+
+    def owned(self, t, lead=0):
+        """View of the owned planes and rows of a box tensor whose x3 axis is `lead` (x2 follows it)."""
+        idx = [slice(None)] * t.dim()
+        idx[lead], idx[lead + 1] = self.layout.L3.owned, self.layout.L2.owned
+        return t[tuple(idx)]
+
+
+def exchange_local_box(domains):
+    """exchange_box for boxes that live in ONE process (list index = rank): x3 phase, then x2 phase, each reading everything before
+    it writes anything."""
+    import torch
+    for axis, attr, tax in ((3, "L3", 0), (2, "L2", 1)):
+        new = []
+        for d in domains:
+            L, got = getattr(d.layout, attr), {}
+            for name in ("I", "T"):
+                t = getattr(d, name)
+                if L.lo_cut:
+                    src = domains[d.layout.peer(axis, L.left)]
+                    got[(name, "lo")] = _axis_slice(getattr(src, name), tax, getattr(src.layout, attr).send_hi()).to(t.device, copy=True)
+                if L.hi_cut:
+                    src = domains[d.layout.peer(axis, L.right)]
+                    got[(name, "hi")] = _axis_slice(getattr(src, name), tax, getattr(src.layout, attr).send_lo()).to(t.device, copy=True)
+            new.append(got)
+        for d, got in zip(domains, new):
+            L = getattr(d.layout, attr)
+            for (name, side), v in got.items():
+                _axis_slice(getattr(d, name), tax, L.recv_lo() if side == "lo" else L.recv_hi()).copy_(v)
+    if torch.cuda.is_available():
+        torch.cuda.synchronize()

@@ -93,3 +93,86 @@ def test_exchange_over_gloo(tmp_path, world, n3, periodic):
     p = subprocess.run(cmd, capture_output=True, text=True, timeout=300, env=env)
     assert p.returncode == 0, p.stdout[-2000:] + p.stderr[-2000:]
     assert p.stdout.count("ok") == world
+
+
+# ---- two-dimensional (x2 x x3) decomposition --------------------------------------------------------------------------------------
+from paper_2508_15532_b200.dist import BoxLayout, local_grid_box
+
+
+@pytest.mark.parametrize("n2,n3,p2,p3,per2,per3", [(12, 16, 2, 2, False, True), (17, 13, 3, 2, True, False), (8, 40, 1, 4, False, True),
+                                                   (24, 9, 4, 1, True, True)])
+def test_box_layout_partitions_the_mesh(n2, n3, p2, p3, per2, per3):
+    seen = np.zeros((n3, n2), int)
+    for r in range(p2 * p3):
+        B = BoxLayout(n2, n3, per2, per3, r, p2, p3)
+        assert B.rank == B.r3 * p2 + B.r2 and B.peer(2, B.r2) == r and B.peer(3, B.r3) == r
+        seen[B.L3.k0:B.L3.k1, B.L2.k0:B.L2.k1] += 1
+        for axis, L in ((2, B.L2), (3, B.L3)):
+            if L.lo_cut:
+                N = BoxLayout(n2, n3, per2, per3, B.peer(axis, L.left), p2, p3)
+                Ln = N.L2 if axis == 2 else N.L3
+                assert (L.planes[L.recv_lo()] == Ln.planes[Ln.send_hi()]).all()
+                # the neighbour along one axis has my position along the other
+                assert (N.r3 == B.r3) if axis == 2 else (N.r2 == B.r2)
+    assert (seen == 1).all()
+
+
+def test_local_grid_box_boundaries():
+    grid = dict(n=(8, 24, 20), x0=(0.0, 2.0, 1.0), dx=(0.1, 0.25, 0.5), bc_lo=("outflow", "reflect", "periodic"),
+                bc_hi=("outflow", "outflow", "periodic"), zero_lo=(0, 2, 0), zero_hi=(0, 3, 0))
+    g = local_grid_box(grid, BoxLayout(24, 20, False, True, 0, 2, 2))          # r2 = 0, r3 = 0
+    assert g["n"] == (8, 12 + MARGIN, 10 + 2 * MARGIN)
+    assert g["bc_lo"] == ("outflow", "reflect", "outflow") and g["bc_hi"] == ("outflow", "outflow", "outflow")
+    assert g["zero_lo"] == (0, 2, 0) and g["zero_hi"] == (0, 0, 0)             # the upper x2 side is a cut: no band there
+    assert g["x0"][1] == 2.0 and abs(g["x0"][2] - (1.0 - MARGIN * 0.5)) < 1e-15
+    g = local_grid_box(grid, BoxLayout(24, 20, False, True, 3, 2, 2))          # r2 = 1, r3 = 1
+    assert g["bc_lo"][1] == "outflow" and g["bc_hi"][1] == "outflow" and g["zero_lo"][1] == 0 and g["zero_hi"][1] == 3
+    assert abs(g["x0"][1] - (2.0 + (12 - MARGIN) * 0.25)) < 1e-15
+
+
+WORKER2 = textwrap.dedent('''
+    import os, sys
+    import numpy as np, torch, torch.distributed as dist
+    sys.path.insert(0, sys.argv[1])
+    from paper_2508_15532_b200.dist import BoxLayout, exchange_box
+    n2, n3, p2, p3 = (int(x) for x in sys.argv[2:6])
+    per2, per3 = sys.argv[6] == "1", sys.argv[7] == "1"
+    dist.init_process_group("gloo")
+    rank, world = dist.get_rank(), dist.get_world_size()
+    assert world == p2 * p3
+    B = BoxLayout(n2, n3, per2, per3, rank, p2, p3)
+    K = torch.as_tensor(B.L3.planes, dtype=torch.float64)[:, None, None]
+    J = torch.as_tensor(B.L2.planes, dtype=torch.float64)[None, :, None]
+    def make(width):
+        want = K * 1000 + J * 10 + torch.arange(width, dtype=torch.float64)[None, None, :]
+        t = torch.full(want.shape, -1.0, dtype=torch.float64)
+        t[B.L3.owned, B.L2.owned] = want[B.L3.owned, B.L2.owned]
+        return t, want
+    (A, wa), (C, wc) = make(3), make(1)
+    Cs = C[..., 0].clone()                      # a tensor without trailing axes, like T
+    for _ in range(2):
+        exchange_box(B, [A, Cs], [0, 0], [1, 1])
+    assert torch.equal(A, wa), (rank, (A - wa).abs().max())
+    assert torch.equal(Cs, wc[..., 0])
+    dist.barrier()
+    dist.destroy_process_group()
+    print("ok", rank)
+''')
+
+
+@pytest.mark.parametrize("p2,p3,n2,n3,per2,per3", [(2, 2, 11, 13, False, True), (2, 2, 9, 9, True, True), (3, 1, 14, 5, False, False),
+                                                   (2, 3, 10, 14, False, False)])
+def test_box_exchange_over_gloo(tmp_path, p2, p3, n2, n3, per2, per3):
+    """Margins AND corner blocks of every box equal the global field after the two-phase exchange (real processes, gloo)."""
+    script = tmp_path / "worker2.py"
+    script.write_text(WORKER2)
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(p2 * p3),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), str(script), ROOT, str(n2), str(n3), str(p2), str(p3),
+           "1" if per2 else "0", "1" if per3 else "0"]
+    env = dict(os.environ, OMP_NUM_THREADS="1")
+    p = subprocess.run(cmd, capture_output=True, text=True, timeout=300, env=env)
+    assert p.returncode == 0, p.stdout[-2000:] + p.stderr[-2000:]
+    assert p.stdout.count("ok") == p2 * p3

@@ -99,3 +99,50 @@ def test_rt_step_host_pipeline_equals_rt_step(idx, n):
         assert nf == 0
         for a, b in ((I, hI), (T, hT), (R, hR), (G, hG)):
             assert torch.equal(a.cpu(), b)
+
+
+# ---- two-dimensional (x2 x x3) decomposition: every box of a process grid held in one process ---------------------------------------
+@pytest.mark.parametrize("idx,n,p2,p3", [(4, (10, 20, 16), 2, 2), (3, (7, 12, 13), 2, 2), (3, (6, 13, 9), 3, 1), (4, (8, 16, 24), 2, 3)])
+def test_boxes_reproduce_the_single_domain(idx, n, p2, p3):
+    """I, T, R, G on the owned rows and planes of every box against the single-domain run -- bit for bit in flat space; in a curved
+    metric a box cut along x2 evaluates its geometry at x0_local + (j + 1/2) dx, which differs from the global x0 + (j_global + 1/2) dx
+    in the last bit, so the comparison is to rounding (1e-13) there -- and every box's margins (corner blocks included) equal to the
+    neighbours' owned values after the two-phase exchange."""
+    from paper_2508_15532_b200 import rt
+    from paper_2508_15532_b200.dist import BoxDomain, exchange_local_box
+    cfg = W.config(idx, n=n)
+    kind, params = cfg["metric"]
+    probe = rt.RtContext(cfg["grid"], kind, params, cfg["level"], cfg["options"])
+    f = W.fields(cfg, probe.directions()["nhat"], probe.geometry("e_c"))
+    if idx == 3:
+        f["I0"] = f["I0"] + np.random.default_rng(3).uniform(0.5, 1.0, size=f["I0"].shape) / (4 * np.pi)
+    dt = cfg["dt"] if cfg["dt"] is not None else min(probe.cfl_dt())
+    probe.close()
+    one = _single(cfg, f, dt, 3)
+    exact = kind == "minkowski" or p2 == 1
+    doms = [BoxDomain(cfg, r, p2, p3) for r in range(p2 * p3)]
+    for d in doms:
+        d.set_fields(f)
+    for _ in range(3):
+        for d in doms:
+            d.ctx.step(d.I, d.T, dt, d.R, d.G)
+        exchange_local_box(doms)
+    for name, lead in (("I", 0), ("T", 0), ("R", 1), ("G", 1)):
+        whole = getattr(one, name)
+        for d in doms:
+            L2, L3 = d.layout.L2, d.layout.L3
+            idx_w = [slice(None)] * whole.dim()
+            idx_w[lead], idx_w[lead + 1] = slice(L3.k0, L3.k1), slice(L2.k0, L2.k1)
+            part = d.owned(getattr(d, name), lead)
+            if exact:
+                assert torch.equal(part, whole[tuple(idx_w)]), (name, d.layout.rank, float((part - whole[tuple(idx_w)]).abs().max()))
+            else:
+                scale = float(one.R.abs().max()) / dt if name == "G" else float(whole.abs().max())
+                assert float((part - whole[tuple(idx_w)]).abs().max()) <= 1e-13 * scale, (name, d.layout.rank)
+    full = torch.zeros_like(one.I)   # the decomposed run's own global field, from the owned parts
+    for d in doms:
+        L2, L3 = d.layout.L2, d.layout.L3
+        full[L3.k0:L3.k1, L2.k0:L2.k1] = d.owned(d.I, 0)
+    for d in doms:   # margins and corners hold the neighbours' owned values
+        want = full[torch.as_tensor(d.layout.L3.planes, device=one.I.device)][:, torch.as_tensor(d.layout.L2.planes, device=one.I.device)]
+        assert torch.equal(d.I, want), d.layout.rank
