@@ -41,6 +41,7 @@ def parse():
                     help="N > 1: slab decomposition along x3 with halo exchange -- the mesh grows with N (slab, weak scaling, default) or "
                          "stays the config's (slab-strong: strong scaling, 8 halo planes per rank on fewer owned ones; box: the config's mesh cut "
                          "along x2 and x3, dist.BoxDomain) -- or independent replicas")
+    ap.add_argument("--overlap", action="store_true", help="N > 1, slab modes: boundary planes first, their transfer overlapped with the whole-slab step (dist.SlabDomain.step_overlapped)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--size", default=None, help="override grid, e.g. 64x48x32 (debug)")
@@ -276,7 +277,10 @@ def run_gpu(args, rank, world):
         ctx, I, T, R, G = slab.ctx, slab.I, slab.T, slab.R, slab.G
         dev = ctx.device
         units = slab.owned_units                     # cells this rank OWNS x directions (halo planes are not counted)
-        step = lambda: slab.step(dt)
+        ov = bool(args.overlap and hasattr(slab, "enable_overlap") and slab.enable_overlap())
+        if args.overlap:
+            multi += "; boundary first, transfer overlapped with the whole-slab step" if ov else "; --overlap not applicable here (plain exchange)"
+        step = (lambda: slab.step(dt, overlap=True)) if ov else (lambda: slab.step(dt))
     else:
         ctx, f, I, T, dt = setup_gpu(cfg, device)
         dev = ctx.device

@@ -146,3 +146,85 @@ def test_boxes_reproduce_the_single_domain(idx, n, p2, p3):
     for d in doms:   # margins and corners hold the neighbours' owned values
         want = full[torch.as_tensor(d.layout.L3.planes, device=one.I.device)][:, torch.as_tensor(d.layout.L2.planes, device=one.I.device)]
         assert torch.equal(d.I, want), d.layout.rank
+
+
+# ---- boundary first: the planes a neighbour needs, stepped ahead of the slab, are the slab's own result -----------
+@pytest.mark.parametrize("idx,n,world", [(4, (12, 10, 32), 2), (3, (9, 8, 36), 3), (5, (8, 6, 24), 2)])
+def test_boundary_first_planes_equal_the_whole_slab_step(idx, n, world):
+    from paper_2508_15532_b200 import rt
+    from paper_2508_15532_b200.dist import SlabDomain, exchange_local
+    cfg = W.config(idx, n=n)
+    kind, params = cfg["metric"]
+    probe = rt.RtContext(cfg["grid"], kind, params, cfg["level"], cfg["options"])
+    f = W.fields(cfg, probe.directions()["nhat"], probe.geometry("e_c"))
+    f["ghosts"] = {}
+    dt = cfg["dt"] if cfg["dt"] is not None else min(probe.cfl_dt())
+    probe.close()
+    doms = [SlabDomain(cfg, r, world) for r in range(world)]
+    for d in doms:
+        d.set_fields(f)
+        assert d.enable_overlap()
+    m = doms[0].layout.margin
+    for _ in range(3):
+        ahead = [d.boundary_first(dt) for d in doms]
+        for d in doms:
+            d.ctx.step(d.I, d.T, dt, d.R, d.G)
+        for d, a in zip(doms, ahead):
+            L = d.layout
+            assert set(a) == ({"lo"} if L.lo_cut else set()) | ({"hi"} if L.hi_cut else set())
+            for side, (Ia, Ta) in a.items():
+                sl = L.send_lo() if side == "lo" else L.send_hi()
+                assert torch.equal(Ia, d.I[sl]) and torch.equal(Ta, d.T[sl]), (L.rank, side)
+        exchange_local(doms)
+    assert not SlabDomain(cfg, 0, 1).enable_overlap()          # nothing to overlap on one rank
+
+
+OVERLAP_WORKER = """
+import sys
+import numpy as np, torch, torch.distributed as dist
+sys.path.insert(0, sys.argv[1])
+import rt_workloads as W
+from paper_2508_15532_b200 import rt
+from paper_2508_15532_b200.dist import SlabDomain
+dist.init_process_group("gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+cfg = W.config(4, n=(12, 10, 32))
+kind, params = cfg["metric"]
+probe = rt.RtContext(cfg["grid"], kind, params, cfg["level"], cfg["options"])
+f = W.fields(cfg, probe.directions()["nhat"], probe.geometry("e_c"))
+f["ghosts"] = {}
+dt = min(probe.cfl_dt())
+probe.close()
+res = []
+for overlap in (False, True):
+    d = SlabDomain(cfg, rank, world)
+    d.set_fields(f)
+    if overlap:
+        assert d.enable_overlap()
+    for _ in range(3):
+        d.step(dt, overlap=overlap)
+    torch.cuda.synchronize()
+    res.append((d.I.clone(), d.T.clone(), d.R.clone(), d.G.clone()))
+for a, b in zip(*res):
+    assert torch.equal(a, b), float((a - b).abs().max())
+dist.barrier()
+dist.destroy_process_group()
+print("ok", rank)
+"""
+
+
+def test_overlapped_step_equals_the_plain_step_two_ranks(tmp_path):
+    """Two processes sharing the GPU, halo over gloo (host-staged): boundary-first + transfer on a side stream + whole-slab step gives
+    the state of step-then-exchange, margins included, bit for bit."""
+    import os, socket, subprocess, sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    script = tmp_path / "overlap_worker.py"
+    script.write_text(OVERLAP_WORKER)
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), str(script), root]
+    p = subprocess.run(cmd, capture_output=True, text=True, timeout=600, env=dict(os.environ, OMP_NUM_THREADS="1"))
+    assert p.returncode == 0, p.stdout[-2000:] + p.stderr[-3000:]
+    assert p.stdout.count("ok") == 2
