@@ -193,6 +193,20 @@ enum { RT_K_FACECOEF = 0, RT_K_TRANSPORT = 1, RT_K_ANGULAR = 2, RT_K_SOURCE = 3,
 int rt_profile_enable(rt_ctx *ctx, int on);
 int rt_profile_read(rt_ctx *ctx, double *ms_host, long long *count_host);
 
+/* One step of a rank's slab in a multi-GPU decomposition along x3, the planes its neighbours need FIRST (L778: "treating the boundaries
+ * first and overlapping the transfer with the interior").  `ctx` is the rank's EXTENDED slab: RT_SLAB_MARGIN = 4 planes of halo on every
+ * cut side (the domain of dependence of one predictor-corrector step), OUTFLOW there.  On `halo_stream` the library steps, per cut
+ * side, a sub-slab of 3 x RT_SLAB_MARGIN planes with a context of its own and leaves in the caller's DEVICE send buffers the
+ * RT_SLAB_MARGIN owned planes next to the cut as they will be after this step, bit for bit: send_lo_I [4][ncol][pitch], send_lo_T
+ * [4][ncol] = planes 4..7 of the slab (NULL, both: no cut below), send_hi_* = planes n3-8 .. n3-5 (NULL: no cut above).  On `stream` the
+ * whole slab is stepped exactly as by rt_step (I, T in place; R, G, n_fail as there).  The caller sends / receives on `halo_stream`
+ * (ordered after the library's work there) while `stream` computes, and copies what it received into the halo planes (planes 0..3 and
+ * n3-4 .. n3-1: contiguous) once `stream` has finished the step.  Costs 3 x RT_SLAB_MARGIN extra planes of compute per cut side; not
+ * available with RT_BC_FIXED boundaries (RT_EINVAL).  With all four buffers NULL it is rt_step. */
+#define RT_SLAB_MARGIN 4
+int rt_step_slab(rt_ctx *ctx, double *I_inout_dev, double *T_inout_dev, double *R_out_dev, double *G_out_dev, double dt, int *n_fail_dev,
+                 double *send_lo_I_dev, double *send_lo_T_dev, double *send_hi_I_dev, double *send_hi_T_dev, void *stream, void *halo_stream);
+
 /* Which spatial transport path rt_init selected, to HOST: out[0] = RT_TRANSPORT_* actually used (RT_TRANSPORT_L2 when the
  * tile kernel's conditions do not hold), out[1..3] = the tile in the order of rt_options.transport_tile. */
 int rt_transport_info(const rt_ctx *ctx, int out_host[4]);

@@ -34,6 +34,8 @@ struct rt_ctx {
     // rt_step_host pipeline (x3 slabs with a 4-plane halo, each its own context over the same metric): built on first use
     struct HostSlab { rt_ctx *sub; int k0, k1, ext_lo, ext_hi, n3l; double *I, *T, *R, *G, *rho, *u4; cudaEvent_t done; };
     std::vector<HostSlab> hslabs;
+    HostSlab bslab[2];                 // rt_step_slab: the boundary sub-slabs (3 margins of planes) at the low / high x3 end
+    cudaEvent_t bev_in, bev_cloned; long long bslab_fluid_version; int *d_bfail;
     cudaStream_t hs_in, hs_cmp, hs_out;
     std::vector<cudaEvent_t> hev;      // one event per uploaded chunk
     cudaEvent_t hev_start, hev_end[3];
@@ -279,6 +281,7 @@ extern "C" int rt_init(const rt_grid *grid, const rt_metric *metric, int angle_l
     c->d_fcoef[0] = c->d_fcoef[1] = c->d_fcoef[2] = nullptr;
     c->u4_rest = false; c->d_colflag = nullptr; c->d_cls = nullptr; c->d_paircoef = nullptr; c->d_paircoefz = nullptr; c->d_genlist = nullptr; c->d_srclist = nullptr; c->d_nsel = nullptr; c->d_part_tmp = nullptr; c->part_tmp_bytes = 0;
     c->d_hI = c->d_hT = c->d_hR = c->d_hG = nullptr; c->d_hfail = nullptr;
+    std::memset(c->bslab, 0, sizeof c->bslab); c->bev_in = c->bev_cloned = nullptr; c->bslab_fluid_version = -1; c->d_bfail = nullptr;
     c->d_mapr_xi = c->d_mapr_xim = c->d_mapr_a = c->d_angraw = nullptr; c->d_mapr_back = c->d_mapr_nnb = nullptr; c->d_angup = nullptr;
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_cls, (size_t)ncol * pitch);
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_colflag, colflag_bytes(c->ncol, n3));   // column flags, x3-chunk flags, cell-flag masks
@@ -380,6 +383,13 @@ extern "C" int rt_free(rt_ctx *c) {
         cudaFree(h.I); cudaFree(h.T); cudaFree(h.R); cudaFree(h.G); cudaFree(h.rho); cudaFree(h.u4);
         if (h.done) cudaEventDestroy(h.done);
     }
+    for (auto &h : c->bslab) {
+        if (h.sub) rt_free(h.sub);
+        cudaFree(h.I); cudaFree(h.T); cudaFree(h.rho); cudaFree(h.u4);
+    }
+    if (c->bev_in) cudaEventDestroy(c->bev_in);
+    if (c->bev_cloned) cudaEventDestroy(c->bev_cloned);
+    cudaFree(c->d_bfail);
     for (auto e : c->hev) cudaEventDestroy(e);
     if (c->hev_start) cudaEventDestroy(c->hev_start);
     for (int q = 0; q < 3; ++q) if (c->hev_end[q]) cudaEventDestroy(c->hev_end[q]);
@@ -659,6 +669,89 @@ extern "C" int rt_step(rt_ctx *c, double *I, double *T, double *R_out, double *G
     int rc = stage(c, I, T, I, c->d_Ih, c->d_Th, 0.5 * dt, n_fail, nullptr, nullptr, st);     // predictor
     if (rc != RT_OK) return rc;
     return stage(c, c->d_Ih, c->d_Th, I, I, T, dt, n_fail, R_out, G_out, st);               // corrector
+}
+
+// ---- rt_step_slab: one step of a rank's slab with the planes its neighbours need stepped first ---------------------------------------
+// PAPER.md L778 lists "treating the boundaries first and overlapping the transfer with the interior" as missing from cuHARM's radiation
+// module.  This context is a rank's EXTENDED slab of an x3 decomposition (RT_SLAB_MARGIN planes of halo on every cut side, OUTFLOW
+// there).  On halo_stream a sub-slab of 3 margins of planes at each cut end (halo, the planes to send, as many again: the domain of
+// dependence of one step) is copied out and stepped by a context of its own, and its middle planes -- the owned planes next to the
+// cut as they will be after this step, bit for bit -- land in the caller's send buffers; on `stream` the whole slab is stepped as by
+// rt_step.  The caller sends / receives on halo_stream meanwhile and copies what it received into the halo planes once `stream` is done.
+static int bslab_build(rt_ctx *c, int side) {
+    rt_ctx::HostSlab &h = c->bslab[side];
+    const rt_grid &G = c->grid;
+    const int n3l = 3 * RT_SLAB_MARGIN;
+    std::memset(&h, 0, sizeof h);
+    h.n3l = n3l;
+    h.k0 = side == 0 ? 0 : G.n[2] - n3l;     // first plane of the sub-slab in this context
+    rt_grid g = G;
+    g.n[2] = n3l;
+    g.x0[2] = G.x0[2] + h.k0 * G.dx[2];
+    g.bc_lo[2] = g.bc_hi[2] = RT_BC_OUTFLOW;
+    g.zero_lo[2] = g.zero_hi[2] = 0;
+    int rc = rt_init(&g, &c->metric, c->level, &c->opt, &h.sub);
+    if (rc != RT_OK) return rc;
+    h.sub->is_sub = true;
+    const size_t pc = (size_t)c->ncol, pi = pc * c->pitch;
+    cudaError_t e = cudaMalloc((void **)&h.I, n3l * pi * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&h.T, n3l * pc * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&h.rho, n3l * pc * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&h.u4, 4 * n3l * pc * sizeof(double));
+    if (e != cudaSuccess) { g_last_cuda = (int)e; return e == cudaErrorMemoryAllocation ? RT_ENOMEM : RT_ECUDA; }
+    return RT_OK;
+}
+
+extern "C" int rt_step_slab(rt_ctx *c, double *I, double *T, double *R_out, double *G_out, double dt, int *n_fail,
+                            double *send_lo_I, double *send_lo_T, double *send_hi_I, double *send_hi_T, void *stream, void *halo_stream) {
+    if (!c || !I || !T || (!send_lo_I != !send_lo_T) || (!send_hi_I != !send_hi_T)) return RT_EINVAL;
+    if (!c->fluid_set || fixed_bc_missing(c)) return RT_ESTATE;
+    const int M = RT_SLAB_MARGIN, n3 = c->grid.n[2];
+    const bool lo = send_lo_I != nullptr, hi = send_hi_I != nullptr;
+    if ((lo || hi) && n3 < 3 * M) return RT_EINVAL;                       // the sub-slab must fit
+    for (int a = 0; a < 3; ++a)                                           // caller-supplied ghost data is not cut into the sub-slabs
+        if ((lo || hi) && (c->grid.bc_lo[a] == RT_BC_FIXED || c->grid.bc_hi[a] == RT_BC_FIXED)) return RT_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream, hs = (cudaStream_t)halo_stream;
+    const size_t pc = (size_t)c->ncol, pi = pc * c->pitch;
+    if (lo || hi) {
+        if (!c->bev_in) {
+            CK(cudaEventCreateWithFlags(&c->bev_in, cudaEventDisableTiming));
+            CK(cudaEventCreateWithFlags(&c->bev_cloned, cudaEventDisableTiming));
+            CK(cudaMalloc((void **)&c->d_bfail, sizeof(int)));
+        }
+        for (int side = 0; side < 2; ++side)
+            if ((side == 0 ? lo : hi) && !c->bslab[side].sub) { int rc = bslab_build(c, side); if (rc != RT_OK) return rc; }
+        CK(cudaEventRecord(c->bev_in, st));                                // I, T and the fluid state are current on `stream`
+        CK(cudaStreamWaitEvent(hs, c->bev_in, 0));
+        const bool refluid = c->bslab_fluid_version != c->fluid_version;
+        for (int side = 0; side < 2; ++side) {
+            if (!(side == 0 ? lo : hi)) continue;
+            rt_ctx::HostSlab &h = c->bslab[side];
+            CK(cudaMemcpyAsync(h.I, I + (size_t)h.k0 * pi, h.n3l * pi * sizeof(double), cudaMemcpyDeviceToDevice, hs));
+            CK(cudaMemcpyAsync(h.T, T + (size_t)h.k0 * pc, h.n3l * pc * sizeof(double), cudaMemcpyDeviceToDevice, hs));
+            if (refluid || !h.sub->fluid_set) {
+                CK(cudaMemcpyAsync(h.rho, c->d_rho + (size_t)h.k0 * pc, h.n3l * pc * sizeof(double), cudaMemcpyDeviceToDevice, hs));
+                for (int m = 0; m < 4; ++m)
+                    CK(cudaMemcpyAsync(h.u4 + (size_t)m * h.n3l * pc, c->d_u4 + (size_t)m * c->ncell + (size_t)h.k0 * pc, h.n3l * pc * sizeof(double),
+                                       cudaMemcpyDeviceToDevice, hs));
+                int rc = rt_set_fluid(h.sub, h.rho, h.T, h.u4, hs);
+                if (rc != RT_OK) return rc;
+            }
+        }
+        c->bslab_fluid_version = c->fluid_version;
+        CK(cudaEventRecord(c->bev_cloned, hs));
+        for (int side = 0; side < 2; ++side) {
+            if (!(side == 0 ? lo : hi)) continue;
+            rt_ctx::HostSlab &h = c->bslab[side];
+            int rc = rt_step(h.sub, h.I, h.T, nullptr, nullptr, dt, c->d_bfail, hs);
+            if (rc != RT_OK) return rc;
+            double *sI = side == 0 ? send_lo_I : send_hi_I, *sT = side == 0 ? send_lo_T : send_hi_T;
+            CK(cudaMemcpyAsync(sI, h.I + (size_t)M * pi, M * pi * sizeof(double), cudaMemcpyDeviceToDevice, hs));
+            CK(cudaMemcpyAsync(sT, h.T + (size_t)M * pc, M * pc * sizeof(double), cudaMemcpyDeviceToDevice, hs));
+        }
+        CK(cudaStreamWaitEvent(st, c->bev_cloned, 0));                     // the whole-slab step must not overwrite what is being copied out
+    }
+    return rt_step(c, I, T, R_out, G_out, dt, n_fail, stream);
 }
 
 // H2D -> rt_step -> D2H back to back on one stream (meshes too thin to cut, FIXED boundaries)

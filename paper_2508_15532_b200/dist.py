@@ -187,91 +187,65 @@ class SlabDomain:
         self.exchange_halo()
 
     # ---- boundary first: "treating the boundaries first and overlapping the transfer with the interior" -----------
-    # The planes a neighbour needs are final only after the corrector, so they can leave early only if they are stepped first: on
-    # each cut side a sub-slab of 3 MARGIN planes (the margin, the MARGIN owned planes to send and MARGIN more: the domain of
-    # dependence of one step) is stepped by a context of its own on a side stream, its middle planes are sent, and the transfer
-    # runs while the main stream steps the whole slab; the received planes land in buffers and are copied into the margins at the
-    # end.  The price is 2 x 3 MARGIN extra planes of compute per step for a transfer that takes 1-2 % of a step on NVLink
-    # (DESIGN.md section 8): an option for slow interconnects, not the default.  Same kernels, same values: the planes sent are
-    # bit-identical to those the whole-slab step produces.
+    # The planes a neighbour needs are final only after the corrector, so they can leave early only if they are stepped first.  The
+    # library does that below the ABI (rt_step_slab, include/rt.h): on each cut side a sub-slab of 3 MARGIN planes is stepped by a
+    # context of its own on a side stream, its middle planes land in send buffers, and the transfer runs while the main stream steps
+    # the whole slab; what is received lands in buffers and is copied into the margins at the end.  The price is 2 x 3 MARGIN extra
+    # planes of compute per step for a transfer that takes 1-2 % of a step on NVLink: an option for slow
+    # interconnects, not the default.  Same kernels, same values: the planes sent are bit-identical to the whole-slab step's.
     def enable_overlap(self):
-        """Build the boundary sub-slab contexts.  Returns False (and leaves the plain path in place) where the scheme does not apply:
-        a single rank, fewer than 2 MARGIN owned planes, caller-supplied ghost data."""
-        from . import rt
+        """Allocate the send buffers.  Returns False (the plain path stays) where the scheme does not apply: a single rank, fewer
+        than 2 MARGIN owned planes, caller-supplied ghost data (FIXED boundaries)."""
+        import torch
         L = self.layout
-        if L.world == 1 or (L.k1 - L.k0) < 2 * L.margin or self._has_ghosts or self._rho_d is None:
+        fixed = "fixed" in tuple(self.grid["bc_lo"]) + tuple(self.grid["bc_hi"])
+        if L.world == 1 or (L.k1 - L.k0) < 2 * L.margin or fixed or self.I is None:
             return False
-        kind, params = self.cfg["metric"]
-        m = L.margin
-        for side, cut, sl in (("lo", L.lo_cut, slice(0, 3 * m)), ("hi", L.hi_cut, slice(L.n3_local - 3 * m, L.n3_local))):
-            if not cut:
-                continue
-            g = dict(self.grid)
-            n = list(g["n"]); n[2] = 3 * m; g["n"] = tuple(n)
-            x0 = list(g["x0"]); x0[2] = self.grid["x0"][2] + sl.start * self.grid["dx"][2]; g["x0"] = tuple(x0)
-            bl, bh = list(g["bc_lo"]), list(g["bc_hi"]); bl[2] = bh[2] = "outflow"; g["bc_lo"], g["bc_hi"] = tuple(bl), tuple(bh)
-            zl, zh = list(g.get("zero_lo", (0, 0, 0))), list(g.get("zero_hi", (0, 0, 0))); zl[2] = zh[2] = 0
-            g["zero_lo"], g["zero_hi"] = tuple(zl), tuple(zh)
-            ctx = rt.RtContext(g, kind, params, self.cfg["level"], self.cfg["options"], device=str(self.device))
-            ctx.set_fluid(self._rho_d[sl].contiguous(), self._T0_d[sl].contiguous(), None if self._u4_d is None else self._u4_d[:, sl].contiguous())
-            self._sub[side] = (ctx, sl)
-        return bool(self._sub)
+        mk = lambda t: torch.empty((L.margin,) + tuple(t.shape[1:]), dtype=t.dtype, device=t.device)
+        self._sub = {"lo": (mk(self.I), mk(self.T)) if L.lo_cut else None, "hi": (mk(self.I), mk(self.T)) if L.hi_cut else None}
+        return True
 
-    def boundary_first(self, dt):
-        """Step the cut-side sub-slabs (on the current stream) and return {side: (I planes, T planes)}: the MARGIN owned planes next to
-        each cut as they will be after this step."""
-        m, out = self.layout.margin, {}
-        for side, (ctx, sl) in self._sub.items():
-            Is, Ts = self.I[sl].clone(), self.T[sl].clone()
-            ctx.step(Is, Ts, dt, None, None)
-            out[side] = (Is[m:2 * m], Ts[m:2 * m])
-        return out
+    def boundary_first(self, dt, moments=True):
+        """rt_step_slab on the current stream and a side stream; returns the send buffers {side: (I planes, T planes)} (the MARGIN owned
+        planes next to each cut after this step).  The whole-slab step has been issued on the current stream when this returns."""
+        import torch
+        if self._side is None:
+            self._side = torch.cuda.Stream(device=self.device)
+        self.ctx.step_slab(self.I, self.T, dt, self.R if moments else None, self.G if moments else None, self._sub["lo"], self._sub["hi"], self._side)
+        return {k: v for k, v in self._sub.items() if v is not None}
 
     def step_overlapped(self, dt, moments=True):
         import torch
         import torch.distributed as dist
         L = self.layout
         main = torch.cuda.current_stream(self.device)
-        if self._side is None:
-            self._side = torch.cuda.Stream(device=self.device)
-        side = self._side
-        side.wait_stream(main)
-        cloned = torch.cuda.Event()
+        bufs = self.boundary_first(dt, moments)      # boundary sub-slabs on the side stream, the whole slab on the main stream
         landed = []
-        with torch.cuda.stream(side):
-            m = L.margin
-            subs = {}
-            for sd, (ctx, sl) in self._sub.items():
-                subs[sd] = (self.I[sl].clone(), self.T[sl].clone())
-            cloned.record(side)
-            for sd, (ctx, sl) in self._sub.items():
-                ctx.step(subs[sd][0], subs[sd][1], dt, None, None)
-            # the transfer, from / into buffers (the margins are still being read by the whole-slab step)
+        with torch.cuda.stream(self._side):          # the transfer: ordered after the boundary work, concurrent with the main stream
             stage = dist.get_backend(self.group) == "gloo"
             ops = []
             def send(t, peer):
-                ops.append(dist.P2POp(dist.isend, t.cpu() if stage else t.contiguous(), peer, self.group))
-            def recv(like, dst_sl, tensor, peer):
+                ops.append(dist.P2POp(dist.isend, t.cpu() if stage else t, peer, self.group))
+            def recv(tensor, dst_sl, peer):
+                like = tensor[dst_sl]
                 buf = torch.empty(like.shape, dtype=like.dtype, device="cpu" if stage else like.device)
                 landed.append((tensor, dst_sl, buf))
                 ops.append(dist.P2POp(dist.irecv, buf, peer, self.group))
-            for which in (0, 1):                                  # I, then T: the order of exchange()
+            for which in (0, 1):                     # I, then T: the order of exchange()
                 tensor = self.I if which == 0 else self.T
                 if L.lo_cut:
-                    send(subs["lo"][which][m:2 * m], L.left)
+                    send(bufs["lo"][which], L.left)
                 if L.hi_cut:
-                    send(subs["hi"][which][m:2 * m], L.right)
+                    send(bufs["hi"][which], L.right)
                 if L.hi_cut:
-                    recv(tensor[L.recv_hi()], L.recv_hi(), tensor, L.right)
+                    recv(tensor, L.recv_hi(), L.right)
                 if L.lo_cut:
-                    recv(tensor[L.recv_lo()], L.recv_lo(), tensor, L.left)
+                    recv(tensor, L.recv_lo(), L.left)
             reqs = dist.batch_isend_irecv(ops)
-        main.wait_event(cloned)
-        self.ctx.step(self.I, self.T, dt, self.R if moments else None, self.G if moments else None)   # the whole slab, meanwhile
         for r in reqs:
             r.wait()
-        main.wait_stream(side)
-        for tensor, sl, buf in landed:
+        main.wait_stream(self._side)
+        for tensor, sl, buf in landed:               # (on the main stream: after the whole-slab step)
             tensor[sl].copy_(buf)
 
     def owned(self, t, lead=0):

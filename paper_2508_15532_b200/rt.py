@@ -17,7 +17,7 @@ METRIC = {"minkowski": 0, "mink_cyl": 1, "ks_mks": 2, "snake": 3, "bl_mks": 4, "
 GEOM = dict(g_c=0, e_c=1, einv_c=2, sqrtg_c=3, omega_c=4, n0_c=5, angcoef=6)
 SYMBOLS = ["rt_init", "rt_free", "rt_ndir", "rt_ndir_padded", "rt_get_directions", "rt_get_geometry", "rt_cfl_dt",
            "rt_set_boundary", "rt_set_fluid", "rt_transport", "rt_transport_static", "rt_angular_flux", "rt_source_implicit", "rt_moments",
-           "rt_step", "rt_step_host", "rt_profile_enable", "rt_profile_read", "rt_transport_info", "rt_launch_count", "rt_last_cuda_error", "rt_strerror"]
+           "rt_step", "rt_step_host", "rt_step_slab", "rt_profile_enable", "rt_profile_read", "rt_transport_info", "rt_launch_count", "rt_last_cuda_error", "rt_strerror"]
 
 
 class RtGrid(ctypes.Structure):
@@ -76,6 +76,7 @@ def load_library(path=LIB_PATH):
     lib.rt_moments.argtypes = [vp, vp, vp, vp]
     lib.rt_step.argtypes = [vp, vp, vp, vp, vp, dbl, vp, vp]
     lib.rt_step_host.argtypes = [vp, vp, vp, vp, vp, dbl, vp, vp]
+    lib.rt_step_slab.argtypes = [vp, vp, vp, vp, vp, dbl, vp, vp, vp, vp, vp, vp, vp]
     lib.rt_profile_enable.argtypes = [vp, ci]
     lib.rt_profile_read.argtypes = [vp, vp, vp]
     lib.rt_transport_info.argtypes = [vp, vp]
@@ -224,6 +225,14 @@ class RtContext:
 
     def step(self, I, T, dt, R=None, G=None):
         _check(lib().rt_step(self._h, _ptr(I), _ptr(T), _ptr(R), _ptr(G), float(dt), _ptr(self._nfail), _stream()))
+
+    def step_slab(self, I, T, dt, R, G, send_lo, send_hi, halo_stream):
+        """rt_step_slab: send_lo / send_hi = (I planes [4, N2, N1, pitch], T planes [4, N2, N1]) device tensors or None; the boundary
+        work runs on `halo_stream` (a torch.cuda.Stream), the whole-slab step on the current stream."""
+        sl = (None, None) if send_lo is None else send_lo
+        sh = (None, None) if send_hi is None else send_hi
+        _check(lib().rt_step_slab(self._h, _ptr(I), _ptr(T), _ptr(R), _ptr(G), float(dt), _ptr(self._nfail), _ptr(sl[0]), _ptr(sl[1]),
+                                  _ptr(sh[0]), _ptr(sh[1]), _stream(), ctypes.c_void_p(halo_stream.cuda_stream)))
 
     def step_host(self, I_host, T_host, dt, R_host=None, G_host=None):
         """rt_step_host: HOST tensors (pinned fp64, padded layout); returns the failed-cell count of this call."""

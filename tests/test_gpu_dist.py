@@ -165,17 +165,23 @@ def test_boundary_first_planes_equal_the_whole_slab_step(idx, n, world):
         d.set_fields(f)
         assert d.enable_overlap()
     m = doms[0].layout.margin
+    ref = [SlabDomain(cfg, r, world) for r in range(world)]          # the plain path beside it
+    for d in ref:
+        d.set_fields(f)
     for _ in range(3):
-        ahead = [d.boundary_first(dt) for d in doms]
-        for d in doms:
+        ahead = [d.boundary_first(dt) for d in doms]                  # rt_step_slab: send buffers + the whole-slab step
+        for d in ref:
             d.ctx.step(d.I, d.T, dt, d.R, d.G)
-        for d, a in zip(doms, ahead):
+        torch.cuda.synchronize()
+        for d, r, a in zip(doms, ref, ahead):
             L = d.layout
             assert set(a) == ({"lo"} if L.lo_cut else set()) | ({"hi"} if L.hi_cut else set())
             for side, (Ia, Ta) in a.items():
                 sl = L.send_lo() if side == "lo" else L.send_hi()
                 assert torch.equal(Ia, d.I[sl]) and torch.equal(Ta, d.T[sl]), (L.rank, side)
-        exchange_local(doms)
+            for name in ("I", "T", "R", "G"):                         # and the slab itself is stepped as by rt_step
+                assert torch.equal(getattr(d, name), getattr(r, name)), name
+        exchange_local(doms); exchange_local(ref)
     assert not SlabDomain(cfg, 0, 1).enable_overlap()          # nothing to overlap on one rank
 
 
