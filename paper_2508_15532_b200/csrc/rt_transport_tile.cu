@@ -79,6 +79,13 @@ __device__ __forceinline__ double lds(uint32_t addr) {
     return v;
 }
 
+__device__ __forceinline__ double4 lds4(uint32_t addr) {
+    double4 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+16];" : "=d"(v.z), "=d"(v.w) : "r"(addr));
+    return v;
+}
+
 // x3-plane p (may be out of range by the stencil reach) -> source plane under a PERIODIC / OUTFLOW boundary
 __device__ __forceinline__ int plane_src(int pl, int n3, int bc_lo, int bc_hi) { return nb_index(pl, n3, bc_lo, bc_hi); }
 
@@ -98,6 +105,7 @@ struct TileParams {
     int slotB, bslotB;
     int off_ring, off_base;
     int slotStride, bslotStride, zeroOff, bzeroOff;   // run-time ring geometry (k_transport_tile_gen; the vacuum kernel's is compile-time)
+    int oCx, oCy, oCz, coefB;                          // k_transport_tile_gen: per-face coefficient blocks of a slot (x1 faces, x2 faces, x3 faces), their bytes
     int split;   // opacities present: tiles without an all-vacuum cell are skipped (see the kernel)
 };
 
@@ -449,16 +457,20 @@ k_transport_tile(const __grid_constant__ KParams p, const __grid_constant__ Tile
 // dims, both PLI states at the six faces, Eq 20 or Eq 23 per face from the per-face coefficients of k_facecoef -- the
 // arithmetic of k_transport_gen (rt_transport.cu) with the thirteen operands taken from the ring instead of thirteen global
 // loads, except that the x3 face flux and slope a step has formed are carried to the next step instead of being formed again
-// (the results agree with k_transport_gen's to rounding).  One pair per thread (the Eq 23 path holds ten face coefficients and a five-deep x3 window);
+// (the results agree with k_transport_gen's to rounding).  The per-face coefficients of k_facecoef (five double4 per cell and step,
+// the same for all directions of a cell) ride in the ring as well: three more TMA boxes per plane ([4 x (TX+1) x TY] x1 faces,
+// [4 x TX x (TY+1)] x2 faces, [4 x TX x TY] x3 faces k+1/2) on the slot's barrier, read by the consumers as shared-memory
+// broadcasts.  Through global memory (L1, prefetched a step ahead, 71-79 % hits) they were the kernel's long-scoreboard stalls:
+// 27 % of its time on the all-matter configs.  One pair per thread (the Eq 23 path holds ten face coefficients and a five-deep x3 window);
 // tiles without such a cell leave at once; steps whose cell is all-vacuum only shift the window.
 constexpr int NTG = 480;     // consumer threads of k_transport_tile_gen (+ one producer warp)
 template <bool SAME_BASE>
 __global__ void __launch_bounds__(NTG + 32, 1)
 k_transport_tile_gen(const __grid_constant__ KParams p, const __grid_constant__ TileParams tp,
                      const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapH,
-                     const __grid_constant__ CUtensorMap mapG, const __grid_constant__ CUtensorMap mapD, double *I_out,
-                     const double4 *__restrict__ fc0, const double4 *__restrict__ fc1, const double4 *__restrict__ fc2,
-                     const unsigned char *__restrict__ colflag, double dt) {
+                     const __grid_constant__ CUtensorMap mapG, const __grid_constant__ CUtensorMap mapD,
+                     const __grid_constant__ CUtensorMap mapCx, const __grid_constant__ CUtensorMap mapCy, const __grid_constant__ CUtensorMap mapCz,
+                     double *I_out, const double4 *__restrict__ fc2, const unsigned char *__restrict__ colflag, double dt) {
     constexpr int RP = 1;
     extern __shared__ __align__(1024) unsigned char smem[];
     const uint32_t sbase = smem_u32(smem);
@@ -496,7 +508,14 @@ k_transport_tile_gen(const __grid_constant__ KParams p, const __grid_constant__ 
         if (m >= NS) mbar_wait(bar_empty + 8 * slot, ((m / NS) & 1) ^ 1);
         const int ks = plane_src(m - 2, n3, p.bc_lo[2], p.bc_hi[2]);
         const uint32_t dst = ring + slot * tp.slotStride, bar = bar_full + 8 * slot;
-        mbar_expect_tx(bar, bytes);
+        const int kp = m - 2;                               // the plane itself (coefficients exist for 0 <= kp < n3 only)
+        const bool coef = kp >= 0 && kp < n3;
+        mbar_expect_tx(bar, bytes + (coef ? (uint32_t)tp.coefB : 0u));
+        if (coef) {
+            tma_box(dst + tp.oCx, &mapCx, bar, 0, i0, j0, kp);
+            tma_box(dst + tp.oCy, &mapCy, bar, 0, i0, j0, kp);
+            tma_box(dst + tp.oCz, &mapCz, bar, 0, i0, j0, kp + 1);
+        }
         tma_box(dst, &mapA, bar, s0, i0 - 2, j0, ks);
         if (hlo) tma_box(dst + tp.oHlo, &mapH, bar, s0, i0, j0 - 2, ks);
         if (hhi) tma_box(dst + tp.oHhi, &mapH, bar, s0, i0, j0 + tp.TY, ks);
@@ -598,9 +617,12 @@ k_transport_tile_gen(const __grid_constant__ KParams p, const __grid_constant__ 
     }
     const long long kstride = (long long)p.ncol * p.pitch;
     const int zlo = p.zlo[2], zhi = n3 - p.zhi[2], ncol = p.ncol, n1 = p.n1;
-    const int sxf = p.n2 * (n1 + 1), syf = (p.n2 + 1) * n1;
-    const double4 *px = fc0 + ((long long)j * (n1 + 1) + i), *py = fc1 + ((long long)j * n1 + i), *pz = fc2 + col;
-    if (!pvalid) { px = fc0; py = fc1; pz = fc2; }
+    const double4 *pz = fc2 + col;       // (only for the x3 low face at the start of a run of Eq 23 cells)
+    if (!pvalid) pz = fc2;
+    // this pair's per-face coefficients inside a slot
+    const uint32_t cxl = ring + (uint32_t)(tp.oCx + (lj * (tp.TX + 1) + c) * 32), cyl = ring + (uint32_t)(tp.oCy + (lj * tp.TX + c) * 32);
+    const uint32_t cyh = cyl + (uint32_t)tp.TX * 32u, czh = ring + (uint32_t)(tp.oCz + (lj * tp.TX + c) * 32);
+    (void)n1;
 
     // prologue: planes -2 .. 1 (ring sequence m = 0 .. 3) -> the x3 window
     double w0, w1, w2, w3;
@@ -633,14 +655,10 @@ k_transport_tile_gen(const __grid_constant__ KParams p, const __grid_constant__ 
         }
         const double w4 = lds(a_own + so);
         const bool mat = (mcur >> (k & 31)) & 1u;
-        const bool matn = ((k & 31) == 31 ? mnext : (mcur >> ((k & 31) + 1))) & 1u;
-        if (matn && k + 1 < n3) {   // the per-face coefficients of the next step: towards L1 now (no registers held)
-            pf_l1(px + sxf); pf_l1(py + syf); pf_l1(py + syf + n1); pf_l1(pz + 2 * ncol);
-        }
         // x3: the slope of cell k + 1 is formed every step and carried (it is the next step's own slope)
         const double dz3 = w4 - w3, spz = slope_mc(dz2, dz3);
         if (mat) {
-            const double4 fzh = ld4(pz + ncol), fxl = ld4(px), fxh = ld4(px + 1), fyl = ld4(py), fyh = ld4(py + n1);
+            const double4 fzh = lds4(czh + sk), fxl = lds4(cxl + sk), fxh = lds4(cxl + sk + 32u), fyl = lds4(cyl + sk), fyh = lds4(cyh + sk);
             const double xm2 = lds(a_x[0] + sk), xm1 = lds(a_x[1] + sk), xp1 = lds(a_x[2] + sk), xp2 = lds(a_x[3] + sk);
             const double ym2 = lds(a_y[0] + sk), ym1 = lds(a_y[1] + sk), yp1 = lds(a_y[2] + sk), yp2 = lds(a_y[3] + sk);
             const double cbase = SAME_BASE ? w2 : lds(a_base + sb);
@@ -663,7 +681,7 @@ k_transport_tile_gen(const __grid_constant__ KParams p, const __grid_constant__ 
             if (!SAME_BASE) ready = mbar_test(bar_fullB + 8 * u1, par1) && ready;
         }
         w0 = w1; w1 = w2; w2 = w3; w3 = w4; dz2 = dz3; s0z = spz;
-        outk += kstride; px += sxf; py += syf; pz += ncol;
+        outk += kstride; pz += ncol;
         __syncwarp();
         if (lane == 0) {
             mbar_arrive(bar_empty + 8 * uk);
@@ -705,6 +723,17 @@ bool make_map(CUtensorMap *m, const double *I, const KParams &p, int dch, int w,
               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// per-face coefficients fc[e3][e2][e1] of double4 as a rank-4 fp64 tensor (4 innermost), box = [4 x w faces x h rows x 1 plane]
+bool make_map_fc(CUtensorMap *m, const double4 *fc, int e1, int e2, int e3, int w, int h) {
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return false;
+    const cuuint64_t dims[4] = {4, (cuuint64_t)e1, (cuuint64_t)e2, (cuuint64_t)e3};
+    const cuuint64_t strides[3] = {32, (cuuint64_t)e1 * 32, (cuuint64_t)e1 * e2 * 32};
+    const cuuint32_t box[4] = {4, (cuuint32_t)w, (cuuint32_t)h, 1}, es[4] = {1, 1, 1, 1};
+    return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double4 *>(fc), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 int align_up(int v, int a) { return (v + a - 1) / a * a; }
 
 // shared-memory layout of a tile (see the kernel) for a kernel with rp pairs per thread; returns the dynamic shared memory it needs
@@ -727,12 +756,18 @@ size_t tile_layout(const KParams &p, const int tile[3], bool same, TileParams &t
     t.off_base = t.off_ring + NS * SLOT_STRIDE;
     return (size_t)t.off_base + (same ? 0 : NS * BSLOT_STRIDE);
 }
-// the same for k_transport_tile_gen: its own, smaller ring (strides fitted to the tile), so that most of the SM's shared
-// memory stays L1 cache for the per-face coefficient loads
+// the same for k_transport_tile_gen: its own ring with run-time strides fitted to its tile (one pair per thread: a smaller tile
+// than the vacuum kernel's), each slot followed by the per-face coefficient blocks of its plane
 size_t tile_layout_gen(const KParams &p, const int tile[3], bool same, TileParams &t) {
     tile_layout(p, tile, same, t);
     t.zeroOff = t.slotB;
-    t.slotStride = align_up(t.slotB + 8, 1024);
+    // the per-face coefficients of Eq 23 ride in the same slot as the plane they belong to: [TY][TX+1] x1 faces, [TY+1][TX] x2 faces
+    // of plane k and [TY][TX] x3 faces k+1/2, one double4 each, as three more TMA boxes on the slot's barrier
+    t.oCx = align_up(t.slotB + 8, 128);
+    t.oCy = t.oCx + align_up(t.TY * (t.TX + 1) * 32, 128);
+    t.oCz = t.oCy + align_up((t.TY + 1) * t.TX * 32, 128);
+    t.coefB = (t.TY * (t.TX + 1) + (t.TY + 1) * t.TX + t.TY * t.TX) * 32;
+    t.slotStride = align_up(t.oCz + t.TY * t.TX * 32, 1024);
     t.bzeroOff = t.bslotB;
     t.bslotStride = align_up(t.bslotB + 8, 128);
     t.off_base = t.off_ring + NS * t.slotStride;
@@ -824,20 +859,21 @@ cudaError_t launch_transport_tile_gen(const KParams &p, const double *I_in, cons
     const size_t smem = tile_layout_gen(p, p.tile_gen, same, t);
     if (smem > SMEM_MAX || t.TX * t.TY * t.DCH > NTG || (t.DCH & 1) || t.TX < 2 || t.TX + 4 > 256 || t.DCH > 256)
         return cudaErrorInvalidConfiguration;
-    CUtensorMap mA, mH, mG, mD;
-    if (!make_map(&mA, I_in, p, t.DCH, t.TX + 4, t.TY) || !make_map(&mH, I_in, p, t.DCH, t.TX, 2) || !make_map(&mG, I_in, p, t.DCH, 2, t.TY) ||
-        !make_map(&mD, I_base, p, t.DCH, t.TX, t.TY))
-        return cudaErrorInvalidValue;
+    CUtensorMap mA, mH, mG, mD, mCx, mCy, mCz;
     const double4 *f0 = reinterpret_cast<const double4 *>(fcoef[0]), *f1 = reinterpret_cast<const double4 *>(fcoef[1]),
                   *f2 = reinterpret_cast<const double4 *>(fcoef[2]);
+    if (!make_map(&mA, I_in, p, t.DCH, t.TX + 4, t.TY) || !make_map(&mH, I_in, p, t.DCH, t.TX, 2) || !make_map(&mG, I_in, p, t.DCH, 2, t.TY) ||
+        !make_map(&mD, I_base, p, t.DCH, t.TX, t.TY) || !make_map_fc(&mCx, f0, p.n1 + 1, p.n2, p.n3, t.TX + 1, t.TY) ||
+        !make_map_fc(&mCy, f1, p.n1, p.n2 + 1, p.n3, t.TX, t.TY + 1) || !make_map_fc(&mCz, f2, p.n1, p.n2, p.n3 + 1, t.TX, t.TY))
+        return cudaErrorInvalidValue;
     const unsigned grid = (unsigned)(t.ntx * t.nty * t.nch);
     cudaError_t e;
     if (same) {
         e = cudaFuncSetAttribute(k_transport_tile_gen<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) k_transport_tile_gen<true><<<grid, NTG + 32, smem, st>>>(p, t, mA, mH, mG, mD, I_out, f0, f1, f2, colflag, dt);
+        if (e == cudaSuccess) k_transport_tile_gen<true><<<grid, NTG + 32, smem, st>>>(p, t, mA, mH, mG, mD, mCx, mCy, mCz, I_out, f2, colflag, dt);
     } else {
         e = cudaFuncSetAttribute(k_transport_tile_gen<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) k_transport_tile_gen<false><<<grid, NTG + 32, smem, st>>>(p, t, mA, mH, mG, mD, I_out, f0, f1, f2, colflag, dt);
+        if (e == cudaSuccess) k_transport_tile_gen<false><<<grid, NTG + 32, smem, st>>>(p, t, mA, mH, mG, mD, mCx, mCy, mCz, I_out, f2, colflag, dt);
     }
     ++*launches;
     return e != cudaSuccess ? e : cudaGetLastError();
