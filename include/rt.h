@@ -47,7 +47,7 @@ enum { RT_LIM_MC = 0, RT_LIM_MINMOD = 1, RT_LIM_VANLEER = 2, RT_LIM_NONE = 3 };
 enum { RT_ANG_DONOR = 0, RT_ANG_MAPR = 1 };
 /* how the vacuum (Eq 20) spatial transport gets its stencil operands.  RT_TRANSPORT_TMA (default): a CTA owns a tile of
  * columns x a chunk of directions, a producer warp streams each x3-plane of the tile with its halos once into a ring of
- * shared-memory slots (cp.async.bulk.tensor + mbarrier), 15 consumer warps read all operands from the ring.  Needs the
+ * shared-memory slots (cp.async.bulk.tensor + mbarrier), 23 consumer warps read all operands from the ring.  Needs the
  * monotonised-central limiter and a PERIODIC or OUTFLOW x3 boundary; otherwise, and with RT_TRANSPORT_L2, one thread
  * per (column, direction) loads its operands itself through L1/L2 (the round-1 kernel).  Same arithmetic in the same
  * order: results are bit-identical.  Cells with an Eq 23 face go through k_transport_gen either way. */

@@ -139,6 +139,22 @@ k_cell_batch(KParams p, double *I, double *T, double dt, int *n_fail) {
         const bool interact = have && p.method != 0 && alpha != 0.0;
         const double adt = alpha * dt;
 
+        {   // the NEXT trip's operands towards the SM now: the rows of its cells and their fluid state (a trip is ~15 us of work per warp;
+            // otherwise its first loads -- list entry, then density, then intensities -- are three dependent trips to DRAM)
+            const long long wn = w0 + nwarps * CB + myc;
+            if (wn < nwork) {
+                const long long cn = (long long)__ldg(p.srclist + wn);
+                const char *row = reinterpret_cast<const char *>(I + cn * p.pitch);
+                for (int line = lane / CB; line * 128 < p.pitch * 8; line += 32 / CB)
+                    asm volatile("prefetch.global.L1 [%0];" ::"l"(row + line * 128));
+                if (lane < CB) {
+                    asm volatile("prefetch.global.L1 [%0];" ::"l"(p.rho + cn));
+                    asm volatile("prefetch.global.L1 [%0];" ::"l"(T + cn));
+#pragma unroll
+                    for (int m = 0; m < 4; ++m) asm volatile("prefetch.global.L1 [%0];" ::"l"(p.u4 + m * p.ncell + cn));
+                }
+            }
+        }
         // ---- phase 1: per cell, lanes over directions ----
         double val[CB][MAXV];          // I, then n^0 I / d for the cells that interact
         unsigned livebits = 0u;        // bit c * MAXV + v: direction v of cell c is updated (not masked, not a pad entry)
