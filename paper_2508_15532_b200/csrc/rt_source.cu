@@ -25,6 +25,18 @@ __device__ __forceinline__ double t_m35(double T) {
     return r * r * r * sqrt(r);
 }
 
+// 1 / x for the positive, well-scaled x = d nbar of a direction: the hardware's reciprocal seed (rcp.approx.ftz.f64, ~20 bits) and two
+// Newton steps (4 dependent FMAs, relative error < 2^-52 before the last rounding) instead of the correctly rounded __drcp_rn
+// (its special-case handling and longer dependent chain cost ~5 instructions and ~25 cycles of latency per direction)
+__device__ __forceinline__ double rcp_pos(double x) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);
+    y = fma(y, e, y);
+    e = fma(-x, y, 1.0);
+    return fma(y, e, y);
+}
+
 struct TEq {
     int method;
     double a4, b1, c0;             // methods 1, 2: a4 g(T) + b1 T + c0
@@ -188,7 +200,7 @@ k_cell_batch(KParams p, double *I, double *T, double dt, int *n_fail) {
                             const double nup = e0 + e1 * nx + e2 * ny + e3 * nz;
                             const double nbar = b0 - (b1 * nx + b2 * ny + b3 * nz);        // Eq 5, first row
                             // 1/d and 1/nbar from one reciprocal: 1/(d nbar) times nbar, times d
-                            const double d = nup + nbar * adt_c, r = __drcp_rn(d * nbar);
+                            const double d = nup + nbar * adt_c, r = rcp_pos(d * nbar);
                             const double rd = r * nbar, rn = r * d;
                             const double IbdOm = nbar * nbar * val[c][v] * ws;               // Ibar dOmegabar (S17)
                             E += IbdOm;                                                     // Eq 33
@@ -276,7 +288,7 @@ k_cell_batch(KParams p, double *I, double *T, double dt, int *n_fail) {
                             const double nx = snx[s], ny = sny[s], nz = snz[s];
                             const double nup = e0 + e1 * nx + e2 * ny + e3 * nz;
                             const double nbar = b0 - (b1 * nx + b2 * ny + b3 * nz);
-                            const double dm = nup + nbar * am, dp = nup + nbar * ap, r = __drcp_rn(dp * nbar);
+                            const double dm = nup + nbar * am, dp = nup + nbar * ap, r = rcp_pos(dp * nbar);
                             const double rd = r * nbar, rn = r * dp;
                             val[c][v] = val[c][v] * (dm * rd) + sd * (rd * (rn * rn * rn));
                             Ic[s] = val[c][v];
