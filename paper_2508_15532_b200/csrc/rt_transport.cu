@@ -37,10 +37,10 @@ __global__ void k_facecoef(KParams p, const double *__restrict__ T, double dt, i
         r = make_double4(0.5, -1.0, 0.0, 0.0);
     } else {
         const double et = exp(-tau);
-        const double ft = sqrt(-expm1(-tau * tau) / (tau * tau));
+        const double ft = sqrt(-expm1(-tau * tau)) * __drcp_rn(tau);   // f(tau) = sqrt(1 - e^(-tau^2)) / tau
         double v[4];
         for (int o = 0; o < 4; ++o)
-            v[o] = mirror_sign(q[a] + o - 2, N[a], p.bc_lo[a], p.bc_hi[a]) * (p.u4[(1 + a) * p.ncell + cell[o]] / p.u4[cell[o]]);
+            v[o] = mirror_sign(q[a] + o - 2, N[a], p.bc_lo[a], p.bc_hi[a]) * (p.u4[(1 + a) * p.ncell + cell[o]] * __drcp_rn(p.u4[cell[o]]));   // (reciprocal, not a division)
         const double vL = v[1] + 0.5 * slope_rt(p.limiter, v[1] - v[0], v[2] - v[1]);
         const double vR = v[2] - 0.5 * slope_rt(p.limiter, v[2] - v[1], v[3] - v[2]);
         double wL, wR;

@@ -42,7 +42,11 @@ __device__ __forceinline__ double mirror_sign(int c, int N, int bc_lo, int bc_hi
 }
 __device__ __forceinline__ double alpha_total(const KParams &p, double rho, double T) {
     if (rho < p.rho_floor) return 0.0;   // L468 (i)
-    double aa = (p.kappa_a0 != 0.0) ? p.kappa_a0 * rho * rho * pow(T, -3.5) : 0.0;
+    double aa = 0.0;
+    if (p.kappa_a0 != 0.0) {   // T^-3.5 = (1/T)^3 sqrt(1/T): a reciprocal and a square root instead of pow() (~100 instructions)
+        const double r = __drcp_rn(T);
+        aa = p.kappa_a0 * rho * rho * (r * r * r * sqrt(r));
+    }
     return aa + p.kappa_s * rho;
 }
 
